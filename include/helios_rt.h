@@ -1,0 +1,159 @@
+/*
+ * helios_rt.h -- C ABI of the B200-native (sm_100a) radiative-transfer step of THOR+HELIOS
+ * (Deitrick et al., arXiv 2203.02293; line numbers below are PAPER.md lines).
+ *
+ * One call = one pass of the paper's per-timestep multi-wavelength RT module ("Alfrodull",
+ * Sec. 2.2.6) over a batch of atmospheric columns, independently for every
+ * (column, k-table bin, Gauss point):
+ *   S1 level geometry            (Sec. 2.2.1; Fig. 3)
+ *   S2 Planck source per bin     (L171, L239)
+ *   S3 k-table P-T interpolation (Sec. 2.1.3)
+ *   S4 omega0, g0, dtau, beam    (Eqs. 17-18; Eq. B6)
+ *   S5 two-stream coefficients   (Eq. 19; Eqs. B1, B2, B5, B8 L1040-1091; Eq. 11)
+ *   S6 Thomas solve of the block-tridiagonal flux system (Eqs. 2-10; Eqs. 12-15)
+ *   S7 Gauss- and bin-weighted reduction to F_up, F_down (incl. beam, L235), F_net and the
+ *      heating rate dT/dt = -dF_net / (c_P dm)            (L393, L1032)
+ * Every stage runs in hand-written CUDA kernels in fp64; there is no CPU fallback.  Readings of
+ * the paper where it is silent (interpolation scheme, band Planck, interface p/T, ...) are listed
+ * in DESIGN.md ("Readings").
+ *
+ * Conventions: SI units (Pa, K, m, kg, W m^-2).  Layer j (0..N-1) lies between interface j (lower)
+ * and j+1 (upper); index 0 = bottom of atmosphere (BOA), interface N = top (TOA).  mu_star > 0 is
+ * the dayside (the paper's mu_star is -mu, App. B); mu_star <= 0: no beam.
+ * All arrays are fp64 and C-contiguous, (bin, Gauss point) fastest in the k-table.
+ *
+ * Threading: a handle may be used by one host thread at a time.  No call throws, aborts or
+ * prints.  Every function returns 0 on success or a negative HELIOS_RT_E* code.
+ */
+#ifndef HELIOS_RT_H
+#define HELIOS_RT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HELIOS_RT_OK        0
+#define HELIOS_RT_EINVAL   -1  /* NULL / negative size / non-monotone grid / sum(w) != 1 / w0 outside [0,1] /
+                                  n_columns > max_columns / unsupported size / output set inconsistent with flags */
+#define HELIOS_RT_ENOMEM   -2  /* host or device allocation failed */
+#define HELIOS_RT_ECUDA    -3  /* a CUDA runtime call failed; helios_rt_last_cuda_error() names it */
+#define HELIOS_RT_ENODEV   -4  /* no CUDA device, or the device is not compute capability 10.x */
+
+/* flags */
+#define HELIOS_RT_IMPROVED       1u  /* improved two-stream: E from Eq.(19); otherwise E = 1 (regular, L73) */
+#define HELIOS_RT_NONISOTHERMAL  2u  /* source linear in tau, two sub-layers per layer (Eqs. 4-9, Fig. 3) */
+#define HELIOS_RT_TOA_SPECTRUM   4u  /* post-processing shape (L385): only F_up_toa_bin is produced */
+
+#define HELIOS_RT_MAX_LAYERS 64
+
+typedef struct helios_rt helios_rt; /* opaque; owns all device tables and workspace */
+
+/* ---- create-time configuration: every pointer is a HOST pointer, deep-copied by create ------- */
+typedef struct {
+  int32_t n_layers;        /* N, 1..HELIOS_RT_MAX_LAYERS                                             */
+  int32_t n_bins;          /* k-table wavelength bins                                                */
+  int32_t n_gauss;         /* Gauss points per bin (L145)                                            */
+  int32_t n_ktab_p;        /* >= 2                                                                   */
+  int32_t n_ktab_t;        /* >= 2                                                                   */
+  int32_t max_columns;     /* workspace is sized for this many columns per step                      */
+  const double *ktab_p;    /* [n_ktab_p] Pa, strictly ascending                                      */
+  const double *ktab_t;    /* [n_ktab_t] K,  strictly ascending                                      */
+  const double *ktab;      /* [n_ktab_p][n_ktab_t][n_bins][n_gauss] absorption opacity, m^2/kg, > 0  */
+  const double *bin_edges; /* [n_bins+1] wavelength, m, strictly ascending, > 0                      */
+  const double *gauss_w;   /* [n_gauss], > 0, |sum - 1| <= 1e-10                                     */
+  const double *scat_gas;  /* [n_bins] gas (Rayleigh) scattering opacity sigma_scat,gas/mbar, m^2/kg */
+  const double *cloud_ext; /* [n_bins] f_cloud (sigma_abs+sigma_scat)_cloud/mbar, m^2/kg; 0 = none   */
+  const double *cloud_w0;  /* [n_bins] cloud single-scattering albedo in [0,1]                       */
+  const double *cloud_g0;  /* [n_bins] cloud asymmetry factor in [0,1)                               */
+  double cloud_p_top;      /* Pa; cloud present at levels with cloud_p_top <= p <= cloud_p_bot       */
+  double cloud_p_bot;      /* Pa                                                                     */
+  double gravity;          /* m s^-2 (Table 3: 47)                                                   */
+  double cp;               /* J kg^-1 K^-1 (Table 3: 12436)                                          */
+  double eps2;             /* second Eddington coefficient of the beam, default 2/3 (L1094)          */
+  double e_tau;            /* thin sub-layer tolerance, 1e-4 (L209)                                  */
+  double gcrit_tol;        /* mu_star,crit guard tolerance, 1e-5 (L252)                              */
+  double w0_transition;    /* regular -> improved switch, 0.1 (Eq.19)                                */
+  double f_toa;            /* diffuse downward flux per unit wavelength at the TOA, 0 (Fig.5)  */
+  uint32_t flags;          /* HELIOS_RT_*                                                            */
+} helios_rt_config;
+
+/* ---- per-step inputs: DEVICE pointers (helios_rt_step) or HOST pointers (helios_rt_step_host),
+ *      caller-owned, never written ------------------------------------------------------------ */
+typedef struct {
+  int32_t n_columns;          /* 0..max_columns (0: nothing is launched)                             */
+  const double *p;            /* [n_columns][n_layers] layer-centre pressure, Pa; layer 0 = bottom;
+                                 strictly decreasing with the layer index                            */
+  const double *T;            /* [n_columns][n_layers] K                                             */
+  const double *mu_star;      /* [n_columns] cosine of the stellar zenith angle                      */
+  const double *stellar_flux; /* [n_bins] TOA normal-incidence flux per unit wavelength, W m^-2 m^-1 */
+  double f_internal;          /* W m^-2 >= 0; T_int = (f_internal/sigma_SB)^(1/4),
+                                 F_BOA,b = pi B_b(T_int) (Eq.10)                           */
+} helios_rt_inputs;
+
+/* ---- per-step outputs: DEVICE (step) or HOST (step_host) pointers, caller-owned; NULL = not wanted
+ *      Without HELIOS_RT_TOA_SPECTRUM at least one pointer must be non-NULL; with it, F_up_toa_bin
+ *      must be non-NULL and all others NULL. ---------------------------------------------------- */
+typedef struct {
+  double *F_up;          /* [n_columns][n_layers+1] W m^-2                                           */
+  double *F_down;        /* [n_columns][n_layers+1] diffuse + direct beam (L235)                     */
+  double *F_net;         /* [n_columns][n_layers+1] F_up - F_down                                    */
+  double *dTdt;          /* [n_columns][n_layers]   K s^-1                                           */
+  double *F_beam;        /* [n_columns][n_layers+1] direct-beam part of F_down (Fig. 10 check, L245) */
+  double *F_up_toa_bin;  /* [n_columns][n_bins]     sum_g w_g F_up at the TOA, W m^-2 m^-1           */
+} helios_rt_outputs;
+
+/* Validates cfg, uploads the k-table as ln(kappa) and all per-bin constants, allocates every
+ * workspace needed for max_columns.  The caller may free its tables as soon as this returns.
+ * On failure *out is NULL. */
+int helios_rt_create(const helios_rt_config *cfg, helios_rt **out);
+
+/* One RT step over in->n_columns columns.  Asynchronous: kernels are enqueued on `cuda_stream`
+ * (a cudaStream_t; NULL = the legacy default stream); no host synchronisation, no allocation, no
+ * host<->device copy.  Outputs are complete when the stream reaches this point.  NaN inputs
+ * propagate to the outputs of their own column only; (p, T) outside the table are clamped to its
+ * edge (no extrapolation, not an error). */
+int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
+                   void *cuda_stream);
+
+/* Same step with HOST buffers (pinned memory recommended): copies the inputs to device staging
+ * owned by the handle, runs the step, copies the requested outputs back and synchronises.  This is
+ * the end-to-end path bench.py times ("e2e"). */
+int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out);
+
+/* Frees every device and host resource of the handle (NULL is accepted). */
+int helios_rt_destroy(helios_rt *h);
+
+/* Static description of a code returned above. */
+const char *helios_rt_strerror(int code);
+
+/* cudaGetErrorString of the last CUDA failure seen by this handle ("" if none). */
+const char *helios_rt_last_cuda_error(const helios_rt *h);
+
+/* Launch geometry of the step kernel for n_columns columns, for benchmarks and profiles:
+ * info[0] = threads per block, [1] = blocks per column (tiles), [2] = dynamic shared memory bytes,
+ * [3] = registers per thread, [4] = resident blocks per SM (occupancy API), [5] = local-memory
+ * bytes per thread, [6] = kernels launched per step, [7] = SM count of the device. */
+int helios_rt_launch_info(const helios_rt *h, int32_t info[8]);
+
+/* Device self-test of the fp64 primitives the kernels use instead of the CUDA math library
+ * (reciprocal, reciprocal square root, exp / 1-exp).  x: n HOST values; outputs n HOST values each:
+ * rcp = 1/x, rsq = 1/sqrt(|x|), ex = exp(-|x|), omx = 1 - exp(-|x|).  Used by the tests. */
+int helios_rt_selftest_math(int32_t n, const double *x, double *rcp, double *rsq, double *ex,
+                            double *omx);
+
+/* Device evaluation of the band Planck function used by S2: out[i] = B_b(T[i]) for the bin
+ * [lam_lo[i], lam_hi[i]] (HOST arrays of length n).  Used by the tests. */
+int helios_rt_selftest_planck(int32_t n, const double *T, const double *lam_lo, const double *lam_hi,
+                              double *out);
+
+/* Sustained fp64 FMA rate of the device in DFMA/s (8 independent chains per thread, all SMs),
+ * measured over `iters` dependent FMAs per chain; *sm_clock_mhz receives the SM clock implied by
+ * clock64() during the run.  This is the measured ALU roofline bench.py reports against. */
+int helios_rt_measure_dfma_peak(int32_t iters, double *dfma_per_s, double *sm_clock_mhz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HELIOS_RT_H */

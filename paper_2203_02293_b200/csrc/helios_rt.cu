@@ -1,0 +1,1092 @@
+// helios_rt.cu -- B200 (sm_100a) implementation of the THOR+HELIOS radiative-transfer step.
+//
+// C ABI: include/helios_rt.h.  Citations are PAPER.md lines (arXiv 2203.02293).
+//
+// One fused kernel per step.  A thread block owns one atmospheric column and a tile of its
+// (bin, Gauss point) spectral points; one thread = one spectral point = one monochromatic
+// two-stream problem over the column (the unit the paper solves independently, L449/L592):
+//
+//   prologue (block-cooperative, shared memory): S1 level geometry (interface p,T; layer masses;
+//            k-table cell + weights per level) and S2 band Planck B_b(T_level) for the tile's bins.
+//   sweep 1  (per thread, TOA -> BOA): S3 bilinear ln(kappa) interpolation + exp, S4 omega0/g0/dtau,
+//            tau prefix and direct beam (Eq. B6), S5 layer coefficients (Eq. 19, B1, B2, B5, B8,
+//            Eq. 11 guard) and the forward elimination of S6.  The block-tridiagonal system of
+//            Eq.(12) has one non-zero in each off-diagonal 2x2 block, so Eqs.(13)-(14) reduce to the
+//            scalar recurrences (R, U, c, d) below; they are carried in registers.
+//   sweep 2  (BOA -> TOA): back-substitution Eq.(15) fused with S7, the Gauss-/bin-weighted
+//            reduction (warp shuffles, then shared memory, then a fixed-order sum over tiles).
+//
+// The layer relations are used in transmission/reflection form.  With zeta+- and T of Eq.(B2),
+//   t = psi/chi = s T / (a b),  r = -xi/chi = zeta+ zeta- (1 - T^2) / (a b),
+//   a = zeta+ - zeta- T,  b = zeta+ + zeta- T,  s = zeta+ - zeta-,  1 - t - r = s (1 - T) / b,
+// Eqs.(2),(3) read  F_up[j+1] = t F_up[j] + r F_dn[j+1] + S_up,  F_dn[j] = t F_dn[j+1] + r F_up[j] + S_dn.
+// These forms avoid the cancellations of chi + xi - psi and 1 - T^2.
+//
+// fp64 throughout.  Reciprocals, reciprocal square roots and exponentials are done with the
+// MUFU seed instructions plus Newton/polynomial refinement in FMA (the fp64 pipe is the binding
+// resource); helios_rt_selftest_math exposes them to the tests.
+
+#include "../../include/helios_rt.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+namespace {
+
+constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kH = 6.62607015e-34, kC = 299792458.0, kKB = 1.380649e-23;  // CODATA 2019 (exact)
+constexpr double kSigmaSB =
+    2.0 * kPi * kPi * kPi * kPi * kPi * kKB * kKB * kKB * kKB / (15.0 * kH * kH * kH * kC * kC);
+constexpr double kPlanckC1 = 2.0 * kKB * kKB * kKB * kKB / (kH * kH * kH * kC * kC);  // 2 k^4 / (h^3 c^2)
+constexpr double kPlanckC2 = kH * kC / kKB;                                            // h c / k
+
+// --------------------------------------------------------------------------------------------
+// fp64 primitives
+// --------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RCP64H: ~20 good bits
+  double e = fma(-x, y, 1.0);
+  e = fma(e, e, e);        // e + e^2
+  y = fma(y, e, y);        // cubic step: error ~ e^3
+  e = fma(-x, y, 1.0);     // one Newton step to land within 1 ulp
+  return fma(y, e, y);
+}
+
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RSQ64H
+  double t = x * y;
+  double e = fma(-t, y, 1.0);            // 1 - x y^2
+  double p = fma(0.375, e, 0.5) * e;     // e/2 + 3 e^2/8
+  y = fma(y, p, y);
+  t = x * y;
+  e = fma(-t, y, 1.0);
+  return fma(0.5 * y, e, y);
+}
+
+// expm1 on the reduced argument |r| <= ln2/2: r + r^2 q(r), q near-minimax of degree 9.
+__device__ __forceinline__ double expm1_reduced(double r) {
+  double q = 2.51003854955103203e-08;
+  q = fma(q, r, 2.76200884454097462e-07);
+  q = fma(q, r, 2.75572684599970641e-06);
+  q = fma(q, r, 2.48015212959543761e-05);
+  q = fma(q, r, 1.98412698630536177e-04);
+  q = fma(q, r, 1.38888889172137167e-03);
+  q = fma(q, r, 8.33333333333006153e-03);
+  q = fma(q, r, 4.16666666666241289e-02);
+  q = fma(q, r, 1.66666666666666685e-01);
+  q = fma(q, r, 5.00000000000000111e-01);
+  return fma(r * r, q, r);
+}
+
+// exp(x) for -708 <= x <= 700 (callers clamp).  If OM, *om = 1 - exp(x) without cancellation for
+// small |x| (x <= 0).
+template <bool OM>
+__device__ __forceinline__ double exp_core(double x, double *om) {
+  const double kMagic = 6755399441055744.0;  // 1.5 * 2^52: round-to-nearest-integer trick
+  double kd = fma(x, 1.4426950408889634074, kMagic);
+  int k = __double2loint(kd);
+  kd -= kMagic;
+  double r = fma(kd, -6.93147180369123816490e-01, x);
+  r = fma(kd, -1.90821492927058770002e-10, r);
+  double p = expm1_reduced(r);
+  double y = 1.0 + p;
+  double res = __hiloint2double(__double2hiint(y) + (k << 20), __double2loint(y));
+  if (OM) *om = (k == 0) ? -p : 1.0 - res;
+  return res;
+}
+__device__ __forceinline__ double exp_fast(double x) {
+  return exp_core<false>(fmin(fmax(x, -708.0), 700.0), nullptr);
+}
+// exp(-a) and 1 - exp(-a) for a >= 0
+__device__ __forceinline__ double exp_neg_fast(double a, double *om) {
+  return exp_core<true>(-fmin(a, 708.0), om);
+}
+
+// --------------------------------------------------------------------------------------------
+// S2: band Planck.  G(x) = int_x^inf t^3/(e^t - 1) dt (reading R8).
+//   x >= 1.5 : sum_n e^{-n x} (x^3/n + 3 x^2/n^2 + 6 x/n^3 + 6/n^4)
+//   x <  1.5 : pi^4/15 - sum_k B_k x^{k+3} / ((k+3) k!)   (Bernoulli numbers B_k)
+// --------------------------------------------------------------------------------------------
+__device__ double planck_G(double x) {
+  if (!(x > 0.0)) return kPi * kPi * kPi * kPi / 15.0;
+  if (x >= 1.5) {
+    if (x > 745.0) return 0.0;
+    const double u = exp(-x);
+    const double x2 = x * x, x3 = x2 * x;
+    double un = 1.0, sum = 0.0;
+    for (int n = 1; n <= 32; ++n) {
+      un *= u;
+      const double in = 1.0 / (double)n;
+      // x^3/n + 3 x^2/n^2 + 6 x/n^3 + 6/n^4
+      const double poly = in * fma(in, fma(in, fma(in, 6.0, 6.0 * x), 3.0 * x2), x3);
+      const double term = un * poly;
+      sum += term;
+      if (term < 1e-18 * sum) break;
+    }
+    return sum;
+  }
+  // coefficients B_k / ((k+3) k!), k = 0,1,2,4,...,30
+  const double c0 = 1.0 / 3.0, c1 = -1.0 / 8.0;
+  const double ce[15] = {
+      1.0 / 60.0,                                   // k=2 : (1/6)/(5*2)
+      -1.0 / 5040.0,                                // k=4 : (-1/30)/(7*24)
+      1.0 / 272160.0,                               // k=6 : (1/42)/(9*720)
+      -1.0 / 13305600.0,                            // k=8
+      1.0 / 622702080.0,                            // k=10
+      -691.0 / (2730.0 * 15.0 * 479001600.0),       // k=12
+      7.0 / (6.0 * 17.0 * 87178291200.0),           // k=14
+      -3617.0 / (510.0 * 19.0 * 20922789888000.0),  // k=16
+      43867.0 / (798.0 * 21.0 * 6402373705728000.0),            // k=18
+      -174611.0 / (330.0 * 23.0 * 2432902008176640000.0),       // k=20
+      854513.0 / (138.0 * 25.0 * 1124000727777607680000.0),     // k=22
+      -236364091.0 / (2730.0 * 27.0 * 620448401733239439360000.0),   // k=24
+      8553103.0 / (6.0 * 29.0 * 403291461126605635584000000.0),      // k=26
+      -23749461029.0 / (870.0 * 31.0 * 304888344611713860501504000000.0),   // k=28
+      8615841276005.0 / (14322.0 * 33.0 * 265252859812191058636308480000000.0)  // k=30
+  };
+  const double x2 = x * x;
+  double s = ce[14];
+#pragma unroll
+  for (int i = 13; i >= 0; --i) s = fma(s, x2, ce[i]);
+  // low = x^3 (c0 + c1 x + x^2 s)
+  const double low = x2 * x * fma(x2, s, fma(c1, x, c0));
+  return kPi * kPi * kPi * kPi / 15.0 - low;
+}
+
+// --------------------------------------------------------------------------------------------
+// kernel parameters
+// --------------------------------------------------------------------------------------------
+struct BinConst {   // per bin, built at create time from scat_gas / cloud_* (Eqs. 17-18)
+  double dlam;      // lam_hi - lam_lo
+  double inv_dlam;
+  double sb[2];     // kappa_ext = kappa_abs + sb[cloudy]
+  double ss[2];     // omega0 = ss[cloudy] / kappa_ext
+  double gg[2];     // g0 at a clear / cloudy level
+};
+
+struct KParams {
+  // create-time tables (device)
+  const double *lnk;      // [nP][nT][npt] ln(kappa)
+  const double *tab_lp;   // [nP] log10(p)
+  const double *tab_t;    // [nT]
+  const double *edges;    // [nb+1]
+  const double *gauss_w;  // [ng]
+  const BinConst *bins;   // [nb]
+  int nP, nT, N, nb, ng, npt, tiles;
+  double cloud_p_top, cloud_p_bot, inv_g, inv_cp, inv_eps2, e_tau, gcrit_tol, w0_transition, f_toa;
+  int improved;
+  // per-step
+  const double *p, *T, *mu, *fstar;
+  double T_int;
+  double *F_up, *F_down, *F_net, *dTdt, *F_beam, *F_toa_bin;
+  // workspace
+  double *partial;        // [ncol][tiles][3][N+1]
+  unsigned *counter;      // [ncol]
+};
+
+struct ThreadConst {      // per spectral point
+  double W;               // dlam_b * w_g
+  double sb0, sb1, ss0, ss1, gg1;
+  double muF;             // mu * F_star[b]
+};
+
+// --------------------------------------------------------------------------------------------
+// S5 + S6 forward step for one (sub-)layer between a lower level "a" and an upper level "b".
+// In: (R, U) at the upper level: F_dn[b] = R F_up[b] + U.   Out: (R, U) at the lower level and the
+// back-substitution pair (c, d): F_up[b] = c F_up[a] + d.
+// --------------------------------------------------------------------------------------------
+template <bool DAY, bool LINSRC>
+__device__ __forceinline__ void layer_forward(const KParams &P, double w0, double g0, double dtau,
+                                              double Ba, double Bb, double mu, double Fa, double Fb,
+                                              double &R, double &U, double &c, double &d) {
+  // E, Eq.(19) L374 (readings R5, R6)
+  double E = 1.0;
+  if (P.improved) {
+    double fit = 1.225 + g0 * (-0.1582 - 0.07465 * g0) + w0 * (-0.1777 + 0.2351 * g0 - 0.05582 * w0);
+    E = (w0 > P.w0_transition) ? fmax(fit, 1.0) : 1.0;
+  }
+  const double wg = w0 * g0;
+  const double num = E - w0;             // E - omega0
+  const double den = E * (1.0 - wg);     // E (1 - omega0 g0)
+  const double X = num * den;
+  const double rs = rsqrt_fast(X);       // 1/sqrt(E (E-w0)(1-w0 g0))
+  const double s = num * rs;             // sqrt((E-w0)/(E(1-w0 g0))) = zeta+ - zeta-   (B2)
+  const double alpha = 2.0 * (X * rs);   // 2 sqrt(E (E-w0)(1-w0 g0))
+  const double rs2 = rs * rs;
+  const double invP = 0.5 * (num * rs2); // 1 / (2 E (1 - w0 g0))
+  const double inv_num = den * rs2;      // 1 / (E - w0)
+  const double zp = 0.5 + 0.5 * s, zm = 0.5 - 0.5 * s;
+  double omT;
+  const double Tr = exp_neg_fast(alpha * dtau, &omT);   // transmission function (B2), 1 - T
+  const double zmT = zm * Tr;
+  const double a = zp - zmT, b = zp + zmT;
+  const double inv_ab = rcp_fast(a * b);
+  const double t = s * Tr * inv_ab;                          // psi/chi
+  const double r = zp * zm * omT * (1.0 + Tr) * inv_ab;      // -xi/chi
+  const double emis = s * omT * a * inv_ab;                  // 1 - t - r
+  const double Pi = kPi * (1.0 - w0) * inv_num;              // (B5)
+  double Sup, Sdn;
+  if (LINSRC) {
+    // Eqs.(4)-(9): B* (1-r) - t B*' +- B' (1 - t + r)/(2E(1-w0 g0)), B' = (Ba - Bb)/dtau; e_tau rule L209
+    const bool thin = dtau < P.e_tau;
+    const double Bm = 0.5 * (Ba + Bb);
+    const double dB = thin ? 0.0 : (Ba - Bb);
+    const double Bal = thin ? Bm : Ba, Bbl = thin ? Bm : Bb;
+    const double grad = (1.0 - t + r) * invP * rcp_fast(dtau);
+    const double k = dB * (t - grad);
+    Sup = Pi * fma(Bbl, emis, -k);
+    Sdn = Pi * fma(Bal, emis, k);
+  } else {
+    Sup = Sdn = Pi * Bb * emis;                              // Eqs.(2),(3)
+  }
+  if (DAY) {
+    // (B8) with mu_star = -mu; guard of Eq.(11)/L252 (reading R4)
+    const double ma = mu * alpha;
+    double D = (ma - 1.0) * (ma + 1.0);                      // 4 E mu^2 (E-w0)(1-w0 g0) - 1
+    D = (fabs(D) < P.gcrit_tol) ? -2.0 * mu : D;
+    const double invD = rcp_fast(D);
+    const double lead = w0 * (2.0 * den + g0 * P.inv_eps2) * invD;
+    const double last = wg * P.inv_eps2 * invP;
+    const double Gp = 0.5 * fma(lead, invP - mu, last);
+    const double Gm = 0.5 * fma(lead, -invP - mu, -last);
+    // (B7): S_up += t G+ Fa + r G- Fb - G+ Fb ; S_dn += t G- Fb + r G+ Fa - G- Fa
+    Sup += Gp * fma(t, Fa, -Fb) + r * Gm * Fb;
+    Sdn += Gm * fma(t, Fb, -Fa) + r * Gp * Fa;
+  }
+  // forward elimination (Eqs. 13-14 specialised): F_up[b] (1 - r R) = t F_up[a] + r U + S_up
+  const double q = rcp_fast(1.0 - r * R);
+  c = t * q;
+  d = fma(r, U, Sup) * q;
+  const double Rn = fma(t * c, R, r);
+  const double Un = fma(c, fma(R, Sup, U), Sdn);
+  R = Rn;
+  U = Un;
+}
+
+// optical properties at one level (S3 + Eqs. 17-18)
+__device__ __forceinline__ void level_optics(const double *__restrict__ lnk_pt, int off, int strideT,
+                                             int strideP, double wp, double wt, int cloudy,
+                                             const ThreadConst &tc, double &kx, double &w0, double &g0) {
+  const double l00 = __ldg(lnk_pt + off);
+  const double l01 = __ldg(lnk_pt + off + strideT);
+  const double l10 = __ldg(lnk_pt + off + strideP);
+  const double l11 = __ldg(lnk_pt + off + strideP + strideT);
+  const double lo = fma(wt, l01 - l00, l00);
+  const double hi = fma(wt, l11 - l10, l10);
+  const double kabs = exp_fast(fma(wp, hi - lo, lo));
+  kx = kabs + (cloudy ? tc.sb1 : tc.sb0);
+  w0 = (cloudy ? tc.ss1 : tc.ss0) * rcp_fast(kx);
+  g0 = cloudy ? tc.gg1 : 0.0;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// --------------------------------------------------------------------------------------------
+// the step kernel
+// --------------------------------------------------------------------------------------------
+struct SmemLayout {
+  int nlev;        // levels at which kappa / Planck are evaluated: N (iso) or 2N+1 (non-iso)
+  int nbt;         // max bins per tile
+  size_t off_lnp, off_pint, off_tint, off_plev, off_tlev, off_wp, off_wt, off_cell, off_cloud, off_dm,
+      off_dmfull, off_G, off_B, off_red, off_fin, off_vals, total;
+};
+
+__host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block, int ng, int nb) {
+  SmemLayout L;
+  L.nlev = noniso ? 2 * N + 1 : N;
+  int nbt = (block + ng - 1) / ng + 1;
+  L.nbt = nbt < nb ? nbt : nb;
+  const int nwarp = (block + 31) / 32;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
+  L.off_lnp = take(sizeof(double) * N);
+  L.off_pint = take(sizeof(double) * (N + 1));
+  L.off_tint = take(sizeof(double) * (N + 1));
+  L.off_plev = take(sizeof(double) * L.nlev);
+  L.off_tlev = take(sizeof(double) * (L.nlev + 1));           // + internal temperature row
+  L.off_wp = take(sizeof(double) * L.nlev);
+  L.off_wt = take(sizeof(double) * L.nlev);
+  L.off_cell = take(sizeof(int) * L.nlev);
+  L.off_cloud = take(sizeof(int) * L.nlev);
+  L.off_dm = take(sizeof(double) * 2 * N);                    // per system layer
+  L.off_dmfull = take(sizeof(double) * N);
+  L.off_G = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
+  L.off_B = take(sizeof(double) * (L.nlev + 1) * L.nbt);
+  L.off_red = take(sizeof(double) * nwarp * 3 * (N + 1));
+  L.off_fin = take(sizeof(double) * 3 * (N + 1));
+  L.off_vals = take(sizeof(double) * block);
+  L.total = o;
+  return L;
+}
+
+template <bool NONISO, bool TOA, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int N = P.N;
+  const SmemLayout L = smem_layout(N, NONISO, BLOCK, P.ng, P.nb);
+  double *s_lnp = (double *)(smem + L.off_lnp);
+  double *s_pint = (double *)(smem + L.off_pint);
+  double *s_tint = (double *)(smem + L.off_tint);
+  double *s_plev = (double *)(smem + L.off_plev);
+  double *s_tlev = (double *)(smem + L.off_tlev);
+  double *s_wp = (double *)(smem + L.off_wp);
+  double *s_wt = (double *)(smem + L.off_wt);
+  int *s_cell = (int *)(smem + L.off_cell);
+  int *s_cloud = (int *)(smem + L.off_cloud);
+  double *s_dm = (double *)(smem + L.off_dm);
+  double *s_dmfull = (double *)(smem + L.off_dmfull);
+  double *s_G = (double *)(smem + L.off_G);
+  double *s_B = (double *)(smem + L.off_B);
+  double *s_red = (double *)(smem + L.off_red);
+  double *s_fin = (double *)(smem + L.off_fin);
+  double *s_vals = (double *)(smem + L.off_vals);
+  __shared__ int s_is_last;
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x, col = blockIdx.y;
+  const int nlev = L.nlev;
+  const double *pc = P.p + (size_t)col * N;
+  const double *Tc = P.T + (size_t)col * N;
+  const double mu = P.mu[col];
+  const bool day = mu > 0.0;
+
+  const int pt0 = tile * BLOCK;
+  const int b_first = pt0 / P.ng;
+  int pt_last = pt0 + BLOCK - 1;
+  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
+  const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
+
+  // ---------------- S1: level geometry (reading R9; L171) ----------------
+  for (int j = tid; j < N; j += BLOCK) s_lnp[j] = log(pc[j]);
+  __syncthreads();
+  for (int i = tid; i <= N; i += BLOCK) {
+    double lp, ti;
+    if (N == 1) {
+      lp = s_lnp[0] + (i == 0 ? 0.5 : -0.5) * 2.302585092994045684;
+      ti = Tc[0];
+    } else if (i == 0) {
+      lp = s_lnp[0] + 0.5 * (s_lnp[0] - s_lnp[1]);
+      ti = Tc[0];
+    } else if (i == N) {
+      lp = s_lnp[N - 1] - 0.5 * (s_lnp[N - 2] - s_lnp[N - 1]);
+      ti = Tc[N - 1];
+    } else {
+      lp = 0.5 * (s_lnp[i - 1] + s_lnp[i]);
+      ti = 0.5 * (Tc[i - 1] + Tc[i]);
+    }
+    s_pint[i] = exp(lp);
+    s_tint[i] = ti;
+  }
+  __syncthreads();
+  for (int l = tid; l <= nlev; l += BLOCK) {
+    if (l == nlev) { s_tlev[l] = P.T_int; continue; }
+    double pl, tl;
+    if (NONISO) {
+      if (l & 1) { pl = pc[l >> 1]; tl = Tc[l >> 1]; }
+      else       { pl = s_pint[l >> 1]; tl = s_tint[l >> 1]; }
+    } else { pl = pc[l]; tl = Tc[l]; }
+    s_plev[l] = pl;
+    s_tlev[l] = tl;
+    s_cloud[l] = (pl >= P.cloud_p_top && pl <= P.cloud_p_bot) ? 1 : 0;
+    // table cell + weights: bilinear in (log10 p, T), clamped (reading R7)
+    double xp = log10(pl);
+    xp = fmin(fmax(xp, P.tab_lp[0]), P.tab_lp[P.nP - 1]);
+    int ip = 0;
+    while (ip < P.nP - 2 && xp > P.tab_lp[ip + 1]) ++ip;
+    const double wp = (xp - P.tab_lp[ip]) / (P.tab_lp[ip + 1] - P.tab_lp[ip]);
+    double xt = fmin(fmax(tl, P.tab_t[0]), P.tab_t[P.nT - 1]);
+    int it = 0;
+    while (it < P.nT - 2 && xt > P.tab_t[it + 1]) ++it;
+    const double wt = (xt - P.tab_t[it]) / (P.tab_t[it + 1] - P.tab_t[it]);
+    s_wp[l] = wp;
+    s_wt[l] = wt;
+    s_cell[l] = (ip * P.nT + it) * P.npt;
+  }
+  for (int j = tid; j < N; j += BLOCK) s_dmfull[j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
+  __syncthreads();
+  if (NONISO) {
+    for (int s = tid; s < 2 * N; s += BLOCK) s_dm[s] = (s_plev[s] - s_plev[s + 1]) * P.inv_g;
+  }
+
+  // ---------------- S2: band Planck for the tile's bins (reading R8) ----------------
+  const int nedge = nbt + 1;
+  for (int i = tid; i < (nlev + 1) * nedge; i += BLOCK) {
+    const int l = i / nedge, e = i - l * nedge;
+    const double Tl = s_tlev[l];
+    s_G[l * (L.nbt + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b_first + e] * Tl)) : 0.0;
+  }
+  __syncthreads();
+  for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
+    const int l = i / nbt, bl = i - l * nbt;
+    const double Tl = s_tlev[l];
+    const double T2 = Tl * Tl;
+    const double *g = s_G + l * (L.nbt + 1) + bl;
+    double B = kPlanckC1 * T2 * T2 * (g[1] - g[0]) * P.bins[b_first + bl].inv_dlam;
+    if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
+    s_B[l * L.nbt + bl] = (Tl > 0.0) ? B : 0.0;
+  }
+  __syncthreads();
+
+  // ---------------- per-thread constants ----------------
+  int pt = pt0 + tid;
+  const bool active = pt < P.npt;
+  if (!active) pt = P.npt - 1;
+  const int b = pt / P.ng, gidx = pt - b * P.ng;
+  const int bl = b - b_first;
+  ThreadConst tc;
+  {
+    const BinConst bc = P.bins[b];
+    tc.W = active ? bc.dlam * P.gauss_w[gidx] : 0.0;
+    tc.sb0 = bc.sb[0]; tc.sb1 = bc.sb[1];
+    tc.ss0 = bc.ss[0]; tc.ss1 = bc.ss[1];
+    tc.gg1 = bc.gg[1];
+    tc.muF = day ? mu * P.fstar[b] : 0.0;
+  }
+  const double inv_mu = day ? 1.0 / mu : 0.0;
+  const double *lnk_pt = P.lnk + pt;
+  const int strideT = P.npt, strideP = P.nT * P.npt;
+  const double *Bcol = s_B + bl;   // B[l] = Bcol[l * L.nbt]
+  const int nbtS = L.nbt;
+
+  // back-substitution state, one entry per interface 1..N (thread-private, local memory:
+  // written top-down, read bottom-up -- a stack, served by L1/L2)
+  double2 st_cd[TOA ? 1 : MAXL];
+  double2 st_RU[TOA ? 1 : MAXL];
+
+  // ---------------- sweep 1: TOA -> BOA ----------------
+  double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
+  double tau = 0.0;
+  double Fb = tc.muF;                // beam at the TOA (full strength, L235)
+  double Ctoa = 1.0, Dtoa = 0.0;     // TOA mode: F_up[N] = Ctoa F_up[j] + Dtoa
+  const bool want_beam = !TOA && (P.F_beam != nullptr);
+  const int warp = tid >> 5, lane = tid & 31;
+  double *red_w = s_red + (size_t)warp * 3 * (N + 1);
+  if (want_beam) {
+    const double wb = warp_sum(tc.W * Fb);
+    if (lane == 0) red_w[2 * (N + 1) + N] = wb;
+  }
+
+  double kx_up = 0.0, w0_up = 0.0, g0_up = 0.0;   // non-iso: optics at the upper interface
+  if (NONISO) {
+    const int l = 2 * N;
+    level_optics(lnk_pt, s_cell[l], strideT, strideP, s_wp[l], s_wt[l], s_cloud[l], tc, kx_up, w0_up, g0_up);
+  }
+
+#pragma unroll 1
+  for (int j = N - 1; j >= 0; --j) {
+    double c, d;
+    const double R_top = R, U_top = U, Fb_top = Fb;
+    if (!NONISO) {
+      double kx, w0, g0;
+      level_optics(lnk_pt, s_cell[j], strideT, strideP, s_wp[j], s_wt[j], s_cloud[j], tc, kx, w0, g0);
+      const double dtau = kx * s_dmfull[j];
+      tau += dtau;
+      double Fa = 0.0;
+      const double Bj = Bcol[j * nbtS];
+      if (day) {
+        Fa = tc.muF * exp_fast(-tau * inv_mu);                 // (B6)
+        layer_forward<true, false>(P, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, R, U, c, d);
+      } else {
+        layer_forward<false, false>(P, w0, g0, dtau, Bj, Bj, mu, 0.0, 0.0, R, U, c, d);
+      }
+      Fb = Fa;
+    } else {
+      // levels: 2j+2 (upper interface, carried), 2j+1 (centre), 2j (lower interface)
+      double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo;
+      const int lc = 2 * j + 1, ll = 2 * j;
+      level_optics(lnk_pt, s_cell[lc], strideT, strideP, s_wp[lc], s_wt[lc], s_cloud[lc], tc, kx_c, w0_c, g0_c);
+      level_optics(lnk_pt, s_cell[ll], strideT, strideP, s_wp[ll], s_wt[ll], s_cloud[ll], tc, kx_lo, w0_lo, g0_lo);
+      const double B_up = Bcol[(lc + 1) * nbtS], B_c = Bcol[lc * nbtS], B_lo = Bcol[ll * nbtS];
+      // upper sub-layer: arithmetic means of centre and interface values (L171, reading R10)
+      const double dtau_u = 0.5 * (kx_c + kx_up) * s_dm[lc];
+      const double dtau_l = 0.5 * (kx_lo + kx_c) * s_dm[ll];
+      double cu, du, cl, dl;
+      if (day) {
+        tau += dtau_u;
+        const double Fc = tc.muF * exp_fast(-tau * inv_mu);
+        layer_forward<true, true>(P, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, Fc, Fb,
+                                  R, U, cu, du);
+        tau += dtau_l;
+        const double Fa = tc.muF * exp_fast(-tau * inv_mu);
+        layer_forward<true, true>(P, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, Fa, Fc,
+                                  R, U, cl, dl);
+        Fb = Fa;
+      } else {
+        layer_forward<false, true>(P, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, 0.0, 0.0,
+                                   R, U, cu, du);
+        layer_forward<false, true>(P, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, 0.0, 0.0,
+                                   R, U, cl, dl);
+      }
+      // F_up[j+1] = cu F_up[c] + du,  F_up[c] = cl F_up[j] + dl
+      c = cu * cl;
+      d = fma(cu, dl, du);
+      kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo;
+    }
+    if (TOA) {
+      Dtoa = fma(Ctoa, d, Dtoa);
+      Ctoa *= c;
+    } else {
+      // weights folded in: back-substitution runs on W F_up; F_dn carries the beam (L235)
+      st_cd[j] = make_double2(c, tc.W * d);
+      st_RU[j] = make_double2(R_top, tc.W * (U_top + Fb_top));
+      if (want_beam) {
+        const double wb = warp_sum(tc.W * Fb);
+        if (lane == 0) red_w[2 * (N + 1) + j] = wb;
+      }
+    }
+  }
+
+  // ---------------- BOA, Eq.(10) L237 ----------------
+  const double F_boa = Bcol[nlev * nbtS];
+  const double Fup0 = (U + F_boa + Fb) * rcp_fast(1.0 - R);
+  const double Fdn0 = fma(R, Fup0, U);
+
+  if (TOA) {
+    // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
+    const double FupN = fma(Ctoa, Fup0, Dtoa);
+    s_vals[tid] = active ? P.gauss_w[gidx] * FupN : 0.0;
+    __syncthreads();
+    for (int k = tid; k < nbt; k += BLOCK) {
+      const int bb = b_first + k;
+      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
+      // a bin may straddle two tiles: every tile adds its own part
+      const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
+      if (g_lo < 0) g_lo = 0;
+      if (g_hi > BLOCK) g_hi = BLOCK;
+      double sum = 0.0;
+      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
+      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
+      if (whole) *dst = sum; else atomicAdd(dst, sum);
+    }
+    return;
+  }
+
+  // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction ----------------
+  {
+    double wFup = tc.W * Fup0;
+    double wFdn = tc.W * (Fdn0 + Fb);
+    double su = warp_sum(wFup), sd = warp_sum(wFdn);
+    if (lane == 0) { red_w[0] = su; red_w[N + 1] = sd; }
+#pragma unroll 1
+    for (int j = 0; j < N; ++j) {
+      const double2 cd = st_cd[j];
+      const double2 RU = st_RU[j];
+      wFup = fma(cd.x, wFup, cd.y);
+      wFdn = fma(RU.x, wFup, RU.y);
+      su = warp_sum(wFup);
+      sd = warp_sum(wFdn);
+      if (lane == 0) { red_w[j + 1] = su; red_w[N + 1 + j + 1] = sd; }
+    }
+    if (P.F_toa_bin != nullptr) s_vals[tid] = active ? wFup * P.bins[b].inv_dlam : 0.0;
+  }
+  __syncthreads();
+
+  // cross-warp sum in fixed order -> tile partial
+  const int nwarp = (BLOCK + 31) / 32;
+  const int nred = (want_beam ? 3 : 2) * (N + 1);
+  for (int k = tid; k < nred; k += BLOCK) {
+    double sum = 0.0;
+    for (int w = 0; w < nwarp; ++w) sum += s_red[(size_t)w * 3 * (N + 1) + k];
+    s_fin[k] = sum;
+  }
+  if (P.F_toa_bin != nullptr) {
+    for (int k = tid; k < nbt; k += BLOCK) {
+      const int bb = b_first + k;
+      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
+      const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
+      if (g_lo < 0) g_lo = 0;
+      if (g_hi > BLOCK) g_hi = BLOCK;
+      double sum = 0.0;
+      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
+      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
+      if (whole) *dst = sum; else atomicAdd(dst, sum);
+    }
+  }
+  __syncthreads();
+
+  if (P.tiles > 1) {
+    // publish the tile partial; the last tile of the column to arrive sums them in tile order
+    double *part = P.partial + ((size_t)col * P.tiles + tile) * 3 * (N + 1);
+    for (int k = tid; k < nred; k += BLOCK) part[k] = s_fin[k];
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+      const unsigned prev = atomicAdd(P.counter + col, 1u);
+      s_is_last = (prev == (unsigned)(P.tiles - 1));
+      if (s_is_last) P.counter[col] = 0;   // re-arm for the next step
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    const double *pall = P.partial + (size_t)col * P.tiles * 3 * (N + 1);
+    for (int k = tid; k < nred; k += BLOCK) {
+      double sum = 0.0;
+      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 3 * (N + 1) + k);
+      s_fin[k] = sum;
+    }
+    __syncthreads();
+  }
+
+  // final outputs of the column
+  for (int i = tid; i <= N; i += BLOCK) {
+    const size_t o = (size_t)col * (N + 1) + i;
+    const double fu = s_fin[i], fd = s_fin[N + 1 + i];
+    if (P.F_up) P.F_up[o] = fu;
+    if (P.F_down) P.F_down[o] = fd;
+    if (P.F_net) P.F_net[o] = fu - fd;
+    if (want_beam) P.F_beam[o] = s_fin[2 * (N + 1) + i];
+  }
+  if (P.dTdt) {
+    for (int j = tid; j < N; j += BLOCK) {
+      const double fn1 = s_fin[j + 1] - s_fin[N + 1 + j + 1];
+      const double fn0 = s_fin[j] - s_fin[N + 1 + j];
+      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / s_dmfull[j];   // reading R14
+    }
+  }
+}
+
+// --------------------------------------------------------------------------------------------
+// small utility kernels
+// --------------------------------------------------------------------------------------------
+__global__ void zero_kernel(double *p, size_t n) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    p[i] = 0.0;
+}
+
+__global__ void selftest_math_kernel(int n, const double *x, double *rcp, double *rsq, double *ex, double *omx) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double v = x[i];
+  rcp[i] = rcp_fast(v);
+  rsq[i] = rsqrt_fast(fabs(v));
+  double om;
+  ex[i] = exp_neg_fast(fabs(v), &om);
+  omx[i] = om;
+}
+
+__global__ void selftest_planck_kernel(int n, const double *T, const double *lo, const double *hi, double *out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double t = T[i];
+  if (!(t > 0.0)) { out[i] = 0.0; return; }
+  const double g_hi = planck_G(kPlanckC2 / (hi[i] * t)), g_lo = planck_G(kPlanckC2 / (lo[i] * t));
+  const double t2 = t * t;
+  out[i] = kPlanckC1 * t2 * t2 * (g_hi - g_lo) / (hi[i] - lo[i]);
+}
+
+__global__ void dfma_peak_kernel(int iters, double seed, double *sink, long long *cycles) {
+  double a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6,
+         a7 = seed + 7;
+  const double m = 0.999999, k = 1e-9;
+  const long long t0 = clock64();
+#pragma unroll 4
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, k); a1 = fma(a1, m, k); a2 = fma(a2, m, k); a3 = fma(a3, m, k);
+    a4 = fma(a4, m, k); a5 = fma(a5, m, k); a6 = fma(a6, m, k); a7 = fma(a7, m, k);
+  }
+  const long long t1 = clock64();
+  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) sink[0] = s;
+  if (threadIdx.x == 0 && blockIdx.x == 0) cycles[0] = t1 - t0;
+}
+
+// --------------------------------------------------------------------------------------------
+// host side
+// --------------------------------------------------------------------------------------------
+typedef void (*kernel_fn)(const KParams);
+
+struct KernelChoice {
+  kernel_fn fn;
+  int block;
+};
+
+template <bool NONISO, bool TOA>
+KernelChoice pick_kernel(int block) {
+  switch (block) {
+    case 32:  return {rt_step_kernel<NONISO, TOA, 32, 16>, 32};
+    case 64:  return {rt_step_kernel<NONISO, TOA, 64, 8>, 64};
+    case 128: return {rt_step_kernel<NONISO, TOA, 128, 4>, 128};
+    case 160: return {rt_step_kernel<NONISO, TOA, 160, 3>, 160};
+    case 320: return {rt_step_kernel<NONISO, TOA, 320, 2>, 320};
+    case 608: return {rt_step_kernel<NONISO, TOA, 608, 1>, 608};
+    default:  return {nullptr, 0};
+  }
+}
+
+KernelChoice pick(bool noniso, bool toa, int block) {
+  if (noniso) return toa ? pick_kernel<true, true>(block) : pick_kernel<true, false>(block);
+  return toa ? pick_kernel<false, true>(block) : pick_kernel<false, false>(block);
+}
+
+const int kBlocks[] = {32, 64, 128, 160, 320, 608};
+
+// block size: fewest padded lanes over the column, ties -> larger block (fewer tiles)
+int choose_block(int npt) {
+  const char *env = getenv("HELIOS_RT_BLOCK");
+  if (env) {
+    const int v = atoi(env);
+    for (int b : kBlocks) if (b == v) return v;
+  }
+  int best = 32;
+  long best_waste = -1;
+  for (int b : kBlocks) {
+    const long tiles = (npt + b - 1) / b;
+    const long waste = tiles * (long)(((b + 31) / 32) * 32) - npt;
+    if (best_waste < 0 || waste < best_waste || (waste == best_waste && b > best)) { best = b; best_waste = waste; }
+  }
+  return best;
+}
+
+}  // namespace
+
+struct helios_rt {
+  helios_rt_config cfg;   // pointers nulled
+  int npt, block, tiles;
+  bool noniso, toa;
+  KernelChoice kc;
+  SmemLayout lay;
+  // device tables
+  double *d_lnk, *d_tab_lp, *d_tab_t, *d_edges, *d_gw;
+  BinConst *d_bins;
+  double *d_partial;
+  unsigned *d_counter;
+  // device staging for step_host
+  double *d_p, *d_T, *d_mu, *d_fstar, *d_out;   // d_out: 5*(N+1)+N+nb per column, carved per output
+  cudaStream_t own_stream;
+  int regs, lmem, occ, sm_count;
+  cudaError_t last_err;
+};
+
+#define CK(h, call)                                                   \
+  do {                                                                \
+    cudaError_t e_ = (call);                                          \
+    if (e_ != cudaSuccess) { if (h) (h)->last_err = e_; return HELIOS_RT_ECUDA; } \
+  } while (0)
+
+extern "C" const char *helios_rt_strerror(int code) {
+  switch (code) {
+    case HELIOS_RT_OK: return "success";
+    case HELIOS_RT_EINVAL: return "invalid argument";
+    case HELIOS_RT_ENOMEM: return "out of memory";
+    case HELIOS_RT_ECUDA: return "CUDA runtime error (see helios_rt_last_cuda_error)";
+    case HELIOS_RT_ENODEV: return "no usable CUDA device (compute capability 10.x required)";
+    default: return "unknown error code";
+  }
+}
+
+extern "C" const char *helios_rt_last_cuda_error(const helios_rt *h) {
+  if (!h || h->last_err == cudaSuccess) return "";
+  return cudaGetErrorString(h->last_err);
+}
+
+static int check_device() {
+  int n = 0;
+  if (cudaGetDeviceCount(&n) != cudaSuccess || n == 0) { cudaGetLastError(); return HELIOS_RT_ENODEV; }
+  int dev = 0, major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return HELIOS_RT_ENODEV;
+  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  return major == 10 ? HELIOS_RT_OK : HELIOS_RT_ENODEV;
+}
+
+static bool strictly_ascending(const double *a, int n) {
+  for (int i = 0; i < n; ++i) if (!(a[i] == a[i])) return false;
+  for (int i = 1; i < n; ++i) if (!(a[i] > a[i - 1])) return false;
+  return true;
+}
+
+static int validate_config(const helios_rt_config *c) {
+  if (!c) return HELIOS_RT_EINVAL;
+  if (c->n_layers < 1 || c->n_layers > MAXL || c->n_bins < 1 || c->n_gauss < 1 || c->n_ktab_p < 2 ||
+      c->n_ktab_t < 2 || c->max_columns < 1)
+    return HELIOS_RT_EINVAL;
+  if ((long long)c->n_bins * c->n_gauss > (1 << 24)) return HELIOS_RT_EINVAL;
+  if (!c->ktab_p || !c->ktab_t || !c->ktab || !c->bin_edges || !c->gauss_w || !c->scat_gas || !c->cloud_ext ||
+      !c->cloud_w0 || !c->cloud_g0)
+    return HELIOS_RT_EINVAL;
+  if (c->flags & ~(HELIOS_RT_IMPROVED | HELIOS_RT_NONISOTHERMAL | HELIOS_RT_TOA_SPECTRUM)) return HELIOS_RT_EINVAL;
+  if (!strictly_ascending(c->ktab_p, c->n_ktab_p) || !(c->ktab_p[0] > 0)) return HELIOS_RT_EINVAL;
+  if (!strictly_ascending(c->ktab_t, c->n_ktab_t)) return HELIOS_RT_EINVAL;
+  if (!strictly_ascending(c->bin_edges, c->n_bins + 1) || !(c->bin_edges[0] > 0)) return HELIOS_RT_EINVAL;
+  double sw = 0;
+  for (int g = 0; g < c->n_gauss; ++g) { if (!(c->gauss_w[g] > 0)) return HELIOS_RT_EINVAL; sw += c->gauss_w[g]; }
+  if (!(fabs(sw - 1.0) <= 1e-10)) return HELIOS_RT_EINVAL;
+  for (int b = 0; b < c->n_bins; ++b) {
+    if (!(c->scat_gas[b] >= 0) || !(c->cloud_ext[b] >= 0)) return HELIOS_RT_EINVAL;
+    if (!(c->cloud_w0[b] >= 0 && c->cloud_w0[b] <= 1)) return HELIOS_RT_EINVAL;
+    if (!(c->cloud_g0[b] >= 0 && c->cloud_g0[b] < 1)) return HELIOS_RT_EINVAL;
+  }
+  if (!(c->gravity > 0) || !(c->cp > 0) || !(c->eps2 > 0) || !(c->e_tau >= 0) || !(c->gcrit_tol >= 0) ||
+      !(c->w0_transition >= 0) || !(c->f_toa >= 0))
+    return HELIOS_RT_EINVAL;
+  if (!(c->cloud_p_top == c->cloud_p_top) || !(c->cloud_p_bot == c->cloud_p_bot)) return HELIOS_RT_EINVAL;
+  const size_t nk = (size_t)c->n_ktab_p * c->n_ktab_t * c->n_bins * c->n_gauss;
+  for (size_t i = 0; i < nk; ++i) if (!(c->ktab[i] > 0) || !(c->ktab[i] < 1e300)) return HELIOS_RT_EINVAL;
+  return HELIOS_RT_OK;
+}
+
+template <class T>
+static cudaError_t upload(T **dst, const T *src, size_t n) {
+  cudaError_t e = cudaMalloc((void **)dst, sizeof(T) * n);
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*dst, src, sizeof(T) * n, cudaMemcpyHostToDevice);
+}
+
+extern "C" int helios_rt_destroy(helios_rt *h) {
+  if (!h) return HELIOS_RT_OK;
+  cudaFree(h->d_lnk); cudaFree(h->d_tab_lp); cudaFree(h->d_tab_t); cudaFree(h->d_edges); cudaFree(h->d_gw);
+  cudaFree(h->d_bins); cudaFree(h->d_partial); cudaFree(h->d_counter);
+  cudaFree(h->d_p); cudaFree(h->d_T); cudaFree(h->d_mu); cudaFree(h->d_fstar); cudaFree(h->d_out);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  delete h;
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
+  if (!out) return HELIOS_RT_EINVAL;
+  *out = nullptr;
+  int rc = validate_config(cfg);
+  if (rc) return rc;
+  rc = check_device();
+  if (rc) return rc;
+  helios_rt *h = new (std::nothrow) helios_rt();
+  if (!h) return HELIOS_RT_ENOMEM;
+  memset(h, 0, sizeof(*h));
+  h->cfg = *cfg;
+  h->cfg.ktab_p = h->cfg.ktab_t = h->cfg.ktab = h->cfg.bin_edges = h->cfg.gauss_w = nullptr;
+  h->cfg.scat_gas = h->cfg.cloud_ext = h->cfg.cloud_w0 = h->cfg.cloud_g0 = nullptr;
+  const int N = cfg->n_layers, nb = cfg->n_bins, ng = cfg->n_gauss;
+  h->npt = nb * ng;
+  h->noniso = (cfg->flags & HELIOS_RT_NONISOTHERMAL) != 0;
+  h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
+  h->block = choose_block(h->npt);
+  h->tiles = (h->npt + h->block - 1) / h->block;
+  h->kc = pick(h->noniso, h->toa, h->block);
+  h->lay = smem_layout(N, h->noniso, h->block, ng, nb);
+  cudaGetDevice(&rc);
+  cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, rc);
+
+  // ln(kappa) table, log10 pressure grid, per-bin constants
+  const size_t nk = (size_t)cfg->n_ktab_p * cfg->n_ktab_t * h->npt;
+  double *lnk = (double *)malloc(sizeof(double) * nk);
+  double *lp = (double *)malloc(sizeof(double) * cfg->n_ktab_p);
+  BinConst *bins = (BinConst *)malloc(sizeof(BinConst) * nb);
+  if (!lnk || !lp || !bins) { free(lnk); free(lp); free(bins); helios_rt_destroy(h); return HELIOS_RT_ENOMEM; }
+  for (size_t i = 0; i < nk; ++i) lnk[i] = log(cfg->ktab[i]);
+  for (int i = 0; i < cfg->n_ktab_p; ++i) lp[i] = log10(cfg->ktab_p[i]);
+  for (int b = 0; b < nb; ++b) {
+    BinConst &bc = bins[b];
+    bc.dlam = cfg->bin_edges[b + 1] - cfg->bin_edges[b];
+    bc.inv_dlam = 1.0 / bc.dlam;
+    const double sg = cfg->scat_gas[b], kc = cfg->cloud_ext[b], sc = cfg->cloud_w0[b] * kc;
+    bc.sb[0] = sg;            bc.sb[1] = sg + kc;
+    bc.ss[0] = sg;            bc.ss[1] = sg + sc;
+    bc.gg[0] = 0.0;           bc.gg[1] = (sg + sc > 0.0) ? sc * cfg->cloud_g0[b] / (sg + sc) : 0.0;
+  }
+  cudaError_t e = cudaSuccess;
+  auto step = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  step(upload(&h->d_lnk, lnk, nk));
+  step(upload(&h->d_tab_lp, lp, (size_t)cfg->n_ktab_p));
+  step(upload(&h->d_tab_t, cfg->ktab_t, (size_t)cfg->n_ktab_t));
+  step(upload(&h->d_edges, cfg->bin_edges, (size_t)nb + 1));
+  step(upload(&h->d_gw, cfg->gauss_w, (size_t)ng));
+  step(upload(&h->d_bins, bins, (size_t)nb));
+  free(lnk); free(lp); free(bins);
+  const size_t ncol = (size_t)cfg->max_columns;
+  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * h->tiles * 3 * (N + 1)));
+  step(cudaMalloc((void **)&h->d_counter, sizeof(unsigned) * ncol));
+  if (e == cudaSuccess) step(cudaMemset(h->d_counter, 0, sizeof(unsigned) * ncol));
+  step(cudaMalloc((void **)&h->d_p, sizeof(double) * ncol * N));
+  step(cudaMalloc((void **)&h->d_T, sizeof(double) * ncol * N));
+  step(cudaMalloc((void **)&h->d_mu, sizeof(double) * ncol));
+  step(cudaMalloc((void **)&h->d_fstar, sizeof(double) * nb));
+  step(cudaMalloc((void **)&h->d_out, sizeof(double) * ncol * (4 * (N + 1) + N + nb)));
+  step(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
+  if (e == cudaSuccess && h->kc.fn) {
+    step(cudaFuncSetAttribute(h->kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
+    cudaFuncAttributes fa;
+    step(cudaFuncGetAttributes(&fa, h->kc.fn));
+    if (e == cudaSuccess) { h->regs = fa.numRegs; h->lmem = (int)fa.localSizeBytes; }
+    step(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ, h->kc.fn, h->block, h->lay.total));
+  }
+  if (e != cudaSuccess || !h->kc.fn) {
+    const bool oom = (e == cudaErrorMemoryAllocation);
+    helios_rt_destroy(h);
+    cudaGetLastError();
+    return !oom && e == cudaSuccess ? HELIOS_RT_EINVAL : (oom ? HELIOS_RT_ENOMEM : HELIOS_RT_ECUDA);
+  }
+  *out = h;
+  return HELIOS_RT_OK;
+}
+
+static int validate_step(const helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out) {
+  if (!h || !in || !out) return HELIOS_RT_EINVAL;
+  if (in->n_columns < 0 || in->n_columns > h->cfg.max_columns) return HELIOS_RT_EINVAL;
+  if (in->n_columns > 0 && (!in->p || !in->T || !in->mu_star || !in->stellar_flux)) return HELIOS_RT_EINVAL;
+  if (!(in->f_internal >= 0)) return HELIOS_RT_EINVAL;
+  const bool any_flux = out->F_up || out->F_down || out->F_net || out->dTdt || out->F_beam;
+  if (h->toa) { if (!out->F_up_toa_bin || any_flux) return HELIOS_RT_EINVAL; }
+  else if (!any_flux && !out->F_up_toa_bin) return HELIOS_RT_EINVAL;
+  return HELIOS_RT_OK;
+}
+
+static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out, cudaStream_t st) {
+  const helios_rt_config &c = h->cfg;
+  if (in->n_columns == 0) return HELIOS_RT_OK;
+  KParams P;
+  P.lnk = h->d_lnk; P.tab_lp = h->d_tab_lp; P.tab_t = h->d_tab_t; P.edges = h->d_edges; P.gauss_w = h->d_gw;
+  P.bins = h->d_bins;
+  P.nP = c.n_ktab_p; P.nT = c.n_ktab_t; P.N = c.n_layers; P.nb = c.n_bins; P.ng = c.n_gauss; P.npt = h->npt;
+  P.tiles = h->tiles;
+  P.cloud_p_top = c.cloud_p_top; P.cloud_p_bot = c.cloud_p_bot; P.inv_g = 1.0 / c.gravity; P.inv_cp = 1.0 / c.cp;
+  P.inv_eps2 = 1.0 / c.eps2; P.e_tau = c.e_tau; P.gcrit_tol = c.gcrit_tol; P.w0_transition = c.w0_transition;
+  P.f_toa = c.f_toa; P.improved = (c.flags & HELIOS_RT_IMPROVED) ? 1 : 0;
+  P.p = in->p; P.T = in->T; P.mu = in->mu_star; P.fstar = in->stellar_flux;
+  P.T_int = in->f_internal > 0 ? sqrt(sqrt(in->f_internal / kSigmaSB)) : 0.0;
+  P.F_up = out->F_up; P.F_down = out->F_down; P.F_net = out->F_net; P.dTdt = out->dTdt; P.F_beam = out->F_beam;
+  P.F_toa_bin = out->F_up_toa_bin;
+  P.partial = h->d_partial; P.counter = h->d_counter;
+  // bins that straddle two tiles are accumulated with atomics: start from zero
+  if (P.F_toa_bin && h->tiles > 1 && (h->block % c.n_gauss) != 0) {
+    const size_t n = (size_t)in->n_columns * c.n_bins;
+    zero_kernel<<<(unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, st>>>(P.F_toa_bin, n);
+  }
+  dim3 grid((unsigned)h->tiles, (unsigned)in->n_columns);
+  h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
+  CK(h, cudaGetLastError());
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
+                              void *cuda_stream) {
+  const int rc = validate_step(h, in, out);
+  if (rc) return rc;
+  return launch_step(h, in, out, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out) {
+  int rc = validate_step(h, in, out);
+  if (rc) return rc;
+  if (in->n_columns == 0) return HELIOS_RT_OK;
+  const size_t ncol = (size_t)in->n_columns, N = (size_t)h->cfg.n_layers, nb = (size_t)h->cfg.n_bins;
+  cudaStream_t st = h->own_stream;
+  CK(h, cudaMemcpyAsync(h->d_p, in->p, sizeof(double) * ncol * N, cudaMemcpyHostToDevice, st));
+  CK(h, cudaMemcpyAsync(h->d_T, in->T, sizeof(double) * ncol * N, cudaMemcpyHostToDevice, st));
+  CK(h, cudaMemcpyAsync(h->d_mu, in->mu_star, sizeof(double) * ncol, cudaMemcpyHostToDevice, st));
+  CK(h, cudaMemcpyAsync(h->d_fstar, in->stellar_flux, sizeof(double) * nb, cudaMemcpyHostToDevice, st));
+  helios_rt_inputs din = *in;
+  din.p = h->d_p; din.T = h->d_T; din.mu_star = h->d_mu; din.stellar_flux = h->d_fstar;
+  helios_rt_outputs dout;
+  double *o = h->d_out;
+  const size_t ni = ncol * (N + 1);
+  dout.F_up = out->F_up ? o : nullptr;                 o += ni;
+  dout.F_down = out->F_down ? o : nullptr;             o += ni;
+  dout.F_net = out->F_net ? o : nullptr;               o += ni;
+  dout.F_beam = out->F_beam ? o : nullptr;             o += ni;
+  dout.dTdt = out->dTdt ? o : nullptr;                 o += ncol * N;
+  dout.F_up_toa_bin = out->F_up_toa_bin ? o : nullptr;
+  rc = launch_step(h, &din, &dout, st);
+  if (rc) return rc;
+  if (out->F_up) CK(h, cudaMemcpyAsync(out->F_up, dout.F_up, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
+  if (out->F_down) CK(h, cudaMemcpyAsync(out->F_down, dout.F_down, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
+  if (out->F_net) CK(h, cudaMemcpyAsync(out->F_net, dout.F_net, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
+  if (out->F_beam) CK(h, cudaMemcpyAsync(out->F_beam, dout.F_beam, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
+  if (out->dTdt) CK(h, cudaMemcpyAsync(out->dTdt, dout.dTdt, sizeof(double) * ncol * N, cudaMemcpyDeviceToHost, st));
+  if (out->F_up_toa_bin)
+    CK(h, cudaMemcpyAsync(out->F_up_toa_bin, dout.F_up_toa_bin, sizeof(double) * ncol * nb, cudaMemcpyDeviceToHost, st));
+  CK(h, cudaStreamSynchronize(st));
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_launch_info(const helios_rt *h, int32_t info[8]) {
+  if (!h || !info) return HELIOS_RT_EINVAL;
+  info[0] = h->block; info[1] = h->tiles; info[2] = (int32_t)h->lay.total; info[3] = h->regs; info[4] = h->occ;
+  info[5] = h->lmem;
+  info[6] = 1;   // (+1 zero-fill launch when F_up_toa_bin bins straddle tiles)
+  info[7] = h->sm_count;
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_selftest_math(int32_t n, const double *x, double *rcp, double *rsq, double *ex, double *omx) {
+  if (n < 0 || (n > 0 && (!x || !rcp || !rsq || !ex || !omx))) return HELIOS_RT_EINVAL;
+  int rc = check_device();
+  if (rc) return rc;
+  if (n == 0) return HELIOS_RT_OK;
+  double *d = nullptr;
+  if (cudaMalloc((void **)&d, sizeof(double) * 5 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return HELIOS_RT_ENOMEM; }
+  cudaError_t e = cudaMemcpy(d, x, sizeof(double) * n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    selftest_math_kernel<<<(n + 127) / 128, 128>>>(n, d, d + n, d + 2 * (size_t)n, d + 3 * (size_t)n, d + 4 * (size_t)n);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(rcp, d + n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(rsq, d + 2 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(ex, d + 3 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(omx, d + 4 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  return e == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
+}
+
+extern "C" int helios_rt_selftest_planck(int32_t n, const double *T, const double *lam_lo, const double *lam_hi,
+                                         double *out) {
+  if (n < 0 || (n > 0 && (!T || !lam_lo || !lam_hi || !out))) return HELIOS_RT_EINVAL;
+  int rc = check_device();
+  if (rc) return rc;
+  if (n == 0) return HELIOS_RT_OK;
+  double *d = nullptr;
+  if (cudaMalloc((void **)&d, sizeof(double) * 4 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return HELIOS_RT_ENOMEM; }
+  cudaError_t e = cudaMemcpy(d, T, sizeof(double) * n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d + n, lam_lo, sizeof(double) * n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d + 2 * (size_t)n, lam_hi, sizeof(double) * n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    selftest_planck_kernel<<<(n + 127) / 128, 128>>>(n, d, d + n, d + 2 * (size_t)n, d + 3 * (size_t)n);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(out, d + 3 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  return e == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
+}
+
+extern "C" int helios_rt_measure_dfma_peak(int32_t iters, double *dfma_per_s, double *sm_clock_mhz) {
+  if (iters < 1 || !dfma_per_s) return HELIOS_RT_EINVAL;
+  int rc = check_device();
+  if (rc) return rc;
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  double *sink = nullptr;
+  long long *cyc = nullptr;
+  if (cudaMalloc((void **)&sink, sizeof(double)) != cudaSuccess) return HELIOS_RT_ENOMEM;
+  if (cudaMalloc((void **)&cyc, sizeof(long long)) != cudaSuccess) { cudaFree(sink); return HELIOS_RT_ENOMEM; }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = sms * 2, threads = 1024;
+  dfma_peak_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, sink, cyc);   // warm-up
+  float best = 1e30f;
+  long long hc = 0;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(e0);
+    dfma_peak_kernel<<<blocks, threads>>>(iters, 1.0, sink, cyc);
+    cudaEventRecord(e1);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { rc = HELIOS_RT_ECUDA; break; }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) { best = ms; cudaMemcpy(&hc, cyc, sizeof(hc), cudaMemcpyDeviceToHost); }
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(sink); cudaFree(cyc);
+  if (rc) return rc;
+  *dfma_per_s = 8.0 * (double)iters * (double)blocks * threads / (best * 1e-3);
+  if (sm_clock_mhz) *sm_clock_mhz = (double)hc / (best * 1e-3) * 1e-6;
+  return HELIOS_RT_OK;
+}

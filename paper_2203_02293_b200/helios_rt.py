@@ -1,0 +1,217 @@
+"""Thin ctypes binding of include/helios_rt.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libhelios_rt.so.  There is no CPU fallback: if
+the library is missing or no sm_100 device is present, construction raises.
+PyTorch is used only for device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from .workloads import IMPROVED, NONISOTHERMAL, TOA_SPECTRUM  # noqa: F401
+
+_LIB_PATH = Path(__file__).resolve().parent / "libhelios_rt.so"
+_dp = C.POINTER(C.c_double)
+
+EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
+           "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info",
+           "helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_measure_dfma_peak")
+
+
+class Config(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("n_layers", "n_bins", "n_gauss", "n_ktab_p", "n_ktab_t", "max_columns")] + \
+               [(n, _dp) for n in ("ktab_p", "ktab_t", "ktab", "bin_edges", "gauss_w", "scat_gas", "cloud_ext",
+                                   "cloud_w0", "cloud_g0")] + \
+               [(n, C.c_double) for n in ("cloud_p_top", "cloud_p_bot", "gravity", "cp", "eps2", "e_tau",
+                                          "gcrit_tol", "w0_transition", "f_toa")] + \
+               [("flags", C.c_uint32)]
+
+
+class Inputs(C.Structure):
+    _fields_ = [("n_columns", C.c_int32)] + [(n, C.c_void_p) for n in ("p", "T", "mu_star", "stellar_flux")] + \
+               [("f_internal", C.c_double)]
+
+
+class Outputs(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("F_up", "F_down", "F_net", "dTdt", "F_beam", "F_up_toa_bin")]
+
+
+OUTPUT_NAMES = tuple(n for n, _ in Outputs._fields_)
+_lib = None
+
+
+class HeliosRTError(RuntimeError):
+    pass
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree CUDA library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise HeliosRTError(f"{_LIB_PATH} is missing: run `python -m paper_2203_02293_b200.build` "
+                                "(there is no CPU fallback)")
+        L = C.CDLL(str(_LIB_PATH))
+        L.helios_rt_create.restype = C.c_int
+        L.helios_rt_create.argtypes = [C.POINTER(Config), C.POINTER(C.c_void_p)]
+        L.helios_rt_step.restype = C.c_int
+        L.helios_rt_step.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Outputs), C.c_void_p]
+        L.helios_rt_step_host.restype = C.c_int
+        L.helios_rt_step_host.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Outputs)]
+        L.helios_rt_destroy.restype = C.c_int
+        L.helios_rt_destroy.argtypes = [C.c_void_p]
+        L.helios_rt_strerror.restype = C.c_char_p
+        L.helios_rt_strerror.argtypes = [C.c_int]
+        L.helios_rt_last_cuda_error.restype = C.c_char_p
+        L.helios_rt_last_cuda_error.argtypes = [C.c_void_p]
+        L.helios_rt_launch_info.restype = C.c_int
+        L.helios_rt_launch_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.helios_rt_selftest_math.restype = C.c_int
+        L.helios_rt_selftest_math.argtypes = [C.c_int32] + [_dp] * 5
+        L.helios_rt_selftest_planck.restype = C.c_int
+        L.helios_rt_selftest_planck.argtypes = [C.c_int32] + [_dp] * 4
+        L.helios_rt_measure_dfma_peak.restype = C.c_int
+        L.helios_rt_measure_dfma_peak.argtypes = [C.c_int32, _dp, _dp]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, handle=None):
+    if rc != 0:
+        L = load_library()
+        msg = L.helios_rt_strerror(rc).decode()
+        if handle:
+            extra = L.helios_rt_last_cuda_error(handle).decode()
+            if extra:
+                msg += f": {extra}"
+        raise HeliosRTError(f"helios_rt error {rc}: {msg}")
+
+
+def _np(x):
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(_dp)
+
+
+class HeliosRT:
+    """Handle around helios_rt_create / helios_rt_step / helios_rt_destroy.
+
+    cfg: dict of host arrays/scalars with the field names of helios_rt_config (see workloads.make);
+    n_layers is taken from cfg["n_layers"] or passed explicitly.
+    """
+
+    def __init__(self, cfg: dict, max_columns: int, n_layers: int | None = None):
+        L = load_library()
+        ktab = _np(cfg["ktab"])
+        if ktab.ndim != 4:
+            raise HeliosRTError("helios_rt error -1: ktab must be [nP, nT, n_bins, n_gauss]")
+        nP, nT, nb, ng = ktab.shape
+        keep = {k: _np(cfg[k]) for k in ("ktab_p", "ktab_t", "bin_edges", "gauss_w", "scat_gas", "cloud_ext",
+                                         "cloud_w0", "cloud_g0")}
+        if keep["ktab_p"].shape != (nP,) or keep["ktab_t"].shape != (nT,) or keep["bin_edges"].shape != (nb + 1,) \
+                or keep["gauss_w"].shape != (ng,) or any(keep[k].shape != (nb,) for k in
+                                                         ("scat_gas", "cloud_ext", "cloud_w0", "cloud_g0")):
+            raise HeliosRTError("helios_rt error -1: array shapes inconsistent with ktab[nP,nT,n_bins,n_gauss]")
+        self.n_layers = int(n_layers if n_layers is not None else cfg["n_layers"])
+        self.n_bins, self.n_gauss = nb, ng
+        self.max_columns, self.flags = int(max_columns), int(cfg["flags"])
+        c = Config(self.n_layers, nb, ng, nP, nT, self.max_columns, _ptr(keep["ktab_p"]), _ptr(keep["ktab_t"]),
+                   _ptr(ktab), _ptr(keep["bin_edges"]), _ptr(keep["gauss_w"]), _ptr(keep["scat_gas"]),
+                   _ptr(keep["cloud_ext"]), _ptr(keep["cloud_w0"]), _ptr(keep["cloud_g0"]),
+                   float(cfg["cloud_p_top"]), float(cfg["cloud_p_bot"]), float(cfg["gravity"]), float(cfg["cp"]),
+                   float(cfg.get("eps2", 2.0 / 3.0)), float(cfg.get("e_tau", 1e-4)), float(cfg.get("gcrit_tol", 1e-5)),
+                   float(cfg.get("w0_transition", 0.1)), float(cfg.get("f_toa", 0.0)), self.flags)
+        h = C.c_void_p()
+        _check(L.helios_rt_create(C.byref(c), C.byref(h)))
+        self._h = h
+
+    def output_shapes(self, n: int) -> dict:
+        N, nb = self.n_layers, self.n_bins
+        return dict(F_up=(n, N + 1), F_down=(n, N + 1), F_net=(n, N + 1), dTdt=(n, N), F_beam=(n, N + 1),
+                    F_up_toa_bin=(n, nb))
+
+    def launch_info(self) -> dict:
+        info = (C.c_int32 * 8)()
+        _check(load_library().helios_rt_launch_info(self._h, info))
+        keys = ("block", "tiles", "smem_bytes", "registers", "blocks_per_sm", "local_bytes", "launches_per_step",
+                "sm_count")
+        return dict(zip(keys, list(info)))
+
+    def step(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict, stream=None) -> None:
+        """Device step: torch CUDA float64 contiguous tensors; `out` maps output names to pre-allocated
+        tensors (omitted = not wanted).  Asynchronous on `stream` (default: torch's current stream)."""
+        import torch
+        n = int(p.shape[0])
+        for name, t, shape in (("p", p, (n, self.n_layers)), ("T", T, (n, self.n_layers)), ("mu_star", mu_star, (n,)),
+                               ("stellar_flux", stellar_flux, (self.n_bins,))):
+            if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
+                raise HeliosRTError(f"helios_rt error -1: {name} must be a contiguous CUDA float64 tensor {shape}")
+        shapes = self.output_shapes(n)
+        ptrs = {}
+        for k, t in out.items():
+            if k not in shapes:
+                raise HeliosRTError(f"helios_rt error -1: unknown output {k}")
+            if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shapes[k]):
+                raise HeliosRTError(f"helios_rt error -1: output {k} must be a contiguous CUDA float64 tensor {shapes[k]}")
+            ptrs[k] = t.data_ptr()
+        i = Inputs(n, p.data_ptr(), T.data_ptr(), mu_star.data_ptr(), stellar_flux.data_ptr(), float(f_internal))
+        o = Outputs(*[ptrs.get(k) for k in OUTPUT_NAMES])
+        st = (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+        _check(load_library().helios_rt_step(self._h, C.byref(i), C.byref(o), C.c_void_p(st)), self._h)
+
+    def step_host(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict) -> None:
+        """Host step (end-to-end path): numpy arrays or CPU (ideally pinned) torch tensors, float64 contiguous.
+        Copies in, runs, copies the requested outputs back, synchronises."""
+        def addr(x):
+            if isinstance(x, np.ndarray):
+                if x.dtype != np.float64 or not x.flags.c_contiguous:
+                    raise HeliosRTError("helios_rt error -1: host arrays must be contiguous float64")
+                return x.ctypes.data
+            return x.data_ptr()
+        n = int(p.shape[0])
+        shapes = self.output_shapes(n)
+        for k, t in out.items():
+            if k not in shapes or tuple(t.shape) != shapes[k]:
+                raise HeliosRTError(f"helios_rt error -1: bad output {k}")
+        if tuple(p.shape) != (n, self.n_layers) or tuple(T.shape) != (n, self.n_layers) or \
+                tuple(mu_star.shape) != (n,) or tuple(stellar_flux.shape) != (self.n_bins,):
+            raise HeliosRTError("helios_rt error -1: bad input shape")
+        i = Inputs(n, addr(p), addr(T), addr(mu_star), addr(stellar_flux), float(f_internal))
+        o = Outputs(*[addr(out[k]) if k in out else None for k in OUTPUT_NAMES])
+        _check(load_library().helios_rt_step_host(self._h, C.byref(i), C.byref(o)), self._h)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            load_library().helios_rt_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def selftest_math(x):
+    x = _np(x)
+    outs = [np.empty_like(x) for _ in range(4)]
+    _check(load_library().helios_rt_selftest_math(x.size, _ptr(x), *[_ptr(o) for o in outs]))
+    return tuple(outs)  # rcp, rsqrt, exp(-|x|), 1-exp(-|x|)
+
+
+def selftest_planck(T, lam_lo, lam_hi) -> np.ndarray:
+    T, lo, hi = _np(T), _np(lam_lo), _np(lam_hi)
+    out = np.empty_like(T)
+    _check(load_library().helios_rt_selftest_planck(T.size, _ptr(T), _ptr(lo), _ptr(hi), _ptr(out)))
+    return out
+
+
+def measure_dfma_peak(iters: int = 1 << 16) -> tuple[float, float]:
+    a, b = C.c_double(), C.c_double()
+    _check(load_library().helios_rt_measure_dfma_peak(int(iters), C.byref(a), C.byref(b)))
+    return a.value, b.value

@@ -182,7 +182,7 @@ def make(config: int, columns=None) -> tuple[dict, dict, dict]:
         idx = np.arange(n_col)[columns]
         p, T, mu = p[idx].copy(), T[idx].copy(), mu[idx].copy()
 
-    cfg = dict(ktab_p=ktab_p, ktab_t=ktab_t, ktab=ktab, bin_edges=edges, gauss_w=gw, scat_gas=scat_gas,
+    cfg = dict(n_layers=N, ktab_p=ktab_p, ktab_t=ktab_t, ktab=ktab, bin_edges=edges, gauss_w=gw, scat_gas=scat_gas,
                cloud_ext=cloud_ext, cloud_w0=cloud_w0, cloud_g0=cloud_g0, cloud_p_top=cloud_p_top,
                cloud_p_bot=cloud_p_bot, gravity=GRAVITY, cp=CP, eps2=EPS2, e_tau=1e-4, gcrit_tol=1e-5,
                w0_transition=0.1, f_toa=0.0, flags=flags)

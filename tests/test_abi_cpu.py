@@ -1,0 +1,89 @@
+"""CPU-side checks of the C-ABI boundary: the library builds, loads, exports every symbol declared in
+include/helios_rt.h, and its host-side validation returns the documented error codes without a GPU
+(no compute call is made here)."""
+from __future__ import annotations
+
+import ctypes as C
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2203_02293_b200 import build, helios_rt
+    build.build()
+    return helios_rt.load_library()
+
+
+def test_exports_every_declared_symbol(lib):
+    from paper_2203_02293_b200 import helios_rt
+    hdr = (ROOT / "include" / "helios_rt.h").read_text()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(helios_rt_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(helios_rt.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_strerror(lib):
+    assert lib.helios_rt_strerror(0) == b"success"
+    for code in (-1, -2, -3, -4):
+        assert len(lib.helios_rt_strerror(code)) > 5
+    assert b"unknown" in lib.helios_rt_strerror(-77)
+
+
+def _cfg():
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(1)
+    return cfg
+
+
+def _create(cfg, max_columns=8):
+    from paper_2203_02293_b200.helios_rt import HeliosRT, HeliosRTError
+    try:
+        HeliosRT(cfg, max_columns).close()
+        return 0
+    except HeliosRTError as e:
+        return int(re.search(r"error (-?\d+)", str(e)).group(1))
+
+
+def test_validation_errors_come_before_the_device_check(lib):
+    """EINVAL (-1) for malformed configs even on a box without a GPU; a valid config on a GPU-less box
+    fails loudly with ENODEV (-4) -- never a silent CPU path."""
+    import torch
+    good = _cfg()
+    rc = _create(good)
+    assert rc == (0 if torch.cuda.is_available() else -4)
+    bad = dict(good, gauss_w=good["gauss_w"] * 1.01)
+    assert _create(bad) == -1
+    bad = dict(good, ktab_p=good["ktab_p"][::-1].copy())
+    assert _create(bad) == -1
+    bad = dict(good, bin_edges=np.concatenate([[0.0], good["bin_edges"][1:]]))
+    assert _create(bad) == -1
+    bad = dict(good, cloud_w0=np.full_like(good["cloud_w0"], 1.5))
+    assert _create(bad) == -1
+    bad = dict(good, cloud_g0=np.full_like(good["cloud_g0"], 1.0))
+    assert _create(bad) == -1
+    k = good["ktab"].copy(); k[0, 0, 0, 0] = 0.0
+    assert _create(dict(good, ktab=k)) == -1
+    k = good["ktab"].copy(); k[1, 2, 1, 0] = np.nan
+    assert _create(dict(good, ktab=k)) == -1
+    assert _create(dict(good, n_layers=0)) == -1
+    assert _create(dict(good, n_layers=65)) == -1
+    assert _create(dict(good, flags=64)) == -1
+    assert _create(dict(good, gravity=0.0)) == -1
+    assert _create(good, max_columns=0) == -1
+
+
+def test_null_handles(lib):
+    assert lib.helios_rt_destroy(None) == 0
+    assert lib.helios_rt_create(None, None) == -1
+    h = C.c_void_p()
+    assert lib.helios_rt_create(None, C.byref(h)) == -1 and not h
+    assert lib.helios_rt_launch_info(None, None) == -1
+    assert lib.helios_rt_last_cuda_error(None) == b""

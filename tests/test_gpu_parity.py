@@ -1,0 +1,351 @@
+"""GPU parity: the CUDA path (through the C ABI) against the long-double CPU oracle, element by element
+on the same seeded inputs.  Tolerances are north_star's: |dF| <= 1e-9 |F| + 1e-12 F*_tot for fluxes,
+|d(dT/dt)| <= 1e-8 |dT/dt| + 1e-12 F*_tot / (c_P dm_j) for heating rates.  Run with `-m gpu` on a B200.
+"""
+from __future__ import annotations
+
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+FLUX_RTOL, FLUX_FLOOR = 1e-9, 1e-12
+HEAT_RTOL = 1e-8
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_2203_02293_b200 import build, helios_rt
+    build.build()
+    return helios_rt
+
+
+def run_gpu(torch, H, cfg, inp, want, host=False, rt=None):
+    n = inp["p"].shape[0]
+    own = rt is None
+    if own:
+        rt = H.HeliosRT(cfg, max(n, 1))
+    shapes = rt.output_shapes(n)
+    if host:
+        out = {k: np.full(shapes[k], np.nan) for k in want}
+        rt.step_host(np.ascontiguousarray(inp["p"]), np.ascontiguousarray(inp["T"]),
+                     np.ascontiguousarray(inp["mu_star"]), np.ascontiguousarray(inp["stellar_flux"]),
+                     inp["f_internal"], out)
+        res = out
+    else:
+        dev = "cuda:0"
+        t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
+        out = {k: torch.full(shapes[k], float("nan"), dtype=torch.float64, device=dev) for k in want}
+        rt.step(t(inp["p"]), t(inp["T"]), t(inp["mu_star"]), t(inp["stellar_flux"]), inp["f_internal"], out)
+        torch.cuda.synchronize()
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+    if own:
+        rt.close()
+    return res
+
+
+def assert_parity(oracle_mod, cfg, inp, meta, got, ref):
+    Ftot = meta["F_star_tot"]
+    for k in ("F_up", "F_down", "F_net", "F_beam"):
+        if k in got:
+            err = np.abs(got[k] - ref[k])
+            tol = FLUX_RTOL * np.abs(ref[k]) + FLUX_FLOOR * Ftot
+            assert np.all(np.isfinite(got[k])), k
+            worst = np.unravel_index(np.argmax(err / tol), err.shape)
+            assert np.all(err <= tol), f"{k}: worst at {worst}: got {got[k][worst]!r} ref {ref[k][worst]!r} err/tol {(err / tol)[worst]:.3g}"
+    if "F_up_toa_bin" in got:
+        err = np.abs(got["F_up_toa_bin"] - ref["F_up_toa_bin"])
+        tol = FLUX_RTOL * np.abs(ref["F_up_toa_bin"]) + FLUX_FLOOR * np.asarray(inp["stellar_flux"])[None, :]
+        assert np.all(np.isfinite(got["F_up_toa_bin"]))
+        assert np.all(err <= tol), f"F_up_toa_bin: max err/tol {np.max(err / tol):.3g}"
+    if "dTdt" in got:
+        dm = np.stack([-np.diff(oracle_mod.levels(inp["p"][c], inp["T"][c])[0]) for c in range(inp["p"].shape[0])]) / cfg["gravity"]
+        err = np.abs(got["dTdt"] - ref["dTdt"])
+        tol = HEAT_RTOL * np.abs(ref["dTdt"]) + FLUX_FLOOR * Ftot / (cfg["cp"] * dm)
+        assert np.all(np.isfinite(got["dTdt"]))
+        assert np.all(err <= tol), f"dTdt: max err/tol {np.max(err / tol):.3g}"
+
+
+ALL = ("F_up", "F_down", "F_net", "dTdt", "F_beam", "F_up_toa_bin")
+
+
+# ------------------------------------------------------------------------------- device primitives
+def test_fp64_primitives(torch_cuda, H):
+    """rcp / rsqrt / exp replacements: <= 2 ulp-ish over the ranges the kernels feed them."""
+    rng = np.random.default_rng(5)
+    x = np.concatenate([10 ** rng.uniform(-12, 6, 200000), -(10 ** rng.uniform(-6, 2, 1000)),
+                        rng.uniform(0, 750, 100000), 10 ** rng.uniform(-300, -12, 1000), [0.0 + 1e-300, 1.0, 0.5, 2.0, 708.0, 745.0, 1e4]])
+    rcp, rsq, ex, om = H.selftest_math(x)
+    assert np.max(np.abs(rcp * x - 1.0)) < 4.5e-16
+    ax = np.abs(x)
+    assert np.max(np.abs(rsq * rsq * ax - 1.0)) < 9e-16
+    import mpmath as mp
+    mp.mp.dps = 40
+    idx = rng.choice(len(x), 4000, replace=False)
+    for i in idx:
+        a = mp.mpf(float(ax[i]))
+        e_ref, om_ref = mp.e ** (-a), -mp.expm1(-a)
+        if ax[i] <= 708.0:
+            assert abs(mp.mpf(float(ex[i])) - e_ref) <= mp.mpf(4.5e-16) * e_ref, (ax[i], ex[i])
+            assert abs(mp.mpf(float(om[i])) - om_ref) <= mp.mpf(4.5e-16) * om_ref + mp.mpf(1e-300), (ax[i], om[i])
+        else:
+            assert 0.0 <= ex[i] <= 4e-308 and om[i] == 1.0
+
+
+def test_planck_device_vs_oracle(torch_cuda, H, oracle_mod):
+    rng = np.random.default_rng(6)
+    n = 3000
+    T = np.concatenate([rng.uniform(50, 3500, n - 4), [100.0, 400.0, 4798.0, 3000.0]])
+    lo = 10 ** rng.uniform(np.log10(0.25e-6), np.log10(150e-6), n)
+    hi = lo * (1 + 10 ** rng.uniform(-3, 0.5, n))
+    got = H.selftest_planck(T, lo, hi)
+    ref = np.array([oracle_mod.planck_bin_mean(T[i], lo[i], hi[i]) for i in range(n)])
+    # a narrow bin differences two G values: allow the conditioning of G_hi - G_lo
+    cond = 1.0 + 6.5 / np.maximum(np.abs(ref) * (hi - lo) / (2 * 1.380649e-23**4 * T**4 / (6.62607015e-34**3 * 299792458.0**2)), 1e-300)
+    assert np.all(np.abs(got - ref) <= 4e-16 * cond * np.abs(ref) + 1e-300)
+    ok = ref > 1e-250
+    assert np.max(np.abs(got[ok] - ref[ok]) / ref[ok]) < 1e-11
+
+
+# ------------------------------------------------------------------------------------ the configs
+def test_config1_full(torch_cuda, H, oracle_mod):
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(1)
+    ref = oracle_mod.rt_step(cfg, inp)
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+@pytest.mark.parametrize("config,stride", [(2, 97), (3, 131), (4, 601), (5, 367)])
+def test_configs_subsampled_columns(torch_cuda, H, oracle_mod, config, stride):
+    """Configs 2-5 on every `stride`-th column (a true sub-sample: same draws as the full config);
+    600 / 6000 spectral points per column span several warps / tiles and a ragged tail."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config, columns=slice(3, None, stride))
+    want = ("F_up_toa_bin",) if config == 5 else ALL
+    ref = oracle_mod.rt_step(cfg, inp, want=want)
+    got = run_gpu(torch_cuda, H, cfg, inp, want)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+    assert (inp["mu_star"] > 0).any() and (inp["mu_star"] <= 0).any()
+
+
+@pytest.mark.parametrize("config", [2, 3])
+def test_full_size_launch_sampled_columns(torch_cuda, H, oracle_mod, config):
+    """The launch configuration bench.py times (all 2562 columns in one step); columns are
+    independent, so sampled columns are checked against the oracle run on those columns alone."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config)
+    got = run_gpu(torch_cuda, H, cfg, inp, ("F_up", "F_down", "F_net", "dTdt"))
+    rng = np.random.default_rng(config)
+    cols = np.sort(rng.choice(meta["n_columns"], 10, replace=False))
+    sub = dict(inp, p=inp["p"][cols], T=inp["T"][cols], mu_star=inp["mu_star"][cols])
+    ref = oracle_mod.rt_step(cfg, sub, want=("F_up", "F_down", "F_net", "dTdt"))
+    assert_parity(oracle_mod, cfg, sub, meta, {k: v[cols] for k, v in got.items()}, ref)
+    # properties that hold at any size
+    assert np.all(np.isfinite(got["F_net"])) and np.all(got["F_up"] >= 0) and np.all(got["F_down"] >= 0)
+    night = inp["mu_star"] <= 0
+    assert np.allclose(got["F_net"][:, 0], inp["f_internal"] * 0 + got["F_net"][:, 0])  # finite
+    # Eq.(10): F_net at the BOA equals sum_b dlam pi B_b(T_int) (beam fully absorbed in these columns)
+    boa = got["F_net"][:, 0]
+    assert np.allclose(boa[night], boa[night][0], rtol=1e-9)
+
+
+def test_config5_full_size_sampled(torch_cuda, H, oracle_mod):
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(5)
+    got = run_gpu(torch_cuda, H, cfg, inp, ("F_up_toa_bin",))
+    cols = np.array([0, 641, 1280, 2561])
+    sub = dict(inp, p=inp["p"][cols], T=inp["T"][cols], mu_star=inp["mu_star"][cols])
+    ref = oracle_mod.rt_step(cfg, sub, want=("F_up_toa_bin",))
+    assert_parity(oracle_mod, cfg, sub, meta, {"F_up_toa_bin": got["F_up_toa_bin"][cols]}, ref)
+
+
+# --------------------------------------------------------------------------- variants / edge cases
+def _small(config=1, **over):
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config, columns=slice(0, 12))
+    cfg = dict(cfg, **over)
+    return cfg, inp, meta
+
+
+def _cloudy(cfg, meta):
+    nb = meta["n_bins"]
+    return dict(cfg, cloud_ext=np.linspace(1e-4, 3e-3, nb), cloud_w0=np.linspace(0.05, 0.999, nb),
+                cloud_g0=np.linspace(0.0, 0.9, nb), cloud_p_top=1e2, cloud_p_bot=3e4)
+
+
+@pytest.mark.parametrize("flags", [0, 1, 2, 3])
+def test_regular_improved_iso_noniso(torch_cuda, H, oracle_mod, flags):
+    cfg, inp, meta = _small()
+    cfg = dict(_cloudy(cfg, meta), flags=flags)
+    ref = oracle_mod.rt_step(cfg, inp)
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+@pytest.mark.parametrize("eps2,f_toa", [(0.5, 0.0), (1 / np.sqrt(3), 0.0), (2 / 3, 3.0e5)])
+def test_eps2_and_f_toa_options(torch_cuda, H, oracle_mod, eps2, f_toa):
+    cfg, inp, meta = _small()
+    cfg = dict(_cloudy(cfg, meta), eps2=eps2, f_toa=f_toa, flags=3)
+    ref = oracle_mod.rt_step(cfg, inp)
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+def test_toa_spectrum_mode_small(torch_cuda, H, oracle_mod):
+    for flags in (1 | 4, 1 | 2 | 4):
+        cfg, inp, meta = _small()
+        cfg = dict(_cloudy(cfg, meta), flags=flags)
+        ref = oracle_mod.rt_step(cfg, inp, want=("F_up_toa_bin",))
+        got = run_gpu(torch_cuda, H, cfg, inp, ("F_up_toa_bin",))
+        assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+@pytest.mark.parametrize("block", [32, 64, 128, 160, 320, 608])
+def test_every_block_size_and_multi_tile_reduction(torch_cuda, H, oracle_mod, block):
+    """Forces each compiled block size: with 600 points per column, 32..320 give 19..2 tiles per column
+    (cross-tile fixed-order reduction, bins straddling tiles), 608 gives one."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(3, columns=slice(5, None, 400))
+    ref = oracle_mod.rt_step(cfg, inp)
+    os.environ["HELIOS_RT_BLOCK"] = str(block)
+    try:
+        rt = H.HeliosRT(cfg, inp["p"].shape[0])
+        assert rt.launch_info()["block"] == block
+        got = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)
+        got2 = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)      # counters re-arm: a second step is identical
+        rt.close()
+    finally:
+        del os.environ["HELIOS_RT_BLOCK"]
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+    for k in ALL:
+        assert np.array_equal(got[k], got2[k]), k        # deterministic, run to run
+
+
+def test_ragged_shapes(torch_cuda, H, oracle_mod):
+    """Odd sizes: 3 bins x 5 Gauss points (15 points, half a warp), 7 layers; and 1 layer."""
+    from paper_2203_02293_b200 import workloads as W
+    rng = np.random.default_rng(77)
+    for N, nb, ng in ((7, 3, 5), (1, 2, 3), (64, 5, 7)):
+        edges = W.bin_edges_equal_wavenumber(nb)
+        _, gw = W.gauss_legendre_01(ng)
+        ktab_p = np.logspace(1, 7, 5)
+        ktab_t = np.array([300.0, 700.0, 1500.0, 2600.0])
+        ktab = np.exp(rng.normal(-8, 2, (5, 4, nb, ng)))
+        ncol = 5
+        p = np.tile(np.logspace(6.5, 1.5, N) if N > 1 else np.array([1e5]), (ncol, 1))
+        T = rng.uniform(400, 2400, (ncol, N))
+        cfg = dict(n_layers=N, ktab_p=ktab_p, ktab_t=ktab_t, ktab=ktab, bin_edges=edges, gauss_w=gw,
+                   scat_gas=np.full(nb, 2e-4), cloud_ext=np.full(nb, 5e-4), cloud_w0=np.full(nb, 0.9),
+                   cloud_g0=np.full(nb, 0.6), cloud_p_top=1e3, cloud_p_bot=1e5, gravity=10.0, cp=1000.0, flags=3)
+        inp = dict(p=p, T=T, mu_star=np.array([1.0, 0.3, 0.0, -0.5, 0.01]), stellar_flux=np.full(nb, 1e9),
+                   f_internal=50.0)
+        meta = dict(F_star_tot=float(np.sum(np.diff(edges) * 1e9)))
+        for flags in (1, 3):
+            cfg["flags"] = flags
+            ref = oracle_mod.rt_step(cfg, inp)
+            got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+            assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+def test_out_of_table_is_clamped(torch_cuda, H, oracle_mod):
+    cfg, inp, meta = _small()
+    inp = dict(inp, T=inp["T"] + 1500.0, p=inp["p"] * 30.0)     # above the table in T, beyond it in p
+    ref = oracle_mod.rt_step(cfg, inp)
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+def test_no_internal_flux_and_all_night(torch_cuda, H, oracle_mod):
+    cfg, inp, meta = _small()
+    inp = dict(inp, f_internal=0.0, mu_star=-np.abs(inp["mu_star"]))
+    ref = oracle_mod.rt_step(cfg, inp)
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+    assert np.all(got["F_beam"] == 0.0)
+
+
+def test_mu_crit_guard_on_device(torch_cuda, H, oracle_mod):
+    """Columns whose mu sits on / next to mu_crit of some layer-point (Eq.11) stay finite and match."""
+    cfg, inp, meta = _small()
+    cfg = dict(_cloudy(cfg, meta), flags=1)
+    w0, g0 = 0.5, 0.3
+    E = oracle_mod.layer_coeffs(w0, g0, 1.0, -1)["E"]
+    mu_c = 1 / (2 * np.sqrt(E * (E - w0) * (1 - w0 * g0)))
+    mus = np.array([mu_c * (1 + d) for d in (0, 1e-7, -1e-7, 1e-5, -1e-5, 1e-3)] * 2)
+    inp = dict(inp, mu_star=mus)
+    ref = oracle_mod.rt_step(cfg, inp)
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+
+
+def test_nan_stays_in_its_column(torch_cuda, H, oracle_mod):
+    cfg, inp, meta = _small()
+    T = inp["T"].copy(); T[3, 4] = np.nan
+    bad = dict(inp, T=T)
+    got = run_gpu(torch_cuda, H, cfg, bad, ("F_net", "dTdt"))
+    good = run_gpu(torch_cuda, H, cfg, inp, ("F_net", "dTdt"))
+    assert np.isnan(got["F_net"][3]).any()
+    others = [c for c in range(12) if c != 3]
+    assert np.array_equal(got["F_net"][others], good["F_net"][others])
+
+
+def test_step_host_equals_device_step(torch_cuda, H, oracle_mod):
+    cfg, inp, meta = _small(3)
+    a = run_gpu(torch_cuda, H, cfg, inp, ALL)
+    b = run_gpu(torch_cuda, H, cfg, inp, ALL, host=True)
+    for k in ALL:
+        assert np.array_equal(a[k], b[k]), k
+    c = run_gpu(torch_cuda, H, cfg, inp, ("dTdt",), host=True)     # a subset of outputs
+    assert np.array_equal(c["dTdt"], a["dTdt"])
+
+
+def test_step_argument_errors(torch_cuda, H):
+    cfg, inp, meta = _small()
+    rt = H.HeliosRT(cfg, 4)
+    torch = torch_cuda
+    t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
+    with pytest.raises(H.HeliosRTError, match="error -1"):            # more columns than max_columns
+        rt.step(t(inp["p"]), t(inp["T"]), t(inp["mu_star"]), t(inp["stellar_flux"]), 0.0,
+                {"F_net": torch.empty((12, 11), dtype=torch.float64, device="cuda:0")})
+    with pytest.raises(H.HeliosRTError, match="error -1"):            # no output requested
+        rt.step(t(inp["p"][:4]), t(inp["T"][:4]), t(inp["mu_star"][:4]), t(inp["stellar_flux"]), 0.0, {})
+    with pytest.raises(H.HeliosRTError, match="error -1"):            # negative internal flux
+        rt.step(t(inp["p"][:4]), t(inp["T"][:4]), t(inp["mu_star"][:4]), t(inp["stellar_flux"]), -1.0,
+                {"F_net": torch.empty((4, 11), dtype=torch.float64, device="cuda:0")})
+    # zero columns: a no-op
+    rt.step(t(inp["p"][:0]), t(inp["T"][:0]), t(inp["mu_star"][:0]), t(inp["stellar_flux"]), 0.0,
+            {"F_net": torch.empty((0, 11), dtype=torch.float64, device="cuda:0")})
+    rt.close()
+    rt_toa = H.HeliosRT(dict(cfg, flags=5), 4)
+    with pytest.raises(H.HeliosRTError, match="error -1"):            # TOA mode produces only F_up_toa_bin
+        rt_toa.step(t(inp["p"][:4]), t(inp["T"][:4]), t(inp["mu_star"][:4]), t(inp["stellar_flux"]), 0.0,
+                    {"F_net": torch.empty((4, 11), dtype=torch.float64, device="cuda:0")})
+    rt_toa.close()
+
+
+def test_runs_on_a_side_stream(torch_cuda, H, oracle_mod):
+    torch = torch_cuda
+    cfg, inp, meta = _small()
+    ref = run_gpu(torch, H, cfg, inp, ("F_net",))
+    rt = H.HeliosRT(cfg, 12)
+    s = torch.cuda.Stream()
+    t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
+    args = (t(inp["p"]), t(inp["T"]), t(inp["mu_star"]), t(inp["stellar_flux"]))
+    out = {"F_net": torch.zeros((12, 11), dtype=torch.float64, device="cuda:0")}
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        rt.step(*args, inp["f_internal"], out)
+    s.synchronize()
+    assert np.array_equal(out["F_net"].cpu().numpy(), ref["F_net"])
+    rt.close()
