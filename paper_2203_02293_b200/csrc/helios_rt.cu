@@ -114,8 +114,11 @@ __device__ __forceinline__ double exp_neg_fast(double a, double *om) {
 //   x >= 1.5 : sum_n e^{-n x} (x^3/n + 3 x^2/n^2 + 6 x/n^3 + 6/n^4)
 //   x <  1.5 : pi^4/15 - sum_k B_k x^{k+3} / ((k+3) k!)   (Bernoulli numbers B_k)
 // --------------------------------------------------------------------------------------------
-__device__ double planck_G(double x) {
-  if (!(x > 0.0)) return kPi * kPi * kPi * kPi / 15.0;
+// *low receives int_0^x t^3/(e^t-1) dt when x < 1.5 (else -1): a bin whose two edges both lie there is
+// differenced on `low`, which avoids the cancellation against pi^4/15 for narrow Rayleigh-Jeans bins.
+__device__ double planck_G(double x, double *low_out) {
+  *low_out = -1.0;
+  if (!(x > 0.0)) { *low_out = 0.0; return kPi * kPi * kPi * kPi / 15.0; }
   if (x >= 1.5) {
     if (x > 745.0) return 0.0;
     const double u = exp(-x);
@@ -157,7 +160,13 @@ __device__ double planck_G(double x) {
   for (int i = 13; i >= 0; --i) s = fma(s, x2, ce[i]);
   // low = x^3 (c0 + c1 x + x^2 s)
   const double low = x2 * x * fma(x2, s, fma(c1, x, c0));
+  *low_out = low;
   return kPi * kPi * kPi * kPi / 15.0 - low;
+}
+
+// G(x_hi_edge) - G(x_lo_edge) for one bin from the per-edge (G, low) pairs (edge e = lam_lo: larger x)
+__device__ __forceinline__ double planck_dG(double G_lo_edge, double low_lo_edge, double G_hi_edge, double low_hi_edge) {
+  return (low_lo_edge >= 0.0 && low_hi_edge >= 0.0) ? (low_lo_edge - low_hi_edge) : (G_hi_edge - G_lo_edge);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -299,7 +308,7 @@ struct SmemLayout {
   int nlev;        // levels at which kappa / Planck are evaluated: N (iso) or 2N+1 (non-iso)
   int nbt;         // max bins per tile
   size_t off_lnp, off_pint, off_tint, off_plev, off_tlev, off_wp, off_wt, off_cell, off_cloud, off_dm,
-      off_dmfull, off_G, off_B, off_red, off_fin, off_vals, total;
+      off_dmfull, off_G, off_Glow, off_B, off_red, off_fin, off_vals, total;
 };
 
 __host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block, int ng, int nb) {
@@ -322,6 +331,7 @@ __host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block,
   L.off_dm = take(sizeof(double) * 2 * N);                    // per system layer
   L.off_dmfull = take(sizeof(double) * N);
   L.off_G = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
+  L.off_Glow = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
   L.off_B = take(sizeof(double) * (L.nlev + 1) * L.nbt);
   L.off_red = take(sizeof(double) * nwarp * 3 * (N + 1));
   L.off_fin = take(sizeof(double) * 3 * (N + 1));
@@ -347,11 +357,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   double *s_dm = (double *)(smem + L.off_dm);
   double *s_dmfull = (double *)(smem + L.off_dmfull);
   double *s_G = (double *)(smem + L.off_G);
+  double *s_Glow = (double *)(smem + L.off_Glow);
   double *s_B = (double *)(smem + L.off_B);
   double *s_red = (double *)(smem + L.off_red);
   double *s_fin = (double *)(smem + L.off_fin);
   double *s_vals = (double *)(smem + L.off_vals);
-  __shared__ int s_is_last;
+  __shared__ int s_is_last, s_nan;
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x, col = blockIdx.y;
@@ -367,8 +378,16 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   if (pt_last > P.npt - 1) pt_last = P.npt - 1;
   const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
 
+  // NaN in p, T or mu of this column poisons the column's outputs (and only them): the clamps and
+  // selects below would otherwise swallow it.
+  if (tid == 0) s_nan = (mu != mu) ? 1 : 0;
+  __syncthreads();
   // ---------------- S1: level geometry (reading R9; L171) ----------------
-  for (int j = tid; j < N; j += BLOCK) s_lnp[j] = log(pc[j]);
+  for (int j = tid; j < N; j += BLOCK) {
+    const double pj = pc[j], tj = Tc[j];
+    if (pj != pj || tj != tj) s_nan = 1;
+    s_lnp[j] = log(pj);
+  }
   __syncthreads();
   for (int i = tid; i <= N; i += BLOCK) {
     double lp, ti;
@@ -424,7 +443,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   for (int i = tid; i < (nlev + 1) * nedge; i += BLOCK) {
     const int l = i / nedge, e = i - l * nedge;
     const double Tl = s_tlev[l];
-    s_G[l * (L.nbt + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b_first + e] * Tl)) : 0.0;
+    double low = 0.0;
+    s_G[l * (L.nbt + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b_first + e] * Tl), &low) : 0.0;
+    s_Glow[l * (L.nbt + 1) + e] = low;
   }
   __syncthreads();
   for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
@@ -432,7 +453,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
     const double Tl = s_tlev[l];
     const double T2 = Tl * Tl;
     const double *g = s_G + l * (L.nbt + 1) + bl;
-    double B = kPlanckC1 * T2 * T2 * (g[1] - g[0]) * P.bins[b_first + bl].inv_dlam;
+    const double *gl = s_Glow + l * (L.nbt + 1) + bl;
+    double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * P.bins[b_first + bl].inv_dlam;
     if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
     s_B[l * L.nbt + bl] = (Tl > 0.0) ? B : 0.0;
   }
@@ -564,7 +586,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
       const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
       if (g_lo < 0) g_lo = 0;
       if (g_hi > BLOCK) g_hi = BLOCK;
-      double sum = 0.0;
+      double sum = s_nan ? nan("") : 0.0;
       for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
       double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
       if (whole) *dst = sum; else atomicAdd(dst, sum);
@@ -607,7 +629,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
       const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
       if (g_lo < 0) g_lo = 0;
       if (g_hi > BLOCK) g_hi = BLOCK;
-      double sum = 0.0;
+      double sum = s_nan ? nan("") : 0.0;
       for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
       double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
       if (whole) *dst = sum; else atomicAdd(dst, sum);
@@ -639,6 +661,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   }
 
   // final outputs of the column
+  if (s_nan) {
+    __syncthreads();
+    for (int k = tid; k < 3 * (N + 1); k += BLOCK) s_fin[k] = nan("");
+    __syncthreads();
+  }
   for (int i = tid; i <= N; i += BLOCK) {
     const size_t o = (size_t)col * (N + 1) + i;
     const double fu = s_fin[i], fd = s_fin[N + 1 + i];
@@ -680,9 +707,10 @@ __global__ void selftest_planck_kernel(int n, const double *T, const double *lo,
   if (i >= n) return;
   const double t = T[i];
   if (!(t > 0.0)) { out[i] = 0.0; return; }
-  const double g_hi = planck_G(kPlanckC2 / (hi[i] * t)), g_lo = planck_G(kPlanckC2 / (lo[i] * t));
+  double l_hi, l_lo;
+  const double g_hi = planck_G(kPlanckC2 / (hi[i] * t), &l_hi), g_lo = planck_G(kPlanckC2 / (lo[i] * t), &l_lo);
   const double t2 = t * t;
-  out[i] = kPlanckC1 * t2 * t2 * (g_hi - g_lo) / (hi[i] - lo[i]);
+  out[i] = kPlanckC1 * t2 * t2 * planck_dG(g_lo, l_lo, g_hi, l_hi) / (hi[i] - lo[i]);
 }
 
 __global__ void dfma_peak_kernel(int iters, double seed, double *sink, long long *cycles) {
@@ -932,6 +960,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
 static int validate_step(const helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out) {
   if (!h || !in || !out) return HELIOS_RT_EINVAL;
   if (in->n_columns < 0 || in->n_columns > h->cfg.max_columns) return HELIOS_RT_EINVAL;
+  if (in->n_columns == 0) return in->f_internal >= 0 ? HELIOS_RT_OK : HELIOS_RT_EINVAL;   // nothing to do
   if (in->n_columns > 0 && (!in->p || !in->T || !in->mu_star || !in->stellar_flux)) return HELIOS_RT_EINVAL;
   if (!(in->f_internal >= 0)) return HELIOS_RT_EINVAL;
   const bool any_flux = out->F_up || out->F_down || out->F_net || out->dTdt || out->F_beam;
