@@ -48,65 +48,79 @@ constexpr double kPlanckC2 = kH * kC / kKB;                                     
 // --------------------------------------------------------------------------------------------
 // fp64 primitives
 // --------------------------------------------------------------------------------------------
+// MUFU.RCP64H seed (~20 good bits), then y (1 + e + e^2) = (1/x)(1 - e^3): <= 1.5 ulp
 __device__ __forceinline__ double rcp_fast(double x) {
   double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RCP64H: ~20 good bits
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double e = fma(-x, y, 1.0);
-  e = fma(e, e, e);        // e + e^2
-  y = fma(y, e, y);        // cubic step: error ~ e^3
-  e = fma(-x, y, 1.0);     // one Newton step to land within 1 ulp
+  e = fma(e, e, e);
   return fma(y, e, y);
 }
 
+// MUFU.RSQ64H seed, then y (1 + e/2 + 3 e^2/8), e = 1 - x y^2: error O(e^3)
 __device__ __forceinline__ double rsqrt_fast(double x) {
   double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RSQ64H
-  double t = x * y;
-  double e = fma(-t, y, 1.0);            // 1 - x y^2
-  double p = fma(0.375, e, 0.5) * e;     // e/2 + 3 e^2/8
-  y = fma(y, p, y);
-  t = x * y;
-  e = fma(-t, y, 1.0);
-  return fma(0.5 * y, e, y);
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double t = x * y;
+  const double e = fma(-t, y, 1.0);
+  const double p = fma(0.375, e, 0.5) * e;
+  return fma(y, p, y);
 }
 
-// expm1 on the reduced argument |r| <= ln2/2: r + r^2 q(r), q near-minimax of degree 9.
-__device__ __forceinline__ double expm1_reduced(double r) {
-  double q = 2.51003854955103203e-08;
-  q = fma(q, r, 2.76200884454097462e-07);
-  q = fma(q, r, 2.75572684599970641e-06);
-  q = fma(q, r, 2.48015212959543761e-05);
-  q = fma(q, r, 1.98412698630536177e-04);
-  q = fma(q, r, 1.38888889172137167e-03);
-  q = fma(q, r, 8.33333333333006153e-03);
-  q = fma(q, r, 4.16666666666241289e-02);
-  q = fma(q, r, 1.66666666666666685e-01);
-  q = fma(q, r, 5.00000000000000111e-01);
-  return fma(r * r, q, r);
+// positive, non-NaN doubles order like their bit patterns: comparisons on the integer pipes keep the
+// fp64 pipe (the binding resource) for arithmetic
+__device__ __forceinline__ bool gt_pos(double a, double b) { return __double_as_longlong(a) > __double_as_longlong(b); }
+__device__ __forceinline__ bool abs_lt(double a, double b_pos) {
+  return (__double_as_longlong(a) & 0x7fffffffffffffffLL) < __double_as_longlong(b_pos);
 }
 
-// exp(x) for -708 <= x <= 700 (callers clamp).  If OM, *om = 1 - exp(x) without cancellation for
-// small |x| (x <= 0).
-template <bool OM>
-__device__ __forceinline__ double exp_core(double x, double *om) {
-  const double kMagic = 6755399441055744.0;  // 1.5 * 2^52: round-to-nearest-integer trick
-  double kd = fma(x, 1.4426950408889634074, kMagic);
-  int k = __double2loint(kd);
-  kd -= kMagic;
-  double r = fma(kd, -6.93147180369123816490e-01, x);
-  r = fma(kd, -1.90821492927058770002e-10, r);
-  double p = expm1_reduced(r);
-  double y = 1.0 + p;
-  double res = __hiloint2double(__double2hiint(y) + (k << 20), __double2loint(y));
-  if (OM) *om = (k == 0) ? -p : 1.0 - res;
-  return res;
-}
-__device__ __forceinline__ double exp_fast(double x) {
-  return exp_core<false>(fmin(fmax(x, -708.0), 700.0), nullptr);
-}
-// exp(-a) and 1 - exp(-a) for a >= 0
-__device__ __forceinline__ double exp_neg_fast(double a, double *om) {
-  return exp_core<true>(-fmin(a, 708.0), om);
+// exp by table: e^x = 2^m T[j] (1 + p(r)), k = 32 m + j = round(32 x / ln 2), r = x - k ln2/32, |r| <= ln2/64,
+// T[j] = 2^(j/32) (32 doubles in shared memory), p = expm1(r) by its degree-6 Taylor polynomial (remainder
+// r^7/5040 < 4e-18).  10 fp64 instructions.  The single-constant reduction k * fl(ln2/32) is exact to
+// |k| 2.4e-18, i.e. <= 8e-14 relative at |x| = 700 and <= 3e-15 for |x| <= 30 (far inside the 1e-9 budget).
+//   MODE 0: e^x for |x| <= 708;  MODE 1: e^-a, 0 <= a <= 708;  MODE 2: e^-2a, 0 <= a <= 354, and, if OM,
+//   *om = 1 - e^-2a without cancellation.
+__constant__ double kExp2Tab[32] = {
+    1.0, 1.0218971486541166, 1.0442737824274138, 1.0671404006768237,
+    1.0905077326652577, 1.1143867425958924, 1.1387886347566916, 1.1637248587775775,
+    1.189207115002721, 1.215247359980469, 1.241857812073484, 1.2690509571917332,
+    1.2968395546510096, 1.3252366431597413, 1.3542555469368927, 1.383909881963832,
+    1.4142135623730951, 1.4451808069770467, 1.4768261459394993, 1.5091644275934228,
+    1.5422108254079407, 1.5759808451078865, 1.6104903319492543, 1.645755478153965,
+    1.681792830507429, 1.718619298122478, 1.7562521603732995, 1.7947090750031072,
+    1.8340080864093424, 1.8741676341103, 1.9152065613971474, 1.9571441241754002};
+
+template <int MODE, bool OM>
+__device__ __forceinline__ double exp_tab(double x, const double *__restrict__ T32, double *om) {
+  const double kMagic = 6755399441055744.0;      // 1.5 * 2^52: round-to-nearest-integer trick
+  const double kS = 46.16624130844683;           // 32 / ln 2
+  const double kL = 0.02166084939249829;         // ln 2 / 32
+  double kd, p;
+  if (MODE == 0) kd = fma(x, kS, kMagic);
+  else if (MODE == 1) kd = fma(x, -kS, kMagic);
+  else kd = fma(x, -2.0 * kS, kMagic);
+  const int ki = __double2loint(kd);
+  const double kf = kd - kMagic;
+  if (MODE == 2) {
+    // r = -2 x - kf L; with h = -r/2 = x + kf L/2:  p = expm1(-2 h) = h (-2 + h q(h))
+    const double h = fma(kf, 0.5 * kL, x);
+    double q = fma(h, 4.0 / 45.0, -4.0 / 15.0);
+    q = fma(q, h, 2.0 / 3.0);
+    q = fma(q, h, -4.0 / 3.0);
+    q = fma(q, h, 2.0);
+    p = h * fma(h, q, -2.0);
+  } else {
+    const double r = (MODE == 0) ? fma(kf, -kL, x) : fma(kf, -kL, -x);
+    double q = fma(r, 1.0 / 720.0, 1.0 / 120.0);
+    q = fma(q, r, 1.0 / 24.0);
+    q = fma(q, r, 1.0 / 6.0);
+    q = fma(q, r, 0.5);
+    p = fma(r * r, q, r);
+  }
+  const double Tj = T32[ki & 31];
+  const double Ts = __hiloint2double(__double2hiint(Tj) + (ki >> 5) * 1048576, __double2loint(Tj));   // 2^m T[j]
+  if (OM) *om = fma(-Ts, p, 1.0 - Ts);
+  return fma(Ts, p, Ts);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -212,14 +226,15 @@ struct ThreadConst {      // per spectral point
 // back-substitution pair (c, d): F_up[b] = c F_up[a] + d.
 // --------------------------------------------------------------------------------------------
 template <bool DAY, bool LINSRC>
-__device__ __forceinline__ void layer_forward(const KParams &P, double w0, double g0, double dtau,
-                                              double Ba, double Bb, double mu, double Fa, double Fb,
+__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+                                              double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
                                               double &R, double &U, double &c, double &d) {
-  // E, Eq.(19) L374 (readings R5, R6)
+  // E, Eq.(19) L374 (readings R5, R6): E = max(1, fit) if w0 > 0.1 else 1
   double E = 1.0;
   if (P.improved) {
-    double fit = 1.225 + g0 * (-0.1582 - 0.07465 * g0) + w0 * (-0.1777 + 0.2351 * g0 - 0.05582 * w0);
-    E = (w0 > P.w0_transition) ? fmax(fit, 1.0) : 1.0;
+    const double fg = fma(g0, fma(-0.07465, g0, -0.1582), 1.225);
+    const double fit = fma(w0, fma(g0, 0.2351, fma(-0.05582, w0, -0.1777)), fg);
+    E = (gt_pos(w0, P.w0_transition) && gt_pos(fit, 1.0)) ? fit : 1.0;
   }
   const double wg = w0 * g0;
   const double num = E - w0;             // E - omega0
@@ -227,72 +242,59 @@ __device__ __forceinline__ void layer_forward(const KParams &P, double w0, doubl
   const double X = num * den;
   const double rs = rsqrt_fast(X);       // 1/sqrt(E (E-w0)(1-w0 g0))
   const double s = num * rs;             // sqrt((E-w0)/(E(1-w0 g0))) = zeta+ - zeta-   (B2)
-  const double alpha = 2.0 * (X * rs);   // 2 sqrt(E (E-w0)(1-w0 g0))
+  const double ha = X * rs;              // alpha / 2 = sqrt(E (E-w0)(1-w0 g0))
   const double rs2 = rs * rs;
-  const double invP = 0.5 * (num * rs2); // 1 / (2 E (1 - w0 g0))
-  const double inv_num = den * rs2;      // 1 / (E - w0)
-  const double zp = 0.5 + 0.5 * s, zm = 0.5 - 0.5 * s;
+  const double zp = fma(0.5, s, 0.5), zm = fma(-0.5, s, 0.5);
   double omT;
-  const double Tr = exp_neg_fast(alpha * dtau, &omT);   // transmission function (B2), 1 - T
+  const double Tr = exp_tab<2, true>(fmin(ha * dtau, 354.0), T32, &omT);   // transmission function (B2), 1 - T
   const double zmT = zm * Tr;
   const double a = zp - zmT, b = zp + zmT;
   const double inv_ab = rcp_fast(a * b);
-  const double t = s * Tr * inv_ab;                          // psi/chi
-  const double r = zp * zm * omT * (1.0 + Tr) * inv_ab;      // -xi/chi
-  const double emis = s * omT * a * inv_ab;                  // 1 - t - r
-  const double Pi = kPi * (1.0 - w0) * inv_num;              // (B5)
+  const double u = omT * inv_ab;
+  const double t = (s * Tr) * inv_ab;                        // psi/chi
+  const double r = (zp * zm) * (1.0 + Tr) * u;               // -xi/chi
+  const double emis = (s * a) * u;                           // 1 - t - r
+  const double Pi = fma(-kPi, w0, kPi) * (den * rs2);        // (B5): pi (1-w0)/(E-w0)
   double Sup, Sdn;
   if (LINSRC) {
     // Eqs.(4)-(9): B* (1-r) - t B*' +- B' (1 - t + r)/(2E(1-w0 g0)), B' = (Ba - Bb)/dtau; e_tau rule L209
-    const bool thin = dtau < P.e_tau;
+    const bool thin = !gt_pos(dtau, P.e_tau) && dtau != P.e_tau;   // dtau < e_tau
     const double Bm = 0.5 * (Ba + Bb);
     const double dB = thin ? 0.0 : (Ba - Bb);
     const double Bal = thin ? Bm : Ba, Bbl = thin ? Bm : Bb;
+    const double invP = 0.5 * (num * rs2);                   // 1 / (2 E (1 - w0 g0))
     const double grad = (1.0 - t + r) * invP * rcp_fast(dtau);
     const double k = dB * (t - grad);
     Sup = Pi * fma(Bbl, emis, -k);
     Sdn = Pi * fma(Bal, emis, k);
   } else {
-    Sup = Sdn = Pi * Bb * emis;                              // Eqs.(2),(3)
+    Sup = Sdn = (Pi * Bb) * emis;                            // Eqs.(2),(3)
   }
   if (DAY) {
     // (B8) with mu_star = -mu; guard of Eq.(11)/L252 (reading R4)
-    const double ma = mu * alpha;
+    const double ma = mu * (2.0 * ha);
     double D = (ma - 1.0) * (ma + 1.0);                      // 4 E mu^2 (E-w0)(1-w0 g0) - 1
-    D = (fabs(D) < P.gcrit_tol) ? -2.0 * mu : D;
+    D = abs_lt(D, P.gcrit_tol) ? -2.0 * mu : D;
     const double invD = rcp_fast(D);
-    const double lead = w0 * (2.0 * den + g0 * P.inv_eps2) * invD;
-    const double last = wg * P.inv_eps2 * invP;
-    const double Gp = 0.5 * fma(lead, invP - mu, last);
-    const double Gm = 0.5 * fma(lead, -invP - mu, -last);
+    const double hP = 0.5 * (num * rs2);                     // 1 / (2 E (1 - w0 g0))
+    const double ge = g0 * P.inv_eps2;
+    const double lead = (0.5 * w0) * fma(2.0, den, ge) * invD;
+    const double last = (0.5 * w0) * ge * hP;
+    const double Gp = fma(lead, hP - mu, last);
+    const double Gm = -fma(lead, hP + mu, last);
     // (B7): S_up += t G+ Fa + r G- Fb - G+ Fb ; S_dn += t G- Fb + r G+ Fa - G- Fa
-    Sup += Gp * fma(t, Fa, -Fb) + r * Gm * Fb;
-    Sdn += Gm * fma(t, Fb, -Fa) + r * Gp * Fa;
+    const double rGm = r * Gm, rGp = r * Gp;
+    Sup = fma(rGm, Fb, fma(Gp, fma(t, Fa, -Fb), Sup));
+    Sdn = fma(rGp, Fa, fma(Gm, fma(t, Fb, -Fa), Sdn));
   }
   // forward elimination (Eqs. 13-14 specialised): F_up[b] (1 - r R) = t F_up[a] + r U + S_up
-  const double q = rcp_fast(1.0 - r * R);
+  const double q = rcp_fast(fma(-r, R, 1.0));
   c = t * q;
   d = fma(r, U, Sup) * q;
   const double Rn = fma(t * c, R, r);
   const double Un = fma(c, fma(R, Sup, U), Sdn);
   R = Rn;
   U = Un;
-}
-
-// optical properties at one level (S3 + Eqs. 17-18)
-__device__ __forceinline__ void level_optics(const double *__restrict__ lnk_pt, int off, int strideT,
-                                             int strideP, double wp, double wt, int cloudy,
-                                             const ThreadConst &tc, double &kx, double &w0, double &g0) {
-  const double l00 = __ldg(lnk_pt + off);
-  const double l01 = __ldg(lnk_pt + off + strideT);
-  const double l10 = __ldg(lnk_pt + off + strideP);
-  const double l11 = __ldg(lnk_pt + off + strideP + strideT);
-  const double lo = fma(wt, l01 - l00, l00);
-  const double hi = fma(wt, l11 - l10, l10);
-  const double kabs = exp_fast(fma(wp, hi - lo, lo));
-  kx = kabs + (cloudy ? tc.sb1 : tc.sb0);
-  w0 = (cloudy ? tc.ss1 : tc.ss0) * rcp_fast(kx);
-  g0 = cloudy ? tc.gg1 : 0.0;
 }
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -307,8 +309,9 @@ __device__ __forceinline__ double warp_sum(double v) {
 struct SmemLayout {
   int nlev;        // levels at which kappa / Planck are evaluated: N (iso) or 2N+1 (non-iso)
   int nbt;         // max bins per tile
-  size_t off_lnp, off_pint, off_tint, off_plev, off_tlev, off_wp, off_wt, off_cell, off_cloud, off_dm,
-      off_dmfull, off_G, off_Glow, off_B, off_red, off_fin, off_vals, total;
+  int LP;          // N + 1 rounded up to a multiple of 8 (sweep 2 reduces 8 levels at a time)
+  size_t off_lnp, off_pint, off_tint, off_plev, off_tlev, off_cw, off_cell, off_cloud, off_dm,
+      off_dmfull, off_G, off_Glow, off_B, off_red, off_fin, off_vals, off_T32, total;
 };
 
 __host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block, int ng, int nb) {
@@ -316,16 +319,16 @@ __host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block,
   L.nlev = noniso ? 2 * N + 1 : N;
   int nbt = (block + ng - 1) / ng + 1;
   L.nbt = nbt < nb ? nbt : nb;
+  L.LP = (N + 1 + 7) & ~7;
   const int nwarp = (block + 31) / 32;
   size_t o = 0;
-  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
+  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 31) & ~size_t(31); return r; };
   L.off_lnp = take(sizeof(double) * N);
   L.off_pint = take(sizeof(double) * (N + 1));
   L.off_tint = take(sizeof(double) * (N + 1));
   L.off_plev = take(sizeof(double) * L.nlev);
   L.off_tlev = take(sizeof(double) * (L.nlev + 1));           // + internal temperature row
-  L.off_wp = take(sizeof(double) * L.nlev);
-  L.off_wt = take(sizeof(double) * L.nlev);
+  L.off_cw = take(sizeof(double) * 4 * L.nlev);               // bilinear corner weights per level
   L.off_cell = take(sizeof(int) * L.nlev);
   L.off_cloud = take(sizeof(int) * L.nlev);
   L.off_dm = take(sizeof(double) * 2 * N);                    // per system layer
@@ -333,16 +336,66 @@ __host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block,
   L.off_G = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
   L.off_Glow = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
   L.off_B = take(sizeof(double) * (L.nlev + 1) * L.nbt);
-  L.off_red = take(sizeof(double) * nwarp * 3 * (N + 1));
+  L.off_red = take(sizeof(double) * nwarp * 3 * L.LP);
   L.off_fin = take(sizeof(double) * 3 * (N + 1));
   L.off_vals = take(sizeof(double) * block);
+  L.off_T32 = take(sizeof(double) * 32);
   L.total = o;
   return L;
 }
 
+// Sum each of the 16 values v[0..15] over the 32 lanes of the warp by recursive halving: 16 shuffle+add
+// steps instead of 16 x 5.  Returns, in lanes L and L^1, the total of v[L >> 1].  Fixed order: deterministic.
+__device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
+  const unsigned full = 0xffffffffu;
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const double send = b4 ? v[i] : v[i + 8], keep = b4 ? v[i + 8] : v[i];
+    v[i] = keep + __shfl_xor_sync(full, send, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const double send = b3 ? v[i] : v[i + 4], keep = b3 ? v[i + 4] : v[i];
+    v[i] = keep + __shfl_xor_sync(full, send, 8);
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const double send = b2 ? v[i] : v[i + 2], keep = b2 ? v[i + 2] : v[i];
+    v[i] = keep + __shfl_xor_sync(full, send, 4);
+  }
+  {
+    const double send = b1 ? v[0] : v[1], keep = b1 ? v[1] : v[0];
+    v[0] = keep + __shfl_xor_sync(full, send, 2);
+  }
+  return v[0] + __shfl_xor_sync(full, v[0], 1);
+}
+
+struct Rows { double l00, l01, l10, l11; };   // the four k-table corner values of one (level, point)
+
+__device__ __forceinline__ Rows load_rows(const double *__restrict__ lnk_pt, int off, int strideT, int strideP) {
+  Rows r;
+  r.l00 = __ldg(lnk_pt + off);
+  r.l01 = __ldg(lnk_pt + off + strideT);
+  r.l10 = __ldg(lnk_pt + off + strideP);
+  r.l11 = __ldg(lnk_pt + off + strideP + strideT);
+  return r;
+}
+
+// optical properties at one level (S3 + Eqs. 17-18): bilinear ln(kappa) from the four corner rows with the
+// level's corner weights, exp, then kappa_ext, omega0, g0
+__device__ __forceinline__ void level_optics(const Rows &rw, const double *__restrict__ T32, const double4 cw,
+                                             int cloudy, const ThreadConst &tc, double &kx, double &w0, double &g0) {
+  const double lk = fma(cw.w, rw.l11, fma(cw.z, rw.l10, fma(cw.y, rw.l01, cw.x * rw.l00)));
+  const double kabs = exp_tab<0, false>(lk, T32, nullptr);
+  kx = kabs + (cloudy ? tc.sb1 : tc.sb0);
+  w0 = (cloudy ? tc.ss1 : tc.ss0) * rcp_fast(kx);
+  g0 = cloudy ? tc.gg1 : 0.0;
+}
+
 template <bool NONISO, bool TOA, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  extern __shared__ __align__(32) unsigned char smem[];
   const int N = P.N;
   const SmemLayout L = smem_layout(N, NONISO, BLOCK, P.ng, P.nb);
   double *s_lnp = (double *)(smem + L.off_lnp);
@@ -350,8 +403,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   double *s_tint = (double *)(smem + L.off_tint);
   double *s_plev = (double *)(smem + L.off_plev);
   double *s_tlev = (double *)(smem + L.off_tlev);
-  double *s_wp = (double *)(smem + L.off_wp);
-  double *s_wt = (double *)(smem + L.off_wt);
+  double4 *s_cw = (double4 *)(smem + L.off_cw);
   int *s_cell = (int *)(smem + L.off_cell);
   int *s_cloud = (int *)(smem + L.off_cloud);
   double *s_dm = (double *)(smem + L.off_dm);
@@ -362,11 +414,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   double *s_red = (double *)(smem + L.off_red);
   double *s_fin = (double *)(smem + L.off_fin);
   double *s_vals = (double *)(smem + L.off_vals);
+  double *s_T32 = (double *)(smem + L.off_T32);
   __shared__ int s_is_last, s_nan;
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x, col = blockIdx.y;
-  const int nlev = L.nlev;
+  const int nlev = L.nlev, LP = L.LP;
   const double *pc = P.p + (size_t)col * N;
   const double *Tc = P.T + (size_t)col * N;
   const double mu = P.mu[col];
@@ -377,10 +430,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   int pt_last = pt0 + BLOCK - 1;
   if (pt_last > P.npt - 1) pt_last = P.npt - 1;
   const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
+  const int nwa = ((pt_last - pt0) >> 5) + 1;     // warps of this tile that own at least one spectral point
 
   // NaN in p, T or mu of this column poisons the column's outputs (and only them): the clamps and
   // selects below would otherwise swallow it.
   if (tid == 0) s_nan = (mu != mu) ? 1 : 0;
+  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
   __syncthreads();
   // ---------------- S1: level geometry (reading R9; L171) ----------------
   for (int j = tid; j < N; j += BLOCK) {
@@ -428,8 +483,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
     int it = 0;
     while (it < P.nT - 2 && xt > P.tab_t[it + 1]) ++it;
     const double wt = (xt - P.tab_t[it]) / (P.tab_t[it + 1] - P.tab_t[it]);
-    s_wp[l] = wp;
-    s_wt[l] = wt;
+    // corner weights (iP,iT), (iP,iT+1), (iP+1,iT), (iP+1,iT+1)
+    s_cw[l] = make_double4((1.0 - wp) * (1.0 - wt), (1.0 - wp) * wt, wp * (1.0 - wt), wp * wt);
     s_cell[l] = (ip * P.nT + it) * P.npt;
   }
   for (int j = tid; j < N; j += BLOCK) s_dmfull[j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
@@ -466,119 +521,166 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   if (!active) pt = P.npt - 1;
   const int b = pt / P.ng, gidx = pt - b * P.ng;
   const int bl = b - b_first;
-  ThreadConst tc;
-  {
-    const BinConst bc = P.bins[b];
-    tc.W = active ? bc.dlam * P.gauss_w[gidx] : 0.0;
-    tc.sb0 = bc.sb[0]; tc.sb1 = bc.sb[1];
-    tc.ss0 = bc.ss[0]; tc.ss1 = bc.ss[1];
-    tc.gg1 = bc.gg[1];
-    tc.muF = day ? mu * P.fstar[b] : 0.0;
-  }
-  const double inv_mu = day ? 1.0 / mu : 0.0;
-  const double *lnk_pt = P.lnk + pt;
-  const int strideT = P.npt, strideP = P.nT * P.npt;
-  const double *Bcol = s_B + bl;   // B[l] = Bcol[l * L.nbt]
-  const int nbtS = L.nbt;
-
-  // back-substitution state, one entry per interface 1..N (thread-private, local memory:
-  // written top-down, read bottom-up -- a stack, served by L1/L2)
-  double2 st_cd[TOA ? 1 : MAXL];
-  double2 st_RU[TOA ? 1 : MAXL];
-
-  // ---------------- sweep 1: TOA -> BOA ----------------
-  double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
-  double tau = 0.0;
-  double Fb = tc.muF;                // beam at the TOA (full strength, L235)
-  double Ctoa = 1.0, Dtoa = 0.0;     // TOA mode: F_up[N] = Ctoa F_up[j] + Dtoa
-  const bool want_beam = !TOA && (P.F_beam != nullptr);
   const int warp = tid >> 5, lane = tid & 31;
-  double *red_w = s_red + (size_t)warp * 3 * (N + 1);
-  if (want_beam) {
-    const double wb = warp_sum(tc.W * Fb);
-    if (lane == 0) red_w[2 * (N + 1) + N] = wb;
-  }
+  const bool warp_on = warp < nwa;          // a warp without any spectral point only joins the barriers
+  double *red_w = s_red + (size_t)warp * 3 * LP;
+  const bool want_beam = !TOA && (P.F_beam != nullptr);
 
-  double kx_up = 0.0, w0_up = 0.0, g0_up = 0.0;   // non-iso: optics at the upper interface
-  if (NONISO) {
-    const int l = 2 * N;
-    level_optics(lnk_pt, s_cell[l], strideT, strideP, s_wp[l], s_wt[l], s_cloud[l], tc, kx_up, w0_up, g0_up);
-  }
+  if (warp_on) {
+    ThreadConst tc;
+    {
+      const BinConst bc = P.bins[b];
+      tc.W = active ? bc.dlam * P.gauss_w[gidx] : 0.0;
+      tc.sb0 = bc.sb[0]; tc.sb1 = bc.sb[1];
+      tc.ss0 = bc.ss[0]; tc.ss1 = bc.ss[1];
+      tc.gg1 = bc.gg[1];
+      tc.muF = day ? mu * P.fstar[b] : 0.0;
+    }
+    const double inv_mu = day ? 1.0 / mu : 0.0;
+    const double *lnk_pt = P.lnk + pt;
+    const int strideT = P.npt, strideP = P.nT * P.npt;
+    const double *Bcol = s_B + bl;   // B[l] = Bcol[l * L.nbt]
+    const int nbtS = L.nbt;
+    const double *T32 = s_T32;
+
+    // back-substitution state, one entry per interface 1..N (thread-private, local memory:
+    // written top-down, read bottom-up -- a stack, served by L1/L2)
+    double2 st_cd[TOA ? 1 : MAXL];
+    double2 st_RU[TOA ? 1 : MAXL];
+
+    // ---------------- sweep 1: TOA -> BOA ----------------
+    double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
+    double tau = 0.0;
+    double Fb = tc.muF;                // beam at the TOA (full strength, L235)
+    double Ctoa = 1.0, Dtoa = 0.0;     // TOA mode: F_up[N] = Ctoa F_up[j] + Dtoa
+    if (want_beam) {
+      const double wb = warp_sum(tc.W * Fb);
+      if (lane == 0) red_w[2 * LP + N] = wb;
+    }
+
+    double kx_up = 0.0, w0_up = 0.0, g0_up = 0.0;   // non-iso: optics at the upper interface
+    Rows nx;                                        // k-table rows of the next level, loaded one level ahead
+    if (NONISO) {
+      const int l = 2 * N;
+      const Rows top = load_rows(lnk_pt, s_cell[l], strideT, strideP);
+      level_optics(top, T32, s_cw[l], s_cloud[l], tc, kx_up, w0_up, g0_up);
+      nx = load_rows(lnk_pt, s_cell[2 * N - 1], strideT, strideP);
+    } else {
+      nx = load_rows(lnk_pt, s_cell[N - 1], strideT, strideP);
+    }
 
 #pragma unroll 1
-  for (int j = N - 1; j >= 0; --j) {
-    double c, d;
-    const double R_top = R, U_top = U, Fb_top = Fb;
-    if (!NONISO) {
-      double kx, w0, g0;
-      level_optics(lnk_pt, s_cell[j], strideT, strideP, s_wp[j], s_wt[j], s_cloud[j], tc, kx, w0, g0);
-      const double dtau = kx * s_dmfull[j];
-      tau += dtau;
-      double Fa = 0.0;
-      const double Bj = Bcol[j * nbtS];
-      if (day) {
-        Fa = tc.muF * exp_fast(-tau * inv_mu);                 // (B6)
-        layer_forward<true, false>(P, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, R, U, c, d);
-      } else {
-        layer_forward<false, false>(P, w0, g0, dtau, Bj, Bj, mu, 0.0, 0.0, R, U, c, d);
-      }
-      Fb = Fa;
-    } else {
-      // levels: 2j+2 (upper interface, carried), 2j+1 (centre), 2j (lower interface)
-      double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo;
-      const int lc = 2 * j + 1, ll = 2 * j;
-      level_optics(lnk_pt, s_cell[lc], strideT, strideP, s_wp[lc], s_wt[lc], s_cloud[lc], tc, kx_c, w0_c, g0_c);
-      level_optics(lnk_pt, s_cell[ll], strideT, strideP, s_wp[ll], s_wt[ll], s_cloud[ll], tc, kx_lo, w0_lo, g0_lo);
-      const double B_up = Bcol[(lc + 1) * nbtS], B_c = Bcol[lc * nbtS], B_lo = Bcol[ll * nbtS];
-      // upper sub-layer: arithmetic means of centre and interface values (L171, reading R10)
-      const double dtau_u = 0.5 * (kx_c + kx_up) * s_dm[lc];
-      const double dtau_l = 0.5 * (kx_lo + kx_c) * s_dm[ll];
-      double cu, du, cl, dl;
-      if (day) {
-        tau += dtau_u;
-        const double Fc = tc.muF * exp_fast(-tau * inv_mu);
-        layer_forward<true, true>(P, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, Fc, Fb,
-                                  R, U, cu, du);
-        tau += dtau_l;
-        const double Fa = tc.muF * exp_fast(-tau * inv_mu);
-        layer_forward<true, true>(P, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, Fa, Fc,
-                                  R, U, cl, dl);
+    for (int j = N - 1; j >= 0; --j) {
+      double c, d;
+      const double R_top = R, U_top = U, Fb_top = Fb;
+      if (!NONISO) {
+        const Rows cur = nx;
+        if (j > 0) nx = load_rows(lnk_pt, s_cell[j - 1], strideT, strideP);
+        double kx, w0, g0;
+        level_optics(cur, T32, s_cw[j], s_cloud[j], tc, kx, w0, g0);
+        const double dtau = kx * s_dmfull[j];
+        tau += dtau;
+        double Fa = 0.0;
+        const double Bj = Bcol[j * nbtS];
+        if (day) {
+          Fa = tc.muF * exp_tab<1, false>(fmin(tau * inv_mu, 708.0), T32, nullptr);                 // (B6)
+          layer_forward<true, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, R, U, c, d);
+        } else {
+          layer_forward<false, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, 0.0, 0.0, R, U, c, d);
+        }
         Fb = Fa;
       } else {
-        layer_forward<false, true>(P, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, 0.0, 0.0,
-                                   R, U, cu, du);
-        layer_forward<false, true>(P, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, 0.0, 0.0,
-                                   R, U, cl, dl);
+        // levels: 2j+2 (upper interface, carried), 2j+1 (centre), 2j (lower interface)
+        double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo;
+        const int lc = 2 * j + 1, ll = 2 * j;
+        const Rows rc = nx;
+        const Rows rl = load_rows(lnk_pt, s_cell[ll], strideT, strideP);
+        if (j > 0) nx = load_rows(lnk_pt, s_cell[ll - 1], strideT, strideP);
+        level_optics(rc, T32, s_cw[lc], s_cloud[lc], tc, kx_c, w0_c, g0_c);
+        level_optics(rl, T32, s_cw[ll], s_cloud[ll], tc, kx_lo, w0_lo, g0_lo);
+        const double B_up = Bcol[(lc + 1) * nbtS], B_c = Bcol[lc * nbtS], B_lo = Bcol[ll * nbtS];
+        // upper sub-layer: arithmetic means of centre and interface values (L171, reading R10)
+        const double dtau_u = 0.5 * (kx_c + kx_up) * s_dm[lc];
+        const double dtau_l = 0.5 * (kx_lo + kx_c) * s_dm[ll];
+        double cu, du, cl, dl;
+        if (day) {
+          tau += dtau_u;
+          const double Fc = tc.muF * exp_tab<1, false>(fmin(tau * inv_mu, 708.0), T32, nullptr);
+          layer_forward<true, true>(P, T32, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, Fc, Fb,
+                                    R, U, cu, du);
+          tau += dtau_l;
+          const double Fa = tc.muF * exp_tab<1, false>(fmin(tau * inv_mu, 708.0), T32, nullptr);
+          layer_forward<true, true>(P, T32, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, Fa, Fc,
+                                    R, U, cl, dl);
+          Fb = Fa;
+        } else {
+          layer_forward<false, true>(P, T32, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, 0.0,
+                                     0.0, R, U, cu, du);
+          layer_forward<false, true>(P, T32, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, 0.0,
+                                     0.0, R, U, cl, dl);
+        }
+        // F_up[j+1] = cu F_up[c] + du,  F_up[c] = cl F_up[j] + dl
+        c = cu * cl;
+        d = fma(cu, dl, du);
+        kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo;
       }
-      // F_up[j+1] = cu F_up[c] + du,  F_up[c] = cl F_up[j] + dl
-      c = cu * cl;
-      d = fma(cu, dl, du);
-      kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo;
+      if (TOA) {
+        Dtoa = fma(Ctoa, d, Dtoa);
+        Ctoa *= c;
+      } else {
+        // weights folded in: back-substitution runs on W F_up; F_dn carries the beam (L235)
+        st_cd[j] = make_double2(c, tc.W * d);
+        st_RU[j] = make_double2(R_top, tc.W * (U_top + Fb_top));
+        if (want_beam) {
+          const double wb = warp_sum(tc.W * Fb);
+          if (lane == 0) red_w[2 * LP + j] = wb;
+        }
+      }
     }
+
+    // ---------------- BOA, Eq.(10) L237 ----------------
+    const double F_boa = Bcol[nlev * nbtS];
+    const double Fup0 = (U + F_boa + Fb) * rcp_fast(1.0 - R);
+    const double Fdn0 = fma(R, Fup0, U);
+
     if (TOA) {
-      Dtoa = fma(Ctoa, d, Dtoa);
-      Ctoa *= c;
+      // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
+      const double FupN = fma(Ctoa, Fup0, Dtoa);
+      s_vals[tid] = active ? P.gauss_w[gidx] * FupN : 0.0;
     } else {
-      // weights folded in: back-substitution runs on W F_up; F_dn carries the beam (L235)
-      st_cd[j] = make_double2(c, tc.W * d);
-      st_RU[j] = make_double2(R_top, tc.W * (U_top + Fb_top));
-      if (want_beam) {
-        const double wb = warp_sum(tc.W * Fb);
-        if (lane == 0) red_w[2 * (N + 1) + j] = wb;
+      // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 levels at a time ----------------
+      double wFup = tc.W * Fup0;
+      double wFdn = tc.W * (Fdn0 + Fb);
+#pragma unroll 1
+      for (int base = 0; base <= N; base += 8) {
+        double v[16];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int e = base + k - 1;                       // stack entry that lifts level base+k-1 to base+k
+          const int ec = e < 0 ? 0 : (e > N - 1 ? N - 1 : e);
+          const double2 cd = st_cd[ec];
+          const double2 RU = st_RU[ec];
+          const bool upd = (e >= 0) && (e < N);
+          const double nu = fma(cd.x, wFup, cd.y);
+          const double nd = fma(RU.x, nu, RU.y);
+          wFup = upd ? nu : wFup;
+          wFdn = upd ? nd : wFdn;
+          const bool on = (base + k) <= N;
+          v[k] = on ? wFup : 0.0;
+          v[8 + k] = on ? wFdn : 0.0;
+        }
+        const double tot = warp_reduce16(v, lane);
+        const int idx = lane >> 1, lev = base + (idx & 7);
+        if (!(lane & 1) && lev <= N) red_w[(idx >> 3) * LP + lev] = tot;
       }
+      if (P.F_toa_bin != nullptr) s_vals[tid] = active ? wFup * P.bins[b].inv_dlam : 0.0;
     }
+  } else if (TOA || P.F_toa_bin != nullptr) {
+    s_vals[tid] = 0.0;
   }
+  __syncthreads();
 
-  // ---------------- BOA, Eq.(10) L237 ----------------
-  const double F_boa = Bcol[nlev * nbtS];
-  const double Fup0 = (U + F_boa + Fb) * rcp_fast(1.0 - R);
-  const double Fdn0 = fma(R, Fup0, U);
-
-  if (TOA) {
-    // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
-    const double FupN = fma(Ctoa, Fup0, Dtoa);
-    s_vals[tid] = active ? P.gauss_w[gidx] * FupN : 0.0;
-    __syncthreads();
+  if (TOA || P.F_toa_bin != nullptr) {
     for (int k = tid; k < nbt; k += BLOCK) {
       const int bb = b_first + k;
       int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
@@ -591,49 +693,17 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
       double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
       if (whole) *dst = sum; else atomicAdd(dst, sum);
     }
-    return;
   }
-
-  // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction ----------------
-  {
-    double wFup = tc.W * Fup0;
-    double wFdn = tc.W * (Fdn0 + Fb);
-    double su = warp_sum(wFup), sd = warp_sum(wFdn);
-    if (lane == 0) { red_w[0] = su; red_w[N + 1] = sd; }
-#pragma unroll 1
-    for (int j = 0; j < N; ++j) {
-      const double2 cd = st_cd[j];
-      const double2 RU = st_RU[j];
-      wFup = fma(cd.x, wFup, cd.y);
-      wFdn = fma(RU.x, wFup, RU.y);
-      su = warp_sum(wFup);
-      sd = warp_sum(wFdn);
-      if (lane == 0) { red_w[j + 1] = su; red_w[N + 1 + j + 1] = sd; }
-    }
-    if (P.F_toa_bin != nullptr) s_vals[tid] = active ? wFup * P.bins[b].inv_dlam : 0.0;
-  }
-  __syncthreads();
+  if (TOA) return;
 
   // cross-warp sum in fixed order -> tile partial
-  const int nwarp = (BLOCK + 31) / 32;
-  const int nred = (want_beam ? 3 : 2) * (N + 1);
+  const int nq = want_beam ? 3 : 2;
+  const int nred = nq * (N + 1);
   for (int k = tid; k < nred; k += BLOCK) {
+    const int q = k / (N + 1), lev = k - q * (N + 1);
     double sum = 0.0;
-    for (int w = 0; w < nwarp; ++w) sum += s_red[(size_t)w * 3 * (N + 1) + k];
+    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 3 * LP + q * LP + lev];
     s_fin[k] = sum;
-  }
-  if (P.F_toa_bin != nullptr) {
-    for (int k = tid; k < nbt; k += BLOCK) {
-      const int bb = b_first + k;
-      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
-      const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
-      if (g_lo < 0) g_lo = 0;
-      if (g_hi > BLOCK) g_hi = BLOCK;
-      double sum = s_nan ? nan("") : 0.0;
-      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
-      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
-      if (whole) *dst = sum; else atomicAdd(dst, sum);
-    }
   }
   __syncthreads();
 
@@ -693,12 +763,20 @@ __global__ void zero_kernel(double *p, size_t n) {
 
 __global__ void selftest_math_kernel(int n, const double *x, double *rcp, double *rsq, double *ex, double *omx) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ double T32[32];
+  if (threadIdx.x < 32) T32[threadIdx.x] = kExp2Tab[threadIdx.x];
+  __syncthreads();
   if (i >= n) return;
   const double v = x[i];
   rcp[i] = rcp_fast(v);
   rsq[i] = rsqrt_fast(fabs(v));
+  // e^-|x| through the three entry points the step kernel uses: e^-a, e^-2(a/2) (+ 1 - e^-a), e^(-a)
+  const double a = fmin(fabs(v), 708.0);
   double om;
-  ex[i] = exp_neg_fast(fabs(v), &om);
+  const double e2 = exp_tab<2, true>(0.5 * a, T32, &om);
+  const double e1 = exp_tab<1, false>(a, T32, nullptr);
+  const double e0 = exp_tab<0, false>(-a, T32, nullptr);
+  ex[i] = (i % 3 == 0) ? e0 : ((i % 3 == 1) ? e1 : e2);
   omx[i] = om;
 }
 
@@ -740,24 +818,21 @@ struct KernelChoice {
 };
 
 template <bool NONISO, bool TOA>
-KernelChoice pick_kernel(int block) {
-  switch (block) {
-    case 32:  return {rt_step_kernel<NONISO, TOA, 32, 16>, 32};
-    case 64:  return {rt_step_kernel<NONISO, TOA, 64, 8>, 64};
-    case 128: return {rt_step_kernel<NONISO, TOA, 128, 4>, 128};
-    case 160: return {rt_step_kernel<NONISO, TOA, 160, 3>, 160};
-    case 320: return {rt_step_kernel<NONISO, TOA, 320, 2>, 320};
-    case 608: return {rt_step_kernel<NONISO, TOA, 608, 1>, 608};
-    default:  return {nullptr, 0};
-  }
+KernelChoice pick_kernel(int block, int minb) {
+#define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_step_kernel<NONISO, TOA, B, M>, B};
+  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(128, 4) HRT_VARIANT(160, 3) HRT_VARIANT(320, 2) HRT_VARIANT(608, 1)
+  HRT_VARIANT(160, 4) HRT_VARIANT(128, 5) HRT_VARIANT(128, 6) HRT_VARIANT(128, 7) HRT_VARIANT(128, 8)
+  HRT_VARIANT(64, 10) HRT_VARIANT(64, 12) HRT_VARIANT(64, 14) HRT_VARIANT(96, 7) HRT_VARIANT(96, 8)
+#undef HRT_VARIANT
+  return {nullptr, 0};
 }
 
-KernelChoice pick(bool noniso, bool toa, int block) {
-  if (noniso) return toa ? pick_kernel<true, true>(block) : pick_kernel<true, false>(block);
-  return toa ? pick_kernel<false, true>(block) : pick_kernel<false, false>(block);
+KernelChoice pick(bool noniso, bool toa, int block, int minb) {
+  if (noniso) return toa ? pick_kernel<true, true>(block, minb) : pick_kernel<true, false>(block, minb);
+  return toa ? pick_kernel<false, true>(block, minb) : pick_kernel<false, false>(block, minb);
 }
 
-const int kBlocks[] = {32, 64, 128, 160, 320, 608};
+const int kBlocks[] = {32, 64, 96, 128, 160, 320, 608};
 
 // block size: fewest padded lanes over the column, ties -> larger block (fewer tiles)
 int choose_block(int npt) {
@@ -899,7 +974,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
   h->block = choose_block(h->npt);
   h->tiles = (h->npt + h->block - 1) / h->block;
-  h->kc = pick(h->noniso, h->toa, h->block);
+  { const char *mb = getenv("HELIOS_RT_MINB"); h->kc = pick(h->noniso, h->toa, h->block, mb ? atoi(mb) : 0); }
   h->lay = smem_layout(N, h->noniso, h->block, ng, nb);
   cudaGetDevice(&rc);
   cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, rc);
