@@ -34,6 +34,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include <new>
+#include <type_traits>
 
 namespace {
 
@@ -73,6 +74,8 @@ __device__ __forceinline__ bool gt_pos(double a, double b) { return __double_as_
 __device__ __forceinline__ bool abs_lt(double a, double b_pos) {
   return (__double_as_longlong(a) & 0x7fffffffffffffffLL) < __double_as_longlong(b_pos);
 }
+// min(x, c) for x >= 0, c > 0 on the integer pipes
+__device__ __forceinline__ double min_pos(double x, double c) { return gt_pos(x, c) ? c : x; }
 
 // exp by table: e^x = 2^m T[j] (1 + p(r)), k = 32 m + j = round(32 x / ln 2), r = x - k ln2/32, |r| <= ln2/64,
 // T[j] = 2^(j/32) (32 doubles in shared memory), p = expm1(r) by its degree-6 Taylor polynomial (remainder
@@ -89,39 +92,6 @@ __constant__ double kExp2Tab[32] = {
     1.5422108254079407, 1.5759808451078865, 1.6104903319492543, 1.645755478153965,
     1.681792830507429, 1.718619298122478, 1.7562521603732995, 1.7947090750031072,
     1.8340080864093424, 1.8741676341103, 1.9152065613971474, 1.9571441241754002};
-
-template <int MODE, bool OM>
-__device__ __forceinline__ double exp_tab(double x, const double *__restrict__ T32, double *om) {
-  const double kMagic = 6755399441055744.0;      // 1.5 * 2^52: round-to-nearest-integer trick
-  const double kS = 46.16624130844683;           // 32 / ln 2
-  const double kL = 0.02166084939249829;         // ln 2 / 32
-  double kd, p;
-  if (MODE == 0) kd = fma(x, kS, kMagic);
-  else if (MODE == 1) kd = fma(x, -kS, kMagic);
-  else kd = fma(x, -2.0 * kS, kMagic);
-  const int ki = __double2loint(kd);
-  const double kf = kd - kMagic;
-  if (MODE == 2) {
-    // r = -2 x - kf L; with h = -r/2 = x + kf L/2:  p = expm1(-2 h) = h (-2 + h q(h))
-    const double h = fma(kf, 0.5 * kL, x);
-    double q = fma(h, 4.0 / 45.0, -4.0 / 15.0);
-    q = fma(q, h, 2.0 / 3.0);
-    q = fma(q, h, -4.0 / 3.0);
-    q = fma(q, h, 2.0);
-    p = h * fma(h, q, -2.0);
-  } else {
-    const double r = (MODE == 0) ? fma(kf, -kL, x) : fma(kf, -kL, -x);
-    double q = fma(r, 1.0 / 720.0, 1.0 / 120.0);
-    q = fma(q, r, 1.0 / 24.0);
-    q = fma(q, r, 1.0 / 6.0);
-    q = fma(q, r, 0.5);
-    p = fma(r * r, q, r);
-  }
-  const double Tj = T32[ki & 31];
-  const double Ts = __hiloint2double(__double2hiint(Tj) + (ki >> 5) * 1048576, __double2loint(Tj));   // 2^m T[j]
-  if (OM) *om = fma(-Ts, p, 1.0 - Ts);
-  return fma(Ts, p, Ts);
-}
 
 // --------------------------------------------------------------------------------------------
 // S2: band Planck.  G(x) = int_x^inf t^3/(e^t - 1) dt (reading R8).
@@ -194,6 +164,16 @@ struct BinConst {   // per bin, built at create time from scat_gas / cloud_* (Eq
   double gg[2];     // g0 at a clear / cloudy level
 };
 
+// S1 result per (column, level), written by rt_prep_kernel, staged in shared memory by rt_solve_kernel
+struct __align__(16) LevelRec {
+  double c00, c01, c10, c11;  // bilinear weights of the corners (iP,iT), (iP,iT+1), (iP+1,iT), (iP+1,iT+1)
+  unsigned o00, o01, o10, o11;  // offsets of the four corner rows (spectral point 0) in the ln(kappa) table, doubles
+  double dm;                  // column mass of the (sub-)layer whose lower level this is, kg m^-2
+  int cloud;                  // cloud_p_top <= p <= cloud_p_bot
+  int pad;
+};
+static_assert(sizeof(LevelRec) == 64, "LevelRec layout");
+
 struct KParams {
   // create-time tables (device)
   const double *lnk;      // [nP][nT][npt] ln(kappa)
@@ -202,7 +182,7 @@ struct KParams {
   const double *edges;    // [nb+1]
   const double *gauss_w;  // [ng]
   const BinConst *bins;   // [nb]
-  int nP, nT, N, nb, ng, npt, tiles;
+  int nP, nT, N, nlev, nb, ng, npt, tiles;
   double cloud_p_top, cloud_p_bot, inv_g, inv_cp, inv_eps2, e_tau, gcrit_tol, w0_transition, f_toa;
   int improved;
   // per-step
@@ -210,15 +190,68 @@ struct KParams {
   double T_int;
   double *F_up, *F_down, *F_net, *dTdt, *F_beam, *F_toa_bin;
   // workspace
-  double *partial;        // [ncol][tiles][3][N+1]
+  LevelRec *ws_lev;       // [ncol][nlev+1]   record 0 pads the one-level-ahead prefetch (copy of level 0)
+  double *ws_B;           // [ncol][nlev+1][nb] band Planck per level; last row pi B_b(T_int)
+  double *ws_dm;          // [ncol][N]        full-layer column mass (heating rate)
+  int *ws_nan;            // [ncol]           NaN in p, T of the column
+  double *partial;        // [ncol][tiles][4][N+1]
   unsigned *counter;      // [ncol]
 };
 
-struct ThreadConst {      // per spectral point
-  double W;               // dlam_b * w_g
-  double sb0, sb1, ss0, ss1, gg1;
-  double muF;             // mu * F_star[b]
+// constants of the hot loop live in constant memory: an fp64 instruction takes one operand straight from
+// the constant bank, so none of them costs a register, a move or a uniform-register rematerialisation
+struct HotConst {
+  double S, nS, n2S;      // 32/ln2, -32/ln2, -64/ln2
+  double nL, hL;          // -ln2/32, ln2/64
+  double e6, e5, e4, e3;  // 1/720, 1/120, 1/24, 1/6
+  double q4, q3, q2, q1;  // 4/45, -4/15, 2/3, -4/3
+  double fa, fb, fc;      // Eq.(19): 1.225 - 0.1582 g - 0.07465 g^2
+  double fd, fe, ff;      //          + w (-0.1777 + 0.2351 g - 0.05582 w)
+  double pi, npi;
 };
+__constant__ HotConst kHC = {
+    46.16624130844683,     -46.16624130844683,   -92.33248261689366,
+    -0.02166084939249829,  0.010830424696249145,
+    1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0,
+    4.0 / 45.0, -4.0 / 15.0, 2.0 / 3.0, -4.0 / 3.0,
+    1.225, -0.1582, -0.07465,
+    -0.1777, 0.2351, -0.05582,
+    3.14159265358979323846, -3.14159265358979323846};
+
+// exp by table (see kExp2Tab), constants from kHC.
+//   MODE 0: e^x for |x| <= 708;  MODE 1: e^-a, 0 <= a <= 708;  MODE 2: e^-2a, 0 <= a <= 354, and, if OM,
+//   *om = 1 - e^-2a without cancellation.
+template <int MODE, bool OM>
+__device__ __forceinline__ double exp_hot(double x, const double *__restrict__ T32, double *om) {
+  const double kMagic = 6755399441055744.0;      // 1.5 * 2^52: round-to-nearest-integer trick
+  double kd, p;
+  if (MODE == 0) kd = fma(x, kHC.S, kMagic);
+  else if (MODE == 1) kd = fma(x, kHC.nS, kMagic);
+  else kd = fma(x, kHC.n2S, kMagic);
+  const int ki = __double2loint(kd);
+  const double kf = kd - kMagic;
+  if (MODE == 2) {
+    // r = -2 x - kf L; with h = -r/2 = x + kf L/2:  p = expm1(-2 h) = h (-2 + h q(h))
+    const double h = fma(kf, kHC.hL, x);
+    double q = fma(h, kHC.q4, kHC.q3);
+    q = fma(q, h, kHC.q2);
+    q = fma(q, h, kHC.q1);
+    q = fma(q, h, 2.0);
+    p = h * fma(h, q, -2.0);
+  } else {
+    const double r = (MODE == 0) ? fma(kf, kHC.nL, x) : fma(kf, kHC.nL, -x);
+    double q = fma(r, kHC.e6, kHC.e5);
+    q = fma(q, r, kHC.e4);
+    q = fma(q, r, kHC.e3);
+    q = fma(q, r, 0.5);
+    p = fma(r * r, q, r);
+  }
+  const double Tj = T32[ki & 31];
+  const double Ts = __hiloint2double(__double2hiint(Tj) + ((ki >> 5) << 20), __double2loint(Tj));   // 2^m T[j]
+  if (OM) *om = fma(-Ts, p, 1.0 - Ts);
+  return fma(Ts, p, Ts);
+}
+
 
 // --------------------------------------------------------------------------------------------
 // S5 + S6 forward step for one (sub-)layer between a lower level "a" and an upper level "b".
@@ -230,12 +263,9 @@ __device__ __forceinline__ void layer_forward(const KParams &P, const double *__
                                               double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
                                               double &R, double &U, double &c, double &d) {
   // E, Eq.(19) L374 (readings R5, R6): E = max(1, fit) if w0 > 0.1 else 1
-  double E = 1.0;
-  if (P.improved) {
-    const double fg = fma(g0, fma(-0.07465, g0, -0.1582), 1.225);
-    const double fit = fma(w0, fma(g0, 0.2351, fma(-0.05582, w0, -0.1777)), fg);
-    E = (gt_pos(w0, P.w0_transition) && gt_pos(fit, 1.0)) ? fit : 1.0;
-  }
+  const double fg = fma(g0, fma(kHC.fc, g0, kHC.fb), kHC.fa);
+  const double fit = fma(w0, fma(g0, kHC.fe, fma(kHC.ff, w0, kHC.fd)), fg);
+  const double E = (P.improved && gt_pos(w0, P.w0_transition) && gt_pos(fit, 1.0)) ? fit : 1.0;
   const double wg = w0 * g0;
   const double num = E - w0;             // E - omega0
   const double den = E * (1.0 - wg);     // E (1 - omega0 g0)
@@ -246,7 +276,7 @@ __device__ __forceinline__ void layer_forward(const KParams &P, const double *__
   const double rs2 = rs * rs;
   const double zp = fma(0.5, s, 0.5), zm = fma(-0.5, s, 0.5);
   double omT;
-  const double Tr = exp_tab<2, true>(fmin(ha * dtau, 354.0), T32, &omT);   // transmission function (B2), 1 - T
+  const double Tr = exp_hot<2, true>(min_pos(ha * dtau, 354.0), T32, &omT);   // transmission function (B2), 1 - T
   const double zmT = zm * Tr;
   const double a = zp - zmT, b = zp + zmT;
   const double inv_ab = rcp_fast(a * b);
@@ -254,7 +284,7 @@ __device__ __forceinline__ void layer_forward(const KParams &P, const double *__
   const double t = (s * Tr) * inv_ab;                        // psi/chi
   const double r = (zp * zm) * (1.0 + Tr) * u;               // -xi/chi
   const double emis = (s * a) * u;                           // 1 - t - r
-  const double Pi = fma(-kPi, w0, kPi) * (den * rs2);        // (B5): pi (1-w0)/(E-w0)
+  const double Pi = fma(kHC.npi, w0, kHC.pi) * (den * rs2);  // (B5): pi (1-w0)/(E-w0)
   double Sup, Sdn;
   if (LINSRC) {
     // Eqs.(4)-(9): B* (1-r) - t B*' +- B' (1 - t + r)/(2E(1-w0 g0)), B' = (Ba - Bb)/dtau; e_tau rule L209
@@ -303,47 +333,6 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// --------------------------------------------------------------------------------------------
-// the step kernel
-// --------------------------------------------------------------------------------------------
-struct SmemLayout {
-  int nlev;        // levels at which kappa / Planck are evaluated: N (iso) or 2N+1 (non-iso)
-  int nbt;         // max bins per tile
-  int LP;          // N + 1 rounded up to a multiple of 8 (sweep 2 reduces 8 levels at a time)
-  size_t off_lnp, off_pint, off_tint, off_plev, off_tlev, off_cw, off_cell, off_cloud, off_dm,
-      off_dmfull, off_G, off_Glow, off_B, off_red, off_fin, off_vals, off_T32, total;
-};
-
-__host__ __device__ inline SmemLayout smem_layout(int N, bool noniso, int block, int ng, int nb) {
-  SmemLayout L;
-  L.nlev = noniso ? 2 * N + 1 : N;
-  int nbt = (block + ng - 1) / ng + 1;
-  L.nbt = nbt < nb ? nbt : nb;
-  L.LP = (N + 1 + 7) & ~7;
-  const int nwarp = (block + 31) / 32;
-  size_t o = 0;
-  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 31) & ~size_t(31); return r; };
-  L.off_lnp = take(sizeof(double) * N);
-  L.off_pint = take(sizeof(double) * (N + 1));
-  L.off_tint = take(sizeof(double) * (N + 1));
-  L.off_plev = take(sizeof(double) * L.nlev);
-  L.off_tlev = take(sizeof(double) * (L.nlev + 1));           // + internal temperature row
-  L.off_cw = take(sizeof(double) * 4 * L.nlev);               // bilinear corner weights per level
-  L.off_cell = take(sizeof(int) * L.nlev);
-  L.off_cloud = take(sizeof(int) * L.nlev);
-  L.off_dm = take(sizeof(double) * 2 * N);                    // per system layer
-  L.off_dmfull = take(sizeof(double) * N);
-  L.off_G = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
-  L.off_Glow = take(sizeof(double) * (L.nlev + 1) * (L.nbt + 1));
-  L.off_B = take(sizeof(double) * (L.nlev + 1) * L.nbt);
-  L.off_red = take(sizeof(double) * nwarp * 3 * L.LP);
-  L.off_fin = take(sizeof(double) * 3 * (N + 1));
-  L.off_vals = take(sizeof(double) * block);
-  L.off_T32 = take(sizeof(double) * 32);
-  L.total = o;
-  return L;
-}
-
 // Sum each of the 16 values v[0..15] over the 32 lanes of the warp by recursive halving: 16 shuffle+add
 // steps instead of 16 x 5.  Returns, in lanes L and L^1, the total of v[L >> 1].  Fixed order: deterministic.
 __device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
@@ -371,80 +360,48 @@ __device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
   return v[0] + __shfl_xor_sync(full, v[0], 1);
 }
 
-struct Rows { double l00, l01, l10, l11; };   // the four k-table corner values of one (level, point)
+// --------------------------------------------------------------------------------------------
+// rt_prep_kernel: S1 (level geometry, k-table cell + weights per level) and S2 (band Planck per level
+// and bin) for every column.  Grid = (bin chunks of PREP_BINS, columns).  Results go to the handle's
+// workspace (a few tens of MB, L2-resident when rt_solve_kernel reads them back).
+// --------------------------------------------------------------------------------------------
+constexpr int PREP_BLOCK = 256, PREP_BINS = 32;
 
-__device__ __forceinline__ Rows load_rows(const double *__restrict__ lnk_pt, int off, int strideT, int strideP) {
-  Rows r;
-  r.l00 = __ldg(lnk_pt + off);
-  r.l01 = __ldg(lnk_pt + off + strideT);
-  r.l10 = __ldg(lnk_pt + off + strideP);
-  r.l11 = __ldg(lnk_pt + off + strideP + strideT);
-  return r;
+__host__ __device__ inline size_t prep_smem_bytes(int N, int nlev) {
+  return sizeof(double) * ((size_t)N + 2 * (N + 1) + (nlev + 1) + 2 * (size_t)(nlev + 1) * (PREP_BINS + 1));
 }
 
-// optical properties at one level (S3 + Eqs. 17-18): bilinear ln(kappa) from the four corner rows with the
-// level's corner weights, exp, then kappa_ext, omega0, g0
-__device__ __forceinline__ void level_optics(const Rows &rw, const double *__restrict__ T32, const double4 cw,
-                                             int cloudy, const ThreadConst &tc, double &kx, double &w0, double &g0) {
-  const double lk = fma(cw.w, rw.l11, fma(cw.z, rw.l10, fma(cw.y, rw.l01, cw.x * rw.l00)));
-  const double kabs = exp_tab<0, false>(lk, T32, nullptr);
-  kx = kabs + (cloudy ? tc.sb1 : tc.sb0);
-  w0 = (cloudy ? tc.ss1 : tc.ss0) * rcp_fast(kx);
-  g0 = cloudy ? tc.gg1 : 0.0;
-}
-
-template <bool NONISO, bool TOA, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
-  extern __shared__ __align__(32) unsigned char smem[];
-  const int N = P.N;
-  const SmemLayout L = smem_layout(N, NONISO, BLOCK, P.ng, P.nb);
-  double *s_lnp = (double *)(smem + L.off_lnp);
-  double *s_pint = (double *)(smem + L.off_pint);
-  double *s_tint = (double *)(smem + L.off_tint);
-  double *s_plev = (double *)(smem + L.off_plev);
-  double *s_tlev = (double *)(smem + L.off_tlev);
-  double4 *s_cw = (double4 *)(smem + L.off_cw);
-  int *s_cell = (int *)(smem + L.off_cell);
-  int *s_cloud = (int *)(smem + L.off_cloud);
-  double *s_dm = (double *)(smem + L.off_dm);
-  double *s_dmfull = (double *)(smem + L.off_dmfull);
-  double *s_G = (double *)(smem + L.off_G);
-  double *s_Glow = (double *)(smem + L.off_Glow);
-  double *s_B = (double *)(smem + L.off_B);
-  double *s_red = (double *)(smem + L.off_red);
-  double *s_fin = (double *)(smem + L.off_fin);
-  double *s_vals = (double *)(smem + L.off_vals);
-  double *s_T32 = (double *)(smem + L.off_T32);
-  __shared__ int s_is_last, s_nan;
+template <bool NONISO>
+__global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int N = P.N, nlev = P.nlev;
+  double *s_lnp = (double *)smem;                       // [N]
+  double *s_pint = s_lnp + N;                           // [N+1]
+  double *s_tint = s_pint + (N + 1);                    // [N+1]
+  double *s_tlev = s_tint + (N + 1);                    // [nlev+1], last = internal temperature
+  double *s_G = s_tlev + (nlev + 1);                    // [nlev+1][PREP_BINS+1]
+  double *s_Glow = s_G + (size_t)(nlev + 1) * (PREP_BINS + 1);
+  __shared__ int s_nan;
 
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x, col = blockIdx.y;
-  const int nlev = L.nlev, LP = L.LP;
+  const int chunk = blockIdx.x, col = blockIdx.y;
   const double *pc = P.p + (size_t)col * N;
   const double *Tc = P.T + (size_t)col * N;
-  const double mu = P.mu[col];
-  const bool day = mu > 0.0;
-
-  const int pt0 = tile * BLOCK;
-  const int b_first = pt0 / P.ng;
-  int pt_last = pt0 + BLOCK - 1;
-  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
-  const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
-  const int nwa = ((pt_last - pt0) >> 5) + 1;     // warps of this tile that own at least one spectral point
+  const int b0 = chunk * PREP_BINS;
+  const int nbc = (P.nb - b0 < PREP_BINS) ? (P.nb - b0) : PREP_BINS;
 
   // NaN in p, T or mu of this column poisons the column's outputs (and only them): the clamps and
   // selects below would otherwise swallow it.
-  if (tid == 0) s_nan = (mu != mu) ? 1 : 0;
-  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
+  if (tid == 0) { const double mu = P.mu[col]; s_nan = (mu != mu) ? 1 : 0; }
   __syncthreads();
   // ---------------- S1: level geometry (reading R9; L171) ----------------
-  for (int j = tid; j < N; j += BLOCK) {
+  for (int j = tid; j < N; j += PREP_BLOCK) {
     const double pj = pc[j], tj = Tc[j];
     if (pj != pj || tj != tj) s_nan = 1;
     s_lnp[j] = log(pj);
   }
   __syncthreads();
-  for (int i = tid; i <= N; i += BLOCK) {
+  for (int i = tid; i <= N; i += PREP_BLOCK) {
     double lp, ti;
     if (N == 1) {
       lp = s_lnp[0] + (i == 0 ? 0.5 : -0.5) * 2.302585092994045684;
@@ -463,56 +420,203 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
     s_tint[i] = ti;
   }
   __syncthreads();
-  for (int l = tid; l <= nlev; l += BLOCK) {
+  auto p_level = [&](int l) -> double {
+    if (NONISO) return (l & 1) ? pc[l >> 1] : s_pint[l >> 1];
+    return pc[l];
+  };
+  for (int l = tid; l <= nlev; l += PREP_BLOCK) {
     if (l == nlev) { s_tlev[l] = P.T_int; continue; }
-    double pl, tl;
-    if (NONISO) {
-      if (l & 1) { pl = pc[l >> 1]; tl = Tc[l >> 1]; }
-      else       { pl = s_pint[l >> 1]; tl = s_tint[l >> 1]; }
-    } else { pl = pc[l]; tl = Tc[l]; }
-    s_plev[l] = pl;
+    const double pl = p_level(l);
+    const double tl = NONISO ? ((l & 1) ? Tc[l >> 1] : s_tint[l >> 1]) : Tc[l];
     s_tlev[l] = tl;
-    s_cloud[l] = (pl >= P.cloud_p_top && pl <= P.cloud_p_bot) ? 1 : 0;
+    if (chunk != 0) continue;
+    LevelRec rec;
+    rec.cloud = (pl >= P.cloud_p_top && pl <= P.cloud_p_bot) ? 1 : 0;
     // table cell + weights: bilinear in (log10 p, T), clamped (reading R7)
     double xp = log10(pl);
     xp = fmin(fmax(xp, P.tab_lp[0]), P.tab_lp[P.nP - 1]);
     int ip = 0;
     while (ip < P.nP - 2 && xp > P.tab_lp[ip + 1]) ++ip;
     const double wp = (xp - P.tab_lp[ip]) / (P.tab_lp[ip + 1] - P.tab_lp[ip]);
-    double xt = fmin(fmax(tl, P.tab_t[0]), P.tab_t[P.nT - 1]);
+    const double xt = fmin(fmax(tl, P.tab_t[0]), P.tab_t[P.nT - 1]);
     int it = 0;
     while (it < P.nT - 2 && xt > P.tab_t[it + 1]) ++it;
     const double wt = (xt - P.tab_t[it]) / (P.tab_t[it + 1] - P.tab_t[it]);
-    // corner weights (iP,iT), (iP,iT+1), (iP+1,iT), (iP+1,iT+1)
-    s_cw[l] = make_double4((1.0 - wp) * (1.0 - wt), (1.0 - wp) * wt, wp * (1.0 - wt), wp * wt);
-    s_cell[l] = (ip * P.nT + it) * P.npt;
+    rec.c00 = (1.0 - wp) * (1.0 - wt);
+    rec.c01 = (1.0 - wp) * wt;
+    rec.c10 = wp * (1.0 - wt);
+    rec.c11 = wp * wt;
+    rec.o00 = (unsigned)(ip * P.nT + it) * (unsigned)P.npt;
+    rec.o01 = rec.o00 + (unsigned)P.npt;
+    rec.o10 = rec.o00 + (unsigned)P.nT * (unsigned)P.npt;
+    rec.o11 = rec.o10 + (unsigned)P.npt;
+    rec.pad = 0;
+    // column mass below this level down to the next level: full layer (isothermal: level = layer centre,
+    // mass between its two interfaces) or sub-layer (non-isothermal: levels alternate interface / centre)
+    if (NONISO) rec.dm = (l < nlev - 1) ? (pl - p_level(l + 1)) * P.inv_g : 0.0;
+    else rec.dm = (s_pint[l] - s_pint[l + 1]) * P.inv_g;
+    LevelRec *dst = P.ws_lev + (size_t)col * (nlev + 1) + 1 + l;
+    *dst = rec;
+    if (l == 0) dst[-1] = rec;
   }
-  for (int j = tid; j < N; j += BLOCK) s_dmfull[j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
+  if (chunk == 0)
+    for (int j = tid; j < N; j += PREP_BLOCK) P.ws_dm[(size_t)col * N + j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
   __syncthreads();
-  if (NONISO) {
-    for (int s = tid; s < 2 * N; s += BLOCK) s_dm[s] = (s_plev[s] - s_plev[s + 1]) * P.inv_g;
-  }
+  if (chunk == 0 && tid == 0) P.ws_nan[col] = s_nan;
 
-  // ---------------- S2: band Planck for the tile's bins (reading R8) ----------------
-  const int nedge = nbt + 1;
-  for (int i = tid; i < (nlev + 1) * nedge; i += BLOCK) {
+  // ---------------- S2: band Planck for this chunk's bins (reading R8) ----------------
+  const int nedge = nbc + 1;
+  for (int i = tid; i < (nlev + 1) * nedge; i += PREP_BLOCK) {
     const int l = i / nedge, e = i - l * nedge;
     const double Tl = s_tlev[l];
     double low = 0.0;
-    s_G[l * (L.nbt + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b_first + e] * Tl), &low) : 0.0;
-    s_Glow[l * (L.nbt + 1) + e] = low;
+    s_G[l * (PREP_BINS + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b0 + e] * Tl), &low) : 0.0;
+    s_Glow[l * (PREP_BINS + 1) + e] = low;
   }
   __syncthreads();
-  for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
-    const int l = i / nbt, bl = i - l * nbt;
+  for (int i = tid; i < (nlev + 1) * nbc; i += PREP_BLOCK) {
+    const int l = i / nbc, k = i - l * nbc;
     const double Tl = s_tlev[l];
     const double T2 = Tl * Tl;
-    const double *g = s_G + l * (L.nbt + 1) + bl;
-    const double *gl = s_Glow + l * (L.nbt + 1) + bl;
-    double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * P.bins[b_first + bl].inv_dlam;
+    const double *g = s_G + l * (PREP_BINS + 1) + k;
+    const double *gl = s_Glow + l * (PREP_BINS + 1) + k;
+    double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * P.bins[b0 + k].inv_dlam;
     if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
-    s_B[l * L.nbt + bl] = (Tl > 0.0) ? B : 0.0;
+    P.ws_B[((size_t)col * (nlev + 1) + l) * P.nb + b0 + k] = (Tl > 0.0) ? B : 0.0;
   }
+}
+
+// --------------------------------------------------------------------------------------------
+// rt_solve_kernel: S3-S7.  Grid = (tiles per column, columns); a block owns one column and a tile of
+// BLOCK consecutive spectral points (bin-major, Gauss point fastest); one thread = one spectral point.
+// --------------------------------------------------------------------------------------------
+constexpr int STAGE_LD = 36;   // row stride (doubles) of the per-warp 8 x 32 staging tile: conflict-free transpose
+
+struct __align__(16) BinOpt { double sb, ss, gg, pad; };   // per bin of the tile: [0][bin] clear level, [1][bin] cloudy level
+
+struct SolveSmem {
+  int nbt;         // max bins per tile
+  int LP;          // N + 1 rounded up to a multiple of 8 (the reductions handle 8 levels at a time)
+  size_t off_lev, off_B, off_bin, off_red, off_stage, off_fin, off_vals, total;
+};
+
+__host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa) {
+  SolveSmem L;
+  int nbt = (block + ng - 1) / ng + 1;
+  L.nbt = nbt < nb ? nbt : nb;
+  L.LP = (N + 1 + 7) & ~7;
+  const int nwarp = (block + 31) / 32;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
+  L.off_lev = take(sizeof(LevelRec) * (nlev + 1));
+  L.off_B = take(sizeof(double) * (nlev + 1) * L.nbt);
+  L.off_bin = take(sizeof(BinOpt) * 2 * L.nbt);
+  L.off_red = take(toa ? 0 : sizeof(double) * nwarp * 4 * L.LP);       // F_up, R F_up, U + beam, beam
+  L.off_stage = take(toa ? 0 : sizeof(double) * nwarp * 8 * STAGE_LD);
+  L.off_fin = take(toa ? 0 : sizeof(double) * 4 * (N + 1));
+  L.off_vals = take(sizeof(double) * block);
+  L.total = o;
+  return L;
+}
+
+struct Rows { double l00, l01, l10, l11; };   // the four k-table corner values of one (level, point)
+
+// address of element `off` (32-bit, unsigned) of a double array: one IMAD.WIDE.U32
+__device__ __forceinline__ const double *elem_addr(const double *base, unsigned off) {
+  unsigned long long a;
+  asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(a) : "r"(off), "l"((unsigned long long)base));
+  return (const double *)a;
+}
+
+__device__ __forceinline__ Rows load_rows(const double *__restrict__ lnk_pt, const LevelRec *lv) {
+  const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
+  Rows r;
+  r.l00 = __ldg(elem_addr(lnk_pt, o.x));
+  r.l01 = __ldg(elem_addr(lnk_pt, o.y));
+  r.l10 = __ldg(elem_addr(lnk_pt, o.z));
+  r.l11 = __ldg(elem_addr(lnk_pt, o.w));
+  return r;
+}
+
+
+// optical properties at one level (S3 + Eqs. 17-18): bilinear ln(kappa) from the four corner rows with the
+// level's corner weights, exp, then kappa_ext, omega0, g0.  bin0 / bin1: the point's BinOpt for clear / cloudy.
+__device__ __forceinline__ void level_optics(const Rows &rw, const double *__restrict__ T32, const LevelRec *lv,
+                                             const BinOpt *bin0, const BinOpt *bin1, double &kx, double &w0,
+                                             double &g0) {
+  const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
+  const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
+  const double lk = fma(cb.y, rw.l11, fma(cb.x, rw.l10, fma(ca.y, rw.l01, ca.x * rw.l00)));
+  const double kabs = exp_hot<0, false>(lk, T32, nullptr);
+  const BinOpt *bo = lv->cloud ? bin1 : bin0;
+  const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
+  kx = kabs + sbss.x;
+  w0 = sbss.y * rcp_fast(kx);
+  g0 = bo->gg;
+}
+
+// sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
+// base + k.  Lane L sums 8 entries of row L >> 2, two shuffle steps finish the row.  Fixed order.
+__device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, double *__restrict__ dst, int lane) {
+  __syncwarp();
+  const double *row = stage_w + (lane >> 2) * STAGE_LD + (lane & 3);
+  double s = row[0];
+#pragma unroll
+  for (int i = 1; i < 8; ++i) s += row[4 * i];
+  s += __shfl_xor_sync(0xffffffffu, s, 1);
+  s += __shfl_xor_sync(0xffffffffu, s, 2);
+  if ((lane & 3) == 0) dst[lane >> 2] = s;
+  __syncwarp();
+}
+
+template <bool NONISO, bool TOA, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double s_T32[32];
+  __shared__ int s_is_last;
+  const int N = P.N, nlev = P.nlev;
+  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA);
+  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;   // s_lev[-1] pads the prefetch
+  double *s_B = (double *)(smem + L.off_B);
+  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
+  double *s_red = (double *)(smem + L.off_red);
+  double *s_stage = (double *)(smem + L.off_stage);
+  double *s_fin = (double *)(smem + L.off_fin);
+  double *s_vals = (double *)(smem + L.off_vals);
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x, col = blockIdx.y;
+  const int LP = L.LP, nbtS = L.nbt;
+  const double mu = P.mu[col];
+  const bool day = mu > 0.0;
+
+  const int pt0 = tile * BLOCK;
+  const int b_first = pt0 / P.ng;
+  int pt_last = pt0 + BLOCK - 1;
+  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
+  const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
+  const int nwa = ((pt_last - pt0) >> 5) + 1;     // warps of this tile that own at least one spectral point
+
+  // ---------------- stage the column's level records, the tile's Planck values and bin constants ----------------
+  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
+  {
+    const double *src = (const double *)(P.ws_lev + (size_t)col * (nlev + 1));
+    double *dst = (double *)(smem + L.off_lev);
+    for (int i = tid; i < 8 * (nlev + 1); i += BLOCK) dst[i] = src[i];
+    const double *gB = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b_first;
+    for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
+      const int l = i / nbt, k = i - l * nbt;
+      s_B[l * nbtS + k] = gB[(size_t)l * P.nb + k];
+    }
+    for (int i = tid; i < 2 * nbt; i += BLOCK) {
+      const int cl = i / nbt, k = i - cl * nbt;
+      const BinConst bc = P.bins[b_first + k];
+      BinOpt bo;
+      bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gg = bc.gg[cl]; bo.pad = 0.0;
+      s_bin[cl * nbtS + k] = bo;
+    }
+  }
+  const int col_nan = P.ws_nan[col];
   __syncthreads();
 
   // ---------------- per-thread constants ----------------
@@ -523,155 +627,155 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   const int bl = b - b_first;
   const int warp = tid >> 5, lane = tid & 31;
   const bool warp_on = warp < nwa;          // a warp without any spectral point only joins the barriers
-  double *red_w = s_red + (size_t)warp * 3 * LP;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
+  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
   const bool want_beam = !TOA && (P.F_beam != nullptr);
 
   if (warp_on) {
-    ThreadConst tc;
-    {
-      const BinConst bc = P.bins[b];
-      tc.W = active ? bc.dlam * P.gauss_w[gidx] : 0.0;
-      tc.sb0 = bc.sb[0]; tc.sb1 = bc.sb[1];
-      tc.ss0 = bc.ss[0]; tc.ss1 = bc.ss[1];
-      tc.gg1 = bc.gg[1];
-      tc.muF = day ? mu * P.fstar[b] : 0.0;
-    }
+    const double W = active ? P.bins[b].dlam * P.gauss_w[gidx] : 0.0;    // dlam_b * w_g
+    const double muF = day ? mu * P.fstar[b] : 0.0;                      // mu * F_star[b]
     const double inv_mu = day ? 1.0 / mu : 0.0;
     const double *lnk_pt = P.lnk + pt;
-    const int strideT = P.npt, strideP = P.nT * P.npt;
-    const double *Bcol = s_B + bl;   // B[l] = Bcol[l * L.nbt]
-    const int nbtS = L.nbt;
+    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
     const double *T32 = s_T32;
+    double *stage_wr = stage_w + lane;
 
-    // back-substitution state, one entry per interface 1..N (thread-private, local memory:
-    // written top-down, read bottom-up -- a stack, served by L1/L2)
-    double2 st_cd[TOA ? 1 : MAXL];
-    double2 st_RU[TOA ? 1 : MAXL];
+    // back-substitution state per interface i = 0..N (thread-private stack in local memory, written top-down,
+    // read bottom-up): F_up[i] = c F_up[i-1] + d (weight folded into d) and R with F_dn[i] = R F_up[i] + U.
+    // U itself is not kept: sum_points W (U + beam) is reduced on the way down (flush_stage).
+    double2 st_cd[TOA ? 1 : MAXL + 1];
+    double st_R[TOA ? 1 : MAXL + 1];
 
-    // ---------------- sweep 1: TOA -> BOA ----------------
     double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
-    double tau = 0.0;
-    double Fb = tc.muF;                // beam at the TOA (full strength, L235)
+    double Fb = muF;                   // beam at the TOA (full strength, L235)
     double Ctoa = 1.0, Dtoa = 0.0;     // TOA mode: F_up[N] = Ctoa F_up[j] + Dtoa
-    if (want_beam) {
-      const double wb = warp_sum(tc.W * Fb);
-      if (lane == 0) red_w[2 * LP + N] = wb;
-    }
 
-    double kx_up = 0.0, w0_up = 0.0, g0_up = 0.0;   // non-iso: optics at the upper interface
-    Rows nx;                                        // k-table rows of the next level, loaded one level ahead
-    if (NONISO) {
-      const int l = 2 * N;
-      const Rows top = load_rows(lnk_pt, s_cell[l], strideT, strideP);
-      level_optics(top, T32, s_cw[l], s_cloud[l], tc, kx_up, w0_up, g0_up);
-      nx = load_rows(lnk_pt, s_cell[2 * N - 1], strideT, strideP);
-    } else {
-      nx = load_rows(lnk_pt, s_cell[N - 1], strideT, strideP);
-    }
-
-#pragma unroll 1
-    for (int j = N - 1; j >= 0; --j) {
-      double c, d;
-      const double R_top = R, U_top = U, Fb_top = Fb;
-      if (!NONISO) {
-        const Rows cur = nx;
-        if (j > 0) nx = load_rows(lnk_pt, s_cell[j - 1], strideT, strideP);
-        double kx, w0, g0;
-        level_optics(cur, T32, s_cw[j], s_cloud[j], tc, kx, w0, g0);
-        const double dtau = kx * s_dmfull[j];
-        tau += dtau;
-        double Fa = 0.0;
-        const double Bj = Bcol[j * nbtS];
-        if (day) {
-          Fa = tc.muF * exp_tab<1, false>(fmin(tau * inv_mu, 708.0), T32, nullptr);                 // (B6)
-          layer_forward<true, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, R, U, c, d);
-        } else {
-          layer_forward<false, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, 0.0, 0.0, R, U, c, d);
-        }
-        Fb = Fa;
-      } else {
-        // levels: 2j+2 (upper interface, carried), 2j+1 (centre), 2j (lower interface)
-        double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo;
-        const int lc = 2 * j + 1, ll = 2 * j;
-        const Rows rc = nx;
-        const Rows rl = load_rows(lnk_pt, s_cell[ll], strideT, strideP);
-        if (j > 0) nx = load_rows(lnk_pt, s_cell[ll - 1], strideT, strideP);
-        level_optics(rc, T32, s_cw[lc], s_cloud[lc], tc, kx_c, w0_c, g0_c);
-        level_optics(rl, T32, s_cw[ll], s_cloud[ll], tc, kx_lo, w0_lo, g0_lo);
-        const double B_up = Bcol[(lc + 1) * nbtS], B_c = Bcol[lc * nbtS], B_lo = Bcol[ll * nbtS];
-        // upper sub-layer: arithmetic means of centre and interface values (L171, reading R10)
-        const double dtau_u = 0.5 * (kx_c + kx_up) * s_dm[lc];
-        const double dtau_l = 0.5 * (kx_lo + kx_c) * s_dm[ll];
-        double cu, du, cl, dl;
-        if (day) {
-          tau += dtau_u;
-          const double Fc = tc.muF * exp_tab<1, false>(fmin(tau * inv_mu, 708.0), T32, nullptr);
-          layer_forward<true, true>(P, T32, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, Fc, Fb,
-                                    R, U, cu, du);
-          tau += dtau_l;
-          const double Fa = tc.muF * exp_tab<1, false>(fmin(tau * inv_mu, 708.0), T32, nullptr);
-          layer_forward<true, true>(P, T32, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, Fa, Fc,
-                                    R, U, cl, dl);
-          Fb = Fa;
-        } else {
-          layer_forward<false, true>(P, T32, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, 0.0,
-                                     0.0, R, U, cu, du);
-          layer_forward<false, true>(P, T32, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, 0.0,
-                                     0.0, R, U, cl, dl);
-        }
-        // F_up[j+1] = cu F_up[c] + du,  F_up[c] = cl F_up[j] + dl
-        c = cu * cl;
-        d = fma(cu, dl, du);
-        kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo;
-      }
-      if (TOA) {
-        Dtoa = fma(Ctoa, d, Dtoa);
-        Ctoa *= c;
-      } else {
-        // weights folded in: back-substitution runs on W F_up; F_dn carries the beam (L235)
-        st_cd[j] = make_double2(c, tc.W * d);
-        st_RU[j] = make_double2(R_top, tc.W * (U_top + Fb_top));
+    // bookkeeping of interface i with (R, U, Fb) at that interface
+    auto push_interface = [&](int i, double Ri, double Ui, double Fbi) {
+      if (!TOA) {
+        st_R[i] = Ri;
+        stage_wr[(i & 7) * STAGE_LD] = W * (Ui + Fbi);
+        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
         if (want_beam) {
-          const double wb = warp_sum(tc.W * Fb);
-          if (lane == 0) red_w[2 * LP + j] = wb;
+          const double wb = warp_sum(W * Fbi);
+          if (lane == 0) red_w[3 * LP + i] = wb;
         }
       }
-    }
+    };
+
+    // ---------------- sweep 1: TOA -> BOA (one instantiation per day / night: the loop body has no branch) ------
+    auto sweep1 = [&](auto day_tag) {
+      constexpr bool DAY = decltype(day_tag)::value;
+      double tau = 0.0;
+      if (!NONISO) {
+        const LevelRec *lv = s_lev + (N - 1);
+        const double *Bp = s_B + (size_t)(N - 1) * nbtS + bl;
+        Rows nx = load_rows(lnk_pt, lv);   // rows of the next level, loaded one level ahead
+#pragma unroll 2
+        for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
+          const Rows cur = nx;
+          nx = load_rows(lnk_pt, lv - 1);
+          push_interface(j + 1, R, U, Fb);
+          double kx, w0, g0, c, d;
+          level_optics(cur, T32, lv, bin0, bin1, kx, w0, g0);
+          const double dtau = kx * lv->dm;
+          const double Bj = *Bp;
+          double Fa = 0.0;
+          if (DAY) {
+            tau += dtau;
+            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);   // (B6)
+          }
+          layer_forward<DAY, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, R, U, c, d);
+          Fb = Fa;
+          if (TOA) {
+            Dtoa = fma(Ctoa, d, Dtoa);
+            Ctoa *= c;
+          } else {
+            st_cd[j + 1] = make_double2(c, W * d);
+          }
+        }
+      } else {
+        // levels alternate interface (even) / centre (odd); sub-layer s lies between levels s and s+1 and takes
+        // the arithmetic mean of the two levels' kappa_ext, omega0, g0 (L171, reading R10).  The centre unknowns
+        // are eliminated on the fly: F_up[j+1] = cu F_up[centre] + du, F_up[centre] = cl F_up[j] + dl.
+        const LevelRec *lv = s_lev + (nlev - 1);
+        const double *Bp = s_B + (size_t)(nlev - 1) * nbtS + bl;
+        double kx_up, w0_up, g0_up;
+        {
+          const Rows top = load_rows(lnk_pt, lv);
+          level_optics(top, T32, lv, bin0, bin1, kx_up, w0_up, g0_up);
+        }
+        double B_up = *Bp;
+        Rows nxc = load_rows(lnk_pt, lv - 1);   // centre and lower interface of the next layer, one layer ahead
+        Rows nxl = load_rows(lnk_pt, lv - 2);
+#pragma unroll 1
+        for (int j = N - 1; j >= 0; --j, lv -= 2, Bp -= 2 * nbtS) {
+          const Rows rc = nxc, rl = nxl;
+          nxc = load_rows(lnk_pt, lv - 3);
+          nxl = load_rows(lnk_pt, (j > 0) ? lv - 4 : lv - 3);
+          push_interface(j + 1, R, U, Fb);
+          double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo, cu, du, cl, dl;
+          level_optics(rc, T32, lv - 1, bin0, bin1, kx_c, w0_c, g0_c);
+          level_optics(rl, T32, lv - 2, bin0, bin1, kx_lo, w0_lo, g0_lo);
+          const double B_c = Bp[-nbtS], B_lo = Bp[-2 * nbtS];
+          const double dtau_u = 0.5 * (kx_c + kx_up) * lv[-1].dm;
+          const double dtau_l = 0.5 * (kx_lo + kx_c) * lv[-2].dm;
+          double Fc = 0.0, Fa = 0.0;
+          if (DAY) {
+            const double tau_c = tau + dtau_u;
+            tau = tau_c + dtau_l;
+            Fc = muF * exp_hot<1, false>(min_pos(tau_c * inv_mu, 708.0), T32, nullptr);   // (B6)
+            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
+          }
+          layer_forward<DAY, true>(P, T32, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, Fc, Fb,
+                                   R, U, cu, du);
+          layer_forward<DAY, true>(P, T32, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, Fa, Fc,
+                                   R, U, cl, dl);
+          Fb = Fa;
+          kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo; B_up = B_lo;
+          const double cc = cu * cl, dd = fma(cu, dl, du);
+          if (TOA) {
+            Dtoa = fma(Ctoa, dd, Dtoa);
+            Ctoa *= cc;
+          } else {
+            st_cd[j + 1] = make_double2(cc, W * dd);
+          }
+        }
+      }
+    };
+    if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
 
     // ---------------- BOA, Eq.(10) L237 ----------------
-    const double F_boa = Bcol[nlev * nbtS];
+    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
     const double Fup0 = (U + F_boa + Fb) * rcp_fast(1.0 - R);
-    const double Fdn0 = fma(R, Fup0, U);
 
     if (TOA) {
       // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
       const double FupN = fma(Ctoa, Fup0, Dtoa);
       s_vals[tid] = active ? P.gauss_w[gidx] * FupN : 0.0;
     } else {
-      // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 levels at a time ----------------
-      double wFup = tc.W * Fup0;
-      double wFdn = tc.W * (Fdn0 + Fb);
+      push_interface(0, R, U, Fb);
+      st_cd[0] = make_double2(0.0, W * Fup0);
+      // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 interfaces at a time ----------------
+      double wFup = 0.0;
 #pragma unroll 1
       for (int base = 0; base <= N; base += 8) {
         double v[16];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-          const int e = base + k - 1;                       // stack entry that lifts level base+k-1 to base+k
-          const int ec = e < 0 ? 0 : (e > N - 1 ? N - 1 : e);
-          const double2 cd = st_cd[ec];
-          const double2 RU = st_RU[ec];
-          const bool upd = (e >= 0) && (e < N);
+          const int i = base + k;
+          const bool on = i <= N;
+          const int ic = on ? i : N;
+          const double2 cd = st_cd[ic];
+          const double Ri = st_R[ic];
           const double nu = fma(cd.x, wFup, cd.y);
-          const double nd = fma(RU.x, nu, RU.y);
-          wFup = upd ? nu : wFup;
-          wFdn = upd ? nd : wFdn;
-          const bool on = (base + k) <= N;
-          v[k] = on ? wFup : 0.0;
-          v[8 + k] = on ? wFdn : 0.0;
+          wFup = on ? nu : wFup;
+          v[k] = on ? nu : 0.0;
+          v[8 + k] = on ? Ri * nu : 0.0;
         }
         const double tot = warp_reduce16(v, lane);
-        const int idx = lane >> 1, lev = base + (idx & 7);
-        if (!(lane & 1) && lev <= N) red_w[(idx >> 3) * LP + lev] = tot;
+        const int idx = lane >> 1;
+        if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
       }
       if (P.F_toa_bin != nullptr) s_vals[tid] = active ? wFup * P.bins[b].inv_dlam : 0.0;
     }
@@ -688,7 +792,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
       const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
       if (g_lo < 0) g_lo = 0;
       if (g_hi > BLOCK) g_hi = BLOCK;
-      double sum = s_nan ? nan("") : 0.0;
+      double sum = col_nan ? nan("") : 0.0;
       for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
       double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
       if (whole) *dst = sum; else atomicAdd(dst, sum);
@@ -696,20 +800,20 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
   }
   if (TOA) return;
 
-  // cross-warp sum in fixed order -> tile partial
-  const int nq = want_beam ? 3 : 2;
+  // cross-warp sum in fixed order -> tile partial: F_up, R F_up, U + beam, beam
+  const int nq = want_beam ? 4 : 3;
   const int nred = nq * (N + 1);
   for (int k = tid; k < nred; k += BLOCK) {
     const int q = k / (N + 1), lev = k - q * (N + 1);
     double sum = 0.0;
-    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 3 * LP + q * LP + lev];
+    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
     s_fin[k] = sum;
   }
   __syncthreads();
 
   if (P.tiles > 1) {
     // publish the tile partial; the last tile of the column to arrive sums them in tile order
-    double *part = P.partial + ((size_t)col * P.tiles + tile) * 3 * (N + 1);
+    double *part = P.partial + ((size_t)col * P.tiles + tile) * 4 * (N + 1);
     for (int k = tid; k < nred; k += BLOCK) part[k] = s_fin[k];
     __threadfence();
     __syncthreads();
@@ -721,34 +825,31 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_step_kernel(const KParams P) {
     __syncthreads();
     if (!s_is_last) return;
     __threadfence();
-    const double *pall = P.partial + (size_t)col * P.tiles * 3 * (N + 1);
+    const double *pall = P.partial + (size_t)col * P.tiles * 4 * (N + 1);
     for (int k = tid; k < nred; k += BLOCK) {
       double sum = 0.0;
-      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 3 * (N + 1) + k);
+      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 4 * (N + 1) + k);
       s_fin[k] = sum;
     }
     __syncthreads();
   }
 
-  // final outputs of the column
-  if (s_nan) {
-    __syncthreads();
-    for (int k = tid; k < 3 * (N + 1); k += BLOCK) s_fin[k] = nan("");
-    __syncthreads();
-  }
+  // final outputs of the column: F_down = sum W R F_up + sum W (U + beam)
+  const double poison = col_nan ? nan("") : 0.0;
   for (int i = tid; i <= N; i += BLOCK) {
     const size_t o = (size_t)col * (N + 1) + i;
-    const double fu = s_fin[i], fd = s_fin[N + 1 + i];
+    const double fu = s_fin[i] + poison, fd = s_fin[N + 1 + i] + s_fin[2 * (N + 1) + i] + poison;
     if (P.F_up) P.F_up[o] = fu;
     if (P.F_down) P.F_down[o] = fd;
     if (P.F_net) P.F_net[o] = fu - fd;
-    if (want_beam) P.F_beam[o] = s_fin[2 * (N + 1) + i];
+    if (want_beam) P.F_beam[o] = s_fin[3 * (N + 1) + i] + poison;
   }
   if (P.dTdt) {
+    const double *dm = P.ws_dm + (size_t)col * N;
     for (int j = tid; j < N; j += BLOCK) {
-      const double fn1 = s_fin[j + 1] - s_fin[N + 1 + j + 1];
-      const double fn0 = s_fin[j] - s_fin[N + 1 + j];
-      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / s_dmfull[j];   // reading R14
+      const double fn1 = s_fin[j + 1] - (s_fin[N + 1 + j + 1] + s_fin[2 * (N + 1) + j + 1]);
+      const double fn0 = s_fin[j] - (s_fin[N + 1 + j] + s_fin[2 * (N + 1) + j]);
+      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / dm[j] + poison;   // reading R14
     }
   }
 }
@@ -773,9 +874,9 @@ __global__ void selftest_math_kernel(int n, const double *x, double *rcp, double
   // e^-|x| through the three entry points the step kernel uses: e^-a, e^-2(a/2) (+ 1 - e^-a), e^(-a)
   const double a = fmin(fabs(v), 708.0);
   double om;
-  const double e2 = exp_tab<2, true>(0.5 * a, T32, &om);
-  const double e1 = exp_tab<1, false>(a, T32, nullptr);
-  const double e0 = exp_tab<0, false>(-a, T32, nullptr);
+  const double e2 = exp_hot<2, true>(0.5 * a, T32, &om);
+  const double e1 = exp_hot<1, false>(a, T32, nullptr);
+  const double e0 = exp_hot<0, false>(-a, T32, nullptr);
   ex[i] = (i % 3 == 0) ? e0 : ((i % 3 == 1) ? e1 : e2);
   omx[i] = om;
 }
@@ -819,10 +920,9 @@ struct KernelChoice {
 
 template <bool NONISO, bool TOA>
 KernelChoice pick_kernel(int block, int minb) {
-#define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_step_kernel<NONISO, TOA, B, M>, B};
+#define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, B, M>, B};
   HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(128, 4) HRT_VARIANT(160, 3) HRT_VARIANT(320, 2) HRT_VARIANT(608, 1)
-  HRT_VARIANT(160, 4) HRT_VARIANT(128, 5) HRT_VARIANT(128, 6) HRT_VARIANT(128, 7) HRT_VARIANT(128, 8)
-  HRT_VARIANT(64, 10) HRT_VARIANT(64, 12) HRT_VARIANT(64, 14) HRT_VARIANT(96, 7) HRT_VARIANT(96, 8)
+  HRT_VARIANT(160, 4) HRT_VARIANT(128, 5) HRT_VARIANT(64, 10) HRT_VARIANT(96, 7) HRT_VARIANT(320, 1) HRT_VARIANT(128, 3)
 #undef HRT_VARIANT
   return {nullptr, 0};
 }
@@ -834,21 +934,33 @@ KernelChoice pick(bool noniso, bool toa, int block, int minb) {
 
 const int kBlocks[] = {32, 64, 96, 128, 160, 320, 608};
 
-// block size: fewest padded lanes over the column, ties -> larger block (fewer tiles)
+// block size: columns with many spectral points use 128-thread tiles (4-5 resident blocks per SM keep the fp64
+// pipe fed while other blocks sit in their prologue or reductions: measured best on configs 2-5); small
+// columns take the block with the fewest padded lanes, ties -> larger block (fewer tiles)
 int choose_block(int npt) {
   const char *env = getenv("HELIOS_RT_BLOCK");
   if (env) {
     const int v = atoi(env);
     for (int b : kBlocks) if (b == v) return v;
   }
+  if (npt >= 256) return 128;
   int best = 32;
   long best_waste = -1;
-  for (int b : kBlocks) {
+  for (int b : {32, 64, 96, 128}) {
     const long tiles = (npt + b - 1) / b;
     const long waste = tiles * (long)(((b + 31) / 32) * 32) - npt;
     if (best_waste < 0 || waste < best_waste || (waste == best_waste && b > best)) { best = b; best_waste = waste; }
   }
   return best;
+}
+
+// resident blocks per SM the kernel is compiled for (register cap): isothermal 128 x 5 (96 registers),
+// non-isothermal 128 x 4 (128 registers)
+int choose_minb(int block, bool noniso) {
+  const char *mb = getenv("HELIOS_RT_MINB");
+  if (mb) return atoi(mb);
+  if (block == 128) return noniso ? 4 : 5;
+  return 0;
 }
 
 }  // namespace
@@ -858,12 +970,16 @@ struct helios_rt {
   int npt, block, tiles;
   bool noniso, toa;
   KernelChoice kc;
-  SmemLayout lay;
+  SolveSmem lay;
+  int nlev;
   // device tables
   double *d_lnk, *d_tab_lp, *d_tab_t, *d_edges, *d_gw;
   BinConst *d_bins;
   double *d_partial;
   unsigned *d_counter;
+  LevelRec *d_ws_lev;
+  double *d_ws_B, *d_ws_dm;
+  int *d_ws_nan;
   // device staging for step_host
   double *d_p, *d_T, *d_mu, *d_fstar, *d_out;   // d_out: 5*(N+1)+N+nb per column, carved per output
   cudaStream_t own_stream;
@@ -914,6 +1030,7 @@ static int validate_config(const helios_rt_config *c) {
       c->n_ktab_t < 2 || c->max_columns < 1)
     return HELIOS_RT_EINVAL;
   if ((long long)c->n_bins * c->n_gauss > (1 << 24)) return HELIOS_RT_EINVAL;
+  if ((long long)c->n_ktab_p * c->n_ktab_t * c->n_bins * c->n_gauss >= (1LL << 31)) return HELIOS_RT_EINVAL;   // 32-bit table offsets
   if (!c->ktab_p || !c->ktab_t || !c->ktab || !c->bin_edges || !c->gauss_w || !c->scat_gas || !c->cloud_ext ||
       !c->cloud_w0 || !c->cloud_g0)
     return HELIOS_RT_EINVAL;
@@ -949,6 +1066,7 @@ extern "C" int helios_rt_destroy(helios_rt *h) {
   if (!h) return HELIOS_RT_OK;
   cudaFree(h->d_lnk); cudaFree(h->d_tab_lp); cudaFree(h->d_tab_t); cudaFree(h->d_edges); cudaFree(h->d_gw);
   cudaFree(h->d_bins); cudaFree(h->d_partial); cudaFree(h->d_counter);
+  cudaFree(h->d_ws_lev); cudaFree(h->d_ws_B); cudaFree(h->d_ws_dm); cudaFree(h->d_ws_nan);
   cudaFree(h->d_p); cudaFree(h->d_T); cudaFree(h->d_mu); cudaFree(h->d_fstar); cudaFree(h->d_out);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   delete h;
@@ -974,8 +1092,9 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
   h->block = choose_block(h->npt);
   h->tiles = (h->npt + h->block - 1) / h->block;
-  { const char *mb = getenv("HELIOS_RT_MINB"); h->kc = pick(h->noniso, h->toa, h->block, mb ? atoi(mb) : 0); }
-  h->lay = smem_layout(N, h->noniso, h->block, ng, nb);
+  h->kc = pick(h->noniso, h->toa, h->block, choose_minb(h->block, h->noniso));
+  h->nlev = h->noniso ? 2 * N + 1 : N;
+  h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa);
   cudaGetDevice(&rc);
   cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, rc);
 
@@ -1006,7 +1125,11 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(upload(&h->d_bins, bins, (size_t)nb));
   free(lnk); free(lp); free(bins);
   const size_t ncol = (size_t)cfg->max_columns;
-  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * h->tiles * 3 * (N + 1)));
+  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * h->tiles * 4 * (N + 1)));
+  step(cudaMalloc((void **)&h->d_ws_lev, sizeof(LevelRec) * ncol * (h->nlev + 1)));
+  step(cudaMalloc((void **)&h->d_ws_B, sizeof(double) * ncol * (h->nlev + 1) * nb));
+  step(cudaMalloc((void **)&h->d_ws_dm, sizeof(double) * ncol * N));
+  step(cudaMalloc((void **)&h->d_ws_nan, sizeof(int) * ncol));
   step(cudaMalloc((void **)&h->d_counter, sizeof(unsigned) * ncol));
   if (e == cudaSuccess) step(cudaMemset(h->d_counter, 0, sizeof(unsigned) * ncol));
   step(cudaMalloc((void **)&h->d_p, sizeof(double) * ncol * N));
@@ -1017,6 +1140,8 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
   if (e == cudaSuccess && h->kc.fn) {
     step(cudaFuncSetAttribute(h->kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
+    step(cudaFuncSetAttribute(h->noniso ? rt_prep_kernel<true> : rt_prep_kernel<false>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prep_smem_bytes(N, h->nlev)));
     cudaFuncAttributes fa;
     step(cudaFuncGetAttributes(&fa, h->kc.fn));
     if (e == cudaSuccess) { h->regs = fa.numRegs; h->lmem = (int)fa.localSizeBytes; }
@@ -1050,7 +1175,7 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   KParams P;
   P.lnk = h->d_lnk; P.tab_lp = h->d_tab_lp; P.tab_t = h->d_tab_t; P.edges = h->d_edges; P.gauss_w = h->d_gw;
   P.bins = h->d_bins;
-  P.nP = c.n_ktab_p; P.nT = c.n_ktab_t; P.N = c.n_layers; P.nb = c.n_bins; P.ng = c.n_gauss; P.npt = h->npt;
+  P.nP = c.n_ktab_p; P.nT = c.n_ktab_t; P.N = c.n_layers; P.nlev = h->nlev; P.nb = c.n_bins; P.ng = c.n_gauss; P.npt = h->npt;
   P.tiles = h->tiles;
   P.cloud_p_top = c.cloud_p_top; P.cloud_p_bot = c.cloud_p_bot; P.inv_g = 1.0 / c.gravity; P.inv_cp = 1.0 / c.cp;
   P.inv_eps2 = 1.0 / c.eps2; P.e_tau = c.e_tau; P.gcrit_tol = c.gcrit_tol; P.w0_transition = c.w0_transition;
@@ -1060,11 +1185,17 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.F_up = out->F_up; P.F_down = out->F_down; P.F_net = out->F_net; P.dTdt = out->dTdt; P.F_beam = out->F_beam;
   P.F_toa_bin = out->F_up_toa_bin;
   P.partial = h->d_partial; P.counter = h->d_counter;
+  P.ws_lev = h->d_ws_lev; P.ws_B = h->d_ws_B; P.ws_dm = h->d_ws_dm; P.ws_nan = h->d_ws_nan;
   // bins that straddle two tiles are accumulated with atomics: start from zero
   if (P.F_toa_bin && h->tiles > 1 && (h->block % c.n_gauss) != 0) {
     const size_t n = (size_t)in->n_columns * c.n_bins;
     zero_kernel<<<(unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, st>>>(P.F_toa_bin, n);
   }
+  dim3 pgrid((unsigned)((c.n_bins + PREP_BINS - 1) / PREP_BINS), (unsigned)in->n_columns);
+  const size_t psm = prep_smem_bytes(c.n_layers, h->nlev);
+  if (h->noniso) rt_prep_kernel<true><<<pgrid, PREP_BLOCK, psm, st>>>(P);
+  else rt_prep_kernel<false><<<pgrid, PREP_BLOCK, psm, st>>>(P);
+  CK(h, cudaGetLastError());
   dim3 grid((unsigned)h->tiles, (unsigned)in->n_columns);
   h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
   CK(h, cudaGetLastError());
@@ -1116,7 +1247,7 @@ extern "C" int helios_rt_launch_info(const helios_rt *h, int32_t info[8]) {
   if (!h || !info) return HELIOS_RT_EINVAL;
   info[0] = h->block; info[1] = h->tiles; info[2] = (int32_t)h->lay.total; info[3] = h->regs; info[4] = h->occ;
   info[5] = h->lmem;
-  info[6] = 1;   // (+1 zero-fill launch when F_up_toa_bin bins straddle tiles)
+  info[6] = 2;   // rt_prep_kernel + rt_solve_kernel (+1 zero-fill launch when F_up_toa_bin bins straddle tiles)
   info[7] = h->sm_count;
   return HELIOS_RT_OK;
 }
