@@ -137,6 +137,16 @@ const char *helios_rt_last_cuda_error(const helios_rt *h);
  * bytes per thread, [6] = kernels launched per step, [7] = SM count of the device. */
 int helios_rt_launch_info(const helios_rt *h, int32_t info[8]);
 
+/* Per-kernel timing for benchmarks.  With profiling on, every step records three CUDA events on the
+ * launching stream (before rt_prep_kernel, between the two kernels, after rt_solve_kernel) into a ring of
+ * 256 steps; no synchronisation is added.  Turning it on or off clears the ring. */
+int helios_rt_set_profiling(helios_rt *h, int32_t on);
+
+/* Waits for the recorded steps (at most the last 256 since the previous call) and returns their number
+ * and the SUMS of the two kernels' event times in milliseconds: S1+S2 (rt_prep_kernel) and S3-S7
+ * (rt_solve_kernel, the dominant kernel of the roofline).  Clears the ring. */
+int helios_rt_kernel_times(helios_rt *h, int32_t *n_steps, double *prep_ms, double *solve_ms);
+
 /* Device self-test of the fp64 primitives the kernels use instead of the CUDA math library
  * (reciprocal, reciprocal square root, exp / 1-exp).  x: n HOST values; outputs n HOST values each:
  * rcp = 1/x, rsq = 1/sqrt(|x|), ex = exp(-|x|), omx = 1 - exp(-|x|).  Used by the tests. */

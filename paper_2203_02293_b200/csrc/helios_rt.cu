@@ -985,7 +985,13 @@ struct helios_rt {
   cudaStream_t own_stream;
   int regs, lmem, occ, sm_count;
   cudaError_t last_err;
+  // per-kernel timing (helios_rt_set_profiling): a ring of event triples (before prep, between, after solve)
+  int profiling;
+  cudaEvent_t *prof_ev;      // [kProfRing][3]
+  long long prof_head;       // triples recorded since the last read
 };
+
+constexpr int kProfRing = 256;
 
 #define CK(h, call)                                                   \
   do {                                                                \
@@ -1069,6 +1075,10 @@ extern "C" int helios_rt_destroy(helios_rt *h) {
   cudaFree(h->d_ws_lev); cudaFree(h->d_ws_B); cudaFree(h->d_ws_dm); cudaFree(h->d_ws_nan);
   cudaFree(h->d_p); cudaFree(h->d_T); cudaFree(h->d_mu); cudaFree(h->d_fstar); cudaFree(h->d_out);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  if (h->prof_ev) {
+    for (int i = 0; i < 3 * kProfRing; ++i) if (h->prof_ev[i]) cudaEventDestroy(h->prof_ev[i]);
+    free(h->prof_ev);
+  }
   delete h;
   return HELIOS_RT_OK;
 }
@@ -1191,14 +1201,18 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
     const size_t n = (size_t)in->n_columns * c.n_bins;
     zero_kernel<<<(unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, st>>>(P.F_toa_bin, n);
   }
+  cudaEvent_t *ev = h->profiling ? h->prof_ev + 3 * (h->prof_head % kProfRing) : nullptr;
+  if (ev) CK(h, cudaEventRecord(ev[0], st));
   dim3 pgrid((unsigned)((c.n_bins + PREP_BINS - 1) / PREP_BINS), (unsigned)in->n_columns);
   const size_t psm = prep_smem_bytes(c.n_layers, h->nlev);
   if (h->noniso) rt_prep_kernel<true><<<pgrid, PREP_BLOCK, psm, st>>>(P);
   else rt_prep_kernel<false><<<pgrid, PREP_BLOCK, psm, st>>>(P);
   CK(h, cudaGetLastError());
+  if (ev) CK(h, cudaEventRecord(ev[1], st));
   dim3 grid((unsigned)h->tiles, (unsigned)in->n_columns);
   h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
   CK(h, cudaGetLastError());
+  if (ev) { CK(h, cudaEventRecord(ev[2], st)); ++h->prof_head; }
   return HELIOS_RT_OK;
 }
 
@@ -1240,6 +1254,36 @@ extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, con
   if (out->F_up_toa_bin)
     CK(h, cudaMemcpyAsync(out->F_up_toa_bin, dout.F_up_toa_bin, sizeof(double) * ncol * nb, cudaMemcpyDeviceToHost, st));
   CK(h, cudaStreamSynchronize(st));
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_set_profiling(helios_rt *h, int32_t on) {
+  if (!h) return HELIOS_RT_EINVAL;
+  if (on && !h->prof_ev) {
+    h->prof_ev = (cudaEvent_t *)calloc(3 * kProfRing, sizeof(cudaEvent_t));
+    if (!h->prof_ev) return HELIOS_RT_ENOMEM;
+    for (int i = 0; i < 3 * kProfRing; ++i) CK(h, cudaEventCreate(&h->prof_ev[i]));
+  }
+  h->profiling = on ? 1 : 0;
+  h->prof_head = 0;
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_kernel_times(helios_rt *h, int32_t *n_steps, double *prep_ms, double *solve_ms) {
+  if (!h || !n_steps || !prep_ms || !solve_ms) return HELIOS_RT_EINVAL;
+  *n_steps = 0; *prep_ms = 0.0; *solve_ms = 0.0;
+  if (!h->prof_ev) return HELIOS_RT_OK;
+  const long long n = h->prof_head < kProfRing ? h->prof_head : kProfRing;
+  for (long long k = h->prof_head - n; k < h->prof_head; ++k) {
+    cudaEvent_t *ev = h->prof_ev + 3 * (k % kProfRing);
+    CK(h, cudaEventSynchronize(ev[2]));
+    float a = 0.f, b = 0.f;
+    CK(h, cudaEventElapsedTime(&a, ev[0], ev[1]));
+    CK(h, cudaEventElapsedTime(&b, ev[1], ev[2]));
+    *prep_ms += a; *solve_ms += b;
+  }
+  *n_steps = (int32_t)n;
+  h->prof_head = 0;
   return HELIOS_RT_OK;
 }
 

@@ -18,6 +18,7 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
            "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info",
+           "helios_rt_set_profiling", "helios_rt_kernel_times",
            "helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_measure_dfma_peak")
 
 
@@ -69,6 +70,10 @@ def load_library() -> C.CDLL:
         L.helios_rt_last_cuda_error.argtypes = [C.c_void_p]
         L.helios_rt_launch_info.restype = C.c_int
         L.helios_rt_launch_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.helios_rt_set_profiling.restype = C.c_int
+        L.helios_rt_set_profiling.argtypes = [C.c_void_p, C.c_int32]
+        L.helios_rt_kernel_times.restype = C.c_int
+        L.helios_rt_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_int32), _dp, _dp]
         L.helios_rt_selftest_math.restype = C.c_int
         L.helios_rt_selftest_math.argtypes = [C.c_int32] + [_dp] * 5
         L.helios_rt_selftest_planck.restype = C.c_int
@@ -141,6 +146,15 @@ class HeliosRT:
         keys = ("block", "tiles", "smem_bytes", "registers", "blocks_per_sm", "local_bytes", "launches_per_step",
                 "sm_count")
         return dict(zip(keys, list(info)))
+
+    def set_profiling(self, on: bool) -> None:
+        _check(load_library().helios_rt_set_profiling(self._h, 1 if on else 0), self._h)
+
+    def kernel_times(self) -> tuple[int, float, float]:
+        """(steps recorded, sum of rt_prep_kernel ms, sum of rt_solve_kernel ms) since the last call."""
+        n, a, b = C.c_int32(), C.c_double(), C.c_double()
+        _check(load_library().helios_rt_kernel_times(self._h, C.byref(n), C.byref(a), C.byref(b)), self._h)
+        return n.value, a.value, b.value
 
     def step(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict, stream=None) -> None:
         """Device step: torch CUDA float64 contiguous tensors; `out` maps output names to pre-allocated
