@@ -922,7 +922,7 @@ template <bool NONISO, bool TOA>
 KernelChoice pick_kernel(int block, int minb) {
 #define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, B, M>, B};
   HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(128, 4) HRT_VARIANT(160, 3) HRT_VARIANT(320, 2) HRT_VARIANT(608, 1)
-  HRT_VARIANT(160, 4) HRT_VARIANT(128, 5) HRT_VARIANT(64, 10) HRT_VARIANT(96, 7) HRT_VARIANT(320, 1) HRT_VARIANT(128, 3)
+  HRT_VARIANT(160, 4) HRT_VARIANT(128, 6) HRT_VARIANT(128, 5) HRT_VARIANT(64, 10) HRT_VARIANT(96, 7) HRT_VARIANT(320, 1) HRT_VARIANT(128, 3)
 #undef HRT_VARIANT
   return {nullptr, 0};
 }

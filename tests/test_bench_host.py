@@ -66,8 +66,8 @@ def test_algorithmic_work_is_the_locked_count():
     meta = dict(n_columns=2562, n_layers=40, n_bins=30, n_gauss=20)
     mu = np.r_[np.full(1281, 0.5), np.full(1281, -0.5)]
     slots = bench.algorithmic_slots(meta, 1, mu)
-    assert slots == 40 * 600 * (1281 * 232.0 + 1281 * 160.0)
-    assert bench.algorithmic_slots(meta, 3, mu) == 40 * 600 * (1281 * 544.0 + 1281 * 400.0)
+    assert slots == 40 * 600 * (1281 * 156.0 + 1281 * 108.0)
+    assert bench.algorithmic_slots(meta, 3, mu) == 40 * 600 * (1281 * 368.0 + 1281 * 272.0)
     cfg = dict(ktab=np.zeros((20, 30, 30, 20)))
     b = bench.algorithmic_bytes(meta, cfg, toa=False)
     assert b == 8 * (2 * 2562 * 40 + 2562 + 30) + 8 * (3 * 2562 * 41 + 2562 * 40) + 20 * 30 * 600 * 8
