@@ -58,7 +58,7 @@ class _Config(C.Structure):
                                    "cloud_ext", "cloud_w0", "cloud_g0")] + \
                [(n, C.c_double) for n in ("cloud_p_top", "cloud_p_bot", "gravity", "cp", "eps2",
                                           "e_tau", "gcrit_tol", "w0_transition", "f_toa")] + \
-               [("flags", C.c_uint32)]
+               [("flags", C.c_uint32), ("n_iterations", C.c_int32)]
 
 
 class _Inputs(C.Structure):
@@ -88,6 +88,8 @@ def lib(real: str = "ld") -> C.CDLL:
         mono = [C.c_int] + [_dp] * 5 + [C.c_double] * 8 + [C.c_int] * 2
         L.oracle_column_mono.restype = None
         L.oracle_column_mono.argtypes = mono + [_dp] * 3
+        L.oracle_column_mono_iter.restype = None
+        L.oracle_column_mono_iter.argtypes = mono + [C.c_int] + [_dp] * 3
         L.oracle_assemble_blocks.restype = None
         L.oracle_assemble_blocks.argtypes = mono + [_dp] * 5
         L.oracle_rt_step.restype = C.c_int
@@ -160,6 +162,15 @@ def column_mono(dtau, w0, g0, B_lo, B_hi, mu, Fstar, F_boa, *, improved=True, li
     return fu, fd, fb
 
 
+def column_mono_iter(dtau, w0, g0, B_lo, B_hi, mu, Fstar, F_boa, n_iter, *, improved=True, linear_source=False,
+                     real="ld", **opts):
+    """The pair-wise iterative scheme Thomas replaces, n_iter iterations from zero fluxes."""
+    L, keep, args = _mono_args(dtau, w0, g0, B_lo, B_hi, mu, Fstar, F_boa, improved, linear_source, opts)
+    fu, fd, fb = np.empty(L + 1), np.empty(L + 1), np.empty(L + 1)
+    lib(real).oracle_column_mono_iter(*args, int(n_iter), _p(fu), _p(fd), _p(fb))
+    return fu, fd, fb
+
+
 def assemble_blocks(dtau, w0, g0, B_lo, B_hi, mu, Fstar, F_boa, *, improved=True, linear_source=False,
                     real="ld", **opts):
     """The 2x2 blocks A, B, C [L+1,2,2], D [L+1,2] of Eq.(12) and F_beam [L+1]."""
@@ -196,7 +207,7 @@ def rt_step(cfg: dict, inp: dict, *, real: str = "ld", threads: int | None = Non
                 _p(keep["gauss_w"]), _p(keep["scat_gas"]), _p(keep["cloud_ext"]), _p(keep["cloud_w0"]),
                 _p(keep["cloud_g0"]), float(cfg["cloud_p_top"]), float(cfg["cloud_p_bot"]),
                 float(cfg["gravity"]), float(cfg["cp"]), o["eps2"], o["e_tau"], o["gcrit_tol"],
-                o["w0_transition"], o["f_toa"], int(cfg["flags"]))
+                o["w0_transition"], o["f_toa"], int(cfg["flags"]), int(cfg.get("n_iterations", 0)))
     i = _Inputs(ncol, _p(p), _p(T), _p(keep["mu_star"]), _p(keep["stellar_flux"]), float(inp["f_internal"]))
     shapes = dict(F_up=(ncol, N + 1), F_down=(ncol, N + 1), F_net=(ncol, N + 1), dTdt=(ncol, N),
                   F_beam=(ncol, N + 1), F_up_toa_bin=(ncol, nb))

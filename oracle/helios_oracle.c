@@ -20,7 +20,9 @@
  * across one layer; dense LU of the assembled system; the converged pair-wise iteration the
  * paper replaces; pure-absorption closed form; conservative scattering; opaque isothermal
  * limit; layer-splitting exactness; BOA condition; Planck integrals vs quadrature and
- * sigma*T^4; bilinear reproduction; guard branches; 40-digit worked example.
+ * sigma*T^4; bilinear reproduction; guard branches; 40-digit worked example.  The pair-wise
+ * iteration (column_mono_iterative) is pinned by its limit (= dense LU of the system) and by
+ * the non-scattering case, where one iteration is already the closed form.
  *
  * Index conventions (SURVEY.md "Conventions"): layer j (0..N-1) lies between interface j
  * (lower) and j+1 (upper); interface 0 = BOA, interface N = TOA; tau measured from the TOA
@@ -389,6 +391,57 @@ static void column_mono(int L, const real *dtau, const real *w0, const real *g0,
     free(r);
 }
 
+/* The scheme Thomas's algorithm replaces (L258-270, L397): "iterate the two-stream solutions, across the
+ * entire atmosphere, for a finite number of times" (N = 200 in HELIOS, ~10 in Oreshenko et al. 2016).
+ * Reading R23 (the paper does not print the sweep): all diffuse fluxes start at 0; one iteration is one upward
+ * pass -- Eq.(10) at the BOA, then Eq.(2)/(4),(7) layer by layer with the downward fluxes of the previous
+ * iteration -- followed by one downward pass -- F_dn,top = f_toa, then Eq.(3)/(6),(9) with the upward fluxes just
+ * computed.  The rows are exactly those of assemble():
+ *   chi F_up[s+1] = psi F_up[s] - xi F_dn[s+1] + rhs_up[s],   chi F_dn[s] = psi F_dn[s+1] - xi F_up[s] + rhs_dn[s]. */
+static void column_mono_iterative(int L, const real *dtau, const real *w0, const real *g0, const real *B_lo,
+                                  const real *B_hi, real mu, real Fstar, real F_boa, const rt_opts *o,
+                                  int n_iter, real *F_up, real *F_dn, real *F_beam)
+{
+    int n = L + 1;
+    real *r = malloc(sizeof(real) * 14 * n);
+    real *A = r, *Bm = A + 4 * n, *C = Bm + 4 * n, *D = C + 4 * n;
+    assemble(L, dtau, w0, g0, B_lo, B_hi, mu, Fstar, F_boa, o, A, Bm, C, D, F_beam);
+    for (int l = 0; l < n; ++l) { F_up[l] = 0; F_dn[l] = 0; }
+    for (int it = 0; it < n_iter; ++it) {
+        F_up[0] = F_dn[0] + D[0];                                   /* Eq.(10): D[0] = F_BOA + F_beam[0] */
+        for (int s = 0; s < L; ++s) {                               /* upward pass */
+            real chi = Bm[(s + 1) * 4 + 0], xi = Bm[(s + 1) * 4 + 1], psi = -A[(s + 1) * 4 + 0];
+            F_up[s + 1] = (psi * F_up[s] - xi * F_dn[s + 1] + D[(s + 1) * 2 + 0]) / chi;
+        }
+        F_dn[L] = D[L * 2 + 1];                                     /* f_toa */
+        for (int s = L - 1; s >= 0; --s) {                          /* downward pass */
+            real xi = Bm[s * 4 + 2], chi = Bm[s * 4 + 3], psi = -C[s * 4 + 3];
+            F_dn[s] = (psi * F_dn[s + 1] - xi * F_up[s] + D[s * 2 + 1]) / chi;
+        }
+    }
+    free(r);
+}
+
+void oracle_column_mono_iter(int L, const double *dtau, const double *w0, const double *g0,
+                             const double *B_lo, const double *B_hi, double mu, double Fstar,
+                             double F_boa, double eps2, double e_tau, double gcrit_tol,
+                             double w0_transition, double f_toa, int improved, int linear_source,
+                             int n_iter, double *F_up, double *F_dn, double *F_beam)
+{
+    rt_opts o = make_opts(eps2, e_tau, gcrit_tol, w0_transition, f_toa, improved, linear_source);
+    int n = L + 1;
+    real *r = malloc(sizeof(real) * (5 * L + 3 * n));
+    real *dt = r, *w = dt + L, *g = w + L, *bl = g + L, *bh = bl + L;
+    real *fu = bh + L, *fd = fu + n, *fb = fd + n;
+    for (int s = 0; s < L; ++s) {
+        dt[s] = (real)dtau[s]; w[s] = (real)w0[s]; g[s] = (real)g0[s];
+        bl[s] = (real)B_lo[s]; bh[s] = (real)B_hi[s];
+    }
+    column_mono_iterative(L, dt, w, g, bl, bh, (real)mu, (real)Fstar, (real)F_boa, &o, n_iter, fu, fd, fb);
+    for (int l = 0; l < n; ++l) { F_up[l] = (double)fu[l]; F_dn[l] = (double)fd[l]; F_beam[l] = (double)fb[l]; }
+    free(r);
+}
+
 void oracle_column_mono(int L, const double *dtau, const double *w0, const double *g0,
                         const double *B_lo, const double *B_hi, double mu, double Fstar,
                         double F_boa, double eps2, double e_tau, double gcrit_tol,
@@ -419,6 +472,7 @@ typedef struct {
     const double *scat_gas, *cloud_ext, *cloud_w0, *cloud_g0;
     double cloud_p_top, cloud_p_bot, gravity, cp, eps2, e_tau, gcrit_tol, w0_transition, f_toa;
     uint32_t flags;
+    int32_t n_iterations;   /* 0: Thomas (Eqs. 13-15); > 0: that many pair-wise iterations (L258-270) instead */
 } oracle_config;
 
 typedef struct {
@@ -521,8 +575,12 @@ int oracle_rt_step(const oracle_config *cfg, const oracle_inputs *in, const orac
                         dtau[i] = k * dm_sys[i];
                     }
                 }
-                column_mono(L, dtau, w0, g0, B_lo, B_hi, mu, (real)in->stellar_flux[b], F_boa, &o,
-                            Fu, Fd, Fb);
+                if (cfg->n_iterations > 0)
+                    column_mono_iterative(L, dtau, w0, g0, B_lo, B_hi, mu, (real)in->stellar_flux[b], F_boa, &o,
+                                          cfg->n_iterations, Fu, Fd, Fb);
+                else
+                    column_mono(L, dtau, w0, g0, B_lo, B_hi, mu, (real)in->stellar_flux[b], F_boa, &o,
+                                Fu, Fd, Fb);
                 /* O9 reduction: bin weight dlam, Gauss weight w_g; interfaces only */
                 const real wgt = dlam * (real)cfg->gauss_w[g];
                 const int stride = noniso ? 2 : 1;

@@ -94,6 +94,18 @@ def icosahedral_grid(g_level: int) -> np.ndarray:
     return np.array(verts)
 
 
+def grid_geometry(g_level: int):
+    """Longitude, latitude (radians) and control-volume solid angle A_i / R_p^2 of every vertex of the
+    icosahedral grid (Eq. 25): the control volumes are the spherical Voronoi cells of the
+    vertices.  Inputs of the phase-curve reduction; no method arithmetic."""
+    from scipy.spatial import SphericalVoronoi
+    xyz = icosahedral_grid(g_level)
+    lon = np.mod(np.arctan2(xyz[:, 1], xyz[:, 0]), 2.0 * np.pi)      # 0 <= phi < 2 pi (L533)
+    lat = np.arcsin(np.clip(xyz[:, 2], -1.0, 1.0))
+    area = SphericalVoronoi(xyz, radius=1.0).calculate_areas()
+    return lon, lat, np.ascontiguousarray(area)
+
+
 def _ktable(rng, ktab_p, ktab_t, n_bins, n_gauss):
     """ln kappa = ln(1e-4) + 2 z_sorted[b,g] + a_b/2 ln(P/bar) + c_b (T-1500)/1500 + 0.3 eta[iP,iT,b];
     log-normal (median 1e-3 cm^2/g = 1e-4 m^2/kg, sigma_ln = 2), ascending in g within each bin as
