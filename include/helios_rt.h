@@ -122,6 +122,15 @@ int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_out
  * the end-to-end path bench.py times ("e2e"). */
 int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out);
 
+/* the scheme Thomas's algorithm replaces (L258-270, L397), as a measured comparison:
+ * same step, but the flux system is "solved" by n_iterations pair-wise sweeps over the atmosphere (all diffuse
+ * fluxes start at 0; one iteration = one upward pass, Eq.(10) then Eq.(2), with the previous downward fluxes,
+ * followed by one downward pass, Eq.(3), with the upward fluxes just computed; HELIOS used 200, Oreshenko et
+ * al. ~10; reading R23).  Same arguments and outputs as helios_rt_step; HELIOS_RT_TOA_SPECTRUM handles are not
+ * supported (EINVAL); n_iterations >= 1. */
+int helios_rt_step_iterative(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
+                             int32_t n_iterations, void *cuda_stream);
+
 /* Frees every device and host resource of the handle (NULL is accepted). */
 int helios_rt_destroy(helios_rt *h);
 
@@ -146,6 +155,38 @@ int helios_rt_set_profiling(helios_rt *h, int32_t on);
  * and the SUMS of the two kernels' event times in milliseconds: S1+S2 (rt_prep_kernel) and S3-S7
  * (rt_solve_kernel, the dominant kernel of the roofline).  Clears the ring. */
 int helios_rt_kernel_times(helios_rt *h, int32_t *n_steps, double *prep_ms, double *solve_ms);
+
+/* ---- the steps either side of the RT step.  DEVICE pointers, fp64,
+ *      C-contiguous, caller-owned; asynchronous on `cuda_stream`; no allocation, no synchronisation (so they can
+ *      be captured in a CUDA graph together with helios_rt_step). ------------------------------------------- */
+
+/* Post-processing column extension (L385): p_ext, T_ext [n_columns][n_layers + n_extra] receive the input
+ * column followed by n_extra layers above the model top, equally spaced in ln p with the per-layer ratio
+ * q = min(p[N-1]/p[N-2], (p_min/p[N-1])^(1/n_extra)) (so the new top is <= p_min; reading R21) and
+ * T = T[N-1] ("isothermal above the original model top"). */
+int helios_rt_extend_top(int32_t n_columns, int32_t n_layers, int32_t n_extra, double p_min, const double *p,
+                         const double *T, double *p_ext, double *T_ext, void *cuda_stream);
+
+/* Phase curve on the icosahedral grid, Eqs.(25)-(26) (L546-552):
+ *   F_phase_bin[a][b] = sum_i F_toa_bin[i][b] / pi * mu_i(alpha_a) * area[i],
+ *   mu_i = cos(lat_i) cos(lon_i - alpha_a) where that cosine is > 0 (visible hemisphere, modulo 2 pi), else 0;
+ * area[i] = A_i / R_p^2.  If F_phase_band is non-NULL also the wavelength integral of Eq.(23) (L521):
+ *   F_phase_band[a] = sum_b |[bin_edges[b], bin_edges[b+1]] n [lam1, lam2]| * F_phase_bin[a][b]
+ * (HST-WFC3: 1.1-1.7 um).  F_toa_bin [n_columns][n_bins] is the TOA_SPECTRUM output of helios_rt_step; lon, lat,
+ * area [n_columns] (radians, steradians); alpha [n_phases]; bin_edges [n_bins+1]; F_phase_bin
+ * [n_phases][n_bins] (required); F_phase_band [n_phases] or NULL.  The column sum runs in index order:
+ * deterministic. */
+int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t n_phases, const double *F_toa_bin,
+                          const double *lon, const double *lat, const double *area, const double *alpha,
+                          const double *bin_edges, double lam1, double lam2, double *F_phase_bin,
+                          double *F_phase_band, void *cuda_stream);
+
+/* "1-D mode" (Sec. 3): explicit temperature step T <- T + dt * dTdt (dTdt NULL: T unchanged) followed
+ * by the hydrostatic re-balance of Eq.(20) on the fixed altitude grid z [n_layers] (m, ascending): p[.][0] =
+ * p_ref, p_i = p_{i-1} (1/dz - g/(2 R_d T_{i-1})) / (1/dz + g/(2 R_d T_i)) (sign of the denominator: reading
+ * R25), rho = p / (R_d T) (rho may be NULL).  T [n_columns][n_layers] is updated in place; p, rho are outputs. */
+int helios_rt_advance_1d(int32_t n_columns, int32_t n_layers, double dt, double gravity, double R_d, double p_ref,
+                         const double *z, const double *dTdt, double *T, double *p, double *rho, void *cuda_stream);
 
 /* Device self-test of the fp64 primitives the kernels use instead of the CUDA math library
  * (reciprocal, reciprocal square root, exp / 1-exp).  x: n HOST values; outputs n HOST values each:

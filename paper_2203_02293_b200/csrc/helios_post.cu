@@ -1,0 +1,211 @@
+// helios_post.cu -- the steps either side of the RT step, sm_100a.
+//
+//   helios_rt_extend_top   PAPER.md L385: columns extended isothermally to <= p_min before the post-processing step
+//   helios_rt_phase_curve  Eqs.(25)-(26) L546-552 (+ the wavelength integral of Eq.(23))
+//   helios_rt_advance_1d   Sec. 3 "1-D mode": T <- T + dt dT/dt, hydrostatic re-balance Eq.(20)
+//
+// C ABI: include/helios_rt.h.  All pointers are DEVICE pointers; every call is asynchronous on the given
+// stream, allocates nothing and synchronises nothing, so the calls can be captured in a CUDA graph together
+// with helios_rt_step.  Readings R21-R26: DESIGN.md.
+
+#include "../../include/helios_rt.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+namespace {
+
+constexpr double kPi = 3.14159265358979323846;
+
+int device_ok() {
+  static int cached = 1;   // the device check is made once: later calls may sit inside a CUDA-graph capture
+  if (cached <= 0) return cached;
+  const auto done = [&](int rc) { if (rc == HELIOS_RT_OK) cached = 0; return rc; };
+  int n = 0;
+  if (cudaGetDeviceCount(&n) != cudaSuccess || n == 0) { cudaGetLastError(); return HELIOS_RT_ENODEV; }
+  int dev = 0, major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return HELIOS_RT_ENODEV;
+  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  return done(major == 10 ? HELIOS_RT_OK : HELIOS_RT_ENODEV);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// extend_top: one thread per column.  n_extra layers above the top layer, equally spaced in ln p with the ratio
+// q = min(p[N-1]/p[N-2], (p_min/p[N-1])^(1/n_extra)) (reading R21); T = T[N-1] (L385).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void extend_top_kernel(int ncol, int N, int n_extra, double p_min, const double *__restrict__ p,
+                                  const double *__restrict__ T, double *__restrict__ p_ext, double *__restrict__ T_ext) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncol) return;
+  const double *pc = p + (size_t)c * N, *Tc = T + (size_t)c * N;
+  double *po = p_ext + (size_t)c * (N + n_extra), *To = T_ext + (size_t)c * (N + n_extra);
+  for (int j = 0; j < N; ++j) { po[j] = pc[j]; To[j] = Tc[j]; }
+  if (n_extra == 0) return;
+  const double p_top = pc[N - 1], T_top = Tc[N - 1];
+  const double q_own = (N > 1) ? p_top / pc[N - 2] : sqrt(0.1);
+  const double q_need = pow(p_min / p_top, 1.0 / (double)n_extra);
+  const double q = fmin(q_own, q_need);
+  for (int k = 1; k <= n_extra; ++k) {
+    po[N - 1 + k] = p_top * pow(q, (double)k);
+    To[N - 1 + k] = T_top;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// phase_curve: out[a][b] = sum_i F[i][b] * w_a[i],  w_a[i] = cos(lat_i) max(cos(lon_i - alpha_a), 0) A_i / (pi R_p^2)
+// (Eqs. 25-26; visibility modulo 2 pi, reading R22).  Grid = (bin tiles of 128, phase tiles of 8); a block walks
+// all columns in chunks of 128: each thread first builds the 8 weights of one column of the chunk in shared
+// memory, then accumulates its bin over the chunk (F rows read coalesced, weights broadcast from shared memory).
+// The sum over columns runs in index order inside one thread: deterministic.  HBM-bound on F (read once per
+// phase tile; n_columns x n_bins x 8 B, L2-resident for the paper's sizes).
+// ---------------------------------------------------------------------------------------------------------
+constexpr int PC_BINS = 128, PC_PH = 8, PC_COLS = 128;
+
+__global__ void __launch_bounds__(PC_BINS) phase_curve_kernel(int ncol, int nb, int nph, const double *__restrict__ F,
+                                                               const double *__restrict__ lon,
+                                                               const double *__restrict__ lat,
+                                                               const double *__restrict__ area,
+                                                               const double *__restrict__ alpha,
+                                                               double *__restrict__ out) {
+  __shared__ double s_w[PC_PH][PC_COLS];
+  __shared__ double s_alpha[PC_PH];
+  const int tid = threadIdx.x;
+  const int bin = blockIdx.x * PC_BINS + tid;
+  const int ph0 = blockIdx.y * PC_PH;
+  if (tid < PC_PH) s_alpha[tid] = (ph0 + tid < nph) ? alpha[ph0 + tid] : 0.0;
+  __syncthreads();
+  double acc[PC_PH];
+#pragma unroll
+  for (int k = 0; k < PC_PH; ++k) acc[k] = 0.0;
+  for (int c0 = 0; c0 < ncol; c0 += PC_COLS) {
+    const int i = c0 + tid;
+    if (i < ncol) {
+      const double lo = lon[i], cl = cos(lat[i]) * (area[i] / kPi);
+#pragma unroll
+      for (int k = 0; k < PC_PH; ++k) {
+        const double c = cos(lo - s_alpha[k]);
+        s_w[k][tid] = (c > 0.0) ? cl * c : 0.0;     // Eq.(26)
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < PC_PH; ++k) s_w[k][tid] = 0.0;
+    }
+    __syncthreads();
+    if (bin < nb) {
+      const int nj = (ncol - c0 < PC_COLS) ? (ncol - c0) : PC_COLS;
+      const double *Fp = F + (size_t)c0 * nb + bin;
+#pragma unroll 4
+      for (int j = 0; j < nj; ++j) {
+        const double f = __ldg(Fp + (size_t)j * nb);
+#pragma unroll
+        for (int k = 0; k < PC_PH; ++k) acc[k] = fma(s_w[k][j], f, acc[k]);   // Eq.(25)
+      }
+    }
+    __syncthreads();
+  }
+  if (bin < nb)
+#pragma unroll
+    for (int k = 0; k < PC_PH; ++k)
+      if (ph0 + k < nph) out[(size_t)(ph0 + k) * nb + bin] = acc[k];
+}
+
+// band integral of Eq.(23): out[a] = sum_b overlap([edges[b], edges[b+1]], [lam1, lam2]) * F[a][b] (reading R24).
+// One block per phase; fixed-order tree reduction.
+__global__ void __launch_bounds__(256) phase_band_kernel(int nb, const double *__restrict__ edges, double lam1, double lam2,
+                                                         const double *__restrict__ Fph, double *__restrict__ out) {
+  __shared__ double s[256];
+  const int a = blockIdx.x, tid = threadIdx.x;
+  double sum = 0.0;
+  for (int b = tid; b < nb; b += 256) {
+    const double lo = fmax(edges[b], lam1), hi = fmin(edges[b + 1], lam2);
+    const double w = (hi > lo) ? hi - lo : 0.0;
+    sum = fma(w, Fph[(size_t)a * nb + b], sum);
+  }
+  s[tid] = sum;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (tid < o) s[tid] += s[tid + o];
+    __syncthreads();
+  }
+  if (tid == 0) out[a] = s[0];
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// advance_1d: one thread per column.  T <- T + dt dT/dt (reading R26); p[0] = p_ref and Eq.(20) upward with the
+// sign of reading R25; rho = p / (R_d T).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void advance_1d_kernel(int ncol, int N, double dt, double gravity, double R_d, double p_ref,
+                                  const double *__restrict__ z, const double *__restrict__ dTdt, double *__restrict__ T,
+                                  double *__restrict__ p, double *__restrict__ rho) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncol) return;
+  double *Tc = T + (size_t)c * N, *pc = p + (size_t)c * N;
+  const double *hc = dTdt ? dTdt + (size_t)c * N : nullptr;
+  const double g2R = gravity / (2.0 * R_d);
+  double T_prev = hc ? __dadd_rn(Tc[0], __dmul_rn(dt, hc[0])) : Tc[0];
+  double p_prev = p_ref;
+  Tc[0] = T_prev;
+  pc[0] = p_prev;
+  if (rho) rho[(size_t)c * N] = p_prev / (R_d * T_prev);
+  for (int i = 1; i < N; ++i) {
+    const double Ti = hc ? __dadd_rn(Tc[i], __dmul_rn(dt, hc[i])) : Tc[i];
+    const double inv_dz = 1.0 / (z[i] - z[i - 1]);
+    const double pi = p_prev * (inv_dz - g2R / T_prev) / (inv_dz + g2R / Ti);
+    Tc[i] = Ti;
+    pc[i] = pi;
+    if (rho) rho[(size_t)c * N + i] = pi / (R_d * Ti);
+    T_prev = Ti;
+    p_prev = pi;
+  }
+}
+
+}  // namespace
+
+extern "C" int helios_rt_extend_top(int32_t n_columns, int32_t n_layers, int32_t n_extra, double p_min, const double *p,
+                                    const double *T, double *p_ext, double *T_ext, void *cuda_stream) {
+  if (n_columns < 0 || n_layers < 1 || n_extra < 0 || !(p_min > 0.0)) return HELIOS_RT_EINVAL;
+  if (n_columns > 0 && (!p || !T || !p_ext || !T_ext)) return HELIOS_RT_EINVAL;
+  const int rc = device_ok();
+  if (rc) return rc;
+  if (n_columns == 0) return HELIOS_RT_OK;
+  extend_top_kernel<<<(n_columns + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(n_columns, n_layers, n_extra, p_min, p, T,
+                                                                                    p_ext, T_ext);
+  return cudaGetLastError() == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
+}
+
+extern "C" int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t n_phases, const double *F_toa_bin,
+                                     const double *lon, const double *lat, const double *area, const double *alpha,
+                                     const double *bin_edges, double lam1, double lam2, double *F_phase_bin,
+                                     double *F_phase_band, void *cuda_stream) {
+  if (n_columns < 0 || n_bins < 1 || n_phases < 0) return HELIOS_RT_EINVAL;
+  if (n_phases > 0 && (!alpha || !F_phase_bin)) return HELIOS_RT_EINVAL;
+  if (n_columns > 0 && (!F_toa_bin || !lon || !lat || !area)) return HELIOS_RT_EINVAL;
+  if (F_phase_band && (!bin_edges || !(lam2 >= lam1))) return HELIOS_RT_EINVAL;
+  const int rc = device_ok();
+  if (rc) return rc;
+  if (n_phases == 0) return HELIOS_RT_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  dim3 grid((unsigned)((n_bins + PC_BINS - 1) / PC_BINS), (unsigned)((n_phases + PC_PH - 1) / PC_PH));
+  phase_curve_kernel<<<grid, PC_BINS, 0, st>>>(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, F_phase_bin);
+  if (cudaGetLastError() != cudaSuccess) return HELIOS_RT_ECUDA;
+  if (F_phase_band) {
+    phase_band_kernel<<<(unsigned)n_phases, 256, 0, st>>>(n_bins, bin_edges, lam1, lam2, F_phase_bin, F_phase_band);
+    if (cudaGetLastError() != cudaSuccess) return HELIOS_RT_ECUDA;
+  }
+  return HELIOS_RT_OK;
+}
+
+extern "C" int helios_rt_advance_1d(int32_t n_columns, int32_t n_layers, double dt, double gravity, double R_d, double p_ref,
+                                    const double *z, const double *dTdt, double *T, double *p, double *rho,
+                                    void *cuda_stream) {
+  if (n_columns < 0 || n_layers < 1 || !(gravity > 0.0) || !(R_d > 0.0) || !(p_ref > 0.0) || !(dt == dt))
+    return HELIOS_RT_EINVAL;
+  if (n_columns > 0 && (!z || !T || !p)) return HELIOS_RT_EINVAL;
+  const int rc = device_ok();
+  if (rc) return rc;
+  if (n_columns == 0) return HELIOS_RT_OK;
+  advance_1d_kernel<<<(n_columns + 63) / 64, 64, 0, (cudaStream_t)cuda_stream>>>(n_columns, n_layers, dt, gravity, R_d, p_ref, z,
+                                                                                 dTdt, T, p, rho);
+  return cudaGetLastError() == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
+}

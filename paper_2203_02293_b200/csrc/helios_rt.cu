@@ -254,14 +254,13 @@ __device__ __forceinline__ double exp_hot(double x, const double *__restrict__ T
 
 
 // --------------------------------------------------------------------------------------------
-// S5 + S6 forward step for one (sub-)layer between a lower level "a" and an upper level "b".
-// In: (R, U) at the upper level: F_dn[b] = R F_up[b] + U.   Out: (R, U) at the lower level and the
-// back-substitution pair (c, d): F_up[b] = c F_up[a] + d.
+// S5 for one (sub-)layer between a lower level "a" and an upper level "b": transmission t = psi/chi, reflection
+// r = -xi/chi and the sources of  F_up[b] = t F_up[a] + r F_dn[b] + S_up,  F_dn[a] = t F_dn[b] + r F_up[a] + S_dn.
 // --------------------------------------------------------------------------------------------
 template <bool DAY, bool LINSRC>
-__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, double g0,
-                                              double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
-                                              double &R, double &U, double &c, double &d) {
+__device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+                                             double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
+                                             double &t_out, double &r_out, double &Sup_out, double &Sdn_out) {
   // E, Eq.(19) L374 (readings R5, R6): E = max(1, fit) if w0 > 0.1 else 1
   const double fg = fma(g0, fma(kHC.fc, g0, kHC.fb), kHC.fa);
   const double fit = fma(w0, fma(g0, kHC.fe, fma(kHC.ff, w0, kHC.fd)), fg);
@@ -317,6 +316,18 @@ __device__ __forceinline__ void layer_forward(const KParams &P, const double *__
     Sup = fma(rGm, Fb, fma(Gp, fma(t, Fa, -Fb), Sup));
     Sdn = fma(rGp, Fa, fma(Gm, fma(t, Fb, -Fa), Sdn));
   }
+  t_out = t; r_out = r; Sup_out = Sup; Sdn_out = Sdn;
+}
+
+// S5 + S6 forward step: layer_coeffs, then the forward elimination.
+// In: (R, U) at the upper level: F_dn[b] = R F_up[b] + U.   Out: (R, U) at the lower level and the
+// back-substitution pair (c, d): F_up[b] = c F_up[a] + d.
+template <bool DAY, bool LINSRC>
+__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+                                              double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
+                                              double &R, double &U, double &c, double &d) {
+  double t, r, Sup, Sdn;
+  layer_coeffs<DAY, LINSRC>(P, T32, w0, g0, dtau, Ba, Bb, mu, Fa, Fb, t, r, Sup, Sdn);
   // forward elimination (Eqs. 13-14 specialised): F_up[b] (1 - r R) = t F_up[a] + r U + S_up
   const double q = rcp_fast(fma(-r, R, 1.0));
   c = t * q;
@@ -569,6 +580,94 @@ __device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, 
   __syncwarp();
 }
 
+// stage the column's level records, the tile's Planck values and per-bin optical constants in shared memory
+template <int BLOCK>
+__device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &L, unsigned char *smem, double *s_T32,
+                                             int col, int b_first, int nbt, int tid) {
+  const int nlev = P.nlev, nbtS = L.nbt;
+  double *s_B = (double *)(smem + L.off_B);
+  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
+  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
+  {
+    const double *src = (const double *)(P.ws_lev + (size_t)col * (nlev + 1));
+    double *dst = (double *)(smem + L.off_lev);
+    for (int i = tid; i < 8 * (nlev + 1); i += BLOCK) dst[i] = src[i];
+    const double *gB = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b_first;
+    for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
+      const int l = i / nbt, k = i - l * nbt;
+      s_B[l * nbtS + k] = gB[(size_t)l * P.nb + k];
+    }
+    for (int i = tid; i < 2 * nbt; i += BLOCK) {
+      const int cl = i / nbt, k = i - cl * nbt;
+      const BinConst bc = P.bins[b_first + k];
+      BinOpt bo;
+      bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gg = bc.gg[cl]; bo.pad = 0.0;
+      s_bin[cl * nbtS + k] = bo;
+    }
+  }
+}
+
+// cross-warp sum of the per-warp interface sums (s_red: [warp][4][LP] = F_up, diffuse F_dn part 1, part 2 (+ beam),
+// beam), tile partials in fixed order, and the column's outputs written by its last tile
+template <int BLOCK>
+__device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSmem &L, double *s_red, double *s_fin,
+                                                int *s_is_last_p, int nwa, bool want_beam, int col, int tile, int col_nan) {
+  const int N = P.N, LP = L.LP, tid = threadIdx.x;
+  int &s_is_last = *s_is_last_p;
+  // cross-warp sum in fixed order -> tile partial: F_up, R F_up, U + beam, beam
+  const int nq = want_beam ? 4 : 3;
+  const int nred = nq * (N + 1);
+  for (int k = tid; k < nred; k += BLOCK) {
+    const int q = k / (N + 1), lev = k - q * (N + 1);
+    double sum = 0.0;
+    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
+    s_fin[k] = sum;
+  }
+  __syncthreads();
+
+  if (P.tiles > 1) {
+    // publish the tile partial; the last tile of the column to arrive sums them in tile order
+    double *part = P.partial + ((size_t)col * P.tiles + tile) * 4 * (N + 1);
+    for (int k = tid; k < nred; k += BLOCK) part[k] = s_fin[k];
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+      const unsigned prev = atomicAdd(P.counter + col, 1u);
+      s_is_last = (prev == (unsigned)(P.tiles - 1));
+      if (s_is_last) P.counter[col] = 0;   // re-arm for the next step
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    const double *pall = P.partial + (size_t)col * P.tiles * 4 * (N + 1);
+    for (int k = tid; k < nred; k += BLOCK) {
+      double sum = 0.0;
+      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 4 * (N + 1) + k);
+      s_fin[k] = sum;
+    }
+    __syncthreads();
+  }
+
+  // final outputs of the column: F_down = sum W R F_up + sum W (U + beam)
+  const double poison = col_nan ? nan("") : 0.0;
+  for (int i = tid; i <= N; i += BLOCK) {
+    const size_t o = (size_t)col * (N + 1) + i;
+    const double fu = s_fin[i] + poison, fd = s_fin[N + 1 + i] + s_fin[2 * (N + 1) + i] + poison;
+    if (P.F_up) P.F_up[o] = fu;
+    if (P.F_down) P.F_down[o] = fd;
+    if (P.F_net) P.F_net[o] = fu - fd;
+    if (want_beam) P.F_beam[o] = s_fin[3 * (N + 1) + i] + poison;
+  }
+  if (P.dTdt) {
+    const double *dm = P.ws_dm + (size_t)col * N;
+    for (int j = tid; j < N; j += BLOCK) {
+      const double fn1 = s_fin[j + 1] - (s_fin[N + 1 + j + 1] + s_fin[2 * (N + 1) + j + 1]);
+      const double fn0 = s_fin[j] - (s_fin[N + 1 + j] + s_fin[2 * (N + 1) + j]);
+      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / dm[j] + poison;   // reading R14
+    }
+  }
+}
+
 template <bool NONISO, bool TOA, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -597,25 +696,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
   const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
   const int nwa = ((pt_last - pt0) >> 5) + 1;     // warps of this tile that own at least one spectral point
 
-  // ---------------- stage the column's level records, the tile's Planck values and bin constants ----------------
-  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
-  {
-    const double *src = (const double *)(P.ws_lev + (size_t)col * (nlev + 1));
-    double *dst = (double *)(smem + L.off_lev);
-    for (int i = tid; i < 8 * (nlev + 1); i += BLOCK) dst[i] = src[i];
-    const double *gB = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b_first;
-    for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
-      const int l = i / nbt, k = i - l * nbt;
-      s_B[l * nbtS + k] = gB[(size_t)l * P.nb + k];
-    }
-    for (int i = tid; i < 2 * nbt; i += BLOCK) {
-      const int cl = i / nbt, k = i - cl * nbt;
-      const BinConst bc = P.bins[b_first + k];
-      BinOpt bo;
-      bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gg = bc.gg[cl]; bo.pad = 0.0;
-      s_bin[cl * nbtS + k] = bo;
-    }
-  }
+  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid);
   const int col_nan = P.ws_nan[col];
   __syncthreads();
 
@@ -800,58 +881,136 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
   }
   if (TOA) return;
 
-  // cross-warp sum in fixed order -> tile partial: F_up, R F_up, U + beam, beam
-  const int nq = want_beam ? 4 : 3;
-  const int nred = nq * (N + 1);
-  for (int k = tid; k < nred; k += BLOCK) {
-    const int q = k / (N + 1), lev = k - q * (N + 1);
-    double sum = 0.0;
-    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
-    s_fin[k] = sum;
-  }
+  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
+}
+
+// --------------------------------------------------------------------------------------------
+// rt_iter_kernel: the scheme Thomas's algorithm replaces (L258-270, L397), as a measured
+// comparison.  Same decomposition, staging and S3-S5 arithmetic as rt_solve_kernel; instead of the forward
+// elimination the (t, r, S_up, S_dn) of every system layer go to thread-private arrays, and the flux arrays are
+// swept n_iter times: upward pass Eq.(10) + Eq.(2) with the previous downward fluxes, downward pass Eq.(3) with the
+// upward fluxes just computed; all diffuse fluxes start at 0 (reading R23).  The non-isothermal system keeps its
+// centre levels as unknowns (2N system layers, L311-313).  S7 as in the Thomas path (column_epilogue).
+// --------------------------------------------------------------------------------------------
+template <bool NONISO, int BLOCK>
+__global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const int n_iter) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double s_T32[32];
+  __shared__ int s_is_last;
+  constexpr int MAXS = NONISO ? 2 * MAXL : MAXL;   // system layers
+  const int N = P.N, nlev = P.nlev;
+  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, false);
+  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
+  double *s_B = (double *)(smem + L.off_B);
+  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
+  double *s_red = (double *)(smem + L.off_red);
+  double *s_fin = (double *)(smem + L.off_fin);
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x, col = blockIdx.y;
+  const int LP = L.LP, nbtS = L.nbt;
+  const double mu = P.mu[col];
+  const bool day = mu > 0.0;
+  const int pt0 = tile * BLOCK;
+  const int b_first = pt0 / P.ng;
+  int pt_last = pt0 + BLOCK - 1;
+  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
+  const int nbt = pt_last / P.ng - b_first + 1;
+  const int nwa = ((pt_last - pt0) >> 5) + 1;
+  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid);
+  const int col_nan = P.ws_nan[col];
   __syncthreads();
 
-  if (P.tiles > 1) {
-    // publish the tile partial; the last tile of the column to arrive sums them in tile order
-    double *part = P.partial + ((size_t)col * P.tiles + tile) * 4 * (N + 1);
-    for (int k = tid; k < nred; k += BLOCK) part[k] = s_fin[k];
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      const unsigned prev = atomicAdd(P.counter + col, 1u);
-      s_is_last = (prev == (unsigned)(P.tiles - 1));
-      if (s_is_last) P.counter[col] = 0;   // re-arm for the next step
-    }
-    __syncthreads();
-    if (!s_is_last) return;
-    __threadfence();
-    const double *pall = P.partial + (size_t)col * P.tiles * 4 * (N + 1);
-    for (int k = tid; k < nred; k += BLOCK) {
-      double sum = 0.0;
-      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 4 * (N + 1) + k);
-      s_fin[k] = sum;
-    }
-    __syncthreads();
-  }
+  int pt = pt0 + tid;
+  const bool active = pt < P.npt;
+  if (!active) pt = P.npt - 1;
+  const int b = pt / P.ng, gidx = pt - b * P.ng;
+  const int bl = b - b_first;
+  const int warp = tid >> 5, lane = tid & 31;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
 
-  // final outputs of the column: F_down = sum W R F_up + sum W (U + beam)
-  const double poison = col_nan ? nan("") : 0.0;
-  for (int i = tid; i <= N; i += BLOCK) {
-    const size_t o = (size_t)col * (N + 1) + i;
-    const double fu = s_fin[i] + poison, fd = s_fin[N + 1 + i] + s_fin[2 * (N + 1) + i] + poison;
-    if (P.F_up) P.F_up[o] = fu;
-    if (P.F_down) P.F_down[o] = fd;
-    if (P.F_net) P.F_net[o] = fu - fd;
-    if (want_beam) P.F_beam[o] = s_fin[3 * (N + 1) + i] + poison;
-  }
-  if (P.dTdt) {
-    const double *dm = P.ws_dm + (size_t)col * N;
-    for (int j = tid; j < N; j += BLOCK) {
-      const double fn1 = s_fin[j + 1] - (s_fin[N + 1 + j + 1] + s_fin[2 * (N + 1) + j + 1]);
-      const double fn0 = s_fin[j] - (s_fin[N + 1 + j] + s_fin[2 * (N + 1) + j]);
-      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / dm[j] + poison;   // reading R14
+  if (warp < nwa) {
+    const double W = active ? P.bins[b].dlam * P.gauss_w[gidx] : 0.0;
+    const double muF = day ? mu * P.fstar[b] : 0.0;
+    const double inv_mu = day ? 1.0 / mu : 0.0;
+    const double *lnk_pt = P.lnk + pt;
+    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
+    const double *T32 = s_T32;
+    const int LS = NONISO ? 2 * N : N;             // system layers; level s = lower end of system layer s
+
+    double a_t[MAXS], a_r[MAXS], a_su[MAXS], a_sd[MAXS];
+    double fu[MAXS + 1], fd[MAXS + 1], bm[MAXS + 1];
+
+    // ---- S3-S5 per system layer, TOA -> BOA (tau and the beam are running prefixes) ----
+    auto coeffs = [&](auto day_tag) {
+      constexpr bool DAY = decltype(day_tag)::value;
+      double tau = 0.0, Fb = muF;
+      bm[LS] = Fb;
+      if (!NONISO) {
+        for (int j = N - 1; j >= 0; --j) {
+          const LevelRec *lv = s_lev + j;
+          double kx, w0, g0;
+          level_optics(load_rows(lnk_pt, lv), T32, lv, bin0, bin1, kx, w0, g0);
+          const double dtau = kx * lv->dm;
+          const double Bj = s_B[(size_t)j * nbtS + bl];
+          double Fa = 0.0;
+          if (DAY) {
+            tau += dtau;
+            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
+          }
+          layer_coeffs<DAY, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, a_t[j], a_r[j], a_su[j], a_sd[j]);
+          bm[j] = Fa;
+          Fb = Fa;
+        }
+      } else {
+        double kx_up, w0_up, g0_up;
+        {
+          const LevelRec *lv = s_lev + LS;
+          level_optics(load_rows(lnk_pt, lv), T32, lv, bin0, bin1, kx_up, w0_up, g0_up);
+        }
+        double B_up = s_B[(size_t)LS * nbtS + bl];
+        for (int sl = LS - 1; sl >= 0; --sl) {
+          const LevelRec *lv = s_lev + sl;
+          double kx_lo, w0_lo, g0_lo;
+          level_optics(load_rows(lnk_pt, lv), T32, lv, bin0, bin1, kx_lo, w0_lo, g0_lo);
+          const double B_lo = s_B[(size_t)sl * nbtS + bl];
+          const double dtau = 0.5 * (kx_lo + kx_up) * lv->dm;
+          double Fa = 0.0;
+          if (DAY) {
+            tau += dtau;
+            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
+          }
+          layer_coeffs<DAY, true>(P, T32, 0.5 * (w0_lo + w0_up), 0.5 * (g0_lo + g0_up), dtau, B_lo, B_up, mu, Fa, Fb,
+                                  a_t[sl], a_r[sl], a_su[sl], a_sd[sl]);
+          bm[sl] = Fa;
+          Fb = Fa;
+          kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo; B_up = B_lo;
+        }
+      }
+    };
+    if (day) coeffs(std::true_type{}); else coeffs(std::false_type{});
+
+    // ---- n_iter pair-wise sweeps over the whole atmosphere ----
+    for (int l = 0; l <= LS; ++l) { fu[l] = 0.0; fd[l] = 0.0; }
+    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
+    for (int it = 0; it < n_iter; ++it) {
+      fu[0] = fd[0] + F_boa + bm[0];                                        // Eq.(10)
+      for (int sl = 0; sl < LS; ++sl) fu[sl + 1] = fma(a_t[sl], fu[sl], fma(a_r[sl], fd[sl + 1], a_su[sl]));   // Eq.(2)
+      fd[LS] = P.f_toa;
+      for (int sl = LS - 1; sl >= 0; --sl) fd[sl] = fma(a_t[sl], fd[sl + 1], fma(a_r[sl], fu[sl], a_sd[sl]));  // Eq.(3)
+    }
+
+    // ---- S7: weighted sums over the warp at the interfaces ----
+    const int stride = NONISO ? 2 : 1;
+    for (int i = 0; i <= N; ++i) {
+      const double su = warp_sum(W * fu[i * stride]);
+      const double sd = warp_sum(W * fd[i * stride]);
+      const double sb = warp_sum(W * bm[i * stride]);
+      if (lane == 0) { red_w[i] = su; red_w[LP + i] = sd; red_w[2 * LP + i] = sb; red_w[3 * LP + i] = sb; }
     }
   }
+  __syncthreads();
+  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, P.F_beam != nullptr, col, tile, col_nan);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -921,8 +1080,8 @@ struct KernelChoice {
 template <bool NONISO, bool TOA>
 KernelChoice pick_kernel(int block, int minb) {
 #define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, B, M>, B};
-  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(128, 4) HRT_VARIANT(160, 3) HRT_VARIANT(320, 2) HRT_VARIANT(608, 1)
-  HRT_VARIANT(160, 4) HRT_VARIANT(128, 6) HRT_VARIANT(128, 5) HRT_VARIANT(64, 10) HRT_VARIANT(96, 7) HRT_VARIANT(320, 1) HRT_VARIANT(128, 3)
+  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(96, 7) HRT_VARIANT(128, 4) HRT_VARIANT(128, 5) HRT_VARIANT(128, 6)
+  HRT_VARIANT(128, 3) HRT_VARIANT(64, 10)
 #undef HRT_VARIANT
   return {nullptr, 0};
 }
@@ -932,7 +1091,18 @@ KernelChoice pick(bool noniso, bool toa, int block, int minb) {
   return toa ? pick_kernel<false, true>(block, minb) : pick_kernel<false, false>(block, minb);
 }
 
-const int kBlocks[] = {32, 64, 96, 128, 160, 320, 608};
+typedef void (*iter_fn)(const KParams, const int);
+iter_fn pick_iter(bool noniso, int block) {
+  switch (block) {
+    case 32: return noniso ? rt_iter_kernel<true, 32> : rt_iter_kernel<false, 32>;
+    case 64: return noniso ? rt_iter_kernel<true, 64> : rt_iter_kernel<false, 64>;
+    case 96: return noniso ? rt_iter_kernel<true, 96> : rt_iter_kernel<false, 96>;
+    case 128: return noniso ? rt_iter_kernel<true, 128> : rt_iter_kernel<false, 128>;
+  }
+  return nullptr;
+}
+
+const int kBlocks[] = {32, 64, 96, 128};
 
 // block size: columns with many spectral points use 128-thread tiles (4-5 resident blocks per SM keep the fp64
 // pipe fed while other blocks sit in their prologue or reductions: measured best on configs 2-5); small
@@ -1152,6 +1322,9 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     step(cudaFuncSetAttribute(h->kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
     step(cudaFuncSetAttribute(h->noniso ? rt_prep_kernel<true> : rt_prep_kernel<false>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prep_smem_bytes(N, h->nlev)));
+    if (!h->toa && pick_iter(h->noniso, h->block))
+      step(cudaFuncSetAttribute(pick_iter(h->noniso, h->block), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)solve_smem(N, h->nlev, h->block, ng, nb, false).total));
     cudaFuncAttributes fa;
     step(cudaFuncGetAttributes(&fa, h->kc.fn));
     if (e == cudaSuccess) { h->regs = fa.numRegs; h->lmem = (int)fa.localSizeBytes; }
@@ -1179,7 +1352,8 @@ static int validate_step(const helios_rt *h, const helios_rt_inputs *in, const h
   return HELIOS_RT_OK;
 }
 
-static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out, cudaStream_t st) {
+static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out, cudaStream_t st,
+                       int n_iter = 0) {
   const helios_rt_config &c = h->cfg;
   if (in->n_columns == 0) return HELIOS_RT_OK;
   KParams P;
@@ -1210,7 +1384,14 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   CK(h, cudaGetLastError());
   if (ev) CK(h, cudaEventRecord(ev[1], st));
   dim3 grid((unsigned)h->tiles, (unsigned)in->n_columns);
-  h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
+  if (n_iter > 0) {
+    iter_fn fn = pick_iter(h->noniso, h->block);
+    if (!fn) return HELIOS_RT_EINVAL;
+    const SolveSmem lay = solve_smem(c.n_layers, h->nlev, h->block, c.n_gauss, c.n_bins, false);
+    fn<<<grid, h->block, lay.total, st>>>(P, n_iter);
+  } else {
+    h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
+  }
   CK(h, cudaGetLastError());
   if (ev) { CK(h, cudaEventRecord(ev[2], st)); ++h->prof_head; }
   return HELIOS_RT_OK;
@@ -1221,6 +1402,14 @@ extern "C" int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const he
   const int rc = validate_step(h, in, out);
   if (rc) return rc;
   return launch_step(h, in, out, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int helios_rt_step_iterative(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
+                                        int32_t n_iterations, void *cuda_stream) {
+  const int rc = validate_step(h, in, out);
+  if (rc) return rc;
+  if (n_iterations < 1 || h->toa || out->F_up_toa_bin) return HELIOS_RT_EINVAL;
+  return launch_step(h, in, out, (cudaStream_t)cuda_stream, n_iterations);
 }
 
 extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out) {

@@ -18,7 +18,8 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
            "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info",
-           "helios_rt_set_profiling", "helios_rt_kernel_times",
+           "helios_rt_set_profiling", "helios_rt_kernel_times", "helios_rt_step_iterative",
+           "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_advance_1d",
            "helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_measure_dfma_peak")
 
 
@@ -70,6 +71,14 @@ def load_library() -> C.CDLL:
         L.helios_rt_last_cuda_error.argtypes = [C.c_void_p]
         L.helios_rt_launch_info.restype = C.c_int
         L.helios_rt_launch_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.helios_rt_step_iterative.restype = C.c_int
+        L.helios_rt_step_iterative.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Outputs), C.c_int32, C.c_void_p]
+        L.helios_rt_extend_top.restype = C.c_int
+        L.helios_rt_extend_top.argtypes = [C.c_int32] * 3 + [C.c_double] + [C.c_void_p] * 5
+        L.helios_rt_phase_curve.restype = C.c_int
+        L.helios_rt_phase_curve.argtypes = [C.c_int32] * 3 + [C.c_void_p] * 6 + [C.c_double] * 2 + [C.c_void_p] * 3
+        L.helios_rt_advance_1d.restype = C.c_int
+        L.helios_rt_advance_1d.argtypes = [C.c_int32] * 2 + [C.c_double] * 4 + [C.c_void_p] * 6
         L.helios_rt_set_profiling.restype = C.c_int
         L.helios_rt_set_profiling.argtypes = [C.c_void_p, C.c_int32]
         L.helios_rt_kernel_times.restype = C.c_int
@@ -156,7 +165,12 @@ class HeliosRT:
         _check(load_library().helios_rt_kernel_times(self._h, C.byref(n), C.byref(a), C.byref(b)), self._h)
         return n.value, a.value, b.value
 
-    def step(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict, stream=None) -> None:
+    def step_iterative(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict, n_iterations: int,
+                       stream=None) -> None:
+        """The pair-wise iterative scheme Thomas replaces (helios_rt_step_iterative); arguments as `step`."""
+        self.step(p, T, mu_star, stellar_flux, f_internal, out, stream=stream, _n_iter=int(n_iterations))
+
+    def step(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict, stream=None, _n_iter=None) -> None:
         """Device step: torch CUDA float64 contiguous tensors; `out` maps output names to pre-allocated
         tensors (omitted = not wanted).  Asynchronous on `stream` (default: torch's current stream)."""
         import torch
@@ -176,7 +190,11 @@ class HeliosRT:
         i = Inputs(n, p.data_ptr(), T.data_ptr(), mu_star.data_ptr(), stellar_flux.data_ptr(), float(f_internal))
         o = Outputs(*[ptrs.get(k) for k in OUTPUT_NAMES])
         st = (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
-        _check(load_library().helios_rt_step(self._h, C.byref(i), C.byref(o), C.c_void_p(st)), self._h)
+        if _n_iter is None:
+            _check(load_library().helios_rt_step(self._h, C.byref(i), C.byref(o), C.c_void_p(st)), self._h)
+        else:
+            _check(load_library().helios_rt_step_iterative(self._h, C.byref(i), C.byref(o), _n_iter, C.c_void_p(st)),
+                   self._h)
 
     def step_host(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict) -> None:
         """Host step (end-to-end path): numpy arrays or CPU (ideally pinned) torch tensors, float64 contiguous.
@@ -209,6 +227,48 @@ class HeliosRT:
             self.close()
         except Exception:
             pass
+
+
+def _dev(t, shape, name):
+    import torch
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise HeliosRTError(f"helios_rt error -1: {name} must be a contiguous CUDA float64 tensor {tuple(shape)}")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    import torch
+    return C.c_void_p((stream if stream is not None else torch.cuda.current_stream()).cuda_stream)
+
+
+def extend_top(p, T, n_extra: int, p_min: float, p_ext, T_ext, stream=None) -> None:
+    """helios_rt_extend_top on CUDA tensors: p, T [n, N] -> p_ext, T_ext [n, N + n_extra] (pre-allocated)."""
+    n, N = p.shape
+    _check(load_library().helios_rt_extend_top(n, N, int(n_extra), float(p_min), _dev(p, (n, N), "p"), _dev(T, (n, N), "T"),
+                                               _dev(p_ext, (n, N + n_extra), "p_ext"),
+                                               _dev(T_ext, (n, N + n_extra), "T_ext"), _stream(stream)))
+
+
+def phase_curve(F_toa_bin, lon, lat, area, alpha, F_phase_bin, bin_edges=None, lam1=0.0, lam2=0.0, F_phase_band=None,
+                stream=None) -> None:
+    """helios_rt_phase_curve on CUDA tensors (Eqs. 25-26; band integral of Eq. 23 if F_phase_band is given)."""
+    n, nb = F_toa_bin.shape
+    na = alpha.shape[0]
+    _check(load_library().helios_rt_phase_curve(
+        n, nb, na, _dev(F_toa_bin, (n, nb), "F_toa_bin"), _dev(lon, (n,), "lon"), _dev(lat, (n,), "lat"),
+        _dev(area, (n,), "area"), _dev(alpha, (na,), "alpha"),
+        None if bin_edges is None else _dev(bin_edges, (nb + 1,), "bin_edges"), float(lam1), float(lam2),
+        _dev(F_phase_bin, (na, nb), "F_phase_bin"),
+        None if F_phase_band is None else _dev(F_phase_band, (na,), "F_phase_band"), _stream(stream)))
+
+
+def advance_1d(dt: float, gravity: float, R_d: float, p_ref: float, z, dTdt, T, p, rho=None, stream=None) -> None:
+    """helios_rt_advance_1d on CUDA tensors: T [n, N] updated in place, p (and rho) written."""
+    n, N = T.shape
+    _check(load_library().helios_rt_advance_1d(
+        n, N, float(dt), float(gravity), float(R_d), float(p_ref), _dev(z, (N,), "z"),
+        None if dTdt is None else _dev(dTdt, (n, N), "dTdt"), _dev(T, (n, N), "T"), _dev(p, (n, N), "p"),
+        None if rho is None else _dev(rho, (n, N), "rho"), _stream(stream)))
 
 
 def selftest_math(x):

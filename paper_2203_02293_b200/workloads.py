@@ -14,6 +14,10 @@ Configs (BASELINE.json `configs`):
   3  wasp43b-ni  as 2, non-isothermal, T_int = 400 K
   4  hires       10242 x 40 x (30 x 20) non-isothermal
   5  spectrum    2562 x 40 x (300 x 20) isothermal, TOA spectrum only
+  6  postproc the post-processing step of PAPER.md L385: 2562 columns x 40 layers from
+                 1e3 to 1e-3 bar, extended by 20 isothermal layers to 1 ubar (-> 60 layers), opacity sampling at
+                 R = 500 (3255 wavelength points x 1 "Gauss point", Fig. 7), TOA spectrum only; with the grid's
+                 lon / lat / control-volume areas and 64 orbital phases for the phase curve (Eqs. 23-26)
 """
 from __future__ import annotations
 
@@ -136,8 +140,10 @@ def make(config: int, columns=None) -> tuple[dict, dict, dict]:
 
     `columns`: optional index array / slice selecting a subset of the columns AFTER generation (the
     random draws are always those of the full config, so a subset is a true sub-sample)."""
+    if config == 6:
+        return _make_postproc(columns)
     if config not in (1, 2, 3, 4, 5):
-        raise ValueError("config must be 1..5")
+        raise ValueError("config must be 1..6")
     rng = np.random.default_rng(_SEED_BASE + config)
     if config == 1:
         n_col, N, nb, ng = 64, 10, 4, 4
@@ -203,4 +209,45 @@ def make(config: int, columns=None) -> tuple[dict, dict, dict]:
     meta = dict(config=config, n_columns=p.shape[0], n_layers=N, n_bins=nb, n_gauss=ng,
                 F_star_tot=float(np.sum(np.diff(edges) * stellar)),
                 name={1: "tiny", 2: "wasp43b-iso", 3: "wasp43b-noniso", 4: "hires-noniso", 5: "spectrum-toa"}[config])
+    return cfg, inp, meta
+
+
+def _make_postproc(columns=None, n_col_level: int = 4, nb: int = 3255, N: int = 40, n_extra: int = 20):
+    """Config 6: see the module docstring.  cfg["n_layers"] is the EXTENDED layer count (what the RT handle is
+    created with); inp["p"], inp["T"] are the model's own 40 layers; meta carries n_extra, p_min and the
+    phase-curve inputs."""
+    rng = np.random.default_rng(_SEED_BASE + 6)
+    ktab_p = np.logspace(-6, 3, 20) * BAR
+    ktab_t = np.linspace(100.0, 3000.0, 30)
+    p1 = np.logspace(3, -3, N) * BAR
+    edges = 0.3e-6 * (200.0 / 0.3) ** (np.arange(nb + 1) / nb)          # R = lam/dlam ~ 500 (PAPER.md L385, Fig. 7)
+    gw = np.array([1.0])
+    ktab, z = _ktable(rng, ktab_p, ktab_t, nb, 1)
+    lam_c = 0.5 * (edges[:-1] + edges[1:])
+    # stellar spectrum: bin-mean blackbody; the bins are narrow, a 21-point Simpson rule is exact to 1e-10
+    stellar = np.pi * _blackbody_bin_mean_quadrature(T_STAR, edges, n=21) * (R_STAR / SEMI_MAJOR) ** 2
+    xyz = icosahedral_grid(n_col_level)
+    mu = xyz[:, 0].copy()
+    T = _guillot_like(p1, mu, 100.0)
+    phi = rng.uniform(0.0, 2.0 * np.pi, 2)
+    b = np.arange(nb)
+    cloud_w0 = 0.5 + 0.499 * np.sin(3.0 * np.pi * b / nb + phi[0])
+    cloud_g0 = 0.45 + 0.45 * np.cos(2.0 * np.pi * b / nb + phi[1])
+    cloud_ext = 10.0 * np.exp(np.log(1e-4) + 2.0 * z[:, 0])
+    scat_gas = 1e-6 * (lam_c / 1e-6) ** -4.0
+    lon, lat, area = grid_geometry(n_col_level)
+    p = np.broadcast_to(p1, (xyz.shape[0], N)).copy()
+    if columns is not None:
+        idx = np.arange(xyz.shape[0])[columns]
+        p, T, mu, lon, lat, area = p[idx].copy(), T[idx].copy(), mu[idx].copy(), lon[idx].copy(), lat[idx].copy(), area[idx].copy()
+    cfg = dict(n_layers=N + n_extra, ktab_p=ktab_p, ktab_t=ktab_t, ktab=ktab, bin_edges=edges, gauss_w=gw,
+               scat_gas=scat_gas, cloud_ext=cloud_ext, cloud_w0=cloud_w0, cloud_g0=cloud_g0, cloud_p_top=1e-3 * BAR,
+               cloud_p_bot=1.0 * BAR, gravity=GRAVITY, cp=CP, eps2=EPS2, e_tau=1e-4, gcrit_tol=1e-5, w0_transition=0.1,
+               f_toa=0.0, flags=IMPROVED | TOA_SPECTRUM)
+    inp = dict(p=np.ascontiguousarray(p), T=np.ascontiguousarray(T), mu_star=mu, stellar_flux=stellar,
+               f_internal=SIGMA_SB * 100.0**4)
+    meta = dict(config=6, n_columns=p.shape[0], n_layers=N + n_extra, n_model_layers=N, n_extra=n_extra, p_min=1e-6 * BAR,
+                n_bins=nb, n_gauss=1, F_star_tot=float(np.sum(np.diff(edges) * stellar)), name="postproc-R500",
+                lon=lon, lat=lat, area=area, alpha=np.linspace(-np.pi, np.pi, 64, endpoint=False),
+                band=(1.1e-6, 1.7e-6))
     return cfg, inp, meta

@@ -1,0 +1,286 @@
+"""GPU parity of the NEXT rows against their oracles, through the C ABI:
+NEXT-2 column extension + opacity-sampling step + phase curve, NEXT-3 1-D mode (explicit T step + Eq. 20),
+NEXT-4 the pair-wise iterative scheme.  Run with `-m gpu` on a B200."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+FLUX_RTOL, FLUX_FLOOR = 1e-9, 1e-12
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_2203_02293_b200 import build, helios_rt
+    build.build()
+    return helios_rt
+
+
+def _t(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
+
+
+# ------------------------------------------------------------------------------------------ NEXT-4
+@pytest.mark.parametrize("noniso", [False, True])
+@pytest.mark.parametrize("n_iter", [1, 2, 7, 200])
+def test_iterative_scheme_matches_the_oracle_iteration_by_iteration(torch_cuda, H, noniso, n_iter):
+    import oracle
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(1, columns=slice(0, 16))
+    nb = meta["n_bins"]
+    cfg = dict(cfg, cloud_ext=np.linspace(1e-4, 3e-3, nb), cloud_w0=np.linspace(0.05, 0.97, nb),
+               cloud_g0=np.linspace(0.0, 0.9, nb), cloud_p_top=1e2, cloud_p_bot=3e4,
+               flags=cfg["flags"] | (W.NONISOTHERMAL if noniso else 0))
+    want = ("F_up", "F_down", "F_net", "F_beam")
+    ref = oracle.rt_step(dict(cfg, n_iterations=n_iter), inp, want=want)
+    rt = H.HeliosRT(cfg, 16)
+    shapes = rt.output_shapes(16)
+    out = {k: torch.full(shapes[k], float("nan"), dtype=torch.float64, device="cuda:0") for k in want}
+    rt.step_iterative(_t(torch, inp["p"]), _t(torch, inp["T"]), _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"]),
+                      inp["f_internal"], out, n_iter)
+    torch.cuda.synchronize()
+    for k in want:
+        got = out[k].cpu().numpy()
+        tol = FLUX_RTOL * np.abs(ref[k]) + FLUX_FLOOR * meta["F_star_tot"]
+        assert np.all(np.isfinite(got)), k
+        assert np.all(np.abs(got - ref[k]) <= tol), f"{k}: max err/tol {np.max(np.abs(got - ref[k]) / tol):.3g}"
+    if n_iter == 200:    # converged: equals the Thomas path of the same handle
+        out2 = {k: torch.empty(shapes[k], dtype=torch.float64, device="cuda:0") for k in want}
+        rt.step(_t(torch, inp["p"]), _t(torch, inp["T"]), _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"]),
+                inp["f_internal"], out2)
+        torch.cuda.synchronize()
+        a, b = out["F_net"].cpu().numpy(), out2["F_net"].cpu().numpy()
+        assert np.all(np.abs(a - b) <= 1e-8 * np.abs(b) + 1e-11 * meta["F_star_tot"])
+    rt.close()
+
+
+def test_iterative_scheme_config2_columns(torch_cuda, H):
+    """600 points per column (5 tiles, ragged last tile), day and night columns, 12 iterations."""
+    import oracle
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(2, columns=slice(5, None, 427))
+    n = meta["n_columns"]
+    want = ("F_up", "F_down", "F_net", "dTdt")
+    ref = oracle.rt_step(dict(cfg, n_iterations=12), inp, want=want)
+    rt = H.HeliosRT(cfg, n)
+    shapes = rt.output_shapes(n)
+    out = {k: torch.empty(shapes[k], dtype=torch.float64, device="cuda:0") for k in want}
+    rt.step_iterative(_t(torch, inp["p"]), _t(torch, inp["T"]), _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"]),
+                      inp["f_internal"], out, 12)
+    torch.cuda.synchronize()
+    for k in ("F_up", "F_down", "F_net"):
+        got = out[k].cpu().numpy()
+        tol = FLUX_RTOL * np.abs(ref[k]) + FLUX_FLOOR * meta["F_star_tot"]
+        assert np.all(np.abs(got - ref[k]) <= tol), f"{k}: max err/tol {np.max(np.abs(got - ref[k]) / tol):.3g}"
+    assert (inp["mu_star"] > 0).any() and (inp["mu_star"] <= 0).any()
+    rt.close()
+
+
+def test_iterative_rejects_bad_arguments(torch_cuda, H):
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(1, columns=slice(0, 2))
+    rt = H.HeliosRT(cfg, 2)
+    out = {"F_net": torch.empty(rt.output_shapes(2)["F_net"], dtype=torch.float64, device="cuda:0")}
+    args = (_t(torch, inp["p"]), _t(torch, inp["T"]), _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"]), inp["f_internal"])
+    with pytest.raises(H.HeliosRTError, match="error -1"):
+        rt.step_iterative(*args, out, 0)
+    rt.close()
+    rt = H.HeliosRT(dict(cfg, flags=cfg["flags"] | W.TOA_SPECTRUM), 2)
+    out = {"F_up_toa_bin": torch.empty(rt.output_shapes(2)["F_up_toa_bin"], dtype=torch.float64, device="cuda:0")}
+    with pytest.raises(H.HeliosRTError, match="error -1"):
+        rt.step_iterative(*args, out, 5)
+    rt.close()
+
+
+# ------------------------------------------------------------------------------------------ NEXT-2
+def test_extend_top_matches_the_oracle(torch_cuda, H):
+    from oracle import postproc
+    torch = torch_cuda
+    rng = np.random.default_rng(8)
+    p = np.sort(10 ** rng.uniform(1, 8, (300, 17)), axis=1)[:, ::-1].copy()
+    T = rng.uniform(300, 2500, p.shape)
+    for n_extra, p_min in ((0, 0.1), (1, 0.1), (9, 0.1), (20, 1e-3), (5, 1e6)):
+        ref_p, ref_T = postproc.extend_top(p, T, n_extra, p_min)
+        pe = torch.full((300, 17 + n_extra), float("nan"), dtype=torch.float64, device="cuda:0")
+        Te = torch.full_like(pe, float("nan"))
+        H.extend_top(_t(torch, p), _t(torch, T), n_extra, p_min, pe, Te)
+        torch.cuda.synchronize()
+        assert np.allclose(pe.cpu().numpy(), ref_p, rtol=1e-13, atol=0)
+        assert np.array_equal(Te.cpu().numpy(), ref_T)
+
+
+def test_extend_top_single_layer_and_empty(torch_cuda, H):
+    from oracle import postproc
+    torch = torch_cuda
+    p, T = np.array([[1e4]]), np.array([[900.0]])
+    ref_p, ref_T = postproc.extend_top(p, T, 3, 1.0)
+    pe = torch.empty((1, 4), dtype=torch.float64, device="cuda:0")
+    Te = torch.empty_like(pe)
+    H.extend_top(_t(torch, p), _t(torch, T), 3, 1.0, pe, Te)
+    torch.cuda.synchronize()
+    assert np.allclose(pe.cpu().numpy(), ref_p, rtol=1e-13) and np.array_equal(Te.cpu().numpy(), ref_T)
+    e = torch.empty((0, 4), dtype=torch.float64, device="cuda:0")
+    H.extend_top(torch.empty((0, 1), dtype=torch.float64, device="cuda:0"), torch.empty((0, 1), dtype=torch.float64, device="cuda:0"),
+                 3, 1.0, e, e.clone())
+
+
+@pytest.mark.parametrize("ncol_level,nb,nph", [(4, 30, 37), (3, 301, 8), (2, 5, 1)])
+def test_phase_curve_matches_the_oracle(torch_cuda, H, ncol_level, nb, nph):
+    """Full grid (2562 / 642 / 162 columns: several 128-column chunks and a ragged tail), bins spanning several
+    128-bin tiles with a ragged tail, phases spanning several 8-phase tiles with a ragged tail."""
+    from oracle import postproc
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    lon, lat, area = W.grid_geometry(ncol_level)
+    rng = np.random.default_rng(9)
+    F = 10 ** rng.uniform(-2, 4, (lon.size, nb))
+    alpha = rng.uniform(-np.pi, np.pi, nph)
+    edges = W.bin_edges_equal_wavenumber(nb) if nb > 5 else np.array([1.0, 1.2, 1.4, 1.5, 1.65, 1.9]) * 1e-6
+    lam1, lam2 = 1.1e-6, 1.7e-6
+    ref, ref_band = postproc.phase_curve(F, lon, lat, area, alpha, edges, lam1, lam2)
+    out = torch.full((nph, nb), float("nan"), dtype=torch.float64, device="cuda:0")
+    band = torch.full((nph,), float("nan"), dtype=torch.float64, device="cuda:0")
+    H.phase_curve(_t(torch, F), _t(torch, lon), _t(torch, lat), _t(torch, area), _t(torch, alpha), out,
+                  bin_edges=_t(torch, edges), lam1=lam1, lam2=lam2, F_phase_band=band)
+    torch.cuda.synchronize()
+    got, got_band = out.cpu().numpy(), band.cpu().numpy()
+    assert np.all(np.abs(got - ref) <= 1e-12 * np.abs(ref).max(axis=0, keepdims=True) + 1e-13 * np.abs(ref))
+    assert np.allclose(got_band, ref_band, rtol=1e-12, atol=1e-13 * np.abs(ref_band).max())
+    # run to run deterministic
+    out2 = torch.empty_like(out)
+    H.phase_curve(_t(torch, F), _t(torch, lon), _t(torch, lat), _t(torch, area), _t(torch, alpha), out2)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
+
+
+def test_postprocessing_pipeline_extension_step_phase_curve(torch_cuda, H):
+    """Config 6 on a column sub-sample with the first 700 of its 3255 wavelength points: extend_top -> RT step
+    (opacity sampling, n_gauss = 1, TOA spectrum) -> phase curve, every stage against the oracle's."""
+    import oracle
+    from oracle import postproc
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(6, columns=slice(7, None, 160))
+    nbs = 700
+    cfg = dict(cfg, ktab=np.ascontiguousarray(cfg["ktab"][:, :, :nbs]), bin_edges=cfg["bin_edges"][:nbs + 1].copy(),
+               **{k: cfg[k][:nbs].copy() for k in ("scat_gas", "cloud_ext", "cloud_w0", "cloud_g0")})
+    inp = dict(inp, stellar_flux=inp["stellar_flux"][:nbs].copy())
+    n, N, ne = meta["n_columns"], meta["n_model_layers"], meta["n_extra"]
+    # oracle pipeline
+    pe_ref, Te_ref = postproc.extend_top(inp["p"], inp["T"], ne, meta["p_min"])
+    assert np.all(pe_ref[:, -1] <= meta["p_min"] * (1 + 1e-12))
+    ref = oracle.rt_step(cfg, dict(inp, p=pe_ref, T=Te_ref), want=("F_up_toa_bin",))["F_up_toa_bin"]
+    ph_ref, band_ref = postproc.phase_curve(ref, meta["lon"], meta["lat"], meta["area"], meta["alpha"], cfg["bin_edges"], *meta["band"])
+    # CUDA pipeline
+    pe = torch.empty((n, N + ne), dtype=torch.float64, device="cuda:0")
+    Te = torch.empty_like(pe)
+    H.extend_top(_t(torch, inp["p"]), _t(torch, inp["T"]), ne, meta["p_min"], pe, Te)
+    rt = H.HeliosRT(cfg, n)
+    spec = torch.full((n, nbs), float("nan"), dtype=torch.float64, device="cuda:0")
+    rt.step(pe, Te, _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"]), inp["f_internal"], {"F_up_toa_bin": spec})
+    ph = torch.empty((meta["alpha"].size, nbs), dtype=torch.float64, device="cuda:0")
+    band = torch.empty((meta["alpha"].size,), dtype=torch.float64, device="cuda:0")
+    H.phase_curve(spec, _t(torch, meta["lon"]), _t(torch, meta["lat"]), _t(torch, meta["area"]), _t(torch, meta["alpha"]), ph,
+                  bin_edges=_t(torch, cfg["bin_edges"]), lam1=meta["band"][0], lam2=meta["band"][1], F_phase_band=band)
+    torch.cuda.synchronize()
+    got = spec.cpu().numpy()
+    tol = FLUX_RTOL * np.abs(ref) + FLUX_FLOOR * inp["stellar_flux"][None, :]
+    assert np.all(np.isfinite(got)) and np.all(np.abs(got - ref) <= tol), f"max err/tol {np.max(np.abs(got - ref) / tol):.3g}"
+    assert np.allclose(ph.cpu().numpy(), ph_ref, rtol=2e-9, atol=1e-12 * np.abs(ph_ref).max())
+    assert np.allclose(band.cpu().numpy(), band_ref, rtol=2e-9, atol=1e-12 * np.abs(band_ref).max())
+    rt.close()
+
+
+# ------------------------------------------------------------------------------------------ NEXT-3
+def test_advance_1d_matches_the_oracle(torch_cuda, H):
+    from oracle import onedim
+    torch = torch_cuda
+    rng = np.random.default_rng(10)
+    n, N = 200, 40
+    z = np.cumsum(rng.uniform(2e4, 9e4, N))
+    T = rng.uniform(600, 2500, (n, N))
+    h = rng.normal(0, 1e-3, (n, N))
+    g, R, pref, dt = 47.0, 3553.0, 1e8, 300.0
+    T_ref = onedim.advance_temperature(T, h, dt)
+    p_ref, rho_ref = onedim.hydrostatic_rebalance(z, T_ref, pref, g, R)
+    dT = _t(torch, T)
+    dp = torch.full((n, N), float("nan"), dtype=torch.float64, device="cuda:0")
+    drho = torch.full_like(dp, float("nan"))
+    H.advance_1d(dt, g, R, pref, _t(torch, z), _t(torch, h), dT, dp, drho)
+    torch.cuda.synchronize()
+    assert np.array_equal(dT.cpu().numpy(), T_ref)
+    assert np.allclose(dp.cpu().numpy(), p_ref, rtol=1e-13, atol=0)
+    assert np.allclose(drho.cpu().numpy(), rho_ref, rtol=1e-13, atol=0)
+    # dTdt = NULL: re-balance only
+    dT2 = _t(torch, T)
+    H.advance_1d(dt, g, R, pref, _t(torch, z), None, dT2, dp, None)
+    torch.cuda.synchronize()
+    assert np.array_equal(dT2.cpu().numpy(), T)
+    assert np.allclose(dp.cpu().numpy(), onedim.hydrostatic_rebalance(z, T, pref, g, R)[0], rtol=1e-13)
+
+
+@pytest.mark.parametrize("graph", [False, True])
+def test_one_d_mode_loop_matches_the_oracle(torch_cuda, H, graph):
+    """Sec. 3: 30 steps of (RT step -> T += dt dT/dt -> Eq. 20) for 4 zenith angles (0, 30, 60, 89 degrees, L410) and a
+    nightside column, all on the device -- plain launches, or the step pair captured once in a CUDA graph and
+    replayed -- against the oracle's loop."""
+    import oracle
+    from oracle import onedim
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(1, columns=slice(0, 5))
+    N = meta["n_layers"]
+    mu = np.array([1.0, np.cos(np.pi / 6), 0.5, np.cos(np.radians(89.0)), -0.3])
+    g, R, dt, K = cfg["gravity"], 3553.0, 300.0, 30
+    T0 = inp["T"][:5].copy()
+    # altitude grid in hydrostatic balance with the initial column (so the first re-balance reproduces ~p)
+    H_scale = R * T0.mean() / g
+    z = H_scale * np.log(inp["p"][0, 0] / inp["p"][0])
+    pref = float(inp["p"][0, 0])
+    step_inp = dict(inp, mu_star=mu)
+    ref_p, ref_T = onedim.run(lambda p, T: oracle.rt_step(cfg, dict(step_inp, p=p, T=T), want=("dTdt",))["dTdt"],
+                              z, T0, pref, g, R, dt, K)
+    rt = H.HeliosRT(cfg, 5)
+    dT, dz = _t(torch, T0), _t(torch, z)
+    dp = torch.empty((5, N), dtype=torch.float64, device="cuda:0")
+    dh = torch.empty((5, N), dtype=torch.float64, device="cuda:0")
+    dmu, dfs = _t(torch, mu), _t(torch, inp["stellar_flux"])
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        H.advance_1d(0.0, g, R, pref, dz, None, dT, dp, None, stream=s)
+
+        def pair():
+            rt.step(dp, dT, dmu, dfs, inp["f_internal"], {"dTdt": dh}, stream=s)
+            H.advance_1d(dt, g, R, pref, dz, dh, dT, dp, None, stream=s)
+        if graph:
+            pair()                          # warm-up launch outside the capture, then rewind the state
+            dT.copy_(_t(torch, T0))
+            H.advance_1d(0.0, g, R, pref, dz, None, dT, dp, None, stream=s)
+            s.synchronize()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr, stream=s):
+                pair()
+            # the capture itself does not execute: K replays
+            for _ in range(K):
+                gr.replay()
+        else:
+            for _ in range(K):
+                pair()
+    torch.cuda.synchronize()
+    assert np.allclose(dT.cpu().numpy(), ref_T, rtol=1e-9, atol=0)
+    assert np.allclose(dp.cpu().numpy(), ref_p, rtol=1e-9, atol=0)
+    assert np.abs(ref_T - T0).max() > 1e-3       # the loop did move the temperatures
+    rt.close()
