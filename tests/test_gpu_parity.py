@@ -225,10 +225,10 @@ def test_toa_spectrum_mode_small(torch_cuda, H, oracle_mod):
         assert_parity(oracle_mod, cfg, inp, meta, got, ref)
 
 
-@pytest.mark.parametrize("block", [32, 64, 128, 160, 320, 608])
+@pytest.mark.parametrize("block", [32, 64, 96, 128])
 def test_every_block_size_and_multi_tile_reduction(torch_cuda, H, oracle_mod, block):
-    """Forces each compiled block size: with 600 points per column, 32..320 give 19..2 tiles per column
-    (cross-tile fixed-order reduction, bins straddling tiles), 608 gives one."""
+    """Forces each compiled block size: with 600 points per column, 32..128 give 19..5 tiles per column
+    (cross-tile fixed-order reduction, bins straddling tiles)."""
     from paper_2203_02293_b200 import workloads as W
     cfg, inp, meta = W.make(3, columns=slice(5, None, 400))
     ref = oracle_mod.rt_step(cfg, inp)
