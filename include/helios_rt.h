@@ -174,12 +174,16 @@ int helios_rt_extend_top(int32_t n_columns, int32_t n_layers, int32_t n_extra, d
  *   F_phase_band[a] = sum_b |[bin_edges[b], bin_edges[b+1]] n [lam1, lam2]| * F_phase_bin[a][b]
  * (HST-WFC3: 1.1-1.7 um).  F_toa_bin [n_columns][n_bins] is the TOA_SPECTRUM output of helios_rt_step; lon, lat,
  * area [n_columns] (radians, steradians); alpha [n_phases]; bin_edges [n_bins+1]; F_phase_bin
- * [n_phases][n_bins] (required); F_phase_band [n_phases] or NULL.  The column sum runs in index order:
- * deterministic. */
+ * [n_phases][n_bins] (required); F_phase_band [n_phases] or NULL; workspace: DEVICE scratch of
+ * helios_rt_phase_curve_workspace_bytes(...) bytes, caller-owned (partial sums per chunk of 128 columns).
+ * The column sum runs in a fixed order (within a chunk, then over chunks): deterministic run to run. */
 int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t n_phases, const double *F_toa_bin,
                           const double *lon, const double *lat, const double *area, const double *alpha,
                           const double *bin_edges, double lam1, double lam2, double *F_phase_bin,
-                          double *F_phase_band, void *cuda_stream);
+                          double *F_phase_band, double *workspace, void *cuda_stream);
+
+/* Size in bytes of the scratch buffer helios_rt_phase_curve needs (>= 8; negative = HELIOS_RT_EINVAL). */
+int64_t helios_rt_phase_curve_workspace_bytes(int32_t n_columns, int32_t n_bins, int32_t n_phases);
 
 /* "1-D mode" (Sec. 3): explicit temperature step T <- T + dt * dTdt (dTdt NULL: T unchanged) followed
  * by the hydrostatic re-balance of Eq.(20) on the fixed altitude grid z [n_layers] (m, ascending): p[.][0] =

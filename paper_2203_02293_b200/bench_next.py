@@ -60,12 +60,13 @@ def bench_postproc(torch, H, W, steps):
     spec = torch.empty((n, nb), dtype=torch.float64, device=dev)
     ph = torch.empty((na, nb), dtype=torch.float64, device=dev)
     band = torch.empty((na,), dtype=torch.float64, device=dev)
+    pc_ws = H.phase_curve_workspace(n, nb, na, dev)
     flush = torch.empty(L2_FLUSH_BYTES // 8, dtype=torch.float64, device=dev)
     st = torch.cuda.current_stream()
     f_ext = lambda: H.extend_top(d["p"], d["T"], ne, meta["p_min"], pe, Te)
     f_step = lambda: rt.step(pe, Te, d["mu"], d["fs"], inp["f_internal"], {"F_up_toa_bin": spec})
     f_pc = lambda: H.phase_curve(spec, d["lon"], d["lat"], d["area"], d["alpha"], ph, bin_edges=d["edges"],
-                                 lam1=meta["band"][0], lam2=meta["band"][1], F_phase_band=band)
+                                 lam1=meta["band"][0], lam2=meta["band"][1], F_phase_band=band, workspace=pc_ws)
 
     def pipeline():
         f_ext(); f_step(); f_pc()
@@ -74,6 +75,14 @@ def bench_postproc(torch, H, W, steps):
     ms_ext, _ = _timed(torch, f_ext, steps, flush, st)
     ms_step, _ = _timed(torch, f_step, steps, flush, st)
     ms_pc, _ = _timed(torch, f_pc, steps, flush, st)
+    rt.set_profiling(True)
+    for _ in range(5):
+        flush.fill_(1.0)
+        f_step()
+    torch.cuda.synchronize()
+    k, prep_ms, solve_ms = rt.kernel_times()
+    prep_ms, solve_ms = prep_ms / k, solve_ms / k
+    rt.set_profiling(False)
     peaks = _peaks()
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     pc_bytes = 8.0 * (n * nb + na * nb + 3 * n + na)       # F read once, phase spectra written once
@@ -89,9 +98,10 @@ def bench_postproc(torch, H, W, steps):
             "phase_curve": {"bound": "hbm", "algorithmic_bytes": pc_bytes, "achieved_gbs": pc_bytes / (ms_pc * 1e-3) * 1e-9,
                             "peak_gbs": hbm, "frac": pc_bytes / (ms_pc * 1e-3) * 1e-9 / hbm,
                             "fp64_gflops": pc_flops / (ms_pc * 1e-3) * 1e-9,
-                            "note": "2 launches (phase_curve_kernel + phase_band_kernel); F is re-read once per 8-phase tile "
-                                    "from L2; cold-L2 time, so launch latency and the DRAM read of F dominate"},
-            "gpu_launches": steps * 5}
+                            "note": "3 launches (phase_partial_kernel, phase_reduce_kernel, phase_band_kernel); F is read once "
+                                    "per 32 phases; cold L2"},
+            "rt_step_kernels_ms": {"rt_prep_kernel": prep_ms, "rt_solve_kernel": solve_ms},
+            "gpu_launches": steps * 6}
     rt.close()
     return line
 

@@ -54,60 +54,72 @@ __global__ void extend_top_kernel(int ncol, int N, int n_extra, double p_min, co
 
 // ---------------------------------------------------------------------------------------------------------
 // phase_curve: out[a][b] = sum_i F[i][b] * w_a[i],  w_a[i] = cos(lat_i) max(cos(lon_i - alpha_a), 0) A_i / (pi R_p^2)
-// (Eqs. 25-26; visibility modulo 2 pi, reading R22).  Grid = (bin tiles of 128, phase tiles of 8); a block walks
-// all columns in chunks of 128: each thread first builds the 8 weights of one column of the chunk in shared
-// memory, then accumulates its bin over the chunk (F rows read coalesced, weights broadcast from shared memory).
-// The sum over columns runs in index order inside one thread: deterministic.  HBM-bound on F (read once per
-// phase tile; n_columns x n_bins x 8 B, L2-resident for the paper's sizes).
+// (Eqs. 25-26; visibility modulo 2 pi, reading R22).  Two launches, F read once per 32 phases:
+//   phase_partial_kernel  grid = (bin tiles of 128, column chunks of 128, phase tiles of 32).  Each thread first
+//       builds the 32 weights of one column of the chunk in shared memory, then accumulates its bin over the
+//       chunk's columns in index order: F rows read coalesced, weights broadcast from shared memory two at a time,
+//       32 independent FMA chains in registers.  Writes part[chunk][phase][bin] to the caller's workspace.
+//   phase_reduce_kernel   out[a][b] = sum over chunks in chunk order.
+// Both sums run in a fixed order: deterministic run to run.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int PC_BINS = 128, PC_PH = 8, PC_COLS = 128;
+constexpr int PC_BINS = 128, PC_PH = 32, PC_COLS = 128;
 
-__global__ void __launch_bounds__(PC_BINS) phase_curve_kernel(int ncol, int nb, int nph, const double *__restrict__ F,
-                                                               const double *__restrict__ lon,
-                                                               const double *__restrict__ lat,
-                                                               const double *__restrict__ area,
-                                                               const double *__restrict__ alpha,
-                                                               double *__restrict__ out) {
-  __shared__ double s_w[PC_PH][PC_COLS];
+__global__ void __launch_bounds__(PC_BINS) phase_partial_kernel(int ncol, int nb, int nph, const double *__restrict__ F,
+                                                                 const double *__restrict__ lon,
+                                                                 const double *__restrict__ lat,
+                                                                 const double *__restrict__ area,
+                                                                 const double *__restrict__ alpha,
+                                                                 double *__restrict__ part) {
+  __shared__ __align__(16) double s_w[PC_COLS][PC_PH];
   __shared__ double s_alpha[PC_PH];
   const int tid = threadIdx.x;
   const int bin = blockIdx.x * PC_BINS + tid;
-  const int ph0 = blockIdx.y * PC_PH;
+  const int chunk = blockIdx.y, c0 = chunk * PC_COLS;
+  const int ph0 = blockIdx.z * PC_PH;
   if (tid < PC_PH) s_alpha[tid] = (ph0 + tid < nph) ? alpha[ph0 + tid] : 0.0;
   __syncthreads();
-  double acc[PC_PH];
-#pragma unroll
-  for (int k = 0; k < PC_PH; ++k) acc[k] = 0.0;
-  for (int c0 = 0; c0 < ncol; c0 += PC_COLS) {
+  {
     const int i = c0 + tid;
     if (i < ncol) {
       const double lo = lon[i], cl = cos(lat[i]) * (area[i] / kPi);
-#pragma unroll
       for (int k = 0; k < PC_PH; ++k) {
         const double c = cos(lo - s_alpha[k]);
-        s_w[k][tid] = (c > 0.0) ? cl * c : 0.0;     // Eq.(26)
+        s_w[tid][k] = (c > 0.0) ? cl * c : 0.0;     // Eq.(26)
       }
     } else {
-#pragma unroll
-      for (int k = 0; k < PC_PH; ++k) s_w[k][tid] = 0.0;
+      for (int k = 0; k < PC_PH; ++k) s_w[tid][k] = 0.0;
     }
-    __syncthreads();
-    if (bin < nb) {
-      const int nj = (ncol - c0 < PC_COLS) ? (ncol - c0) : PC_COLS;
-      const double *Fp = F + (size_t)c0 * nb + bin;
-#pragma unroll 4
-      for (int j = 0; j < nj; ++j) {
-        const double f = __ldg(Fp + (size_t)j * nb);
-#pragma unroll
-        for (int k = 0; k < PC_PH; ++k) acc[k] = fma(s_w[k][j], f, acc[k]);   // Eq.(25)
-      }
-    }
-    __syncthreads();
   }
-  if (bin < nb)
+  __syncthreads();
+  if (bin >= nb) return;
+  double acc[PC_PH];
 #pragma unroll
-    for (int k = 0; k < PC_PH; ++k)
-      if (ph0 + k < nph) out[(size_t)(ph0 + k) * nb + bin] = acc[k];
+  for (int k = 0; k < PC_PH; ++k) acc[k] = 0.0;
+  const int nj = (ncol - c0 < PC_COLS) ? (ncol - c0) : PC_COLS;
+  const double *Fp = F + (size_t)c0 * nb + bin;
+#pragma unroll 2
+  for (int j = 0; j < nj; ++j) {
+    const double f = __ldg(Fp + (size_t)j * nb);
+    const double2 *w2 = reinterpret_cast<const double2 *>(&s_w[j][0]);
+#pragma unroll
+    for (int k = 0; k < PC_PH / 2; ++k) {
+      const double2 w = w2[k];
+      acc[2 * k] = fma(w.x, f, acc[2 * k]);         // Eq.(25)
+      acc[2 * k + 1] = fma(w.y, f, acc[2 * k + 1]);
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < PC_PH; ++k)
+    if (ph0 + k < nph) part[((size_t)chunk * nph + ph0 + k) * nb + bin] = acc[k];
+}
+
+__global__ void __launch_bounds__(256) phase_reduce_kernel(int nchunk, size_t n_out, const double *__restrict__ part,
+                                                           double *__restrict__ out) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n_out) return;
+  double sum = 0.0;
+  for (int c = 0; c < nchunk; ++c) sum += part[(size_t)c * n_out + i];
+  out[i] = sum;
 }
 
 // band integral of Eq.(23): out[a] = sum_b overlap([edges[b], edges[b+1]], [lam1, lam2]) * F[a][b] (reading R24).
@@ -174,20 +186,32 @@ extern "C" int helios_rt_extend_top(int32_t n_columns, int32_t n_layers, int32_t
   return cudaGetLastError() == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
 }
 
+extern "C" int64_t helios_rt_phase_curve_workspace_bytes(int32_t n_columns, int32_t n_bins, int32_t n_phases) {
+  if (n_columns < 0 || n_bins < 1 || n_phases < 0) return HELIOS_RT_EINVAL;
+  const int64_t nchunk = (n_columns + PC_COLS - 1) / PC_COLS;
+  return (int64_t)sizeof(double) * (nchunk > 0 ? nchunk : 1) * n_phases * n_bins;
+}
+
 extern "C" int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t n_phases, const double *F_toa_bin,
                                      const double *lon, const double *lat, const double *area, const double *alpha,
                                      const double *bin_edges, double lam1, double lam2, double *F_phase_bin,
-                                     double *F_phase_band, void *cuda_stream) {
+                                     double *F_phase_band, double *workspace, void *cuda_stream) {
   if (n_columns < 0 || n_bins < 1 || n_phases < 0) return HELIOS_RT_EINVAL;
   if (n_phases > 0 && (!alpha || !F_phase_bin)) return HELIOS_RT_EINVAL;
-  if (n_columns > 0 && (!F_toa_bin || !lon || !lat || !area)) return HELIOS_RT_EINVAL;
+  if (n_columns > 0 && n_phases > 0 && (!F_toa_bin || !lon || !lat || !area || !workspace)) return HELIOS_RT_EINVAL;
   if (F_phase_band && (!bin_edges || !(lam2 >= lam1))) return HELIOS_RT_EINVAL;
   const int rc = device_ok();
   if (rc) return rc;
   if (n_phases == 0) return HELIOS_RT_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  dim3 grid((unsigned)((n_bins + PC_BINS - 1) / PC_BINS), (unsigned)((n_phases + PC_PH - 1) / PC_PH));
-  phase_curve_kernel<<<grid, PC_BINS, 0, st>>>(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, F_phase_bin);
+  const int nchunk = (n_columns + PC_COLS - 1) / PC_COLS;
+  const size_t n_out = (size_t)n_phases * n_bins;
+  if (nchunk > 0) {
+    dim3 grid((unsigned)((n_bins + PC_BINS - 1) / PC_BINS), (unsigned)nchunk, (unsigned)((n_phases + PC_PH - 1) / PC_PH));
+    phase_partial_kernel<<<grid, PC_BINS, 0, st>>>(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, workspace);
+    if (cudaGetLastError() != cudaSuccess) return HELIOS_RT_ECUDA;
+  }
+  phase_reduce_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, st>>>(nchunk, n_out, workspace, F_phase_bin);
   if (cudaGetLastError() != cudaSuccess) return HELIOS_RT_ECUDA;
   if (F_phase_band) {
     phase_band_kernel<<<(unsigned)n_phases, 256, 0, st>>>(n_bins, bin_edges, lam1, lam2, F_phase_bin, F_phase_band);

@@ -39,6 +39,10 @@
 namespace {
 
 constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
+#ifndef HRT_ISO_UNROLL
+#define HRT_ISO_UNROLL 2
+#endif
+constexpr int kIsoUnroll = HRT_ISO_UNROLL;   // unroll factor of the isothermal sweep-1 loop (measured: see DESIGN.md)
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kH = 6.62607015e-34, kC = 299792458.0, kKB = 1.380649e-23;  // CODATA 2019 (exact)
 constexpr double kSigmaSB =
@@ -100,19 +104,24 @@ __constant__ double kExp2Tab[32] = {
 // --------------------------------------------------------------------------------------------
 // *low receives int_0^x t^3/(e^t-1) dt when x < 1.5 (else -1): a bin whose two edges both lie there is
 // differenced on `low`, which avoids the cancellation against pi^4/15 for narrow Rayleigh-Jeans bins.
+__constant__ double kInvN[33] = {
+    0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8, 1.0 / 9, 1.0 / 10, 1.0 / 11, 1.0 / 12, 1.0 / 13,
+    1.0 / 14, 1.0 / 15, 1.0 / 16, 1.0 / 17, 1.0 / 18, 1.0 / 19, 1.0 / 20, 1.0 / 21, 1.0 / 22, 1.0 / 23, 1.0 / 24, 1.0 / 25,
+    1.0 / 26, 1.0 / 27, 1.0 / 28, 1.0 / 29, 1.0 / 30, 1.0 / 31, 1.0 / 32};
+
 __device__ double planck_G(double x, double *low_out) {
   *low_out = -1.0;
   if (!(x > 0.0)) { *low_out = 0.0; return kPi * kPi * kPi * kPi / 15.0; }
   if (x >= 1.5) {
     if (x > 745.0) return 0.0;
     const double u = exp(-x);
-    const double x2 = x * x, x3 = x2 * x;
+    const double x2 = x * x, x3 = x2 * x, c1 = 6.0 * x, c2 = 3.0 * x2;
     double un = 1.0, sum = 0.0;
     for (int n = 1; n <= 32; ++n) {
       un *= u;
-      const double in = 1.0 / (double)n;
+      const double in = kInvN[n];   // 1/n, correctly rounded: same value as the division, without its ~25 instructions
       // x^3/n + 3 x^2/n^2 + 6 x/n^3 + 6/n^4
-      const double poly = in * fma(in, fma(in, fma(in, 6.0, 6.0 * x), 3.0 * x2), x3);
+      const double poly = in * fma(in, fma(in, fma(in, 6.0, c1), c2), x3);
       const double term = un * poly;
       sum += term;
       if (term < 1e-18 * sum) break;
@@ -393,6 +402,7 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
   double *s_G = s_tlev + (nlev + 1);                    // [nlev+1][PREP_BINS+1]
   double *s_Glow = s_G + (size_t)(nlev + 1) * (PREP_BINS + 1);
   __shared__ int s_nan;
+  __shared__ short s_rep[2 * MAXL + 2];
 
   const int tid = threadIdx.x;
   const int chunk = blockIdx.x, col = blockIdx.y;
@@ -476,9 +486,17 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
   if (chunk == 0 && tid == 0) P.ws_nan[col] = s_nan;
 
   // ---------------- S2: band Planck for this chunk's bins (reading R8) ----------------
+  // a level whose temperature equals that of the level below it (an isothermal stretch, e.g. the extension above the
+  // model top, L385) shares that level's cumulative integrals: s_rep[l] = first level of the run
   const int nedge = nbc + 1;
+  if (tid == 0) {
+    s_rep[0] = 0;
+    for (int l = 1; l <= nlev; ++l) s_rep[l] = (s_tlev[l] == s_tlev[l - 1]) ? s_rep[l - 1] : l;
+  }
+  __syncthreads();
   for (int i = tid; i < (nlev + 1) * nedge; i += PREP_BLOCK) {
     const int l = i / nedge, e = i - l * nedge;
+    if (s_rep[l] != l) continue;
     const double Tl = s_tlev[l];
     double low = 0.0;
     s_G[l * (PREP_BINS + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b0 + e] * Tl), &low) : 0.0;
@@ -489,8 +507,8 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
     const int l = i / nbc, k = i - l * nbc;
     const double Tl = s_tlev[l];
     const double T2 = Tl * Tl;
-    const double *g = s_G + l * (PREP_BINS + 1) + k;
-    const double *gl = s_Glow + l * (PREP_BINS + 1) + k;
+    const double *g = s_G + s_rep[l] * (PREP_BINS + 1) + k;
+    const double *gl = s_Glow + s_rep[l] * (PREP_BINS + 1) + k;
     double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * P.bins[b0 + k].inv_dlam;
     if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
     P.ws_B[((size_t)col * (nlev + 1) + l) * P.nb + b0 + k] = (Tl > 0.0) ? B : 0.0;
@@ -511,7 +529,7 @@ struct SolveSmem {
   size_t off_lev, off_B, off_bin, off_red, off_stage, off_fin, off_vals, total;
 };
 
-__host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa) {
+__host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa, bool bdirect = false) {
   SolveSmem L;
   int nbt = (block + ng - 1) / ng + 1;
   L.nbt = nbt < nb ? nbt : nb;
@@ -520,7 +538,7 @@ __host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int 
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
   L.off_lev = take(sizeof(LevelRec) * (nlev + 1));
-  L.off_B = take(sizeof(double) * (nlev + 1) * L.nbt);
+  L.off_B = take(bdirect ? 0 : sizeof(double) * (nlev + 1) * L.nbt);   // bdirect: B read straight from the workspace
   L.off_bin = take(sizeof(BinOpt) * 2 * L.nbt);
   L.off_red = take(toa ? 0 : sizeof(double) * nwarp * 4 * L.LP);       // F_up, R F_up, U + beam, beam
   L.off_stage = take(toa ? 0 : sizeof(double) * nwarp * 8 * STAGE_LD);
@@ -583,7 +601,7 @@ __device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, 
 // stage the column's level records, the tile's Planck values and per-bin optical constants in shared memory
 template <int BLOCK>
 __device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &L, unsigned char *smem, double *s_T32,
-                                             int col, int b_first, int nbt, int tid) {
+                                             int col, int b_first, int nbt, int tid, bool stage_B = true) {
   const int nlev = P.nlev, nbtS = L.nbt;
   double *s_B = (double *)(smem + L.off_B);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
@@ -593,10 +611,11 @@ __device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &
     double *dst = (double *)(smem + L.off_lev);
     for (int i = tid; i < 8 * (nlev + 1); i += BLOCK) dst[i] = src[i];
     const double *gB = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b_first;
-    for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
-      const int l = i / nbt, k = i - l * nbt;
-      s_B[l * nbtS + k] = gB[(size_t)l * P.nb + k];
-    }
+    if (stage_B)
+      for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
+        const int l = i / nbt, k = i - l * nbt;
+        s_B[l * nbtS + k] = gB[(size_t)l * P.nb + k];
+      }
     for (int i = tid; i < 2 * nbt; i += BLOCK) {
       const int cl = i / nbt, k = i - cl * nbt;
       const BinConst bc = P.bins[b_first + k];
@@ -668,13 +687,16 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSme
   }
 }
 
-template <bool NONISO, bool TOA, int BLOCK, int MINB>
+template <bool NONISO, bool TOA, bool BDIRECT, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ double s_T32[32];
   __shared__ int s_is_last;
   const int N = P.N, nlev = P.nlev;
-  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA);
+  // one Gauss point per bin (opacity sampling, L385): every thread has its own bin, so the Planck values are read
+  // coalesced straight from the workspace instead of being staged (64 KB per block otherwise)
+  constexpr bool bdirect = BDIRECT;   // host: n_gauss == 1
+  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA, bdirect);
   const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;   // s_lev[-1] pads the prefetch
   double *s_B = (double *)(smem + L.off_B);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
@@ -696,7 +718,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
   const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
   const int nwa = ((pt_last - pt0) >> 5) + 1;     // warps of this tile that own at least one spectral point
 
-  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid);
+  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid, !bdirect);
   const int col_nan = P.ws_nan[col];
   __syncthreads();
 
@@ -720,12 +742,18 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
     const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
     const double *T32 = s_T32;
     double *stage_wr = stage_w + lane;
+    // B of level l: Bbase[l * Bstride] (global workspace row, or the staged tile in shared memory)
+    const double *Bbase = s_B + bl;
+    if (BDIRECT) Bbase = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b;
+    const int Bstride = BDIRECT ? P.nb : nbtS;
 
     // back-substitution state per interface i = 0..N (thread-private stack in local memory, written top-down,
     // read bottom-up): F_up[i] = c F_up[i-1] + d (weight folded into d) and R with F_dn[i] = R F_up[i] + U.
     // U itself is not kept: sum_points W (U + beam) is reduced on the way down (flush_stage).
-    double2 st_cd[TOA ? 1 : MAXL + 1];
-    double st_R[TOA ? 1 : MAXL + 1];
+    // Entries N+1 .. LP-1 pad the last group of 8 in sweep 2 with the identity (c = 1, d = 0, R = 0).
+    constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
+    double2 st_cd[STK];
+    double st_R[STK];
 
     double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
     double Fb = muF;                   // beam at the TOA (full strength, L235)
@@ -750,10 +778,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
       double tau = 0.0;
       if (!NONISO) {
         const LevelRec *lv = s_lev + (N - 1);
-        const double *Bp = s_B + (size_t)(N - 1) * nbtS + bl;
+        const double *Bp = Bbase + (size_t)(N - 1) * Bstride;
         Rows nx = load_rows(lnk_pt, lv);   // rows of the next level, loaded one level ahead
-#pragma unroll 2
-        for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
+#pragma unroll kIsoUnroll
+        for (int j = N - 1; j >= 0; --j, --lv, Bp -= Bstride) {
           const Rows cur = nx;
           nx = load_rows(lnk_pt, lv - 1);
           push_interface(j + 1, R, U, Fb);
@@ -780,7 +808,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
         // the arithmetic mean of the two levels' kappa_ext, omega0, g0 (L171, reading R10).  The centre unknowns
         // are eliminated on the fly: F_up[j+1] = cu F_up[centre] + du, F_up[centre] = cl F_up[j] + dl.
         const LevelRec *lv = s_lev + (nlev - 1);
-        const double *Bp = s_B + (size_t)(nlev - 1) * nbtS + bl;
+        const double *Bp = Bbase + (size_t)(nlev - 1) * Bstride;
         double kx_up, w0_up, g0_up;
         {
           const Rows top = load_rows(lnk_pt, lv);
@@ -790,7 +818,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
         Rows nxc = load_rows(lnk_pt, lv - 1);   // centre and lower interface of the next layer, one layer ahead
         Rows nxl = load_rows(lnk_pt, lv - 2);
 #pragma unroll 1
-        for (int j = N - 1; j >= 0; --j, lv -= 2, Bp -= 2 * nbtS) {
+        for (int j = N - 1; j >= 0; --j, lv -= 2, Bp -= 2 * Bstride) {
           const Rows rc = nxc, rl = nxl;
           nxc = load_rows(lnk_pt, lv - 3);
           nxl = load_rows(lnk_pt, (j > 0) ? lv - 4 : lv - 3);
@@ -798,7 +826,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
           double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo, cu, du, cl, dl;
           level_optics(rc, T32, lv - 1, bin0, bin1, kx_c, w0_c, g0_c);
           level_optics(rl, T32, lv - 2, bin0, bin1, kx_lo, w0_lo, g0_lo);
-          const double B_c = Bp[-nbtS], B_lo = Bp[-2 * nbtS];
+          const double B_c = Bp[-Bstride], B_lo = Bp[-2 * Bstride];
           const double dtau_u = 0.5 * (kx_c + kx_up) * lv[-1].dm;
           const double dtau_l = 0.5 * (kx_lo + kx_c) * lv[-2].dm;
           double Fc = 0.0, Fa = 0.0;
@@ -827,7 +855,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
     if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
 
     // ---------------- BOA, Eq.(10) L237 ----------------
-    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
+    const double F_boa = Bbase[(size_t)nlev * Bstride];
     const double Fup0 = (U + F_boa + Fb) * rcp_fast(1.0 - R);
 
     if (TOA) {
@@ -838,21 +866,19 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
       push_interface(0, R, U, Fb);
       st_cd[0] = make_double2(0.0, W * Fup0);
       // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 interfaces at a time ----------------
+      for (int i = N + 1; i < LP; ++i) { st_cd[i] = make_double2(1.0, 0.0); st_R[i] = 0.0; }
       double wFup = 0.0;
 #pragma unroll 1
       for (int base = 0; base <= N; base += 8) {
         double v[16];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-          const int i = base + k;
-          const bool on = i <= N;
-          const int ic = on ? i : N;
-          const double2 cd = st_cd[ic];
-          const double Ri = st_R[ic];
-          const double nu = fma(cd.x, wFup, cd.y);
-          wFup = on ? nu : wFup;
-          v[k] = on ? nu : 0.0;
-          v[8 + k] = on ? Ri * nu : 0.0;
+          // levels beyond N repeat F_up[N] into rows of the reduction buffer that are never read
+          const double2 cd = st_cd[base + k];
+          const double Ri = st_R[base + k];
+          wFup = fma(cd.x, wFup, cd.y);
+          v[k] = wFup;
+          v[8 + k] = Ri * wFup;
         }
         const double tot = warp_reduce16(v, lane);
         const int idx = lane >> 1;
@@ -1077,18 +1103,22 @@ struct KernelChoice {
   int block;
 };
 
-template <bool NONISO, bool TOA>
+template <bool NONISO, bool TOA, bool BDIRECT>
 KernelChoice pick_kernel(int block, int minb) {
-#define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, B, M>, B};
-  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(96, 7) HRT_VARIANT(128, 4) HRT_VARIANT(128, 5) HRT_VARIANT(128, 6)
-  HRT_VARIANT(128, 3) HRT_VARIANT(64, 10)
+#define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, BDIRECT, B, M>, B};
+  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(96, 7) HRT_VARIANT(128, 4) HRT_VARIANT(128, 5)
 #undef HRT_VARIANT
   return {nullptr, 0};
 }
 
-KernelChoice pick(bool noniso, bool toa, int block, int minb) {
-  if (noniso) return toa ? pick_kernel<true, true>(block, minb) : pick_kernel<true, false>(block, minb);
-  return toa ? pick_kernel<false, true>(block, minb) : pick_kernel<false, false>(block, minb);
+template <bool BDIRECT>
+KernelChoice pick_b(bool noniso, bool toa, int block, int minb) {
+  if (noniso) return toa ? pick_kernel<true, true, BDIRECT>(block, minb) : pick_kernel<true, false, BDIRECT>(block, minb);
+  return toa ? pick_kernel<false, true, BDIRECT>(block, minb) : pick_kernel<false, false, BDIRECT>(block, minb);
+}
+
+KernelChoice pick(bool noniso, bool toa, bool bdirect, int block, int minb) {
+  return bdirect ? pick_b<true>(noniso, toa, block, minb) : pick_b<false>(noniso, toa, block, minb);
 }
 
 typedef void (*iter_fn)(const KParams, const int);
@@ -1272,9 +1302,9 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
   h->block = choose_block(h->npt);
   h->tiles = (h->npt + h->block - 1) / h->block;
-  h->kc = pick(h->noniso, h->toa, h->block, choose_minb(h->block, h->noniso));
+  h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso));
   h->nlev = h->noniso ? 2 * N + 1 : N;
-  h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa);
+  h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa, ng == 1);
   cudaGetDevice(&rc);
   cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, rc);
 

@@ -13,13 +13,17 @@ import numpy as np
 
 from .workloads import IMPROVED, NONISOTHERMAL, TOA_SPECTRUM  # noqa: F401
 
-_LIB_PATH = Path(__file__).resolve().parent / "libhelios_rt.so"
+import os
+
+# HELIOS_RT_LIBRARY: developer override for A/B-ing builds of the same source; the default is the in-tree build
+_LIB_PATH = Path(os.environ.get("HELIOS_RT_LIBRARY") or Path(__file__).resolve().parent / "libhelios_rt.so")
 _dp = C.POINTER(C.c_double)
 
 EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
            "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info",
            "helios_rt_set_profiling", "helios_rt_kernel_times", "helios_rt_step_iterative",
-           "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_advance_1d",
+           "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_phase_curve_workspace_bytes",
+           "helios_rt_advance_1d",
            "helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_measure_dfma_peak")
 
 
@@ -76,7 +80,9 @@ def load_library() -> C.CDLL:
         L.helios_rt_extend_top.restype = C.c_int
         L.helios_rt_extend_top.argtypes = [C.c_int32] * 3 + [C.c_double] + [C.c_void_p] * 5
         L.helios_rt_phase_curve.restype = C.c_int
-        L.helios_rt_phase_curve.argtypes = [C.c_int32] * 3 + [C.c_void_p] * 6 + [C.c_double] * 2 + [C.c_void_p] * 3
+        L.helios_rt_phase_curve.argtypes = [C.c_int32] * 3 + [C.c_void_p] * 6 + [C.c_double] * 2 + [C.c_void_p] * 4
+        L.helios_rt_phase_curve_workspace_bytes.restype = C.c_int64
+        L.helios_rt_phase_curve_workspace_bytes.argtypes = [C.c_int32] * 3
         L.helios_rt_advance_1d.restype = C.c_int
         L.helios_rt_advance_1d.argtypes = [C.c_int32] * 2 + [C.c_double] * 4 + [C.c_void_p] * 6
         L.helios_rt_set_profiling.restype = C.c_int
@@ -249,17 +255,33 @@ def extend_top(p, T, n_extra: int, p_min: float, p_ext, T_ext, stream=None) -> N
                                                _dev(T_ext, (n, N + n_extra), "T_ext"), _stream(stream)))
 
 
+def phase_curve_workspace(n_columns: int, n_bins: int, n_phases: int, device="cuda"):
+    """A scratch tensor of the size helios_rt_phase_curve needs."""
+    import torch
+    nbytes = load_library().helios_rt_phase_curve_workspace_bytes(int(n_columns), int(n_bins), int(n_phases))
+    if nbytes < 0:
+        _check(int(nbytes))
+    return torch.empty(max(nbytes // 8, 1), dtype=torch.float64, device=device)
+
+
 def phase_curve(F_toa_bin, lon, lat, area, alpha, F_phase_bin, bin_edges=None, lam1=0.0, lam2=0.0, F_phase_band=None,
-                stream=None) -> None:
-    """helios_rt_phase_curve on CUDA tensors (Eqs. 25-26; band integral of Eq. 23 if F_phase_band is given)."""
+                workspace=None, stream=None) -> None:
+    """helios_rt_phase_curve on CUDA tensors (Eqs. 25-26; band integral of Eq. 23 if F_phase_band is given).
+    `workspace`: tensor from phase_curve_workspace (allocated here if omitted -- pass it to stay allocation-free)."""
     n, nb = F_toa_bin.shape
     na = alpha.shape[0]
+    if workspace is None:
+        workspace = phase_curve_workspace(n, nb, na, F_toa_bin.device)
+    need = load_library().helios_rt_phase_curve_workspace_bytes(n, nb, na)
+    if not (workspace.is_cuda and workspace.is_contiguous() and workspace.numel() * workspace.element_size() >= need):
+        raise HeliosRTError("helios_rt error -1: workspace too small")
     _check(load_library().helios_rt_phase_curve(
         n, nb, na, _dev(F_toa_bin, (n, nb), "F_toa_bin"), _dev(lon, (n,), "lon"), _dev(lat, (n,), "lat"),
         _dev(area, (n,), "area"), _dev(alpha, (na,), "alpha"),
         None if bin_edges is None else _dev(bin_edges, (nb + 1,), "bin_edges"), float(lam1), float(lam2),
         _dev(F_phase_bin, (na, nb), "F_phase_bin"),
-        None if F_phase_band is None else _dev(F_phase_band, (na,), "F_phase_band"), _stream(stream)))
+        None if F_phase_band is None else _dev(F_phase_band, (na,), "F_phase_band"), workspace.data_ptr(),
+        _stream(stream)))
 
 
 def advance_1d(dt: float, gravity: float, R_d: float, p_ref: float, z, dTdt, T, p, rho=None, stream=None) -> None:
