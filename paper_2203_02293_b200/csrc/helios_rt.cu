@@ -39,10 +39,10 @@
 namespace {
 
 constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
-#ifndef HRT_ISO_UNROLL
-#define HRT_ISO_UNROLL 2
-#endif
-constexpr int kIsoUnroll = HRT_ISO_UNROLL;   // unroll factor of the isothermal sweep-1 loop (measured: see DESIGN.md)
+// unroll factors of the isothermal sweep-1 loop, measured on B200: with the back-substitution
+// stack 1 is best (config 2: 0.760 / 0.787 / 0.891 ms at 1 / 2 / 4), the stack-free TOA mode prefers 4 (config 5:
+// 5.31 / 5.13 / 4.98 ms)
+constexpr int kIsoUnroll = 1, kIsoUnrollToa = 4;
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kH = 6.62607015e-34, kC = 299792458.0, kKB = 1.380649e-23;  // CODATA 2019 (exact)
 constexpr double kSigmaSB =
@@ -494,24 +494,42 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
     for (int l = 1; l <= nlev; ++l) s_rep[l] = (s_tlev[l] == s_tlev[l - 1]) ? s_rep[l - 1] : l;
   }
   __syncthreads();
-  for (int i = tid; i < (nlev + 1) * nedge; i += PREP_BLOCK) {
-    const int l = i / nedge, e = i - l * nedge;
-    if (s_rep[l] != l) continue;
-    const double Tl = s_tlev[l];
-    double low = 0.0;
-    s_G[l * (PREP_BINS + 1) + e] = (Tl > 0.0) ? planck_G(kPlanckC2 / (P.edges[b0 + e] * Tl), &low) : 0.0;
-    s_Glow[l * (PREP_BINS + 1) + e] = low;
+  // warp w takes levels w, w + 8, ...; lane e takes edge e of the chunk (no integer division, one edge per lane);
+  // the chunk's last edge (index 32) is done afterwards, one level per thread
+  const int wrp = tid >> 5, lane = tid & 31;
+  {
+    const double lam_e = (lane < nedge) ? P.edges[b0 + lane] : 1.0;
+    for (int l = wrp; l <= nlev; l += PREP_BLOCK / 32) {
+      if (s_rep[l] != l || lane >= nedge) continue;
+      const double Tl = s_tlev[l];
+      double low = 0.0;
+      s_G[l * (PREP_BINS + 1) + lane] = (Tl > 0.0) ? planck_G(kPlanckC2 / (lam_e * Tl), &low) : 0.0;
+      s_Glow[l * (PREP_BINS + 1) + lane] = low;
+    }
+    if (nedge == PREP_BINS + 1) {
+      const double lam_last = P.edges[b0 + PREP_BINS];
+      for (int l = tid; l <= nlev; l += PREP_BLOCK) {
+        if (s_rep[l] != l) continue;
+        const double Tl = s_tlev[l];
+        double low = 0.0;
+        s_G[l * (PREP_BINS + 1) + PREP_BINS] = (Tl > 0.0) ? planck_G(kPlanckC2 / (lam_last * Tl), &low) : 0.0;
+        s_Glow[l * (PREP_BINS + 1) + PREP_BINS] = low;
+      }
+    }
   }
   __syncthreads();
-  for (int i = tid; i < (nlev + 1) * nbc; i += PREP_BLOCK) {
-    const int l = i / nbc, k = i - l * nbc;
-    const double Tl = s_tlev[l];
-    const double T2 = Tl * Tl;
-    const double *g = s_G + s_rep[l] * (PREP_BINS + 1) + k;
-    const double *gl = s_Glow + s_rep[l] * (PREP_BINS + 1) + k;
-    double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * P.bins[b0 + k].inv_dlam;
-    if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
-    P.ws_B[((size_t)col * (nlev + 1) + l) * P.nb + b0 + k] = (Tl > 0.0) ? B : 0.0;
+  if (lane < nbc) {
+    const double inv_dlam = P.bins[b0 + lane].inv_dlam;
+    double *dst = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b0 + lane;
+    for (int l = wrp; l <= nlev; l += PREP_BLOCK / 32) {
+      const double Tl = s_tlev[l];
+      const double T2 = Tl * Tl;
+      const double *g = s_G + s_rep[l] * (PREP_BINS + 1) + lane;
+      const double *gl = s_Glow + s_rep[l] * (PREP_BINS + 1) + lane;
+      double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * inv_dlam;
+      if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
+      dst[(size_t)l * P.nb] = (Tl > 0.0) ? B : 0.0;
+    }
   }
 }
 
@@ -780,7 +798,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
         const LevelRec *lv = s_lev + (N - 1);
         const double *Bp = Bbase + (size_t)(N - 1) * Bstride;
         Rows nx = load_rows(lnk_pt, lv);   // rows of the next level, loaded one level ahead
-#pragma unroll kIsoUnroll
+#pragma unroll (TOA ? kIsoUnrollToa : kIsoUnroll)
         for (int j = N - 1; j >= 0; --j, --lv, Bp -= Bstride) {
           const Rows cur = nx;
           nx = load_rows(lnk_pt, lv - 1);
