@@ -537,13 +537,14 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
 // rt_solve_kernel: S3-S7.  Grid = (tiles per column, columns); a block owns one column and a tile of
 // BLOCK consecutive spectral points (bin-major, Gauss point fastest); one thread = one spectral point.
 // --------------------------------------------------------------------------------------------
+constexpr int STAGE_LD = 36;   // row stride (doubles) of the per-warp 8 x 32 staging tile: conflict-free transpose
 
 struct __align__(16) BinOpt { double sb, ss, gg, pad; };   // per bin of the tile: [0][bin] clear level, [1][bin] cloudy level
 
 struct SolveSmem {
   int nbt;         // max bins per tile
   int LP;          // N + 1 rounded up to a multiple of 8 (the reductions handle 8 levels at a time)
-  size_t off_lev, off_B, off_bin, off_red, off_fin, off_vals, total;
+  size_t off_lev, off_B, off_bin, off_red, off_stage, off_fin, off_vals, total;
 };
 
 __host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa, bool bdirect = false) {
@@ -557,8 +558,9 @@ __host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int 
   L.off_lev = take(sizeof(LevelRec) * (nlev + 1));
   L.off_B = take(bdirect ? 0 : sizeof(double) * (nlev + 1) * L.nbt);   // bdirect: B read straight from the workspace
   L.off_bin = take(sizeof(BinOpt) * 2 * L.nbt);
-  L.off_red = take(toa ? 0 : sizeof(double) * nwarp * 3 * L.LP);       // per warp: F_up, F_down (incl. beam), beam
-  L.off_fin = take(toa ? 0 : sizeof(double) * 3 * (N + 1));
+  L.off_red = take(toa ? 0 : sizeof(double) * nwarp * 4 * L.LP);       // F_up, R F_up, U + beam, beam
+  L.off_stage = take(toa ? 0 : sizeof(double) * nwarp * 8 * STAGE_LD);
+  L.off_fin = take(toa ? 0 : sizeof(double) * 4 * (N + 1));
   L.off_vals = take(sizeof(double) * block);
   L.total = o;
   return L;
@@ -600,6 +602,20 @@ __device__ __forceinline__ void level_optics(const Rows &rw, const double *__res
   g0 = bo->gg;
 }
 
+// sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
+// base + k.  Lane L sums 8 entries of row L >> 2, two shuffle steps finish the row.  Fixed order.
+__device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, double *__restrict__ dst, int lane) {
+  __syncwarp();
+  const double *row = stage_w + (lane >> 2) * STAGE_LD + (lane & 3);
+  double s = row[0];
+#pragma unroll
+  for (int i = 1; i < 8; ++i) s += row[4 * i];
+  s += __shfl_xor_sync(0xffffffffu, s, 1);
+  s += __shfl_xor_sync(0xffffffffu, s, 2);
+  if ((lane & 3) == 0) dst[lane >> 2] = s;
+  __syncwarp();
+}
+
 // stage the column's level records, the tile's Planck values and per-bin optical constants in shared memory
 template <int BLOCK>
 __device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &L, unsigned char *smem, double *s_T32,
@@ -628,27 +644,27 @@ __device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &
   }
 }
 
-// cross-warp sum of the per-warp interface sums (s_red: [warp][3][LP] = F_up, F_down incl. beam, beam), tile
-// partials in fixed order, and the column's outputs written by its last tile
+// cross-warp sum of the per-warp interface sums (s_red: [warp][4][LP] = F_up, diffuse F_dn part 1, part 2 (+ beam),
+// beam), tile partials in fixed order, and the column's outputs written by its last tile
 template <int BLOCK>
 __device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSmem &L, double *s_red, double *s_fin,
                                                 int *s_is_last_p, int nwa, bool want_beam, int col, int tile, int col_nan) {
   const int N = P.N, LP = L.LP, tid = threadIdx.x;
   int &s_is_last = *s_is_last_p;
-  // cross-warp sum in fixed order -> tile partial: F_up, F_down, beam
-  const int nq = want_beam ? 3 : 2;
+  // cross-warp sum in fixed order -> tile partial: F_up, R F_up, U + beam, beam
+  const int nq = want_beam ? 4 : 3;
   const int nred = nq * (N + 1);
   for (int k = tid; k < nred; k += BLOCK) {
     const int q = k / (N + 1), lev = k - q * (N + 1);
     double sum = 0.0;
-    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 3 * LP + q * LP + lev];
+    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
     s_fin[k] = sum;
   }
   __syncthreads();
 
   if (P.tiles > 1) {
     // publish the tile partial; the last tile of the column to arrive sums them in tile order
-    double *part = P.partial + ((size_t)col * P.tiles + tile) * 3 * (N + 1);
+    double *part = P.partial + ((size_t)col * P.tiles + tile) * 4 * (N + 1);
     for (int k = tid; k < nred; k += BLOCK) part[k] = s_fin[k];
     __threadfence();
     __syncthreads();
@@ -660,30 +676,30 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSme
     __syncthreads();
     if (!s_is_last) return;
     __threadfence();
-    const double *pall = P.partial + (size_t)col * P.tiles * 3 * (N + 1);
+    const double *pall = P.partial + (size_t)col * P.tiles * 4 * (N + 1);
     for (int k = tid; k < nred; k += BLOCK) {
       double sum = 0.0;
-      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 3 * (N + 1) + k);
+      for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 4 * (N + 1) + k);
       s_fin[k] = sum;
     }
     __syncthreads();
   }
 
-  // final outputs of the column
+  // final outputs of the column: F_down = sum W R F_up + sum W (U + beam)
   const double poison = col_nan ? nan("") : 0.0;
   for (int i = tid; i <= N; i += BLOCK) {
     const size_t o = (size_t)col * (N + 1) + i;
-    const double fu = s_fin[i] + poison, fd = s_fin[N + 1 + i] + poison;
+    const double fu = s_fin[i] + poison, fd = s_fin[N + 1 + i] + s_fin[2 * (N + 1) + i] + poison;
     if (P.F_up) P.F_up[o] = fu;
     if (P.F_down) P.F_down[o] = fd;
     if (P.F_net) P.F_net[o] = fu - fd;
-    if (want_beam) P.F_beam[o] = s_fin[2 * (N + 1) + i] + poison;
+    if (want_beam) P.F_beam[o] = s_fin[3 * (N + 1) + i] + poison;
   }
   if (P.dTdt) {
     const double *dm = P.ws_dm + (size_t)col * N;
     for (int j = tid; j < N; j += BLOCK) {
-      const double fn1 = s_fin[j + 1] - s_fin[N + 1 + j + 1];
-      const double fn0 = s_fin[j] - s_fin[N + 1 + j];
+      const double fn1 = s_fin[j + 1] - (s_fin[N + 1 + j + 1] + s_fin[2 * (N + 1) + j + 1]);
+      const double fn0 = s_fin[j] - (s_fin[N + 1 + j] + s_fin[2 * (N + 1) + j]);
       P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / dm[j] + poison;   // reading R14
     }
   }
@@ -703,6 +719,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
   double *s_B = (double *)(smem + L.off_B);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
   double *s_red = (double *)(smem + L.off_red);
+  double *s_stage = (double *)(smem + L.off_stage);
   double *s_fin = (double *)(smem + L.off_fin);
   double *s_vals = (double *)(smem + L.off_vals);
 
@@ -731,7 +748,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
   const int bl = b - b_first;
   const int warp = tid >> 5, lane = tid & 31;
   const bool warp_on = warp < nwa;          // a warp without any spectral point only joins the barriers
-  double *red_w = s_red + (size_t)warp * 3 * LP;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
+  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
   const bool want_beam = !TOA && (P.F_beam != nullptr);
 
   if (warp_on) {
@@ -741,6 +759,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
     const double *lnk_pt = P.lnk + pt;
     const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
     const double *T32 = s_T32;
+    double *stage_wr = stage_w + lane;
     // B of level l: Bbase[l * Bstride] (global workspace row, or the staged tile in shared memory)
     const double *Bbase = s_B + bl;
     if (BDIRECT) Bbase = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b;
@@ -748,11 +767,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
 
     // back-substitution state per interface i = 0..N (thread-private stack in local memory, written top-down,
     // read bottom-up): F_up[i] = c F_up[i-1] + d (weight folded into d) and R with F_dn[i] = R F_up[i] + U.
-    // st_RU holds (R, W (U + beam)): sweep 2 forms W F_dn = R (W F_up) + W (U + beam), beam included (L235).
+    // U itself is not kept: sum_points W (U + beam) is reduced on the way down (flush_stage).
     // Entries N+1 .. LP-1 pad the last group of 8 in sweep 2 with the identity (c = 1, d = 0, R = 0).
     constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
     double2 st_cd[STK];
-    double2 st_RU[STK];
+    double st_R[STK];
 
     double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
     double Fb = muF;                   // beam at the TOA (full strength, L235)
@@ -761,10 +780,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
     // bookkeeping of interface i with (R, U, Fb) at that interface
     auto push_interface = [&](int i, double Ri, double Ui, double Fbi) {
       if (!TOA) {
-        st_RU[i] = make_double2(Ri, W * (Ui + Fbi));
+        st_R[i] = Ri;
+        stage_wr[(i & 7) * STAGE_LD] = W * (Ui + Fbi);
+        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
         if (want_beam) {
           const double wb = warp_sum(W * Fbi);
-          if (lane == 0) red_w[2 * LP + i] = wb;
+          if (lane == 0) red_w[3 * LP + i] = wb;
         }
       }
     };
@@ -863,7 +884,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
       push_interface(0, R, U, Fb);
       st_cd[0] = make_double2(0.0, W * Fup0);
       // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 interfaces at a time ----------------
-      for (int i = N + 1; i < LP; ++i) { st_cd[i] = make_double2(1.0, 0.0); st_RU[i] = make_double2(0.0, 0.0); }
+      for (int i = N + 1; i < LP; ++i) { st_cd[i] = make_double2(1.0, 0.0); st_R[i] = 0.0; }
       double wFup = 0.0;
 #pragma unroll 1
       for (int base = 0; base <= N; base += 8) {
@@ -872,10 +893,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
         for (int k = 0; k < 8; ++k) {
           // levels beyond N repeat F_up[N] into rows of the reduction buffer that are never read
           const double2 cd = st_cd[base + k];
-          const double2 ru = st_RU[base + k];
+          const double Ri = st_R[base + k];
           wFup = fma(cd.x, wFup, cd.y);
           v[k] = wFup;
-          v[8 + k] = fma(ru.x, wFup, ru.y);
+          v[8 + k] = Ri * wFup;
         }
         const double tot = warp_reduce16(v, lane);
         const int idx = lane >> 1;
@@ -950,7 +971,7 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
   const int b = pt / P.ng, gidx = pt - b * P.ng;
   const int bl = b - b_first;
   const int warp = tid >> 5, lane = tid & 31;
-  double *red_w = s_red + (size_t)warp * 3 * LP;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
 
   if (warp < nwa) {
     const double W = active ? P.bins[b].dlam * P.gauss_w[gidx] : 0.0;
@@ -1029,7 +1050,7 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
       const double su = warp_sum(W * fu[i * stride]);
       const double sd = warp_sum(W * fd[i * stride]);
       const double sb = warp_sum(W * bm[i * stride]);
-      if (lane == 0) { red_w[i] = su; red_w[LP + i] = sd + sb; red_w[2 * LP + i] = sb; }
+      if (lane == 0) { red_w[i] = su; red_w[LP + i] = sd; red_w[2 * LP + i] = sb; red_w[3 * LP + i] = sb; }
     }
   }
   __syncthreads();
@@ -1332,7 +1353,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(upload(&h->d_bins, bins, (size_t)nb));
   free(lnk); free(lp); free(bins);
   const size_t ncol = (size_t)cfg->max_columns;
-  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * h->tiles * 3 * (N + 1)));
+  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * h->tiles * 4 * (N + 1)));
   step(cudaMalloc((void **)&h->d_ws_lev, sizeof(LevelRec) * ncol * (h->nlev + 1)));
   step(cudaMalloc((void **)&h->d_ws_B, sizeof(double) * ncol * (h->nlev + 1) * nb));
   step(cudaMalloc((void **)&h->d_ws_dm, sizeof(double) * ncol * N));
