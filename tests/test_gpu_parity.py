@@ -247,10 +247,11 @@ def test_every_block_size_and_multi_tile_reduction(torch_cuda, H, oracle_mod, bl
 
 
 def test_ragged_shapes(torch_cuda, H, oracle_mod):
-    """Odd sizes: 3 bins x 5 Gauss points (15 points, half a warp), 7 layers; and 1 layer."""
+    """Odd sizes: 3 bins x 5 Gauss points (15 points, half a warp), 7 layers; 1 layer; the maximum 64 layers; a single
+    spectral point; and one Gauss point per bin (the opacity-sampling kernel variant) with all outputs, 150 bins."""
     from paper_2203_02293_b200 import workloads as W
     rng = np.random.default_rng(77)
-    for N, nb, ng in ((7, 3, 5), (1, 2, 3), (64, 5, 7)):
+    for N, nb, ng in ((7, 3, 5), (1, 2, 3), (64, 5, 7), (9, 1, 1), (12, 150, 1)):
         edges = W.bin_edges_equal_wavenumber(nb)
         _, gw = W.gauss_legendre_01(ng)
         ktab_p = np.logspace(1, 7, 5)
