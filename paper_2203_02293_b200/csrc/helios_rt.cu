@@ -1124,7 +1124,7 @@ struct KernelChoice {
 template <bool NONISO, bool TOA, bool BDIRECT>
 KernelChoice pick_kernel(int block, int minb) {
 #define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, BDIRECT, B, M>, B};
-  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(96, 7) HRT_VARIANT(128, 4) HRT_VARIANT(128, 5)
+  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(96, 7) HRT_VARIANT(128, 4) HRT_VARIANT(128, 5) HRT_VARIANT(128, 6)
 #undef HRT_VARIANT
   return {nullptr, 0};
 }
@@ -1172,12 +1172,13 @@ int choose_block(int npt) {
   return best;
 }
 
-// resident blocks per SM the kernel is compiled for (register cap): isothermal 128 x 5 (96 registers),
-// non-isothermal 128 x 4 (128 registers)
-int choose_minb(int block, bool noniso) {
+// resident blocks per SM the kernel is compiled for (register cap), measured on B200: isothermal with the
+// back-substitution stack 128 x 6 (80 registers, no spills: config 2 0.718 ms against 0.762 at 5 and 0.747 at 7),
+// TOA mode 128 x 5 (96 registers), non-isothermal 128 x 4 (128 registers)
+int choose_minb(int block, bool noniso, bool toa) {
   const char *mb = getenv("HELIOS_RT_MINB");
   if (mb) return atoi(mb);
-  if (block == 128) return noniso ? 4 : 5;
+  if (block == 128) return noniso ? 4 : (toa ? 5 : 6);
   return 0;
 }
 
@@ -1320,7 +1321,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
   h->block = choose_block(h->npt);
   h->tiles = (h->npt + h->block - 1) / h->block;
-  h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso));
+  h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso, h->toa));
   h->nlev = h->noniso ? 2 * N + 1 : N;
   h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa, ng == 1);
   cudaGetDevice(&rc);
