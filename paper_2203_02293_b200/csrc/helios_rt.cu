@@ -43,6 +43,10 @@ constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
 // stack 1 is best (config 2: 0.760 / 0.787 / 0.891 ms at 1 / 2 / 4), the stack-free TOA mode prefers 4 (config 5:
 // 5.31 / 5.13 / 4.98 ms)
 constexpr int kIsoUnroll = 1, kIsoUnrollToa = 4;
+#ifndef HRT_U2
+#define HRT_U2 1
+#endif
+constexpr int kIsoUnrollToa2 = HRT_U2;   // rt_solve2_kernel, TOA mode
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kH = 6.62607015e-34, kC = 299792458.0, kKB = 1.380649e-23;  // CODATA 2019 (exact)
 constexpr double kSigmaSB =
@@ -547,9 +551,10 @@ struct SolveSmem {
   size_t off_lev, off_B, off_bin, off_red, off_stage, off_fin, off_vals, total;
 };
 
-__host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa, bool bdirect = false) {
+__host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa, bool bdirect = false,
+                                                int ppt = 1) {
   SolveSmem L;
-  int nbt = (block + ng - 1) / ng + 1;
+  int nbt = (block * ppt + ng - 1) / ng + 1;   // ppt: spectral points per thread (rt_solve2_kernel: 2)
   L.nbt = nbt < nb ? nbt : nb;
   L.LP = (N + 1 + 7) & ~7;
   const int nwarp = (block + 31) / 32;
@@ -561,7 +566,7 @@ __host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int 
   L.off_red = take(toa ? 0 : sizeof(double) * nwarp * 4 * L.LP);       // F_up, R F_up, U + beam, beam
   L.off_stage = take(toa ? 0 : sizeof(double) * nwarp * 8 * STAGE_LD);
   L.off_fin = take(toa ? 0 : sizeof(double) * 4 * (N + 1));
-  L.off_vals = take(sizeof(double) * block);
+  L.off_vals = take(sizeof(double) * block * ppt);
   L.total = o;
   return L;
 }
@@ -929,6 +934,208 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) 
 }
 
 // --------------------------------------------------------------------------------------------
+// rt_solve2_kernel: the isothermal S3-S7 path with TWO adjacent spectral points per thread (same bin: needs an even
+// number of Gauss points).  Same algorithm and arithmetic as rt_solve_kernel<false, TOA, false, ...>; what changes is
+// the instruction mix: everything that depends only on (column, level, bin) -- the level record, corner weights, row
+// addresses (one 16-byte load per corner instead of two 8-byte ones), Planck value, bin constants, hot constants,
+// loop control -- is issued once for the two points, the two dependence chains interleave in one warp (ILP 2), and
+// the staging / butterfly reductions handle the pair's sum.  A tile is 2 x BLOCK points.
+// --------------------------------------------------------------------------------------------
+struct Rows2 { double2 l00, l01, l10, l11; };
+
+__device__ __forceinline__ Rows2 load_rows2(const double *__restrict__ lnk_pt, const LevelRec *lv) {
+  const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
+  Rows2 r;
+  r.l00 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.x)));
+  r.l01 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.y)));
+  r.l10 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.z)));
+  r.l11 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.w)));
+  return r;
+}
+
+template <bool TOA, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) rt_solve2_kernel(const KParams P) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double s_T32[32];
+  __shared__ int s_is_last;
+  constexpr int TP = 2 * BLOCK;   // points per tile
+  const int N = P.N, nlev = P.nlev;
+  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA, false, 2);
+  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
+  double *s_B = (double *)(smem + L.off_B);
+  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
+  double *s_red = (double *)(smem + L.off_red);
+  double *s_stage = (double *)(smem + L.off_stage);
+  double *s_fin = (double *)(smem + L.off_fin);
+  double *s_vals = (double *)(smem + L.off_vals);
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x, col = blockIdx.y;
+  const int LP = L.LP, nbtS = L.nbt;
+  const double mu = P.mu[col];
+  const bool day = mu > 0.0;
+
+  const int pt0 = tile * TP;
+  const int b_first = pt0 / P.ng;
+  int pt_last = pt0 + TP - 1;
+  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
+  const int nbt = pt_last / P.ng - b_first + 1;
+  const int nwa = ((pt_last - pt0) >> 6) + 1;     // warps that own at least one pair of points
+
+  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid, true);
+  const int col_nan = P.ws_nan[col];
+  __syncthreads();
+
+  // the pair (pt, pt + 1): pt is even and n_gauss is even, so both points lie in bin b
+  int pt = pt0 + 2 * tid;
+  const bool active = pt < P.npt;
+  if (!active) pt = P.npt - 2;
+  const int b = pt / P.ng, gidx = pt - b * P.ng;
+  const int bl = b - b_first;
+  const int warp = tid >> 5, lane = tid & 31;
+  const bool warp_on = warp < nwa;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
+  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
+  const bool want_beam = !TOA && (P.F_beam != nullptr);
+
+  if (warp_on) {
+    const double dlam = P.bins[b].dlam;
+    const double W0 = active ? dlam * P.gauss_w[gidx] : 0.0, W1 = active ? dlam * P.gauss_w[gidx + 1] : 0.0;
+    const double muF = day ? mu * P.fstar[b] : 0.0;
+    const double inv_mu = day ? 1.0 / mu : 0.0;
+    const double *lnk_pt = P.lnk + pt;
+    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
+    const double *T32 = s_T32;
+    double *stage_wr = stage_w + lane;
+
+    constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
+    double2 st_cd0[STK], st_cd1[STK];   // (c, W d) of the two points
+    double2 st_R[STK];                  // (R0, R1)
+
+    double R0 = 0.0, R1 = 0.0, U0 = P.f_toa, U1 = P.f_toa;
+    double Fb0 = muF, Fb1 = muF;
+    double Ct0 = 1.0, Dt0 = 0.0, Ct1 = 1.0, Dt1 = 0.0;
+
+    auto push_interface = [&](int i) {
+      if (!TOA) {
+        st_R[i] = make_double2(R0, R1);
+        stage_wr[(i & 7) * STAGE_LD] = fma(W0, U0 + Fb0, W1 * (U1 + Fb1));
+        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
+        if (want_beam) {
+          const double wb = warp_sum(fma(W0, Fb0, W1 * Fb1));
+          if (lane == 0) red_w[3 * LP + i] = wb;
+        }
+      }
+    };
+
+    auto sweep1 = [&](auto day_tag) {
+      constexpr bool DAY = decltype(day_tag)::value;
+      double tau0 = 0.0, tau1 = 0.0;
+      const LevelRec *lv = s_lev + (N - 1);
+      const double *Bp = s_B + (size_t)(N - 1) * nbtS + bl;
+      Rows2 nx = load_rows2(lnk_pt, lv);
+#pragma unroll (TOA ? kIsoUnrollToa2 : 1)
+      for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
+        const Rows2 cur = nx;
+        nx = load_rows2(lnk_pt, lv - 1);
+        push_interface(j + 1);
+        // S3 + Eqs. 17-18 for the pair: shared corner weights and bin constants
+        const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
+        const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
+        const double lk0 = fma(cb.y, cur.l11.x, fma(cb.x, cur.l10.x, fma(ca.y, cur.l01.x, ca.x * cur.l00.x)));
+        const double lk1 = fma(cb.y, cur.l11.y, fma(cb.x, cur.l10.y, fma(ca.y, cur.l01.y, ca.x * cur.l00.y)));
+        const double ka0 = exp_hot<0, false>(lk0, T32, nullptr), ka1 = exp_hot<0, false>(lk1, T32, nullptr);
+        const BinOpt *bo = lv->cloud ? bin1 : bin0;
+        const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
+        const double g0 = bo->gg, dm = lv->dm, Bj = *Bp;
+        const double kx0 = ka0 + sbss.x, kx1 = ka1 + sbss.x;
+        const double w00 = sbss.y * rcp_fast(kx0), w01 = sbss.y * rcp_fast(kx1);
+        const double dtau0 = kx0 * dm, dtau1 = kx1 * dm;
+        double Fa0 = 0.0, Fa1 = 0.0;
+        if (DAY) {
+          tau0 += dtau0;
+          tau1 += dtau1;
+          Fa0 = muF * exp_hot<1, false>(min_pos(tau0 * inv_mu, 708.0), T32, nullptr);   // (B6)
+          Fa1 = muF * exp_hot<1, false>(min_pos(tau1 * inv_mu, 708.0), T32, nullptr);
+        }
+        double c0, d0, c1, d1;
+        layer_forward<DAY, false>(P, T32, w00, g0, dtau0, Bj, Bj, mu, Fa0, Fb0, R0, U0, c0, d0);
+        layer_forward<DAY, false>(P, T32, w01, g0, dtau1, Bj, Bj, mu, Fa1, Fb1, R1, U1, c1, d1);
+        Fb0 = Fa0;
+        Fb1 = Fa1;
+        if (TOA) {
+          Dt0 = fma(Ct0, d0, Dt0); Ct0 *= c0;
+          Dt1 = fma(Ct1, d1, Dt1); Ct1 *= c1;
+        } else {
+          st_cd0[j + 1] = make_double2(c0, W0 * d0);
+          st_cd1[j + 1] = make_double2(c1, W1 * d1);
+        }
+      }
+    };
+    if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
+
+    // BOA, Eq.(10)
+    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
+    const double Fup00 = (U0 + F_boa + Fb0) * rcp_fast(1.0 - R0), Fup01 = (U1 + F_boa + Fb1) * rcp_fast(1.0 - R1);
+
+    if (TOA) {
+      const double2 gw = make_double2(P.gauss_w[gidx], P.gauss_w[gidx + 1]);
+      s_vals[2 * tid] = active ? gw.x * fma(Ct0, Fup00, Dt0) : 0.0;
+      s_vals[2 * tid + 1] = active ? gw.y * fma(Ct1, Fup01, Dt1) : 0.0;
+    } else {
+      push_interface(0);
+      st_cd0[0] = make_double2(0.0, W0 * Fup00);
+      st_cd1[0] = make_double2(0.0, W1 * Fup01);
+      for (int i = N + 1; i < LP; ++i) {
+        st_cd0[i] = make_double2(1.0, 0.0); st_cd1[i] = make_double2(1.0, 0.0); st_R[i] = make_double2(0.0, 0.0);
+      }
+      double wF0 = 0.0, wF1 = 0.0;
+#pragma unroll 1
+      for (int base = 0; base <= N; base += 8) {
+        double v[16];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const double2 a0 = st_cd0[base + k], a1 = st_cd1[base + k], r = st_R[base + k];
+          wF0 = fma(a0.x, wF0, a0.y);
+          wF1 = fma(a1.x, wF1, a1.y);
+          v[k] = wF0 + wF1;
+          v[8 + k] = fma(r.x, wF0, r.y * wF1);
+        }
+        const double tot = warp_reduce16(v, lane);
+        const int idx = lane >> 1;
+        if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
+      }
+      if (P.F_toa_bin != nullptr) {
+        const double inv_dlam = P.bins[b].inv_dlam;
+        s_vals[2 * tid] = active ? wF0 * inv_dlam : 0.0;
+        s_vals[2 * tid + 1] = active ? wF1 * inv_dlam : 0.0;
+      }
+    }
+  } else if (TOA || P.F_toa_bin != nullptr) {
+    s_vals[2 * tid] = 0.0;
+    s_vals[2 * tid + 1] = 0.0;
+  }
+  __syncthreads();
+
+  if (TOA || P.F_toa_bin != nullptr) {
+    for (int k = tid; k < nbt; k += BLOCK) {
+      const int bb = b_first + k;
+      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
+      const bool whole = (g_lo >= 0) && (g_hi <= TP);
+      if (g_lo < 0) g_lo = 0;
+      if (g_hi > TP) g_hi = TP;
+      double sum = col_nan ? nan("") : 0.0;
+      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
+      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
+      if (whole) *dst = sum; else atomicAdd(dst, sum);
+    }
+  }
+  if (TOA) return;
+
+  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
+}
+
+// --------------------------------------------------------------------------------------------
 // rt_iter_kernel: the scheme Thomas's algorithm replaces (L258-270, L397), as a measured
 // comparison.  Same decomposition, staging and S3-S5 arithmetic as rt_solve_kernel; instead of the forward
 // elimination the (t, r, S_up, S_dn) of every system layer go to thread-private arrays, and the flux arrays are
@@ -1139,6 +1346,13 @@ KernelChoice pick(bool noniso, bool toa, bool bdirect, int block, int minb) {
   return bdirect ? pick_b<true>(noniso, toa, block, minb) : pick_b<false>(noniso, toa, block, minb);
 }
 
+KernelChoice pick2(bool toa, int minb) {
+#define HRT_VARIANT2(M) if (minb == M) return {toa ? rt_solve2_kernel<true, 64, M> : rt_solve2_kernel<false, 64, M>, 64};
+  HRT_VARIANT2(5) HRT_VARIANT2(6) HRT_VARIANT2(7) HRT_VARIANT2(8)
+#undef HRT_VARIANT2
+  return {nullptr, 0};
+}
+
 typedef void (*iter_fn)(const KParams, const int);
 iter_fn pick_iter(bool noniso, int block) {
   switch (block) {
@@ -1182,11 +1396,27 @@ int choose_minb(int block, bool noniso, bool toa) {
   return 0;
 }
 
+// two spectral points per thread (rt_solve2_kernel): isothermal columns with an even number of Gauss points and
+// enough points to fill its 128-point tiles; HELIOS_RT_PPT=1|2 overrides
+int choose_ppt(int npt, int ng, bool noniso) {
+  const bool can = !noniso && ng > 1 && (ng % 2) == 0;
+  const char *env = getenv("HELIOS_RT_PPT");
+  if (env) return (atoi(env) == 2 && can) ? 2 : 1;
+  return (can && npt >= 256) ? 2 : 1;
+}
+
+int choose_minb2() {
+  const char *mb = getenv("HELIOS_RT_MINB");
+  if (mb) { const int v = atoi(mb); if (v >= 5 && v <= 8) return v; }
+  return 8;   // 126 registers, no spills: 8 x 64 threads x 2 points per SM
+}
+
 }  // namespace
 
 struct helios_rt {
   helios_rt_config cfg;   // pointers nulled
-  int npt, block, tiles;
+  int npt, block, tiles, ppt;      // solve kernel: threads per block, tiles per column, points per thread
+  int iter_block, iter_tiles;      // rt_iter_kernel keeps one point per thread
   bool noniso, toa;
   KernelChoice kc;
   SolveSmem lay;
@@ -1319,11 +1549,19 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->npt = nb * ng;
   h->noniso = (cfg->flags & HELIOS_RT_NONISOTHERMAL) != 0;
   h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
-  h->block = choose_block(h->npt);
-  h->tiles = (h->npt + h->block - 1) / h->block;
-  h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso, h->toa));
+  h->iter_block = choose_block(h->npt);
+  h->iter_tiles = (h->npt + h->iter_block - 1) / h->iter_block;
   h->nlev = h->noniso ? 2 * N + 1 : N;
-  h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa, ng == 1);
+  h->ppt = choose_ppt(h->npt, ng, h->noniso);
+  if (h->ppt == 2) {
+    h->block = 64;
+    h->kc = pick2(h->toa, choose_minb2());
+  } else {
+    h->block = h->iter_block;
+    h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso, h->toa));
+  }
+  h->tiles = (h->npt + h->block * h->ppt - 1) / (h->block * h->ppt);
+  h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa, ng == 1, h->ppt);
   cudaGetDevice(&rc);
   cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, rc);
 
@@ -1354,7 +1592,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(upload(&h->d_bins, bins, (size_t)nb));
   free(lnk); free(lp); free(bins);
   const size_t ncol = (size_t)cfg->max_columns;
-  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * h->tiles * 4 * (N + 1)));
+  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * (h->tiles > h->iter_tiles ? h->tiles : h->iter_tiles) * 4 * (N + 1)));
   step(cudaMalloc((void **)&h->d_ws_lev, sizeof(LevelRec) * ncol * (h->nlev + 1)));
   step(cudaMalloc((void **)&h->d_ws_B, sizeof(double) * ncol * (h->nlev + 1) * nb));
   step(cudaMalloc((void **)&h->d_ws_dm, sizeof(double) * ncol * N));
@@ -1371,9 +1609,9 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     step(cudaFuncSetAttribute(h->kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
     step(cudaFuncSetAttribute(h->noniso ? rt_prep_kernel<true> : rt_prep_kernel<false>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prep_smem_bytes(N, h->nlev)));
-    if (!h->toa && pick_iter(h->noniso, h->block))
-      step(cudaFuncSetAttribute(pick_iter(h->noniso, h->block), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)solve_smem(N, h->nlev, h->block, ng, nb, false).total));
+    if (!h->toa && pick_iter(h->noniso, h->iter_block))
+      step(cudaFuncSetAttribute(pick_iter(h->noniso, h->iter_block), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)solve_smem(N, h->nlev, h->iter_block, ng, nb, false).total));
     cudaFuncAttributes fa;
     step(cudaFuncGetAttributes(&fa, h->kc.fn));
     if (e == cudaSuccess) { h->regs = fa.numRegs; h->lmem = (int)fa.localSizeBytes; }
@@ -1409,7 +1647,7 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.lnk = h->d_lnk; P.tab_lp = h->d_tab_lp; P.tab_t = h->d_tab_t; P.edges = h->d_edges; P.gauss_w = h->d_gw;
   P.bins = h->d_bins;
   P.nP = c.n_ktab_p; P.nT = c.n_ktab_t; P.N = c.n_layers; P.nlev = h->nlev; P.nb = c.n_bins; P.ng = c.n_gauss; P.npt = h->npt;
-  P.tiles = h->tiles;
+  P.tiles = n_iter > 0 ? h->iter_tiles : h->tiles;
   P.cloud_p_top = c.cloud_p_top; P.cloud_p_bot = c.cloud_p_bot; P.inv_g = 1.0 / c.gravity; P.inv_cp = 1.0 / c.cp;
   P.inv_eps2 = 1.0 / c.eps2; P.e_tau = c.e_tau; P.gcrit_tol = c.gcrit_tol; P.w0_transition = c.w0_transition;
   P.f_toa = c.f_toa; P.improved = (c.flags & HELIOS_RT_IMPROVED) ? 1 : 0;
@@ -1420,7 +1658,7 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.partial = h->d_partial; P.counter = h->d_counter;
   P.ws_lev = h->d_ws_lev; P.ws_B = h->d_ws_B; P.ws_dm = h->d_ws_dm; P.ws_nan = h->d_ws_nan;
   // bins that straddle two tiles are accumulated with atomics: start from zero
-  if (P.F_toa_bin && h->tiles > 1 && (h->block % c.n_gauss) != 0) {
+  if (P.F_toa_bin && h->tiles > 1 && ((h->block * h->ppt) % c.n_gauss) != 0) {
     const size_t n = (size_t)in->n_columns * c.n_bins;
     zero_kernel<<<(unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, st>>>(P.F_toa_bin, n);
   }
@@ -1432,12 +1670,12 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   else rt_prep_kernel<false><<<pgrid, PREP_BLOCK, psm, st>>>(P);
   CK(h, cudaGetLastError());
   if (ev) CK(h, cudaEventRecord(ev[1], st));
-  dim3 grid((unsigned)h->tiles, (unsigned)in->n_columns);
+  dim3 grid((unsigned)P.tiles, (unsigned)in->n_columns);
   if (n_iter > 0) {
-    iter_fn fn = pick_iter(h->noniso, h->block);
+    iter_fn fn = pick_iter(h->noniso, h->iter_block);
     if (!fn) return HELIOS_RT_EINVAL;
-    const SolveSmem lay = solve_smem(c.n_layers, h->nlev, h->block, c.n_gauss, c.n_bins, false);
-    fn<<<grid, h->block, lay.total, st>>>(P, n_iter);
+    const SolveSmem lay = solve_smem(c.n_layers, h->nlev, h->iter_block, c.n_gauss, c.n_bins, false);
+    fn<<<grid, h->iter_block, lay.total, st>>>(P, n_iter);
   } else {
     h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
   }
