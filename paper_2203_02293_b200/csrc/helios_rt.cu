@@ -1135,6 +1135,216 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve2_kernel(const KParams P)
   column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
 }
 
+template <bool TOA, int PPT, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) rt_solvem_kernel(const KParams P) {
+  static_assert(PPT == 2 || PPT == 4, "points per thread");
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double s_T32[32];
+  __shared__ int s_is_last;
+  constexpr int TP = PPT * BLOCK;   // points per tile
+  constexpr int H = PPT / 2;        // 16-byte loads per corner row
+  const int N = P.N, nlev = P.nlev;
+  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA, false, PPT);
+  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
+  double *s_B = (double *)(smem + L.off_B);
+  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
+  double *s_red = (double *)(smem + L.off_red);
+  double *s_stage = (double *)(smem + L.off_stage);
+  double *s_fin = (double *)(smem + L.off_fin);
+  double *s_vals = (double *)(smem + L.off_vals);
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x, col = blockIdx.y;
+  const int LP = L.LP, nbtS = L.nbt;
+  const double mu = P.mu[col];
+  const bool day = mu > 0.0;
+
+  const int pt0 = tile * TP;
+  const int b_first = pt0 / P.ng;
+  int pt_last = pt0 + TP - 1;
+  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
+  const int nbt = pt_last / P.ng - b_first + 1;
+  const int nwa = ((pt_last - pt0) / (32 * PPT)) + 1;     // warps that own at least one group of points
+
+  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid, true);
+  const int col_nan = P.ws_nan[col];
+  __syncthreads();
+
+  // the group pt .. pt + PPT - 1: pt and n_gauss are multiples of PPT, so all its points lie in bin b
+  int pt = pt0 + PPT * tid;
+  const bool active = pt < P.npt;
+  if (!active) pt = P.npt - PPT;
+  const int b = pt / P.ng, gidx = pt - b * P.ng;
+  const int bl = b - b_first;
+  const int warp = tid >> 5, lane = tid & 31;
+  const bool warp_on = warp < nwa;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
+  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
+  const bool want_beam = !TOA && (P.F_beam != nullptr);
+
+  if (warp_on) {
+    const double dlam = P.bins[b].dlam;
+    double W[PPT];
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) W[q] = active ? dlam * P.gauss_w[gidx + q] : 0.0;
+    const double muF = day ? mu * P.fstar[b] : 0.0;
+    const double inv_mu = day ? 1.0 / mu : 0.0;
+    const double *lnk_pt = P.lnk + pt;
+    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
+    const double *T32 = s_T32;
+    double *stage_wr = stage_w + lane;
+
+    constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
+    double2 st_cd[STK][PPT];   // (c, W d) per point
+    double st_R[STK][PPT];
+
+    double R[PPT], U[PPT], Fb[PPT], Ct[PPT], Dt[PPT];
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) { R[q] = 0.0; U[q] = P.f_toa; Fb[q] = muF; Ct[q] = 1.0; Dt[q] = 0.0; }
+
+    auto push_interface = [&](int i) {
+      if (!TOA) {
+        double su = 0.0, sb = 0.0;
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) { st_R[i][q] = R[q]; su = fma(W[q], U[q] + Fb[q], su); sb = fma(W[q], Fb[q], sb); }
+        stage_wr[(i & 7) * STAGE_LD] = su;
+        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
+        if (want_beam) {
+          const double wb = warp_sum(sb);
+          if (lane == 0) red_w[3 * LP + i] = wb;
+        }
+      }
+    };
+
+    struct RowsM { double2 l00[H], l01[H], l10[H], l11[H]; };
+    auto load_rows_m = [&](const LevelRec *lv) {
+      const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
+      RowsM r;
+#pragma unroll
+      for (int h = 0; h < H; ++h) {
+        r.l00[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.x)) + h);
+        r.l01[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.y)) + h);
+        r.l10[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.z)) + h);
+        r.l11[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.w)) + h);
+      }
+      return r;
+    };
+
+    auto sweep1 = [&](auto day_tag) {
+      constexpr bool DAY = decltype(day_tag)::value;
+      double tau[PPT];
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) tau[q] = 0.0;
+      const LevelRec *lv = s_lev + (N - 1);
+      const double *Bp = s_B + (size_t)(N - 1) * nbtS + bl;
+      RowsM nx = load_rows_m(lv);
+#pragma unroll 1
+      for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
+        const RowsM cur = nx;
+        nx = load_rows_m(lv - 1);
+        push_interface(j + 1);
+        const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
+        const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
+        const BinOpt *bo = lv->cloud ? bin1 : bin0;
+        const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
+        const double g0 = bo->gg, dm = lv->dm, Bj = *Bp;
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) {
+          const int h = q >> 1;
+          const double r00 = (q & 1) ? cur.l00[h].y : cur.l00[h].x, r01 = (q & 1) ? cur.l01[h].y : cur.l01[h].x;
+          const double r10 = (q & 1) ? cur.l10[h].y : cur.l10[h].x, r11 = (q & 1) ? cur.l11[h].y : cur.l11[h].x;
+          const double lk = fma(cb.y, r11, fma(cb.x, r10, fma(ca.y, r01, ca.x * r00)));
+          const double kx = exp_hot<0, false>(lk, T32, nullptr) + sbss.x;
+          const double w0 = sbss.y * rcp_fast(kx);
+          const double dtau = kx * dm;
+          double Fa = 0.0;
+          if (DAY) {
+            tau[q] += dtau;
+            Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);   // (B6)
+          }
+          double c, d;
+          layer_forward<DAY, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb[q], R[q], U[q], c, d);
+          Fb[q] = Fa;
+          if (TOA) {
+            Dt[q] = fma(Ct[q], d, Dt[q]);
+            Ct[q] *= c;
+          } else {
+            st_cd[j + 1][q] = make_double2(c, W[q] * d);
+          }
+        }
+      }
+    };
+    if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
+
+    // BOA, Eq.(10)
+    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
+    double Fup0[PPT];
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) Fup0[q] = (U[q] + F_boa + Fb[q]) * rcp_fast(1.0 - R[q]);
+
+    if (TOA) {
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? P.gauss_w[gidx + q] * fma(Ct[q], Fup0[q], Dt[q]) : 0.0;
+    } else {
+      push_interface(0);
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) st_cd[0][q] = make_double2(0.0, W[q] * Fup0[q]);
+      for (int i = N + 1; i < LP; ++i)
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) { st_cd[i][q] = make_double2(1.0, 0.0); st_R[i][q] = 0.0; }
+      double wF[PPT];
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) wF[q] = 0.0;
+#pragma unroll 1
+      for (int base = 0; base <= N; base += 8) {
+        double v[16];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          double su = 0.0, sd = 0.0;
+#pragma unroll
+          for (int q = 0; q < PPT; ++q) {
+            const double2 a = st_cd[base + k][q];
+            wF[q] = fma(a.x, wF[q], a.y);
+            su += wF[q];
+            sd = fma(st_R[base + k][q], wF[q], sd);
+          }
+          v[k] = su;
+          v[8 + k] = sd;
+        }
+        const double tot = warp_reduce16(v, lane);
+        const int idx = lane >> 1;
+        if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
+      }
+      if (P.F_toa_bin != nullptr) {
+        const double inv_dlam = P.bins[b].inv_dlam;
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? wF[q] * inv_dlam : 0.0;
+      }
+    }
+  } else if (TOA || P.F_toa_bin != nullptr) {
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = 0.0;
+  }
+  __syncthreads();
+
+  if (TOA || P.F_toa_bin != nullptr) {
+    for (int k = tid; k < nbt; k += BLOCK) {
+      const int bb = b_first + k;
+      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
+      const bool whole = (g_lo >= 0) && (g_hi <= TP);
+      if (g_lo < 0) g_lo = 0;
+      if (g_hi > TP) g_hi = TP;
+      double sum = col_nan ? nan("") : 0.0;
+      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
+      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
+      if (whole) *dst = sum; else atomicAdd(dst, sum);
+    }
+  }
+  if (TOA) return;
+
+  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
+}
+
 // --------------------------------------------------------------------------------------------
 // rt_iter_kernel: the scheme Thomas's algorithm replaces (L258-270, L397), as a measured
 // comparison.  Same decomposition, staging and S3-S5 arithmetic as rt_solve_kernel; instead of the forward
@@ -1353,6 +1563,9 @@ KernelChoice pick2(bool toa, int minb) {
   return {nullptr, 0};
 }
 
+// four points per thread: TOA mode only (no stack), 12 warp-sized blocks per SM at 164 registers
+KernelChoice pick4() { return {rt_solvem_kernel<true, 4, 32, 9>, 32}; }
+
 typedef void (*iter_fn)(const KParams, const int);
 iter_fn pick_iter(bool noniso, int block) {
   switch (block) {
@@ -1396,13 +1609,16 @@ int choose_minb(int block, bool noniso, bool toa) {
   return 0;
 }
 
-// two spectral points per thread (rt_solve2_kernel): isothermal columns with an even number of Gauss points and
-// enough points to fill its 128-point tiles; HELIOS_RT_PPT=1|2 overrides
-int choose_ppt(int npt, int ng, bool noniso) {
-  const bool can = !noniso && ng > 1 && (ng % 2) == 0;
+// spectral points per thread: isothermal columns whose number of Gauss points is a multiple of it, with enough points
+// to fill the tiles.  2 (rt_solve2_kernel) with the back-substitution stack; 4 (rt_solvem_kernel) in TOA mode, where no
+// stack competes for the load/store path (measured, config 2 / config 5 solve kernel: 1: 0.716 / 4.97 ms, 2: 0.67 / 4.73,
+// 4: 0.80 / 4.52).  HELIOS_RT_PPT=1|2|4 overrides.
+int choose_ppt(int npt, int ng, bool noniso, bool toa) {
+  const bool can2 = !noniso && ng > 1 && (ng % 2) == 0, can4 = can2 && toa && (ng % 4) == 0;
   const char *env = getenv("HELIOS_RT_PPT");
-  if (env) return (atoi(env) == 2 && can) ? 2 : 1;
-  return (can && npt >= 256) ? 2 : 1;
+  if (env) { const int v = atoi(env); return (v == 4 && can4) ? 4 : ((v >= 2 && can2) ? 2 : 1); }
+  if (npt < 256) return 1;
+  return can4 ? 4 : (can2 ? 2 : 1);
 }
 
 int choose_minb2() {
@@ -1552,8 +1768,11 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->iter_block = choose_block(h->npt);
   h->iter_tiles = (h->npt + h->iter_block - 1) / h->iter_block;
   h->nlev = h->noniso ? 2 * N + 1 : N;
-  h->ppt = choose_ppt(h->npt, ng, h->noniso);
-  if (h->ppt == 2) {
+  h->ppt = choose_ppt(h->npt, ng, h->noniso, h->toa);
+  if (h->ppt == 4) {
+    h->block = 32;
+    h->kc = pick4();
+  } else if (h->ppt == 2) {
     h->block = 64;
     h->kc = pick2(h->toa, choose_minb2());
   } else {
