@@ -204,6 +204,41 @@ def test_postprocessing_pipeline_extension_step_phase_curve(torch_cuda, H):
     rt.close()
 
 
+def test_postprocessing_full_size_sampled(torch_cuda, H):
+    """Config 6 at full size, in the launch configuration bench_next times (2562 columns x 60 layers x 3255 wavelengths):
+    sampled columns of the spectrum against the oracle run on those columns alone (columns are independent), and the
+    phase curve of the full GPU spectrum against the oracle's reduction of the same array."""
+    import oracle
+    from oracle import postproc
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(6)
+    n, N, ne, nb = meta["n_columns"], meta["n_model_layers"], meta["n_extra"], meta["n_bins"]
+    pe = torch.empty((n, N + ne), dtype=torch.float64, device="cuda:0")
+    Te = torch.empty_like(pe)
+    H.extend_top(_t(torch, inp["p"]), _t(torch, inp["T"]), ne, meta["p_min"], pe, Te)
+    rt = H.HeliosRT(cfg, n)
+    spec = torch.full((n, nb), float("nan"), dtype=torch.float64, device="cuda:0")
+    rt.step(pe, Te, _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"]), inp["f_internal"], {"F_up_toa_bin": spec})
+    na = meta["alpha"].size
+    ph = torch.empty((na, nb), dtype=torch.float64, device="cuda:0")
+    band = torch.empty((na,), dtype=torch.float64, device="cuda:0")
+    H.phase_curve(spec, _t(torch, meta["lon"]), _t(torch, meta["lat"]), _t(torch, meta["area"]), _t(torch, meta["alpha"]), ph,
+                  bin_edges=_t(torch, cfg["bin_edges"]), lam1=meta["band"][0], lam2=meta["band"][1], F_phase_band=band)
+    torch.cuda.synchronize()
+    got = spec.cpu().numpy()
+    assert np.all(np.isfinite(got)) and np.all(got >= 0)
+    cols = np.array([0, 1290, 2561])
+    pe_ref, Te_ref = postproc.extend_top(inp["p"][cols], inp["T"][cols], ne, meta["p_min"])
+    ref = oracle.rt_step(cfg, dict(inp, p=pe_ref, T=Te_ref, mu_star=inp["mu_star"][cols]), want=("F_up_toa_bin",))["F_up_toa_bin"]
+    tol = FLUX_RTOL * np.abs(ref) + FLUX_FLOOR * inp["stellar_flux"][None, :]
+    assert np.all(np.abs(got[cols] - ref) <= tol), f"max err/tol {np.max(np.abs(got[cols] - ref) / tol):.3g}"
+    ph_ref, band_ref = postproc.phase_curve(got, meta["lon"], meta["lat"], meta["area"], meta["alpha"][::8], cfg["bin_edges"], *meta["band"])
+    assert np.allclose(ph.cpu().numpy()[::8], ph_ref, rtol=1e-12, atol=1e-13 * np.abs(ph_ref).max())
+    assert np.allclose(band.cpu().numpy()[::8], band_ref, rtol=1e-12)
+    rt.close()
+
+
 # ------------------------------------------------------------------------------------------ NEXT-3
 def test_advance_1d_matches_the_oracle(torch_cuda, H):
     from oracle import onedim

@@ -153,9 +153,9 @@ def test_configs_subsampled_columns(torch_cuda, H, oracle_mod, config, stride):
     assert (inp["mu_star"] > 0).any() and (inp["mu_star"] <= 0).any()
 
 
-@pytest.mark.parametrize("config", [2, 3])
+@pytest.mark.parametrize("config", [2, 3, 4])
 def test_full_size_launch_sampled_columns(torch_cuda, H, oracle_mod, config):
-    """The launch configuration bench.py times (all 2562 columns in one step); columns are
+    """The launch configuration bench.py times (all 2562 / 10242 columns in one step); columns are
     independent, so sampled columns are checked against the oracle run on those columns alone."""
     from paper_2203_02293_b200 import workloads as W
     cfg, inp, meta = W.make(config)
