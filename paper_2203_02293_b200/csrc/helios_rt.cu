@@ -1579,16 +1579,17 @@ iter_fn pick_iter(bool noniso, int block) {
 
 const int kBlocks[] = {32, 64, 96, 128};
 
-// block size: columns with many spectral points use 128-thread tiles (4-5 resident blocks per SM keep the fp64
-// pipe fed while other blocks sit in their prologue or reductions: measured best on configs 2-5); small
-// columns take the block with the fewest padded lanes, ties -> larger block (fewer tiles)
-int choose_block(int npt) {
+// block size of the one-point-per-thread kernels: columns with many spectral points use 128-thread tiles, except the
+// non-isothermal solve kernel, which runs best as 16 warp-sized blocks per SM at 128 registers (config 3 / 4:
+// 1.390 / 5.41 ms against 1.427 / 5.60 at 128 x 4 and 1.460 / 5.73 at 64 x 8); small columns take the block with the
+// fewest padded lanes, ties -> larger block (fewer tiles)
+int choose_block(int npt, bool noniso_solve = false) {
   const char *env = getenv("HELIOS_RT_BLOCK");
   if (env) {
     const int v = atoi(env);
     for (int b : kBlocks) if (b == v) return v;
   }
-  if (npt >= 256) return 128;
+  if (npt >= 256) return noniso_solve ? 32 : 128;
   int best = 32;
   long best_waste = -1;
   for (int b : {32, 64, 96, 128}) {
@@ -1776,7 +1777,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     h->block = 64;
     h->kc = pick2(h->toa, choose_minb2());
   } else {
-    h->block = h->iter_block;
+    h->block = choose_block(h->npt, h->noniso);
     h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso, h->toa));
   }
   h->tiles = (h->npt + h->block * h->ppt - 1) / (h->block * h->ppt);
