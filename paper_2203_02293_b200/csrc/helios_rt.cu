@@ -270,13 +270,30 @@ __device__ __forceinline__ double exp_hot(double x, const double *__restrict__ T
 // S5 for one (sub-)layer between a lower level "a" and an upper level "b": transmission t = psi/chi, reflection
 // r = -xi/chi and the sources of  F_up[b] = t F_up[a] + r F_dn[b] + S_up,  F_dn[a] = t F_dn[b] + r F_up[a] + S_dn.
 // --------------------------------------------------------------------------------------------
+// the terms of S5 that depend on the asymmetry factor g0 alone.  On isothermal columns g0 is a per-(bin, cloud flag)
+// constant, so they are built once at staging time (BinOpt); non-isothermal sub-layers average g0 and build them here.
+struct G0Terms {
+  double g0;
+  double fg;   // Eq.(19): 1.225 - 0.1582 g0 - 0.07465 g0^2
+  double fA;   // Eq.(19): -0.1777 + 0.2351 g0   (fit = fg + w0 (fA - 0.05582 w0))
+  double ge;   // g0 / eps2, (B8)
+};
+__device__ __forceinline__ G0Terms g0_terms(double g0, double inv_eps2) {
+  G0Terms t;
+  t.g0 = g0;
+  t.fg = fma(g0, fma(kHC.fc, g0, kHC.fb), kHC.fa);
+  t.fA = fma(g0, kHC.fe, kHC.fd);
+  t.ge = g0 * inv_eps2;
+  return t;
+}
+
 template <bool DAY, bool LINSRC>
-__device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+__device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__restrict__ T32, double w0, const G0Terms &gt,
                                              double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
                                              double &t_out, double &r_out, double &Sup_out, double &Sdn_out) {
   // E, Eq.(19) L374 (readings R5, R6): E = max(1, fit) if w0 > 0.1 else 1
-  const double fg = fma(g0, fma(kHC.fc, g0, kHC.fb), kHC.fa);
-  const double fit = fma(w0, fma(g0, kHC.fe, fma(kHC.ff, w0, kHC.fd)), fg);
+  const double g0 = gt.g0;
+  const double fit = fma(w0, fma(kHC.ff, w0, gt.fA), gt.fg);
   const double E = (P.improved && gt_pos(w0, P.w0_transition) && gt_pos(fit, 1.0)) ? fit : 1.0;
   const double wg = w0 * g0;
   const double num = E - w0;             // E - omega0
@@ -319,7 +336,7 @@ __device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__r
     D = abs_lt(D, P.gcrit_tol) ? -2.0 * mu : D;
     const double invD = rcp_fast(D);
     const double hP = 0.5 * (num * rs2);                     // 1 / (2 E (1 - w0 g0))
-    const double ge = g0 * P.inv_eps2;
+    const double ge = gt.ge;
     const double lead = (0.5 * w0) * fma(2.0, den, ge) * invD;
     const double last = (0.5 * w0) * ge * hP;
     const double Gp = fma(lead, hP - mu, last);
@@ -336,11 +353,11 @@ __device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__r
 // In: (R, U) at the upper level: F_dn[b] = R F_up[b] + U.   Out: (R, U) at the lower level and the
 // back-substitution pair (c, d): F_up[b] = c F_up[a] + d.
 template <bool DAY, bool LINSRC>
-__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, const G0Terms &gt,
                                               double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
                                               double &R, double &U, double &c, double &d) {
   double t, r, Sup, Sdn;
-  layer_coeffs<DAY, LINSRC>(P, T32, w0, g0, dtau, Ba, Bb, mu, Fa, Fb, t, r, Sup, Sdn);
+  layer_coeffs<DAY, LINSRC>(P, T32, w0, gt, dtau, Ba, Bb, mu, Fa, Fb, t, r, Sup, Sdn);
   // forward elimination (Eqs. 13-14 specialised): F_up[b] (1 - r R) = t F_up[a] + r U + S_up
   const double q = rcp_fast(fma(-r, R, 1.0));
   c = t * q;
@@ -382,6 +399,19 @@ __device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
     v[0] = keep + __shfl_xor_sync(full, send, 2);
   }
   return v[0] + __shfl_xor_sync(full, v[0], 1);
+}
+
+template <bool DAY, bool LINSRC>
+__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+                                              double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
+                                              double &R, double &U, double &c, double &d) {
+  layer_forward<DAY, LINSRC>(P, T32, w0, g0_terms(g0, P.inv_eps2), dtau, Ba, Bb, mu, Fa, Fb, R, U, c, d);
+}
+template <bool DAY, bool LINSRC>
+__device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__restrict__ T32, double w0, double g0,
+                                             double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
+                                             double &t_out, double &r_out, double &Sup_out, double &Sdn_out) {
+  layer_coeffs<DAY, LINSRC>(P, T32, w0, g0_terms(g0, P.inv_eps2), dtau, Ba, Bb, mu, Fa, Fb, t_out, r_out, Sup_out, Sdn_out);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -543,7 +573,9 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
 // --------------------------------------------------------------------------------------------
 constexpr int STAGE_LD = 36;   // row stride (doubles) of the per-warp 8 x 32 staging tile: conflict-free transpose
 
-struct __align__(16) BinOpt { double sb, ss, gg, pad; };   // per bin of the tile: [0][bin] clear level, [1][bin] cloudy level
+// per bin of the tile: [0][bin] clear level, [1][bin] cloudy level.  gt: the g0-only terms of S5 (G0Terms)
+struct __align__(16) BinOpt { double sb, ss; G0Terms gt; double pad[2]; };
+static_assert(sizeof(BinOpt) == 64, "BinOpt layout");
 
 struct SolveSmem {
   int nbt;         // max bins per tile
@@ -604,7 +636,7 @@ __device__ __forceinline__ void level_optics(const Rows &rw, const double *__res
   const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
   kx = kabs + sbss.x;
   w0 = sbss.y * rcp_fast(kx);
-  g0 = bo->gg;
+  g0 = bo->gt.g0;
 }
 
 // sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
@@ -643,7 +675,7 @@ __device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &
       const int cl = i / nbt, k = i - cl * nbt;
       const BinConst bc = P.bins[b_first + k];
       BinOpt bo;
-      bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gg = bc.gg[cl]; bo.pad = 0.0;
+      bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2); bo.pad[0] = bo.pad[1] = 0.0;
       s_bin[cl * nbtS + k] = bo;
     }
   }
@@ -1047,7 +1079,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve2_kernel(const KParams P)
         const double ka0 = exp_hot<0, false>(lk0, T32, nullptr), ka1 = exp_hot<0, false>(lk1, T32, nullptr);
         const BinOpt *bo = lv->cloud ? bin1 : bin0;
         const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
-        const double g0 = bo->gg, dm = lv->dm, Bj = *Bp;
+        const G0Terms gt = bo->gt;
+        const double dm = lv->dm, Bj = *Bp;
         const double kx0 = ka0 + sbss.x, kx1 = ka1 + sbss.x;
         const double w00 = sbss.y * rcp_fast(kx0), w01 = sbss.y * rcp_fast(kx1);
         const double dtau0 = kx0 * dm, dtau1 = kx1 * dm;
@@ -1059,8 +1092,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solve2_kernel(const KParams P)
           Fa1 = muF * exp_hot<1, false>(min_pos(tau1 * inv_mu, 708.0), T32, nullptr);
         }
         double c0, d0, c1, d1;
-        layer_forward<DAY, false>(P, T32, w00, g0, dtau0, Bj, Bj, mu, Fa0, Fb0, R0, U0, c0, d0);
-        layer_forward<DAY, false>(P, T32, w01, g0, dtau1, Bj, Bj, mu, Fa1, Fb1, R1, U1, c1, d1);
+        layer_forward<DAY, false>(P, T32, w00, gt, dtau0, Bj, Bj, mu, Fa0, Fb0, R0, U0, c0, d0);
+        layer_forward<DAY, false>(P, T32, w01, gt, dtau1, Bj, Bj, mu, Fa1, Fb1, R1, U1, c1, d1);
         Fb0 = Fa0;
         Fb1 = Fa1;
         if (TOA) {
@@ -1247,7 +1280,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solvem_kernel(const KParams P)
         const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
         const BinOpt *bo = lv->cloud ? bin1 : bin0;
         const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
-        const double g0 = bo->gg, dm = lv->dm, Bj = *Bp;
+        const G0Terms gt = bo->gt;
+        const double dm = lv->dm, Bj = *Bp;
 #pragma unroll
         for (int q = 0; q < PPT; ++q) {
           const int h = q >> 1;
@@ -1263,7 +1297,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rt_solvem_kernel(const KParams P)
             Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);   // (B6)
           }
           double c, d;
-          layer_forward<DAY, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb[q], R[q], U[q], c, d);
+          layer_forward<DAY, false>(P, T32, w0, gt, dtau, Bj, Bj, mu, Fa, Fb[q], R[q], U[q], c, d);
           Fb[q] = Fa;
           if (TOA) {
             Dt[q] = fma(Ct[q], d, Dt[q]);
