@@ -2,19 +2,21 @@
 //
 // C ABI: include/helios_rt.h.  Citations are PAPER.md lines (arXiv 2203.02293).
 //
-// One fused kernel per step.  A thread block owns one atmospheric column and a tile of its
-// (bin, Gauss point) spectral points; one thread = one spectral point = one monochromatic
-// two-stream problem over the column (the unit the paper solves independently, L449/L592):
+// Two launches per step, both on the caller's stream:
 //
-//   prologue (block-cooperative, shared memory): S1 level geometry (interface p,T; layer masses;
-//            k-table cell + weights per level) and S2 band Planck B_b(T_level) for the tile's bins.
-//   sweep 1  (per thread, TOA -> BOA): S3 bilinear ln(kappa) interpolation + exp, S4 omega0/g0/dtau,
-//            tau prefix and direct beam (Eq. B6), S5 layer coefficients (Eq. 19, B1, B2, B5, B8,
-//            Eq. 11 guard) and the forward elimination of S6.  The block-tridiagonal system of
-//            Eq.(12) has one non-zero in each off-diagonal 2x2 block, so Eqs.(13)-(14) reduce to the
-//            scalar recurrences (R, U, c, d) below; they are carried in registers.
-//   sweep 2  (BOA -> TOA): back-substitution Eq.(15) fused with S7, the Gauss-/bin-weighted
-//            reduction (warp shuffles, then shared memory, then a fixed-order sum over tiles).
+//   rt_prep_kernel   (per column) S1 level geometry -- interface p,T, layer masses, k-table cell + corner weights per
+//                    level -- and S2 band Planck B_b(T_level); results go to the handle's workspace.
+//   rt_solve*_kernel (per spectral point) S3-S7.  A thread block owns one atmospheric column and a tile of its
+//                    (bin, Gauss point) spectral points; one thread = one spectral point = one monochromatic
+//                    two-stream problem over the column (the unit the paper solves independently, L449/L592) --
+//                    or two / four adjacent points of one bin (rt_solve2_kernel / rt_solvem_kernel):
+//     sweep 1 (TOA -> BOA): S3 bilinear ln(kappa) interpolation + exp, S4 omega0/g0/dtau, tau prefix and direct beam
+//              (Eq. B6), S5 layer coefficients (Eq. 19, B1, B2, B5, B8, Eq. 11 guard) and the forward elimination
+//              of S6.  The block-tridiagonal system of Eq.(12) has one non-zero in each off-diagonal 2x2 block, so
+//              Eqs.(13)-(14) reduce to the scalar recurrences (R, U, c, d) below; they are carried in registers.
+//     sweep 2 (BOA -> TOA): back-substitution Eq.(15) fused with S7, the Gauss-/bin-weighted reduction (warp
+//              shuffles, then shared memory, then a fixed-order sum over tiles).
+//   rt_iter_kernel   the pair-wise iterative scheme the paper replaces (helios_rt_step_iterative; comparison only).
 //
 // The layer relations are used in transmission/reflection form.  With zeta+- and T of Eq.(B2),
 //   t = psi/chi = s T / (a b),  r = -xi/chi = zeta+ zeta- (1 - T^2) / (a b),
