@@ -364,3 +364,32 @@ def test_runs_on_a_side_stream(torch_cuda, H, oracle_mod):
     s.synchronize()
     assert np.array_equal(out["F_net"].cpu().numpy(), ref["F_net"])
     rt.close()
+
+
+def test_handle_reuse_fewer_columns_and_interleaved_handles(torch_cuda, H, oracle_mod):
+    """One handle stepped repeatedly with 16, 5, 16 columns (workspace, tile-arrival counters and partial buffers are
+    reused and re-armed), interleaved with a second, non-isothermal handle on the same stream; every step must equal
+    the oracle on its own inputs, and the repeated step must reproduce itself bit for bit."""
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta = W.make(2, columns=slice(1, None, 170))     # 16 columns, 600 points each (5 tiles per column)
+    n = meta["n_columns"]
+    cfg_n = dict(cfg, flags=cfg["flags"] | W.NONISOTHERMAL)
+    want = ("F_up", "F_down", "F_net", "dTdt")
+    ref_a = oracle_mod.rt_step(cfg, inp, want=want)
+    ref_b = oracle_mod.rt_step(cfg_n, inp, want=want)
+    rt_a, rt_b = H.HeliosRT(cfg, n), H.HeliosRT(cfg_n, n)
+    sub = slice(3, 8)
+    inp5 = dict(inp, p=inp["p"][sub], T=inp["T"][sub], mu_star=inp["mu_star"][sub])
+    g1 = run_gpu(torch, H, cfg, inp, want, rt=rt_a)
+    gb = run_gpu(torch, H, cfg_n, inp, want, rt=rt_b)
+    g5 = run_gpu(torch, H, cfg, inp5, want, rt=rt_a)
+    g2 = run_gpu(torch, H, cfg, inp, want, rt=rt_a)
+    assert_parity(oracle_mod, cfg, inp, meta, g1, ref_a)
+    assert_parity(oracle_mod, cfg_n, inp, meta, gb, ref_b)
+    assert_parity(oracle_mod, cfg, inp5, meta, g5, {k: v[sub] for k, v in ref_a.items()})
+    for k in want:
+        assert np.array_equal(g1[k], g2[k]), k
+        assert np.array_equal(g5[k], g1[k][sub]), k
+    rt_a.close()
+    rt_b.close()
