@@ -94,6 +94,8 @@ def lib(real: str = "ld") -> C.CDLL:
         L.oracle_assemble_blocks.argtypes = mono + [_dp] * 5
         L.oracle_rt_step.restype = C.c_int
         L.oracle_rt_step.argtypes = [C.POINTER(_Config), C.POINTER(_Inputs), C.POINTER(_Outputs)]
+        L.oracle_level_optics.restype = None
+        L.oracle_level_optics.argtypes = [C.POINTER(_Config), C.c_double, C.c_double, C.c_int, C.c_int, _dp]
         L.oracle_sizeof_real.restype = C.c_int
         _libs[real] = L
     return _libs[real]
@@ -179,6 +181,24 @@ def assemble_blocks(dtau, w0, g0, B_lo, B_hi, mu, Fstar, F_boa, *, improved=True
     A, B, Cm, D, fb = np.empty(4 * n), np.empty(4 * n), np.empty(4 * n), np.empty(2 * n), np.empty(n)
     lib(real).oracle_assemble_blocks(*args, _p(A), _p(B), _p(Cm), _p(D), _p(fb))
     return A.reshape(n, 2, 2), B.reshape(n, 2, 2), Cm.reshape(n, 2, 2), D.reshape(n, 2), fb
+
+
+def level_optics(cfg: dict, p: float, T: float, b: int, g: int, real: str = "ld"):
+    """(kappa_ext, omega0, g0) at one level for (bin b, Gauss point g): Eqs.(17)-(18) in per-mass units, the
+    function the step itself calls.  cfg as for rt_step."""
+    o = {**_DEFAULTS, **{k: cfg[k] for k in _DEFAULTS if k in cfg}}
+    ktab = _a(cfg["ktab"])
+    nP, nT, nb, ng = ktab.shape
+    keep = {k: _a(cfg[k]) for k in ("ktab_p", "ktab_t", "bin_edges", "gauss_w", "scat_gas", "cloud_ext", "cloud_w0",
+                                    "cloud_g0")}
+    c = _Config(1, nb, ng, nP, nT, _p(keep["ktab_p"]), _p(keep["ktab_t"]), _p(ktab), _p(keep["bin_edges"]),
+                _p(keep["gauss_w"]), _p(keep["scat_gas"]), _p(keep["cloud_ext"]), _p(keep["cloud_w0"]),
+                _p(keep["cloud_g0"]), float(cfg["cloud_p_top"]), float(cfg["cloud_p_bot"]),
+                float(cfg["gravity"]), float(cfg["cp"]), o["eps2"], o["e_tau"], o["gcrit_tol"],
+                o["w0_transition"], o["f_toa"], int(cfg["flags"]), 0)
+    out = np.empty(3)
+    lib(real).oracle_level_optics(C.byref(c), float(p), float(T), int(b), int(g), _p(out))
+    return tuple(out.tolist())
 
 
 def rt_step(cfg: dict, inp: dict, *, real: str = "ld", threads: int | None = None,

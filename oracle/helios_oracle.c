@@ -505,6 +505,15 @@ static void level_optics(const oracle_config *cfg, const ktable *kt, real p, rea
     *g0 = (s_gas + s_c > 0) ? s_c * (real)cfg->cloud_g0[b] / (s_gas + s_c) : 0;
 }
 
+/* exported for the pins of Eqs. 17-18 (tests/test_oracle_pins.py): the same level_optics the step uses; out = {k_ext, w0, g0} */
+void oracle_level_optics(const oracle_config *cfg, double p, double T, int b, int g, double *out3)
+{
+    const ktable kt = {cfg->n_ktab_p, cfg->n_ktab_t, cfg->n_bins, cfg->n_gauss, cfg->ktab_p, cfg->ktab_t, cfg->ktab};
+    real k, w, gg;
+    level_optics(cfg, &kt, (real)p, (real)T, b, g, &k, &w, &gg);
+    out3[0] = (double)k; out3[1] = (double)w; out3[2] = (double)gg;
+}
+
 int oracle_rt_step(const oracle_config *cfg, const oracle_inputs *in, const oracle_outputs *out)
 {
     const int N = cfg->n_layers, nb = cfg->n_bins, ng = cfg->n_gauss, npt = nb * ng;

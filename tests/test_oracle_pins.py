@@ -603,3 +603,187 @@ def test_full_step_opaque_isothermal_atmosphere(oracle_mod):
         assert np.allclose(res["F_up"][:, :-3], ref, rtol=1e-12) and np.allclose(res["F_down"][:, :-3], ref, rtol=1e-12)
         dm = np.abs(np.diff(oracle_mod.levels(one["p"][0], one["T"][0])[0])) / cfg["gravity"]
         assert np.all(np.abs(res["dTdt"][:, :-4]) <= 1e-12 * ref / (cfg["cp"] * dm[:-4]))
+
+
+# ---------------------------------------------------------------- round 2: pins that are not restatements
+# level_optics (Eqs. 17-18), the sub-layer means (L171, reading R10) and the heating rate
+# (L393 / L1032, reading R14) were only checked against numpy re-typings of the same expressions.  The tests
+# below start from what the paper prints (number densities and cross sections; the sentence of L171; energy
+# conservation and Beer's law) and each names the planted mistake it fails on.
+
+AMU = 1.66053906660e-27
+
+
+def _optics_cfg(kappa, scat_gas, cloud_ext, cloud_w0, cloud_g0, p_top=1e2, p_bot=1e5, nb=1, ng=1):
+    """A k-table that is constant in (P, T): kappa_abs = `kappa` at every level."""
+    return dict(ktab_p=np.array([1.0, 1e7]), ktab_t=np.array([100.0, 3000.0]),
+                ktab=np.broadcast_to(np.asarray(kappa, dtype=float).reshape(1, 1, nb, ng), (2, 2, nb, ng)).copy(),
+                bin_edges=np.linspace(1e-6, 2e-6, nb + 1), gauss_w=np.full(ng, 1.0 / ng),
+                scat_gas=np.full(nb, scat_gas), cloud_ext=np.full(nb, cloud_ext), cloud_w0=np.full(nb, cloud_w0),
+                cloud_g0=np.full(nb, cloud_g0), cloud_p_top=p_top, cloud_p_bot=p_bot, gravity=10.0, cp=1e4, flags=1)
+
+
+def test_eq17_eq18_from_number_density_form(oracle_mod):
+    """Eqs.(17),(18) as printed: cross sections per particle weighted by number densities,
+        w0 = (sig_scat,gas + f sig_scat,cloud) / (sig_scat,gas + kappa mbar + f (sig_abs,cloud + sig_scat,cloud)),
+        g0 = f sig_scat,cloud / (sig_scat,gas + f sig_scat,cloud) * g0,cloud,
+    evaluated at 40 digits from hand numbers; the library inputs are those numbers divided by mbar
+    (include/helios_rt.h: scat_gas = sig_scat,gas / mbar, cloud_ext = f (sig_abs + sig_scat)_cloud / mbar,
+    cloud_w0 = sig_scat / (sig_abs + sig_scat)).  Planted mistakes that fail here: s_c <-> k_c (cloud extinction
+    instead of cloud scattering in either numerator), kappa_abs missing from / doubled in the denominator,
+    g0 weighted by the extinction instead of the scattering fraction."""
+    mp.mp.dps = 40
+    mbar = mp.mpf("2.34") * mp.mpf(AMU)                      # L348: 2.34 amu
+    sig_gas = mp.mpf("2.0e-31")                              # m^2 per gas particle
+    kap = mp.mpf("5.0e-5")                                   # m^2 / kg
+    f = mp.mpf("1e-17")                                      # L364
+    sig_abs, sig_sca, g_cl = mp.mpf("1.0e-12"), mp.mpf("3.0e-12"), mp.mpf("0.6")
+    w0_ref = (sig_gas + f * sig_sca) / (sig_gas + kap * mbar + f * (sig_abs + sig_sca))
+    g0_ref = f * sig_sca / (sig_gas + f * sig_sca) * g_cl
+    kext_ref = (sig_gas + kap * mbar + f * (sig_abs + sig_sca)) / mbar
+    cfg = _optics_cfg(float(kap), float(sig_gas / mbar), float(f * (sig_abs + sig_sca) / mbar),
+                      float(sig_sca / (sig_abs + sig_sca)), float(g_cl))
+    kx, w0, g0 = oracle_mod.level_optics(cfg, 1e4, 1000.0, 0, 0)            # inside the cloud deck
+    assert abs(w0 - float(w0_ref)) <= 1e-14 * float(w0_ref)
+    assert abs(g0 - float(g0_ref)) <= 1e-14 * float(g0_ref)
+    assert abs(kx - float(kext_ref)) <= 1e-14 * float(kext_ref)
+    # the hand numbers make the planted mistakes visible: scattering vs extinction differ by 4/3
+    assert abs(float((sig_gas + f * (sig_abs + sig_sca)) / (sig_gas + kap * mbar + f * (sig_abs + sig_sca))) - w0) > 0.05
+    # outside the deck (p < cloud_p_top or p > cloud_p_bot) the cloud terms drop out: f = 0 in Eqs.(17),(18)
+    for p_out in (50.0, 2e5):
+        kx, w0, g0 = oracle_mod.level_optics(cfg, p_out, 1000.0, 0, 0)
+        assert g0 == 0.0
+        assert abs(w0 - float(sig_gas / (sig_gas + kap * mbar))) <= 1e-14 * w0
+        assert abs(kx - float((sig_gas + kap * mbar) / mbar)) <= 1e-14 * kx
+    # deck edges are inclusive (include/helios_rt.h: cloud_p_top <= p <= cloud_p_bot)
+    assert oracle_mod.level_optics(cfg, 1e2, 1000.0, 0, 0)[2] > 0 and oracle_mod.level_optics(cfg, 1e5, 1000.0, 0, 0)[2] > 0
+
+
+def test_eq17_eq18_limits(oracle_mod):
+    """Limits of Eqs.(17),(18): no gas scattering => g0 = g0,cloud exactly and w0 = cloud_w0 k_c / (kappa + k_c);
+    no cloud (cloud_ext = 0) => g0 = 0 and w0 = s / (kappa + s); purely scattering cloud without gas absorption
+    would give w0 -> 1.  A g0 weighted with the extinction instead of the scattering fraction fails the first."""
+    cfg = _optics_cfg(2e-3, 0.0, 6e-3, 0.25, 0.7)
+    kx, w0, g0 = oracle_mod.level_optics(cfg, 1e4, 500.0, 0, 0)
+    assert g0 == 0.7
+    assert abs(w0 - 0.25 * 6e-3 / 8e-3) < 1e-15 and abs(kx - 8e-3) < 1e-17
+    cfg = _optics_cfg(2e-3, 5e-4, 0.0, 0.9, 0.7)
+    kx, w0, g0 = oracle_mod.level_optics(cfg, 1e4, 500.0, 0, 0)
+    assert g0 == 0.0 and abs(w0 - 0.2) < 1e-15 and abs(kx - 2.5e-3) < 1e-17
+    # gas and cloud scattering equal => g0 is exactly half the cloud's (number-density weighting of Eq. 18)
+    cfg = _optics_cfg(1e-3, 3e-3, 6e-3, 0.5, 0.8)
+    assert abs(oracle_mod.level_optics(cfg, 1e4, 500.0, 0, 0)[2] - 0.4) < 1e-15
+
+
+def test_sublayer_means_are_means_of_final_quantities(oracle_mod):
+    """Reading R10 of L171 ("their values in the upper and lower sub-layers are taken to be the arithmetic mean of
+    their central and interface values", said of the opacities AND the single-scattering albedos): a two-layer
+    hand example in which the mean of w0 differs from the w0 of the mean ingredients.  Level values (typed by hand):
+        kappa_abs = 1, 3, 9, 27, 81 e-3 at the five levels (bottom interface, centre 0, interface 1, centre 1, top),
+        gas scattering 1e-3, no cloud  =>  kappa_ext = 2, 4, 10, 28, 82 e-3;  w0 = 1/2, 1/4, 1/10, 1/28, 1/82
+        sub-layer means   kappa_ext: 3, 7, 19, 55 e-3     w0: 3/8, 7/40, 19/280, 55/2296
+        (ingredient averaging would give w0 = 1/3, 1/7, 1/19, 1/55 instead.)
+    The full step must equal column_mono (pinned by the ODE / LU / worked-example tests) fed with the hand values;
+    it must NOT equal column_mono fed with the ingredient-averaged albedos."""
+    sq = np.sqrt(10.0)
+    p = np.array([[1e5, 1e4]])
+    p_lev = np.array([1e5 * sq, 1e5, np.sqrt(1e9), 1e4, 1e4 / sq])          # reading R9, pinned by test_levels_*
+    kap = np.array([1.0, 3.0, 9.0, 27.0, 81.0]) * 1e-3
+    order = np.argsort(p_lev)
+    cfg = dict(ktab_p=p_lev[order], ktab_t=np.array([100.0, 3000.0]),
+               ktab=np.repeat(kap[order].reshape(5, 1, 1, 1), 2, axis=1).copy(),
+               bin_edges=np.array([1e-6, 2e-6]), gauss_w=np.array([1.0]), scat_gas=np.array([1e-3]),
+               cloud_ext=np.array([0.0]), cloud_w0=np.array([0.0]), cloud_g0=np.array([0.0]), cloud_p_top=1.0,
+               cloud_p_bot=2.0, gravity=10.0, cp=1e4, flags=1 | 2)
+    T = np.array([[1500.0, 900.0]])
+    inp = dict(p=p, T=T, mu_star=np.array([0.7]), stellar_flux=np.array([3e9]), f_internal=0.0)
+    res = oracle_mod.rt_step(cfg, inp, want=("F_up", "F_down", "F_beam"))
+    dm = (p_lev[:-1] - p_lev[1:]) / 10.0
+    kx_mean = np.array([3.0, 7.0, 19.0, 55.0]) * 1e-3
+    w_mean = np.array([3 / 8, 7 / 40, 19 / 280, 55 / 2296])
+    w_ingr = np.array([1 / 3, 1 / 7, 1 / 19, 1 / 55])
+    T_lev = np.array([1500.0, 1500.0, 1200.0, 900.0, 900.0])                # reading R9: ends held, interior mean
+    B = np.array([oracle_mod.planck_bin_mean(t, 1e-6, 2e-6) for t in T_lev])
+    dlam = 1e-6
+
+    def mono(w):
+        fu, fd, fb = oracle_mod.column_mono(kx_mean * dm, w, np.zeros(4), B[:-1], B[1:], 0.7, 3e9, 0.0, linear_source=True)
+        return dlam * fu[::2], dlam * (fd + fb)[::2]
+
+    up, dn = mono(w_mean)
+    assert np.allclose(res["F_up"][0], up, rtol=1e-12) and np.allclose(res["F_down"][0], dn, rtol=1e-12)
+    up_bad, dn_bad = mono(w_ingr)
+    assert np.max(np.abs(res["F_up"][0] - up_bad) / np.abs(up)) > 1e-3        # the other reading is far away
+    # the same for the opacity: kappa_ext of a sub-layer is the mean of the two level values (not e.g. the
+    # geometric mean or the lower level's value): tau at the bottom from the beam, Eq.(B6)
+    tau0 = -0.7 * np.log(res["F_beam"][0, 0] / (dlam * 0.7 * 3e9))
+    assert abs(tau0 - float(np.sum(kx_mean * dm))) <= 1e-11 * tau0
+
+
+def _beam_only_case(nb=2, ng=2):
+    """Cold, purely absorbing column under the stellar beam only, opaque at the bottom."""
+    N = 12
+    p = np.logspace(5, 0.5, N)[None, :]
+    kap = np.array([[2e-3, 8e-3], [5e-4, 3e-2]])[:nb, :ng]
+    cfg = _optics_cfg(kap, 0.0, 0.0, 0.0, 0.0, nb=nb, ng=ng)
+    cfg["bin_edges"] = np.array([0.4e-6, 0.9e-6, 2.5e-6])[:nb + 1]       # x = hc/(lam k T) > 100 at T = 50 K: B = 0
+    cfg["gauss_w"] = np.array([0.35, 0.65])[:ng] if ng == 2 else np.array([1.0])
+    inp = dict(p=p, T=np.full((1, N), 50.0), mu_star=np.array([0.05]), stellar_flux=np.array([4e11, 1.5e11])[:nb],
+               f_internal=0.0)
+    return cfg, inp, N, kap
+
+
+def test_heating_rate_energy_closure(oracle_mod):
+    """Reading R14 (L393, L1032: the heating term 'depends on the spatial gradient of the net flux'): whatever the
+    column, the energy deposited per unit area and time, sum_j c_P dm_j dT/dt_j, must equal what enters through the
+    boundaries, F_net[0] - F_net[N] (F_net positive upward): energy conservation, not a re-typing of the difference
+    formula.  dm_j comes from the separately pinned interface pressures.  Fails on: sign flip of dT/dt, dm of the
+    wrong layer (j+1 or the sub-layer), a missing 1/c_P or 1/g, F_net differenced across two layers."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(1)
+    for flags in (W.IMPROVED, W.IMPROVED | W.NONISOTHERMAL):
+        c = dict(cfg, flags=flags)
+        sub = dict(inp, p=inp["p"][:6], T=inp["T"][:6], mu_star=inp["mu_star"][:6])
+        res = oracle_mod.rt_step(c, sub, want=("F_net", "dTdt"))
+        for k in range(6):
+            p_int, _ = oracle_mod.levels(sub["p"][k], sub["T"][k])
+            dm = (p_int[:-1] - p_int[1:]) / c["gravity"]
+            dep = np.sum(c["cp"] * dm * res["dTdt"][k])
+            scale = np.sum(np.abs(c["cp"] * dm * res["dTdt"][k]))
+            assert abs(dep - (res["F_net"][k, 0] - res["F_net"][k, -1])) <= 1e-12 * scale
+            # and layer by layer the deposited power is the flux convergence (sign: net upward flux leaving > entering cools)
+            assert np.allclose(c["cp"] * dm * res["dTdt"][k], res["F_net"][k, :-1] - res["F_net"][k, 1:], rtol=1e-10,
+                               atol=1e-13 * scale)
+
+
+def test_heating_rate_beam_only_closed_form(oracle_mod):
+    """Sign AND scale of dT/dt from a closed form: cold (B = 0), purely absorbing (w0 = 0), no internal flux, opaque at
+    the bottom (so the BOA reflection of Eq. 10 returns nothing): the only flux is the direct beam of Eq.(B6) /
+    Beer's law (L235), F_net = -sum_b dlam_b sum_g w_g mu F*_b exp(-tau/mu), so every layer is HEATED by
+        dT/dt_j = sum_b dlam_b sum_g w_g mu F*_b (exp(-tau_{j+1}/mu) - exp(-tau_j/mu)) / (c_P dm_j)  > 0,
+    tau_j = kappa (p_int,j - p_int,N) / g.  Evaluated at 30 digits.  Fails on: sign flip, dm of a neighbouring
+    layer, missing c_P, dlam or w_g weights dropped, beam not counted in F_down (L235)."""
+    mp.mp.dps = 30
+    cfg, inp, N, kap = _beam_only_case()
+    for flags in (1, 1 | 2):
+        res = oracle_mod.rt_step(dict(cfg, flags=flags), inp, want=("F_up", "F_net", "dTdt"))
+        p_int, _ = oracle_mod.levels(inp["p"][0], inp["T"][0])
+        mu, g, cp = mp.mpf(inp["mu_star"][0]), mp.mpf(10), mp.mpf(1e4)
+        pi = [mp.mpf(float(x)) for x in p_int]
+        ref = []
+        for j in range(N):
+            acc = mp.mpf(0)
+            for b in range(2):
+                dlam = mp.mpf(float(cfg["bin_edges"][b + 1])) - mp.mpf(float(cfg["bin_edges"][b]))
+                for gq in range(2):
+                    k = mp.mpf(float(kap[b, gq]))
+                    t_hi, t_lo = k * (pi[j + 1] - pi[N]) / g, k * (pi[j] - pi[N]) / g
+                    acc += dlam * mp.mpf(float(cfg["gauss_w"][gq])) * mu * mp.mpf(float(inp["stellar_flux"][b])) * \
+                        (mp.e ** (-t_hi / mu) - mp.e ** (-t_lo / mu))
+            ref.append(acc / (cp * (pi[j] - pi[j + 1]) / g))
+        ref = np.array([float(r) for r in ref])
+        assert np.all(ref > 0) and ref.max() > 1e-3                         # a real heating profile
+        assert np.all(res["dTdt"][0] > 0)
+        # (kappa is constant with depth, so the non-isothermal sub-layer treatment must give the same profile)
+        assert np.allclose(res["dTdt"][0], ref, rtol=1e-11, atol=1e-14 * ref.max())
+        assert np.all(np.abs(res["F_up"][0]) <= 1e-40)                        # nothing comes back up (B(50 K) ~ 1e-46)
