@@ -22,8 +22,14 @@
  * the dayside (the paper's mu_star is -mu, App. B); mu_star <= 0: no beam.
  * All arrays are fp64 and C-contiguous, (bin, Gauss point) fastest in the k-table.
  *
- * Threading: a handle may be used by one host thread at a time.  No call throws, aborts or
- * prints.  Every function returns 0 on success or a negative HELIOS_RT_E* code.
+ * Threading: a handle may be used by one host thread at a time, and the steps of one handle must be
+ * stream-ordered (every step uses the handle's workspace, work queues and tile counters: two steps of one handle in
+ * flight on different streams race; use one handle per stream).  The launch shape depends on the problem sizes
+ * only -- never on the environment.  No call throws, aborts or prints.  Every function returns 0 on success or a
+ * negative HELIOS_RT_E* code.
+ *
+ * Test and benchmark hooks are NOT in this header: launch-shape overrides live in helios_rt_debug.h, the device
+ * self-tests and the fp64 FMA microbenchmark in helios_rt_selftest.h (a separate library).
  */
 #ifndef HELIOS_RT_H
 #define HELIOS_RT_H
@@ -109,9 +115,9 @@ typedef struct {
  * On failure *out is NULL. */
 int helios_rt_create(const helios_rt_config *cfg, helios_rt **out);
 
-/* One RT step over in->n_columns columns.  Asynchronous: kernels are enqueued on `cuda_stream`
- * (a cudaStream_t; NULL = the legacy default stream); no host synchronisation, no allocation, no
- * host<->device copy.  Outputs are complete when the stream reaches this point.  NaN inputs
+/* One RT step over in->n_columns columns: ONE kernel launch (rt_step_kernel, S1-S7 fused).  Asynchronous: it is
+ * enqueued on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream); no host synchronisation, no
+ * allocation, no host<->device copy.  Outputs are complete when the stream reaches this point.  NaN inputs
  * propagate to the outputs of their own column only; (p, T) outside the table are clamped to its
  * edge (no extrapolation, not an error). */
 int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
@@ -140,21 +146,11 @@ const char *helios_rt_strerror(int code);
 /* cudaGetErrorString of the last CUDA failure seen by this handle ("" if none). */
 const char *helios_rt_last_cuda_error(const helios_rt *h);
 
-/* Launch geometry of the step kernel for n_columns columns, for benchmarks and profiles:
- * info[0] = threads per block, [1] = blocks per column (tiles), [2] = dynamic shared memory bytes,
- * [3] = registers per thread, [4] = resident blocks per SM (occupancy API), [5] = local-memory
- * bytes per thread, [6] = kernels launched per step, [7] = SM count of the device. */
+/* Launch geometry of the step kernel, for benchmarks and profiles:
+ * info[0] = threads per block, [1] = tiles of the spectral axis per column (the persistent grid is tiles x workers),
+ * [2] = dynamic shared memory bytes, [3] = registers per thread, [4] = resident blocks per SM (occupancy API),
+ * [5] = local-memory bytes per thread, [6] = kernels launched per step (1), [7] = SM count of the device. */
 int helios_rt_launch_info(const helios_rt *h, int32_t info[8]);
-
-/* Per-kernel timing for benchmarks.  With profiling on, every step records three CUDA events on the
- * launching stream (before rt_prep_kernel, between the two kernels, after rt_solve_kernel) into a ring of
- * 256 steps; no synchronisation is added.  Turning it on or off clears the ring. */
-int helios_rt_set_profiling(helios_rt *h, int32_t on);
-
-/* Waits for the recorded steps (at most the last 256 since the previous call) and returns their number
- * and the SUMS of the two kernels' event times in milliseconds: S1+S2 (rt_prep_kernel) and S3-S7
- * (rt_solve_kernel, the dominant kernel of the roofline).  Clears the ring. */
-int helios_rt_kernel_times(helios_rt *h, int32_t *n_steps, double *prep_ms, double *solve_ms);
 
 /* ---- the steps either side of the RT step.  DEVICE pointers, fp64,
  *      C-contiguous, caller-owned; asynchronous on `cuda_stream`; no allocation, no synchronisation (so they can
@@ -191,22 +187,6 @@ int64_t helios_rt_phase_curve_workspace_bytes(int32_t n_columns, int32_t n_bins,
  * R25), rho = p / (R_d T) (rho may be NULL).  T [n_columns][n_layers] is updated in place; p, rho are outputs. */
 int helios_rt_advance_1d(int32_t n_columns, int32_t n_layers, double dt, double gravity, double R_d, double p_ref,
                          const double *z, const double *dTdt, double *T, double *p, double *rho, void *cuda_stream);
-
-/* Device self-test of the fp64 primitives the kernels use instead of the CUDA math library
- * (reciprocal, reciprocal square root, exp / 1-exp).  x: n HOST values; outputs n HOST values each:
- * rcp = 1/x, rsq = 1/sqrt(|x|), ex = exp(-|x|), omx = 1 - exp(-|x|).  Used by the tests. */
-int helios_rt_selftest_math(int32_t n, const double *x, double *rcp, double *rsq, double *ex,
-                            double *omx);
-
-/* Device evaluation of the band Planck function used by S2: out[i] = B_b(T[i]) for the bin
- * [lam_lo[i], lam_hi[i]] (HOST arrays of length n).  Used by the tests. */
-int helios_rt_selftest_planck(int32_t n, const double *T, const double *lam_lo, const double *lam_hi,
-                              double *out);
-
-/* Sustained fp64 FMA rate of the device in DFMA/s (8 independent chains per thread, all SMs),
- * measured over `iters` dependent FMAs per chain; *sm_clock_mhz receives the SM clock implied by
- * clock64() during the run.  This is the measured ALU roofline bench.py reports against. */
-int helios_rt_measure_dfma_peak(int32_t iters, double *dfma_per_s, double *sm_clock_mhz);
 
 #ifdef __cplusplus
 }

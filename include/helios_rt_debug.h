@@ -1,0 +1,35 @@
+/*
+ * helios_rt_debug.h -- NOT part of the product API (include/helios_rt.h).  Launch-shape overrides of the RT step for
+ * tests/ and for tuning runs: the library picks its launch shape from the problem sizes alone (never from the
+ * environment); these two calls let a test force every compiled shape through the same parity checks.
+ */
+#ifndef HELIOS_RT_DEBUG_H
+#define HELIOS_RT_DEBUG_H
+
+#include "helios_rt.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Re-selects the compiled instantiation of rt_step_kernel and the block size of a handle.  A value <= 0 (warps, ppt)
+ * or < 0 (the others) keeps the current / any value.  warps: warps per block (1..maxt/32); ppt: spectral points per
+ * thread (1, 2, 4; n_gauss must be a multiple; non-isothermal handles: 1); rows: 0 = k-table rows by register-prefetched
+ * loads, 1 = by bulk async copies (TMA) into the per-warp shared-memory ring; stk: 1 = back-substitution coefficients in
+ * the global workspace, 0 = thread-private local memory (comparison builds only); maxt, minb: the launch bounds the
+ * instantiation was compiled with (register cap = 65536 / (maxt * minb)).  HELIOS_RT_EINVAL if no such instantiation was
+ * compiled or the shape does not fit an SM; the handle is then unchanged.  Re-allocates the shape-dependent workspace:
+ * must not be called while a step of this handle is in flight. */
+int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t ppt, int32_t rows, int32_t stk, int32_t maxt,
+                               int32_t minb);
+
+/* info[0] = warps per block, [1] = points per thread, [2] = rows, [3] = stk, [4] = maxt, [5] = minb, [6] = tiles per
+ * column, [7] = workers per tile (grid = tiles x workers), [8] = resident blocks per SM, [9] = registers per thread,
+ * [10] = local-memory bytes per thread, [11] = dynamic shared memory bytes, [12] = back-substitution workspace in MiB,
+ * [13] = index of the instantiation, [14] = number of compiled instantiations, [15] = 0. */
+int helios_rt_debug_get_launch(const helios_rt *h, int32_t info[16]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HELIOS_RT_DEBUG_H */

@@ -75,14 +75,6 @@ def bench_postproc(torch, H, W, steps):
     ms_ext, _ = _timed(torch, f_ext, steps, flush, st)
     ms_step, _ = _timed(torch, f_step, steps, flush, st)
     ms_pc, _ = _timed(torch, f_pc, steps, flush, st)
-    rt.set_profiling(True)
-    for _ in range(5):
-        flush.fill_(1.0)
-        f_step()
-    torch.cuda.synchronize()
-    k, prep_ms, solve_ms = rt.kernel_times()
-    prep_ms, solve_ms = prep_ms / k, solve_ms / k
-    rt.set_profiling(False)
     peaks = _peaks()
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     pc_bytes = 8.0 * (n * nb + na * nb + 3 * n + na)       # F read once, phase spectra written once
@@ -100,8 +92,7 @@ def bench_postproc(torch, H, W, steps):
                             "fp64_gflops": pc_flops / (ms_pc * 1e-3) * 1e-9,
                             "note": "3 launches (phase_partial_kernel, phase_reduce_kernel, phase_band_kernel); F is read once "
                                     "per 32 phases; cold L2"},
-            "rt_step_kernels_ms": {"rt_prep_kernel": prep_ms, "rt_solve_kernel": solve_ms},
-            "gpu_launches": steps * 6}
+            "gpu_launches": steps * 5}
     rt.close()
     return line
 

@@ -1,7 +1,10 @@
-"""Build the CUDA C-ABI library in-tree (paper_2203_02293_b200/libhelios_rt.so) for sm_100a.
+"""Build the CUDA C-ABI libraries in-tree for sm_100a:
 
-Every csrc/*.cu is compiled to an object (cached by mtime under csrc/build/) and linked into one shared
-library.  nvcc cross-compiles without a GPU.  `python -m paper_2203_02293_b200.build [--force] [--verbose]`.
+    paper_2203_02293_b200/libhelios_rt.so            the product (include/helios_rt.h, helios_rt_debug.h)
+    paper_2203_02293_b200/libhelios_rt_selftest.so   test / benchmark hooks only (include/helios_rt_selftest.h)
+
+Every csrc/*.cu is compiled to an object (cached by mtime under csrc/build/).  nvcc cross-compiles without a GPU.
+`python -m paper_2203_02293_b200.build [--force] [--verbose]`.
 """
 from __future__ import annotations
 
@@ -15,11 +18,13 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 OBJ = CSRC / "build"
-HDR = ROOT / "include" / "helios_rt.h"
+INC = ROOT / "include"
 LIB = PKG / "libhelios_rt.so"
+LIB_SELFTEST = PKG / "libhelios_rt_selftest.so"
+LIBS = {LIB: ("helios_rt", "helios_post"), LIB_SELFTEST: ("helios_rt_selftest",)}
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC"]
+              "-Xcompiler", "-fPIC", "-split-compile", "0"]
 
 
 def nvcc() -> str:
@@ -39,27 +44,31 @@ def _run(cmd, verbose):
 
 def build(force: bool = False, verbose: bool = False) -> Path:
     sources = sorted(CSRC.glob("*.cu"))
-    deps = [HDR, *CSRC.glob("*.cuh")]
+    deps = [*INC.glob("*.h"), *CSRC.glob("*.cuh"), *CSRC.glob("*.inc")]
     dep_time = max(d.stat().st_mtime for d in deps)
     OBJ.mkdir(exist_ok=True)
-    todo, objs = [], []
+    todo, objs = [], {}
     for src in sources:
         obj = OBJ / (src.stem + ".o")
-        objs.append(obj)
+        objs[src.stem] = obj
         if force or not obj.exists() or obj.stat().st_mtime < max(src.stat().st_mtime, dep_time):
             todo.append((src, obj))
-    if not todo and LIB.exists() and all(LIB.stat().st_mtime >= o.stat().st_mtime for o in objs):
-        return LIB
+
     def compile_one(job):
         src, obj = job
         tmp = obj.with_suffix(f".tmp{os.getpid()}.o")
         _run([nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", "-o", str(tmp), str(src)], verbose)
         os.replace(tmp, obj)
+
     with ThreadPoolExecutor(max_workers=4) as ex:
         list(ex.map(compile_one, todo))
-    tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
-    _run([nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *map(str, objs)], verbose)
-    os.replace(tmp, LIB)
+    for lib, stems in LIBS.items():
+        members = [objs[s] for s in stems]
+        if lib.exists() and all(lib.stat().st_mtime >= o.stat().st_mtime for o in members):
+            continue
+        tmp = lib.with_suffix(f".tmp{os.getpid()}.so")
+        _run([nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *map(str, members)], verbose)
+        os.replace(tmp, lib)
     return LIB
 
 

@@ -1,21 +1,27 @@
 // helios_rt.cu -- B200 (sm_100a) implementation of the THOR+HELIOS radiative-transfer step.
 //
-// C ABI: include/helios_rt.h.  Citations are PAPER.md lines (arXiv 2203.02293).
+// C ABI: include/helios_rt.h.  Citations are PAPER.md lines (arXiv 2203.02293); R-numbers are DESIGN.md readings.
 //
-// Two launches per step, both on the caller's stream:
+// ONE launch per step: rt_step_kernel, a persistent grid of (tiles per column) x (workers) thread blocks.  A block
+// is bound to one tile of the (bin, Gauss point) axis for the whole launch -- so its per-bin optical constants,
+// weights and table addresses are built once -- and pulls atmospheric columns from its tile's queue.  Per column:
 //
-//   rt_prep_kernel   (per column) S1 level geometry -- interface p,T, layer masses, k-table cell + corner weights per
-//                    level -- and S2 band Planck B_b(T_level); results go to the handle's workspace.
-//   rt_solve*_kernel (per spectral point) S3-S7.  A thread block owns one atmospheric column and a tile of its
-//                    (bin, Gauss point) spectral points; one thread = one spectral point = one monochromatic
-//                    two-stream problem over the column (the unit the paper solves independently, L449/L592) --
-//                    or two / four adjacent points of one bin (rt_solve2_kernel / rt_solvem_kernel):
-//     sweep 1 (TOA -> BOA): S3 bilinear ln(kappa) interpolation + exp, S4 omega0/g0/dtau, tau prefix and direct beam
-//              (Eq. B6), S5 layer coefficients (Eq. 19, B1, B2, B5, B8, Eq. 11 guard) and the forward elimination
-//              of S6.  The block-tridiagonal system of Eq.(12) has one non-zero in each off-diagonal 2x2 block, so
-//              Eqs.(13)-(14) reduce to the scalar recurrences (R, U, c, d) below; they are carried in registers.
-//     sweep 2 (BOA -> TOA): back-substitution Eq.(15) fused with S7, the Gauss-/bin-weighted reduction (warp
-//              shuffles, then shared memory, then a fixed-order sum over tiles).
+//   S1  level geometry: interface p, T (R9), layer masses, k-table cell + bilinear corner weights per level
+//   S2  band Planck B_b(T_level) for the tile's bins (piecewise-polynomial G, helios_rt_math.cuh), pi B_b(T_int)
+//       -- both computed by the block itself into shared memory (no second kernel, no workspace round trip)
+//   sweep 1 (TOA -> BOA), one thread = PPT adjacent spectral points of one bin, each a monochromatic two-stream
+//       problem (the unit the paper solves independently, L449/L592): S3 bilinear ln(kappa) + exp (the four
+//       k-table corner rows of a level reach shared memory by one-dimensional bulk async copies -- TMA -- into a
+//       per-warp two-stage ring guarded by mbarriers, or by register-prefetched loads), S4 omega0/g0/dtau, tau
+//       prefix and direct beam (Eq. B6), S5 layer coefficients (Eq. 19, B1, B2, B5, B8, Eq. 11 guard) and the
+//       forward elimination of S6.  The block-tridiagonal system of Eq.(12) has one non-zero in each off-diagonal
+//       2x2 block, so Eqs.(13)-(14) reduce to the scalar recurrences (R, U, c, d) below, carried in registers.
+//       The back-substitution coefficients (c, W d, R) of every interface go to a per-block slab of a global
+//       workspace sized to the resident grid (coalesced 16-byte stores), which the persistent block reuses column
+//       after column, so it lives in L2; its lines are discarded (discard.global.L2) once sweep 2 has read them.
+//   sweep 2 (BOA -> TOA): back-substitution Eq.(15) fused with S7, the Gauss-/bin-weighted reduction (shared-memory
+//       transposes + warp shuffles, then a fixed-order sum over warps and tiles).
+//
 //   rt_iter_kernel   the pair-wise iterative scheme the paper replaces (helios_rt_step_iterative; comparison only).
 //
 // The layer relations are used in transmission/reflection form.  With zeta+- and T of Eq.(B2),
@@ -23,16 +29,11 @@
 //   a = zeta+ - zeta- T,  b = zeta+ + zeta- T,  s = zeta+ - zeta-,  1 - t - r = s (1 - T) / b,
 // Eqs.(2),(3) read  F_up[j+1] = t F_up[j] + r F_dn[j+1] + S_up,  F_dn[j] = t F_dn[j+1] + r F_up[j] + S_dn.
 // These forms avoid the cancellations of chi + xi - psi and 1 - T^2.
-//
-// fp64 throughout.  Reciprocals, reciprocal square roots and exponentials are done with the
-// MUFU seed instructions plus Newton/polynomial refinement in FMA (the fp64 pipe is the binding
-// resource); helios_rt_selftest_math exposes them to the tests.
 
 #include "../../include/helios_rt.h"
+#include "../../include/helios_rt_debug.h"
+#include "helios_rt_math.cuh"
 
-#include <cuda_runtime.h>
-#include <math.h>
-#include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
 #include <new>
@@ -40,136 +41,9 @@
 
 namespace {
 
+using namespace hrt;
+
 constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
-// unroll factors of the isothermal sweep-1 loop, measured on B200: with the back-substitution
-// stack 1 is best (config 2: 0.760 / 0.787 / 0.891 ms at 1 / 2 / 4), the stack-free TOA mode prefers 4 (config 5:
-// 5.31 / 5.13 / 4.98 ms)
-constexpr int kIsoUnroll = 1, kIsoUnrollToa = 4;
-#ifndef HRT_U2
-#define HRT_U2 1
-#endif
-constexpr int kIsoUnrollToa2 = HRT_U2;   // rt_solve2_kernel, TOA mode
-constexpr double kPi = 3.14159265358979323846;
-constexpr double kH = 6.62607015e-34, kC = 299792458.0, kKB = 1.380649e-23;  // CODATA 2019 (exact)
-constexpr double kSigmaSB =
-    2.0 * kPi * kPi * kPi * kPi * kPi * kKB * kKB * kKB * kKB / (15.0 * kH * kH * kH * kC * kC);
-constexpr double kPlanckC1 = 2.0 * kKB * kKB * kKB * kKB / (kH * kH * kH * kC * kC);  // 2 k^4 / (h^3 c^2)
-constexpr double kPlanckC2 = kH * kC / kKB;                                            // h c / k
-
-// --------------------------------------------------------------------------------------------
-// fp64 primitives
-// --------------------------------------------------------------------------------------------
-// MUFU.RCP64H seed (~20 good bits), then y (1 + e + e^2) = (1/x)(1 - e^3): <= 1.5 ulp
-__device__ __forceinline__ double rcp_fast(double x) {
-  double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-x, y, 1.0);
-  e = fma(e, e, e);
-  return fma(y, e, y);
-}
-
-// MUFU.RSQ64H seed, then y (1 + e/2 + 3 e^2/8), e = 1 - x y^2: error O(e^3)
-__device__ __forceinline__ double rsqrt_fast(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double t = x * y;
-  const double e = fma(-t, y, 1.0);
-  const double p = fma(0.375, e, 0.5) * e;
-  return fma(y, p, y);
-}
-
-// positive, non-NaN doubles order like their bit patterns: comparisons on the integer pipes keep the
-// fp64 pipe (the binding resource) for arithmetic
-__device__ __forceinline__ bool gt_pos(double a, double b) { return __double_as_longlong(a) > __double_as_longlong(b); }
-__device__ __forceinline__ bool abs_lt(double a, double b_pos) {
-  return (__double_as_longlong(a) & 0x7fffffffffffffffLL) < __double_as_longlong(b_pos);
-}
-// min(x, c) for x >= 0, c > 0 on the integer pipes
-__device__ __forceinline__ double min_pos(double x, double c) { return gt_pos(x, c) ? c : x; }
-
-// exp by table: e^x = 2^m T[j] (1 + p(r)), k = 32 m + j = round(32 x / ln 2), r = x - k ln2/32, |r| <= ln2/64,
-// T[j] = 2^(j/32) (32 doubles in shared memory), p = expm1(r) by its degree-6 Taylor polynomial (remainder
-// r^7/5040 < 4e-18).  10 fp64 instructions.  The single-constant reduction k * fl(ln2/32) is exact to
-// |k| 2.4e-18, i.e. <= 8e-14 relative at |x| = 700 and <= 3e-15 for |x| <= 30 (far inside the 1e-9 budget).
-//   MODE 0: e^x for |x| <= 708;  MODE 1: e^-a, 0 <= a <= 708;  MODE 2: e^-2a, 0 <= a <= 354, and, if OM,
-//   *om = 1 - e^-2a without cancellation.
-__constant__ double kExp2Tab[32] = {
-    1.0, 1.0218971486541166, 1.0442737824274138, 1.0671404006768237,
-    1.0905077326652577, 1.1143867425958924, 1.1387886347566916, 1.1637248587775775,
-    1.189207115002721, 1.215247359980469, 1.241857812073484, 1.2690509571917332,
-    1.2968395546510096, 1.3252366431597413, 1.3542555469368927, 1.383909881963832,
-    1.4142135623730951, 1.4451808069770467, 1.4768261459394993, 1.5091644275934228,
-    1.5422108254079407, 1.5759808451078865, 1.6104903319492543, 1.645755478153965,
-    1.681792830507429, 1.718619298122478, 1.7562521603732995, 1.7947090750031072,
-    1.8340080864093424, 1.8741676341103, 1.9152065613971474, 1.9571441241754002};
-
-// --------------------------------------------------------------------------------------------
-// S2: band Planck.  G(x) = int_x^inf t^3/(e^t - 1) dt (reading R8).
-//   x >= 1.5 : sum_n e^{-n x} (x^3/n + 3 x^2/n^2 + 6 x/n^3 + 6/n^4)
-//   x <  1.5 : pi^4/15 - sum_k B_k x^{k+3} / ((k+3) k!)   (Bernoulli numbers B_k)
-// --------------------------------------------------------------------------------------------
-// *low receives int_0^x t^3/(e^t-1) dt when x < 1.5 (else -1): a bin whose two edges both lie there is
-// differenced on `low`, which avoids the cancellation against pi^4/15 for narrow Rayleigh-Jeans bins.
-__constant__ double kInvN[33] = {
-    0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8, 1.0 / 9, 1.0 / 10, 1.0 / 11, 1.0 / 12, 1.0 / 13,
-    1.0 / 14, 1.0 / 15, 1.0 / 16, 1.0 / 17, 1.0 / 18, 1.0 / 19, 1.0 / 20, 1.0 / 21, 1.0 / 22, 1.0 / 23, 1.0 / 24, 1.0 / 25,
-    1.0 / 26, 1.0 / 27, 1.0 / 28, 1.0 / 29, 1.0 / 30, 1.0 / 31, 1.0 / 32};
-
-__device__ double planck_G(double x, double *low_out) {
-  *low_out = -1.0;
-  if (!(x > 0.0)) { *low_out = 0.0; return kPi * kPi * kPi * kPi / 15.0; }
-  if (x >= 1.5) {
-    if (x > 745.0) return 0.0;
-    const double u = exp(-x);
-    const double x2 = x * x, x3 = x2 * x, c1 = 6.0 * x, c2 = 3.0 * x2;
-    double un = 1.0, sum = 0.0;
-    // two terms per trip, one convergence test per trip (the terms decrease monotonically)
-    for (int n = 1; n <= 32; n += 2) {
-      const double in1 = kInvN[n], in2 = kInvN[n + 1];   // 1/n, correctly rounded: same value as the division
-      const double un1 = un * u;
-      un = un1 * u;
-      // x^3/n + 3 x^2/n^2 + 6 x/n^3 + 6/n^4
-      const double t1 = un1 * (in1 * fma(in1, fma(in1, fma(in1, 6.0, c1), c2), x3));
-      const double t2 = un * (in2 * fma(in2, fma(in2, fma(in2, 6.0, c1), c2), x3));
-      sum += t1;
-      sum += t2;
-      if (t2 < 1e-18 * sum) break;
-    }
-    return sum;
-  }
-  // coefficients B_k / ((k+3) k!), k = 0,1,2,4,...,30
-  const double c0 = 1.0 / 3.0, c1 = -1.0 / 8.0;
-  const double ce[15] = {
-      1.0 / 60.0,                                   // k=2 : (1/6)/(5*2)
-      -1.0 / 5040.0,                                // k=4 : (-1/30)/(7*24)
-      1.0 / 272160.0,                               // k=6 : (1/42)/(9*720)
-      -1.0 / 13305600.0,                            // k=8
-      1.0 / 622702080.0,                            // k=10
-      -691.0 / (2730.0 * 15.0 * 479001600.0),       // k=12
-      7.0 / (6.0 * 17.0 * 87178291200.0),           // k=14
-      -3617.0 / (510.0 * 19.0 * 20922789888000.0),  // k=16
-      43867.0 / (798.0 * 21.0 * 6402373705728000.0),            // k=18
-      -174611.0 / (330.0 * 23.0 * 2432902008176640000.0),       // k=20
-      854513.0 / (138.0 * 25.0 * 1124000727777607680000.0),     // k=22
-      -236364091.0 / (2730.0 * 27.0 * 620448401733239439360000.0),   // k=24
-      8553103.0 / (6.0 * 29.0 * 403291461126605635584000000.0),      // k=26
-      -23749461029.0 / (870.0 * 31.0 * 304888344611713860501504000000.0),   // k=28
-      8615841276005.0 / (14322.0 * 33.0 * 265252859812191058636308480000000.0)  // k=30
-  };
-  const double x2 = x * x;
-  double s = ce[14];
-#pragma unroll
-  for (int i = 13; i >= 0; --i) s = fma(s, x2, ce[i]);
-  // low = x^3 (c0 + c1 x + x^2 s)
-  const double low = x2 * x * fma(x2, s, fma(c1, x, c0));
-  *low_out = low;
-  return kPi * kPi * kPi * kPi / 15.0 - low;
-}
-
-// G(x_hi_edge) - G(x_lo_edge) for one bin from the per-edge (G, low) pairs (edge e = lam_lo: larger x)
-__device__ __forceinline__ double planck_dG(double G_lo_edge, double low_lo_edge, double G_hi_edge, double low_hi_edge) {
-  return (low_lo_edge >= 0.0 && low_hi_edge >= 0.0) ? (low_lo_edge - low_hi_edge) : (G_hi_edge - G_lo_edge);
-}
 
 // --------------------------------------------------------------------------------------------
 // kernel parameters
@@ -182,7 +56,7 @@ struct BinConst {   // per bin, built at create time from scat_gas / cloud_* (Eq
   double gg[2];     // g0 at a clear / cloudy level
 };
 
-// S1 result per (column, level), written by rt_prep_kernel, staged in shared memory by rt_solve_kernel
+// S1 result per (column, level), built by the block in shared memory
 struct __align__(16) LevelRec {
   double c00, c01, c10, c11;  // bilinear weights of the corners (iP,iT), (iP,iT+1), (iP+1,iT), (iP+1,iT+1)
   unsigned o00, o01, o10, o11;  // offsets of the four corner rows (spectral point 0) in the ln(kappa) table, doubles
@@ -194,13 +68,16 @@ static_assert(sizeof(LevelRec) == 64, "LevelRec layout");
 
 struct KParams {
   // create-time tables (device)
-  const double *lnk;      // [nP][nT][npt] ln(kappa)
+  const double *lnk;      // [nP][nT][row_stride] ln(kappa); rows padded to an even length, + a tail pad
   const double *tab_lp;   // [nP] log10(p)
   const double *tab_t;    // [nT]
   const double *edges;    // [nb+1]
   const double *gauss_w;  // [ng]
   const BinConst *bins;   // [nb]
-  int nP, nT, N, nlev, nb, ng, npt, tiles;
+  const double *gtab;     // Planck polynomial pieces (build_planck_table)
+  int nP, nT, N, nlev, nb, ng, npt, tiles, ncol;
+  unsigned row_stride;
+  double inv_dlp, inv_dt;   // 1 / mean spacing of the table grids: first guess of the cell search
   double cloud_p_top, cloud_p_bot, inv_g, inv_cp, inv_eps2, e_tau, gcrit_tol, w0_transition, f_toa;
   int improved;
   // per-step
@@ -208,75 +85,19 @@ struct KParams {
   double T_int;
   double *F_up, *F_down, *F_net, *dTdt, *F_beam, *F_toa_bin;
   // workspace
-  LevelRec *ws_lev;       // [ncol][nlev+1]   record 0 pads the one-level-ahead prefetch (copy of level 0)
-  double *ws_B;           // [ncol][nlev+1][nb] band Planck per level; last row pi B_b(T_int)
-  double *ws_dm;          // [ncol][N]        full-layer column mass (heating rate)
-  int *ws_nan;            // [ncol]           NaN in p, T of the column
+  double *stack;          // [blocks of the grid][N+1][warps][96 PPT] back-substitution coefficients
+  size_t stack_block;     // doubles per block
   double *partial;        // [ncol][tiles][4][N+1]
-  unsigned *counter;      // [ncol]
+  unsigned *counter;      // [ncol]   tiles of the column that have published their partial sums
+  unsigned *queue;        // [tiles]  next column of each tile's queue;  queue[tiles] = blocks that have finished
 };
-
-// constants of the hot loop live in constant memory: an fp64 instruction takes one operand straight from
-// the constant bank, so none of them costs a register, a move or a uniform-register rematerialisation
-struct HotConst {
-  double S, nS, n2S;      // 32/ln2, -32/ln2, -64/ln2
-  double nL, hL;          // -ln2/32, ln2/64
-  double e6, e5, e4, e3;  // 1/720, 1/120, 1/24, 1/6
-  double q4, q3, q2, q1;  // 4/45, -4/15, 2/3, -4/3
-  double fa, fb, fc;      // Eq.(19): 1.225 - 0.1582 g - 0.07465 g^2
-  double fd, fe, ff;      //          + w (-0.1777 + 0.2351 g - 0.05582 w)
-  double pi, npi;
-};
-__constant__ HotConst kHC = {
-    46.16624130844683,     -46.16624130844683,   -92.33248261689366,
-    -0.02166084939249829,  0.010830424696249145,
-    1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0,
-    4.0 / 45.0, -4.0 / 15.0, 2.0 / 3.0, -4.0 / 3.0,
-    1.225, -0.1582, -0.07465,
-    -0.1777, 0.2351, -0.05582,
-    3.14159265358979323846, -3.14159265358979323846};
-
-// exp by table (see kExp2Tab), constants from kHC.
-//   MODE 0: e^x for |x| <= 708;  MODE 1: e^-a, 0 <= a <= 708;  MODE 2: e^-2a, 0 <= a <= 354, and, if OM,
-//   *om = 1 - e^-2a without cancellation.
-template <int MODE, bool OM>
-__device__ __forceinline__ double exp_hot(double x, const double *__restrict__ T32, double *om) {
-  const double kMagic = 6755399441055744.0;      // 1.5 * 2^52: round-to-nearest-integer trick
-  double kd, p;
-  if (MODE == 0) kd = fma(x, kHC.S, kMagic);
-  else if (MODE == 1) kd = fma(x, kHC.nS, kMagic);
-  else kd = fma(x, kHC.n2S, kMagic);
-  const int ki = __double2loint(kd);
-  const double kf = kd - kMagic;
-  if (MODE == 2) {
-    // r = -2 x - kf L; with h = -r/2 = x + kf L/2:  p = expm1(-2 h) = h (-2 + h q(h))
-    const double h = fma(kf, kHC.hL, x);
-    double q = fma(h, kHC.q4, kHC.q3);
-    q = fma(q, h, kHC.q2);
-    q = fma(q, h, kHC.q1);
-    q = fma(q, h, 2.0);
-    p = h * fma(h, q, -2.0);
-  } else {
-    const double r = (MODE == 0) ? fma(kf, kHC.nL, x) : fma(kf, kHC.nL, -x);
-    double q = fma(r, kHC.e6, kHC.e5);
-    q = fma(q, r, kHC.e4);
-    q = fma(q, r, kHC.e3);
-    q = fma(q, r, 0.5);
-    p = fma(r * r, q, r);
-  }
-  const double Tj = T32[ki & 31];
-  const double Ts = __hiloint2double(__double2hiint(Tj) + ((ki >> 5) << 20), __double2loint(Tj));   // 2^m T[j]
-  if (OM) *om = fma(-Ts, p, 1.0 - Ts);
-  return fma(Ts, p, Ts);
-}
-
 
 // --------------------------------------------------------------------------------------------
 // S5 for one (sub-)layer between a lower level "a" and an upper level "b": transmission t = psi/chi, reflection
 // r = -xi/chi and the sources of  F_up[b] = t F_up[a] + r F_dn[b] + S_up,  F_dn[a] = t F_dn[b] + r F_up[a] + S_dn.
 // --------------------------------------------------------------------------------------------
 // the terms of S5 that depend on the asymmetry factor g0 alone.  On isothermal columns g0 is a per-(bin, cloud flag)
-// constant, so they are built once at staging time (BinOpt); non-isothermal sub-layers average g0 and build them here.
+// constant, so they are built once per block (BinOpt); non-isothermal sub-layers average g0 and build them here.
 struct G0Terms {
   double g0;
   double fg;   // Eq.(19): 1.225 - 0.1582 g0 - 0.07465 g0^2
@@ -379,89 +200,295 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// Sum each of the 16 values v[0..15] over the 32 lanes of the warp by recursive halving: 16 shuffle+add
-// steps instead of 16 x 5.  Returns, in lanes L and L^1, the total of v[L >> 1].  Fixed order: deterministic.
-__device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
-  const unsigned full = 0xffffffffu;
-  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const double send = b4 ? v[i] : v[i + 8], keep = b4 ? v[i + 8] : v[i];
-    v[i] = keep + __shfl_xor_sync(full, send, 16);
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const double send = b3 ? v[i] : v[i + 4], keep = b3 ? v[i + 4] : v[i];
-    v[i] = keep + __shfl_xor_sync(full, send, 8);
-  }
-#pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const double send = b2 ? v[i] : v[i + 2], keep = b2 ? v[i + 2] : v[i];
-    v[i] = keep + __shfl_xor_sync(full, send, 4);
-  }
-  {
-    const double send = b1 ? v[0] : v[1], keep = b1 ? v[1] : v[0];
-    v[0] = keep + __shfl_xor_sync(full, send, 2);
-  }
-  return v[0] + __shfl_xor_sync(full, v[0], 1);
+// --------------------------------------------------------------------------------------------
+// shared-memory layout of one block, PTX helpers
+// --------------------------------------------------------------------------------------------
+constexpr int STAGE_LD = 36;   // row stride (doubles) of the per-warp 8 x 32 staging tile: conflict-free transpose
+constexpr int RING = 2;        // stages of the per-warp k-table row ring (one stage = the rows of one sweep iteration)
+
+// per bin of the tile: [0][bin] clear level, [1][bin] cloudy level.  gt: the g0-only terms of S5 (G0Terms)
+struct __align__(16) BinOpt { double sb, ss; G0Terms gt; double pad[2]; };
+static_assert(sizeof(BinOpt) == 64, "BinOpt layout");
+
+struct Lay {
+  int nbt;         // max bins per tile
+  int LP;          // N + 1 rounded up to a multiple of 8 (the reductions handle 8 interfaces at a time)
+  unsigned off_lev, off_B, off_bin, off_dm, off_red, off_fin, off_vals, off_bar, off_u, total;
+  unsigned u_lnp, u_pint, u_tint, u_tlev, u_G, u_Glow;   // S1/S2 view of the union at off_u
+  unsigned u_stage, u_ring, ring_warp;                   // sweep view: [warp] staging tile; [warp] row ring
+};
+
+// ppt: spectral points per thread; depth: levels per sweep iteration (1 isothermal, 2 non-isothermal); ring: TMA rows
+__host__ __device__ inline Lay make_lay(int N, int nlev, int warps, int ppt, int ng, int nb, bool toa, int depth, bool ring) {
+  Lay L;
+  const int tp = warps * 32 * ppt;
+  const int nbt = (tp + ng - 1) / ng + 1;
+  L.nbt = nbt < nb ? nbt : nb;
+  L.LP = (N + 1 + 7) & ~7;
+  unsigned o = 0;
+  auto take = [&](size_t bytes) { unsigned r = o; o += (unsigned)((bytes + 127) & ~size_t(127)); return r; };
+  L.off_lev = take(sizeof(LevelRec) * (nlev + 1));
+  L.off_B = take(sizeof(double) * (nlev + 1) * L.nbt);
+  L.off_bin = take(sizeof(BinOpt) * 2 * L.nbt);
+  L.off_dm = take(sizeof(double) * N);
+  L.off_red = take(toa ? 0 : sizeof(double) * warps * 4 * L.LP);       // F_up, R F_up, U + beam, beam
+  L.off_fin = take(toa ? 0 : sizeof(double) * 4 * (N + 1));
+  L.off_vals = take(sizeof(double) * tp);
+  L.off_bar = take(8 * RING * warps);
+  L.off_u = o;
+  // S1 / S2 scratch
+  unsigned u = 0;
+  auto utake = [&](size_t bytes) { unsigned r = u; u += (unsigned)((bytes + 15) & ~size_t(15)); return r; };
+  L.u_lnp = utake(sizeof(double) * N);
+  L.u_pint = utake(sizeof(double) * (N + 1));
+  L.u_tint = utake(sizeof(double) * (N + 1));
+  L.u_tlev = utake(sizeof(double) * (nlev + 1));
+  L.u_G = utake(sizeof(double) * (L.nbt + 1) * (nlev + 1));
+  L.u_Glow = utake(sizeof(double) * (L.nbt + 1) * (nlev + 1));
+  const unsigned prep_bytes = u;
+  // sweep scratch
+  u = 0;
+  L.u_stage = utake(toa ? 0 : sizeof(double) * warps * 8 * STAGE_LD);
+  u = (u + 127) & ~127u;
+  L.ring_warp = ring ? (unsigned)(RING * depth * 4 * 32 * ppt * 8) : 0;
+  L.u_ring = utake((size_t)L.ring_warp * warps);
+  const unsigned sweep_bytes = u;
+  L.total = L.off_u + (prep_bytes > sweep_bytes ? prep_bytes : sweep_bytes);
+  return L;
 }
 
-template <bool DAY, bool LINSRC>
-__device__ __forceinline__ void layer_forward(const KParams &P, const double *__restrict__ T32, double w0, double g0,
-                                              double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
-                                              double &R, double &U, double &c, double &d) {
-  layer_forward<DAY, LINSRC>(P, T32, w0, g0_terms(g0, P.inv_eps2), dtau, Ba, Bb, mu, Fa, Fb, R, U, c, d);
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-template <bool DAY, bool LINSRC>
-__device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__restrict__ T32, double w0, double g0,
-                                             double dtau, double Ba, double Bb, double mu, double Fa, double Fb,
-                                             double &t_out, double &r_out, double &Sup_out, double &Sdn_out) {
-  layer_coeffs<DAY, LINSRC>(P, T32, w0, g0_terms(g0, P.inv_eps2), dtau, Ba, Bb, mu, Fa, Fb, t_out, r_out, Sup_out, Sdn_out);
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// one-dimensional bulk async copy global -> shared (TMA; SASS UBLKCP), completion counted on the mbarrier
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "HRT_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra HRT_DONE;\n"
+      "bra HRT_WAIT;\n"
+      "HRT_DONE:\n"
+      "}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+// drop a 128-byte line from L2 without writing it back (its contents are dead)
+__device__ __forceinline__ void l2_discard(const void *p) {
+  asm volatile("discard.global.L2 [%0], 128;" ::"l"(p) : "memory");
+}
+
+// address of element `off` (32-bit, unsigned) of a double array: one IMAD.WIDE.U32
+__device__ __forceinline__ const double *elem_addr(const double *base, unsigned off) {
+  unsigned long long a;
+  asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(a) : "r"(off), "l"((unsigned long long)base));
+  return (const double *)a;
+}
+
+// the four k-table corner values of PPT adjacent spectral points at one level
+template <int PPT> struct RowsT { double v[4][PPT]; };
+
+template <int PPT>
+__device__ __forceinline__ void load_rows_g(RowsT<PPT> &r, const double *__restrict__ lnk_pt, const LevelRec *lv) {
+  const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
+  const unsigned off[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const double *a = elem_addr(lnk_pt, off[c]);
+    if (PPT == 1) {
+      r.v[c][0] = __ldg(a);
+    } else {
+#pragma unroll
+      for (int h = 0; h < PPT / 2; ++h) {
+        const double2 t = __ldg(reinterpret_cast<const double2 *>(a) + h);
+        r.v[c][2 * h] = t.x;
+        r.v[c][2 * h + 1] = t.y;
+      }
+    }
+  }
+}
+
+// st: one level of a ring stage, [4][32 PPT] doubles
+template <int PPT>
+__device__ __forceinline__ void load_rows_s(RowsT<PPT> &r, const double *st, int lane) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const double *a = st + c * 32 * PPT + lane * PPT;
+    if (PPT == 1) {
+      r.v[c][0] = *a;
+    } else {
+#pragma unroll
+      for (int h = 0; h < PPT / 2; ++h) {
+        const double2 t = reinterpret_cast<const double2 *>(a)[h];
+        r.v[c][2 * h] = t.x;
+        r.v[c][2 * h + 1] = t.y;
+      }
+    }
+  }
+}
+
+// Row feed of the sweep: DEPTH levels per iteration, top-down.  ROWS = 0: the next iteration's rows are held in
+// registers (loads issued one iteration ahead).  ROWS = 1: a per-warp ring of RING stages in shared memory, filled by
+// bulk async copies that lane 0 issues two iterations ahead; each stage has its own mbarrier (expect-tx = the
+// stage's bytes); the warp re-arms a stage itself once all its lanes have consumed it, so warps never wait on each
+// other.  `kc` counts iterations since the barriers were initialised and runs across columns: iteration kc uses
+// stage kc % RING in phase (kc / RING) & 1.
+template <int PPT, int DEPTH, int ROWS> struct Feed;
+
+template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 0> {
+  RowsT<PPT> nx[DEPTH];
+  const double *lnk_pt;
+  const LevelRec *lv0;   // record of level 0 (lowest): prefetches below it are clamped
+  __device__ __forceinline__ void load(const LevelRec *lv) {
+#pragma unroll
+    for (int d = 0; d < DEPTH; ++d) {
+      const LevelRec *q = lv - d;
+      load_rows_g<PPT>(nx[d], lnk_pt, q < lv0 ? lv0 : q);
+    }
+  }
+  // lv: highest level of the first iteration
+  __device__ __forceinline__ void prime(const LevelRec *lv, int /*iterations*/) { load(lv); }
+  // returns the rows of this iteration; lv_next: highest level of the next iteration
+  __device__ __forceinline__ void next(RowsT<PPT> (&cur)[DEPTH], const LevelRec *lv_next) {
+#pragma unroll
+    for (int d = 0; d < DEPTH; ++d) cur[d] = nx[d];
+    load(lv_next);
+  }
+  __device__ __forceinline__ void release(const LevelRec *, bool) {}
+};
+
+template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 1> {
+  static constexpr uint32_t ROWB = 32 * PPT * 8, STGB = DEPTH * 4 * ROWB;
+  const double *ring;    // this warp's ring (generic address)
+  uint32_t ring_s, bar_s;
+  const double *lnk_w;   // ln(kappa) table + first spectral point of the warp
+  const LevelRec *lv0;
+  uint32_t kc;
+  int lane;
+  __device__ __forceinline__ void fill(uint32_t stage, const LevelRec *lv) {   // lane 0
+    const uint32_t bar = bar_s + 8 * stage, dst = ring_s + stage * STGB;
+    mbar_expect_tx(bar, STGB);
+#pragma unroll
+    for (int d = 0; d < DEPTH; ++d) {
+      const LevelRec *q = lv - d;
+      q = q < lv0 ? lv0 : q;
+      const uint4 o = *reinterpret_cast<const uint4 *>(&q->o00);
+      bulk_g2s(dst + (d * 4 + 0) * ROWB, lnk_w + o.x, ROWB, bar);
+      bulk_g2s(dst + (d * 4 + 1) * ROWB, lnk_w + o.y, ROWB, bar);
+      bulk_g2s(dst + (d * 4 + 2) * ROWB, lnk_w + o.z, ROWB, bar);
+      bulk_g2s(dst + (d * 4 + 3) * ROWB, lnk_w + o.w, ROWB, bar);
+    }
+  }
+  __device__ __forceinline__ void prime(const LevelRec *lv, int iterations) {
+    if (lane == 0) {
+      fill(kc % RING, lv);
+      if (iterations > 1) fill((kc + 1) % RING, lv - DEPTH);
+    }
+  }
+  __device__ __forceinline__ void next(RowsT<PPT> (&cur)[DEPTH], const LevelRec *) {
+    const uint32_t stage = kc % RING;
+    mbar_wait(bar_s + 8 * stage, (kc / RING) & 1u);
+    const double *st = ring + (size_t)stage * (STGB / 8);
+#pragma unroll
+    for (int d = 0; d < DEPTH; ++d) load_rows_s<PPT>(cur[d], st + d * 4 * 32 * PPT, lane);
+  }
+  // call once the iteration's rows are in registers and have been used; lv_refill: highest level of the iteration
+  // RING ahead (has = false: none left in this column)
+  __device__ __forceinline__ void release(const LevelRec *lv_refill, bool has) {
+    __syncwarp();
+    if (lane == 0 && has) fill(kc % RING, lv_refill);
+    ++kc;
+  }
+};
+
+// sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
+// base + k.  Lane L sums 8 entries of row L >> 2, two shuffle steps finish the row.  Fixed order.
+__device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, double *__restrict__ dst, int lane) {
+  __syncwarp();
+  const double *row = stage_w + (lane >> 2) * STAGE_LD + (lane & 3);
+  double s = row[0];
+#pragma unroll
+  for (int i = 1; i < 8; ++i) s += row[4 * i];
+  s += __shfl_xor_sync(0xffffffffu, s, 1);
+  s += __shfl_xor_sync(0xffffffffu, s, 2);
+  if ((lane & 3) == 0) dst[lane >> 2] = s;
+  __syncwarp();
+}
+
+// back-substitution coefficients of one interface, one warp: 96 PPT doubles.  PPT = 1: [c][W d][R] x 32 lanes;
+// PPT >= 2: 16-byte slots [q: (c, W d)] x 32 lanes, then [h: (R_2h, R_2h+1)] x 32 lanes.  L2 only (.cg).
+template <int PPT>
+__device__ __forceinline__ void stk_store(double *w, int lane, const double (&c)[PPT], const double (&wd)[PPT],
+                                          const double (&R)[PPT]) {
+  if (PPT == 1) {
+    __stcg(w + lane, c[0]);
+    __stcg(w + 32 + lane, wd[0]);
+    __stcg(w + 64 + lane, R[0]);
+  } else {
+    double2 *v = reinterpret_cast<double2 *>(w) + lane;
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) __stcg(v + q * 32, make_double2(c[q], wd[q]));
+#pragma unroll
+    for (int h = 0; h < PPT / 2; ++h) __stcg(v + (PPT + h) * 32, make_double2(R[2 * h], R[2 * h + 1]));
+  }
+}
+template <int PPT>
+__device__ __forceinline__ void stk_load(const double *w, int lane, double (&c)[PPT], double (&wd)[PPT], double (&R)[PPT]) {
+  if (PPT == 1) {
+    c[0] = __ldcg(w + lane);
+    wd[0] = __ldcg(w + 32 + lane);
+    R[0] = __ldcg(w + 64 + lane);
+  } else {
+    const double2 *v = reinterpret_cast<const double2 *>(w) + lane;
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) { const double2 t = __ldcg(v + q * 32); c[q] = t.x; wd[q] = t.y; }
+#pragma unroll
+    for (int h = 0; h < PPT / 2; ++h) { const double2 t = __ldcg(v + (PPT + h) * 32); R[2 * h] = t.x; R[2 * h + 1] = t.y; }
+  }
 }
 
 // --------------------------------------------------------------------------------------------
-// rt_prep_kernel: S1 (level geometry, k-table cell + weights per level) and S2 (band Planck per level
-// and bin) for every column.  Grid = (bin chunks of PREP_BINS, columns).  Results go to the handle's
-// workspace (a few tens of MB, L2-resident when rt_solve_kernel reads them back).
+// S1 + S2 for one column, by the whole block, into shared memory.
+//   S1 (L171, R9, R7): ln p, interface p/T, layer masses, and per level a LevelRec: the four bilinear corner weights
+//       (1-w_p)(1-w_T) ..., the four k-table row offsets, the (sub-)layer column mass and the cloud flag.
+//   S2 (L171, L239, R8): planck_G at every (level, bin edge of the tile) -- consecutive lanes take consecutive levels
+//       of one edge, so a warp's arguments x = hc/(lam k T) stay close and its lanes take the same branch -- then B_b
+//       per (level, bin); the extra level nlev carries T_int and yields F_BOA,b = pi B_b(T_int).
+// Ends with a block barrier; the S1/S2 scratch (union) is dead afterwards.
 // --------------------------------------------------------------------------------------------
-constexpr int PREP_BLOCK = 256, PREP_BINS = 32;
-
-__host__ __device__ inline size_t prep_smem_bytes(int N, int nlev) {
-  return sizeof(double) * ((size_t)N + 2 * (N + 1) + (nlev + 1) + 2 * (size_t)(nlev + 1) * (PREP_BINS + 1));
-}
-
 template <bool NONISO>
-__global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  const int N = P.N, nlev = P.nlev;
-  double *s_lnp = (double *)smem;                       // [N]
-  double *s_pint = s_lnp + N;                           // [N+1]
-  double *s_tint = s_pint + (N + 1);                    // [N+1]
-  double *s_tlev = s_tint + (N + 1);                    // [nlev+1], last = internal temperature
-  double *s_G = s_tlev + (nlev + 1);                    // [nlev+1][PREP_BINS+1]
-  double *s_Glow = s_G + (size_t)(nlev + 1) * (PREP_BINS + 1);
-  __shared__ int s_nan;
-  __shared__ short s_rep[2 * MAXL + 2];
-
-  const int tid = threadIdx.x;
-  const int chunk = blockIdx.x, col = blockIdx.y;
+__device__ __forceinline__ void column_prep(const KParams &P, const Lay &L, unsigned char *smem, int col, int b_first,
+                                            int nbt, int *s_nan) {
+  const int N = P.N, nlev = P.nlev, tid = threadIdx.x, nthr = blockDim.x;
+  unsigned char *un = smem + L.off_u;
+  double *s_lnp = (double *)(un + L.u_lnp), *s_pint = (double *)(un + L.u_pint), *s_tint = (double *)(un + L.u_tint);
+  double *s_tlev = (double *)(un + L.u_tlev), *s_G = (double *)(un + L.u_G), *s_Glow = (double *)(un + L.u_Glow);
+  LevelRec *s_rec = (LevelRec *)(smem + L.off_lev);   // record 0 duplicates level 0 (prefetch pad); level l at [l + 1]
+  double *s_B = (double *)(smem + L.off_B), *s_dm = (double *)(smem + L.off_dm);
   const double *pc = P.p + (size_t)col * N;
   const double *Tc = P.T + (size_t)col * N;
-  const int b0 = chunk * PREP_BINS;
-  const int nbc = (P.nb - b0 < PREP_BINS) ? (P.nb - b0) : PREP_BINS;
 
   // NaN in p, T or mu of this column poisons the column's outputs (and only them): the clamps and
-  // selects below would otherwise swallow it.
-  if (tid == 0) { const double mu = P.mu[col]; s_nan = (mu != mu) ? 1 : 0; }
+  // selects below would otherwise swallow it (R19).
+  if (tid == 0) { const double mu = P.mu[col]; *s_nan = (mu != mu) ? 1 : 0; }
   __syncthreads();
-  // ---------------- S1: level geometry (reading R9; L171) ----------------
-  for (int j = tid; j < N; j += PREP_BLOCK) {
+  for (int j = tid; j < N; j += nthr) {
     const double pj = pc[j], tj = Tc[j];
-    if (pj != pj || tj != tj) s_nan = 1;
+    if (pj != pj || tj != tj) *s_nan = 1;
     s_lnp[j] = log(pj);
   }
   __syncthreads();
-  for (int i = tid; i <= N; i += PREP_BLOCK) {
+  for (int i = tid; i <= N; i += nthr) {
     double lp, ti;
     if (N == 1) {
       lp = s_lnp[0] + (i == 0 ? 0.5 : -0.5) * 2.302585092994045684;
@@ -484,219 +511,82 @@ __global__ void __launch_bounds__(PREP_BLOCK) rt_prep_kernel(const KParams P) {
     if (NONISO) return (l & 1) ? pc[l >> 1] : s_pint[l >> 1];
     return pc[l];
   };
-  for (int l = tid; l <= nlev; l += PREP_BLOCK) {
+  for (int l = tid; l <= nlev; l += nthr) {
     if (l == nlev) { s_tlev[l] = P.T_int; continue; }
     const double pl = p_level(l);
     const double tl = NONISO ? ((l & 1) ? Tc[l >> 1] : s_tint[l >> 1]) : Tc[l];
     s_tlev[l] = tl;
-    if (chunk != 0) continue;
     LevelRec rec;
     rec.cloud = (pl >= P.cloud_p_top && pl <= P.cloud_p_bot) ? 1 : 0;
-    // table cell + weights: bilinear in (log10 p, T), clamped (reading R7)
+    // table cell + weights: bilinear in (log10 p, T), clamped (R7).  Cell = the one with grid[i] < x <= grid[i+1]
+    // (x at or below the first node: cell 0); found from a uniform-grid guess corrected by a walk.
     double xp = log10(pl);
     xp = fmin(fmax(xp, P.tab_lp[0]), P.tab_lp[P.nP - 1]);
-    int ip = 0;
+    int ip = (int)((xp - P.tab_lp[0]) * P.inv_dlp);
+    ip = ip < 0 ? 0 : (ip > P.nP - 2 ? P.nP - 2 : ip);
+    while (ip > 0 && !(xp > P.tab_lp[ip])) --ip;
     while (ip < P.nP - 2 && xp > P.tab_lp[ip + 1]) ++ip;
     const double wp = (xp - P.tab_lp[ip]) / (P.tab_lp[ip + 1] - P.tab_lp[ip]);
     const double xt = fmin(fmax(tl, P.tab_t[0]), P.tab_t[P.nT - 1]);
-    int it = 0;
+    int it = (int)((xt - P.tab_t[0]) * P.inv_dt);
+    it = it < 0 ? 0 : (it > P.nT - 2 ? P.nT - 2 : it);
+    while (it > 0 && !(xt > P.tab_t[it])) --it;
     while (it < P.nT - 2 && xt > P.tab_t[it + 1]) ++it;
     const double wt = (xt - P.tab_t[it]) / (P.tab_t[it + 1] - P.tab_t[it]);
     rec.c00 = (1.0 - wp) * (1.0 - wt);
     rec.c01 = (1.0 - wp) * wt;
     rec.c10 = wp * (1.0 - wt);
     rec.c11 = wp * wt;
-    rec.o00 = (unsigned)(ip * P.nT + it) * (unsigned)P.npt;
-    rec.o01 = rec.o00 + (unsigned)P.npt;
-    rec.o10 = rec.o00 + (unsigned)P.nT * (unsigned)P.npt;
-    rec.o11 = rec.o10 + (unsigned)P.npt;
+    rec.o00 = (unsigned)(ip * P.nT + it) * P.row_stride;
+    rec.o01 = rec.o00 + P.row_stride;
+    rec.o10 = rec.o00 + (unsigned)P.nT * P.row_stride;
+    rec.o11 = rec.o10 + P.row_stride;
     rec.pad = 0;
     // column mass below this level down to the next level: full layer (isothermal: level = layer centre,
     // mass between its two interfaces) or sub-layer (non-isothermal: levels alternate interface / centre)
     if (NONISO) rec.dm = (l < nlev - 1) ? (pl - p_level(l + 1)) * P.inv_g : 0.0;
     else rec.dm = (s_pint[l] - s_pint[l + 1]) * P.inv_g;
-    LevelRec *dst = P.ws_lev + (size_t)col * (nlev + 1) + 1 + l;
-    *dst = rec;
-    if (l == 0) dst[-1] = rec;
+    s_rec[1 + l] = rec;
+    if (l == 0) s_rec[0] = rec;
   }
-  if (chunk == 0)
-    for (int j = tid; j < N; j += PREP_BLOCK) P.ws_dm[(size_t)col * N + j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
+  for (int j = tid; j < N; j += nthr) s_dm[j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
   __syncthreads();
-  if (chunk == 0 && tid == 0) P.ws_nan[col] = s_nan;
 
-  // ---------------- S2: band Planck for this chunk's bins (reading R8) ----------------
-  // a level whose temperature equals that of the level below it (an isothermal stretch, e.g. the extension above the
-  // model top, L385) shares that level's cumulative integrals: s_rep[l] = first level of the run
-  const int nedge = nbc + 1;
-  if (tid == 0) {
-    s_rep[0] = 0;
-    for (int l = 1; l <= nlev; ++l) s_rep[l] = (s_tlev[l] == s_tlev[l - 1]) ? s_rep[l - 1] : l;
-  }
-  __syncthreads();
-  // warp w takes levels w, w + 8, ...; lane e takes edge e of the chunk (no integer division, one edge per lane);
-  // the chunk's last edge (index 32) is done afterwards, one level per thread
-  const int wrp = tid >> 5, lane = tid & 31;
-  {
-    const double lam_e = (lane < nedge) ? P.edges[b0 + lane] : 1.0;
-    for (int l = wrp; l <= nlev; l += PREP_BLOCK / 32) {
-      if (s_rep[l] != l || lane >= nedge) continue;
-      const double Tl = s_tlev[l];
-      double low = 0.0;
-      s_G[l * (PREP_BINS + 1) + lane] = (Tl > 0.0) ? planck_G(kPlanckC2 / (lam_e * Tl), &low) : 0.0;
-      s_Glow[l * (PREP_BINS + 1) + lane] = low;
-    }
-    if (nedge == PREP_BINS + 1) {
-      const double lam_last = P.edges[b0 + PREP_BINS];
-      for (int l = tid; l <= nlev; l += PREP_BLOCK) {
-        if (s_rep[l] != l) continue;
-        const double Tl = s_tlev[l];
-        double low = 0.0;
-        s_G[l * (PREP_BINS + 1) + PREP_BINS] = (Tl > 0.0) ? planck_G(kPlanckC2 / (lam_last * Tl), &low) : 0.0;
-        s_Glow[l * (PREP_BINS + 1) + PREP_BINS] = low;
-      }
-    }
+  // ---------------- S2 ----------------
+  const int nedge = nbt + 1, nlevp = nlev + 1;
+  for (int idx = tid; idx < nedge * nlevp; idx += nthr) {
+    const int e = idx / nlevp, l = idx - e * nlevp;
+    const double Tl = s_tlev[l];
+    double low = 0.0, G = 0.0;
+    if (Tl > 0.0) G = planck_G(kPlanckC2 / (P.edges[b_first + e] * Tl), P.gtab, &low);
+    s_G[idx] = G;
+    s_Glow[idx] = low;
   }
   __syncthreads();
-  if (lane < nbc) {
-    const double inv_dlam = P.bins[b0 + lane].inv_dlam;
-    double *dst = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b0 + lane;
-    for (int l = wrp; l <= nlev; l += PREP_BLOCK / 32) {
-      const double Tl = s_tlev[l];
-      const double T2 = Tl * Tl;
-      const double *g = s_G + s_rep[l] * (PREP_BINS + 1) + lane;
-      const double *gl = s_Glow + s_rep[l] * (PREP_BINS + 1) + lane;
-      double B = kPlanckC1 * T2 * T2 * planck_dG(g[0], gl[0], g[1], gl[1]) * inv_dlam;
-      if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
-      dst[(size_t)l * P.nb] = (Tl > 0.0) ? B : 0.0;
-    }
+  for (int idx = tid; idx < nbt * nlevp; idx += nthr) {
+    const int k = idx / nlevp, l = idx - k * nlevp;
+    const double Tl = s_tlev[l];
+    const double T2 = Tl * Tl;
+    const int g0i = k * nlevp + l, g1i = g0i + nlevp;
+    double B = kPlanckC1 * T2 * T2 * planck_dG(s_G[g0i], s_Glow[g0i], s_G[g1i], s_Glow[g1i]) * P.bins[b_first + k].inv_dlam;
+    if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
+    s_B[l * L.nbt + k] = (Tl > 0.0) ? B : 0.0;
   }
-}
-
-// --------------------------------------------------------------------------------------------
-// rt_solve_kernel: S3-S7.  Grid = (tiles per column, columns); a block owns one column and a tile of
-// BLOCK consecutive spectral points (bin-major, Gauss point fastest); one thread = one spectral point.
-// --------------------------------------------------------------------------------------------
-constexpr int STAGE_LD = 36;   // row stride (doubles) of the per-warp 8 x 32 staging tile: conflict-free transpose
-
-// per bin of the tile: [0][bin] clear level, [1][bin] cloudy level.  gt: the g0-only terms of S5 (G0Terms)
-struct __align__(16) BinOpt { double sb, ss; G0Terms gt; double pad[2]; };
-static_assert(sizeof(BinOpt) == 64, "BinOpt layout");
-
-struct SolveSmem {
-  int nbt;         // max bins per tile
-  int LP;          // N + 1 rounded up to a multiple of 8 (the reductions handle 8 levels at a time)
-  size_t off_lev, off_B, off_bin, off_red, off_stage, off_fin, off_vals, total;
-};
-
-__host__ __device__ inline SolveSmem solve_smem(int N, int nlev, int block, int ng, int nb, bool toa, bool bdirect = false,
-                                                int ppt = 1) {
-  SolveSmem L;
-  int nbt = (block * ppt + ng - 1) / ng + 1;   // ppt: spectral points per thread (rt_solve2_kernel: 2)
-  L.nbt = nbt < nb ? nbt : nb;
-  L.LP = (N + 1 + 7) & ~7;
-  const int nwarp = (block + 31) / 32;
-  size_t o = 0;
-  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
-  L.off_lev = take(sizeof(LevelRec) * (nlev + 1));
-  L.off_B = take(bdirect ? 0 : sizeof(double) * (nlev + 1) * L.nbt);   // bdirect: B read straight from the workspace
-  L.off_bin = take(sizeof(BinOpt) * 2 * L.nbt);
-  L.off_red = take(toa ? 0 : sizeof(double) * nwarp * 4 * L.LP);       // F_up, R F_up, U + beam, beam
-  L.off_stage = take(toa ? 0 : sizeof(double) * nwarp * 8 * STAGE_LD);
-  L.off_fin = take(toa ? 0 : sizeof(double) * 4 * (N + 1));
-  L.off_vals = take(sizeof(double) * block * ppt);
-  L.total = o;
-  return L;
-}
-
-struct Rows { double l00, l01, l10, l11; };   // the four k-table corner values of one (level, point)
-
-// address of element `off` (32-bit, unsigned) of a double array: one IMAD.WIDE.U32
-__device__ __forceinline__ const double *elem_addr(const double *base, unsigned off) {
-  unsigned long long a;
-  asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(a) : "r"(off), "l"((unsigned long long)base));
-  return (const double *)a;
-}
-
-__device__ __forceinline__ Rows load_rows(const double *__restrict__ lnk_pt, const LevelRec *lv) {
-  const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
-  Rows r;
-  r.l00 = __ldg(elem_addr(lnk_pt, o.x));
-  r.l01 = __ldg(elem_addr(lnk_pt, o.y));
-  r.l10 = __ldg(elem_addr(lnk_pt, o.z));
-  r.l11 = __ldg(elem_addr(lnk_pt, o.w));
-  return r;
-}
-
-
-// optical properties at one level (S3 + Eqs. 17-18): bilinear ln(kappa) from the four corner rows with the
-// level's corner weights, exp, then kappa_ext, omega0, g0.  bin0 / bin1: the point's BinOpt for clear / cloudy.
-__device__ __forceinline__ void level_optics(const Rows &rw, const double *__restrict__ T32, const LevelRec *lv,
-                                             const BinOpt *bin0, const BinOpt *bin1, double &kx, double &w0,
-                                             double &g0) {
-  const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
-  const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
-  const double lk = fma(cb.y, rw.l11, fma(cb.x, rw.l10, fma(ca.y, rw.l01, ca.x * rw.l00)));
-  const double kabs = exp_hot<0, false>(lk, T32, nullptr);
-  const BinOpt *bo = lv->cloud ? bin1 : bin0;
-  const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
-  kx = kabs + sbss.x;
-  w0 = sbss.y * rcp_fast(kx);
-  g0 = bo->gt.g0;
-}
-
-// sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
-// base + k.  Lane L sums 8 entries of row L >> 2, two shuffle steps finish the row.  Fixed order.
-__device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, double *__restrict__ dst, int lane) {
-  __syncwarp();
-  const double *row = stage_w + (lane >> 2) * STAGE_LD + (lane & 3);
-  double s = row[0];
-#pragma unroll
-  for (int i = 1; i < 8; ++i) s += row[4 * i];
-  s += __shfl_xor_sync(0xffffffffu, s, 1);
-  s += __shfl_xor_sync(0xffffffffu, s, 2);
-  if ((lane & 3) == 0) dst[lane >> 2] = s;
-  __syncwarp();
-}
-
-// stage the column's level records, the tile's Planck values and per-bin optical constants in shared memory
-template <int BLOCK>
-__device__ __forceinline__ void stage_column(const KParams &P, const SolveSmem &L, unsigned char *smem, double *s_T32,
-                                             int col, int b_first, int nbt, int tid, bool stage_B = true) {
-  const int nlev = P.nlev, nbtS = L.nbt;
-  double *s_B = (double *)(smem + L.off_B);
-  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
-  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
-  {
-    const double *src = (const double *)(P.ws_lev + (size_t)col * (nlev + 1));
-    double *dst = (double *)(smem + L.off_lev);
-    for (int i = tid; i < 8 * (nlev + 1); i += BLOCK) dst[i] = src[i];
-    const double *gB = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b_first;
-    if (stage_B)
-      for (int i = tid; i < (nlev + 1) * nbt; i += BLOCK) {
-        const int l = i / nbt, k = i - l * nbt;
-        s_B[l * nbtS + k] = gB[(size_t)l * P.nb + k];
-      }
-    for (int i = tid; i < 2 * nbt; i += BLOCK) {
-      const int cl = i / nbt, k = i - cl * nbt;
-      const BinConst bc = P.bins[b_first + k];
-      BinOpt bo;
-      bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2); bo.pad[0] = bo.pad[1] = 0.0;
-      s_bin[cl * nbtS + k] = bo;
-    }
-  }
+  __syncthreads();
 }
 
 // cross-warp sum of the per-warp interface sums (s_red: [warp][4][LP] = F_up, diffuse F_dn part 1, part 2 (+ beam),
-// beam), tile partials in fixed order, and the column's outputs written by its last tile
-template <int BLOCK>
-__device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSmem &L, double *s_red, double *s_fin,
-                                                int *s_is_last_p, int nwa, bool want_beam, int col, int tile, int col_nan) {
-  const int N = P.N, LP = L.LP, tid = threadIdx.x;
+// beam), tile partials in fixed order, and the column's outputs written by its last tile.  A tile publishes its
+// partial sums with a release atomic (no L1 invalidation); only the column's last tile takes the acquire fence.
+__device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, unsigned char *smem, int *s_is_last_p,
+                                                int nwa, bool want_beam, int col, int tile, int col_nan) {
+  const int N = P.N, LP = L.LP, tid = threadIdx.x, nthr = blockDim.x;
+  double *s_red = (double *)(smem + L.off_red), *s_fin = (double *)(smem + L.off_fin);
+  const double *s_dm = (const double *)(smem + L.off_dm);
   int &s_is_last = *s_is_last_p;
-  // cross-warp sum in fixed order -> tile partial: F_up, R F_up, U + beam, beam
   const int nq = want_beam ? 4 : 3;
   const int nred = nq * (N + 1);
-  for (int k = tid; k < nred; k += BLOCK) {
+  for (int k = tid; k < nred; k += nthr) {
     const int q = k / (N + 1), lev = k - q * (N + 1);
     double sum = 0.0;
     for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
@@ -705,21 +595,22 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSme
   __syncthreads();
 
   if (P.tiles > 1) {
-    // publish the tile partial; the last tile of the column to arrive sums them in tile order
     double *part = P.partial + ((size_t)col * P.tiles + tile) * 4 * (N + 1);
-    for (int k = tid; k < nred; k += BLOCK) part[k] = s_fin[k];
-    __threadfence();
+    for (int k = tid; k < nred; k += nthr) __stcg(part + k, s_fin[k]);
     __syncthreads();
     if (tid == 0) {
-      const unsigned prev = atomicAdd(P.counter + col, 1u);
+      unsigned prev;
+      asm volatile("atom.add.release.gpu.global.u32 %0, [%1], 1;" : "=r"(prev) : "l"(P.counter + col) : "memory");
       s_is_last = (prev == (unsigned)(P.tiles - 1));
-      if (s_is_last) P.counter[col] = 0;   // re-arm for the next step
+      if (s_is_last) {
+        P.counter[col] = 0;   // re-arm for the next step
+        __threadfence();      // acquire side: the other tiles' partial sums are visible below
+      }
     }
     __syncthreads();
     if (!s_is_last) return;
-    __threadfence();
     const double *pall = P.partial + (size_t)col * P.tiles * 4 * (N + 1);
-    for (int k = tid; k < nred; k += BLOCK) {
+    for (int k = tid; k < nred; k += nthr) {
       double sum = 0.0;
       for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 4 * (N + 1) + k);
       s_fin[k] = sum;
@@ -729,7 +620,7 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSme
 
   // final outputs of the column: F_down = sum W R F_up + sum W (U + beam)
   const double poison = col_nan ? nan("") : 0.0;
-  for (int i = tid; i <= N; i += BLOCK) {
+  for (int i = tid; i <= N; i += nthr) {
     const size_t o = (size_t)col * (N + 1) + i;
     const double fu = s_fin[i] + poison, fd = s_fin[N + 1 + i] + s_fin[2 * (N + 1) + i] + poison;
     if (P.F_up) P.F_up[o] = fu;
@@ -738,688 +629,437 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const SolveSme
     if (want_beam) P.F_beam[o] = s_fin[3 * (N + 1) + i] + poison;
   }
   if (P.dTdt) {
-    const double *dm = P.ws_dm + (size_t)col * N;
-    for (int j = tid; j < N; j += BLOCK) {
+    for (int j = tid; j < N; j += nthr) {
       const double fn1 = s_fin[j + 1] - (s_fin[N + 1 + j + 1] + s_fin[2 * (N + 1) + j + 1]);
       const double fn0 = s_fin[j] - (s_fin[N + 1 + j] + s_fin[2 * (N + 1) + j]);
-      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / dm[j] + poison;   // reading R14
+      P.dTdt[(size_t)col * N + j] = -(fn1 - fn0) * P.inv_cp / s_dm[j] + poison;   // reading R14
     }
   }
 }
 
-template <bool NONISO, bool TOA, bool BDIRECT, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB) rt_solve_kernel(const KParams P) {
-  extern __shared__ __align__(16) unsigned char smem[];
+// --------------------------------------------------------------------------------------------
+// rt_step_kernel: S1-S7.  Persistent grid = (tiles per column, workers): block (t, w) owns tile t of the spectral axis
+// (warps x 32 x PPT consecutive points, bin-major, Gauss point fastest) and takes columns from queue[t].
+//   NONISO  non-isothermal layers (Eqs. 4-9): two sub-layers and two levels per sweep iteration
+//   TOA     HELIOS_RT_TOA_SPECTRUM: only F_up at the top per bin; no back-substitution
+//   PPT     adjacent spectral points of one bin per thread (n_gauss must be a multiple): everything that depends only
+//           on (column, level, bin) is issued once for the group and its PPT dependence chains interleave (ILP)
+//   ROWS    0: k-table rows by register-prefetched loads; 1: by bulk async copies (TMA) into the per-warp ring
+//   STK     back-substitution coefficients: 1 = per-block slab of the global workspace (L2), 0 = thread-private
+//           local memory (kept for comparison builds; SCAP = its capacity in interfaces)
+//   MAXT, MINB  launch bounds (register cap = 65536 / (MAXT MINB)); any block of <= MAXT threads may be launched
+// --------------------------------------------------------------------------------------------
+template <bool NONISO, bool TOA, int PPT, int ROWS, int STK, int SCAP, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
+  static_assert(PPT == 1 || PPT == 2 || PPT == 4, "points per thread");
+  constexpr int DEPTH = NONISO ? 2 : 1;
+  extern __shared__ __align__(128) unsigned char smem[];
   __shared__ double s_T32[32];
-  __shared__ int s_is_last;
+  __shared__ int s_is_last, s_nan, s_col;
   const int N = P.N, nlev = P.nlev;
-  // one Gauss point per bin (opacity sampling, L385): every thread has its own bin, so the Planck values are read
-  // coalesced straight from the workspace instead of being staged (64 KB per block otherwise)
-  constexpr bool bdirect = BDIRECT;   // host: n_gauss == 1
-  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA, bdirect);
-  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;   // s_lev[-1] pads the prefetch
-  double *s_B = (double *)(smem + L.off_B);
-  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
-  double *s_red = (double *)(smem + L.off_red);
-  double *s_stage = (double *)(smem + L.off_stage);
-  double *s_fin = (double *)(smem + L.off_fin);
-  double *s_vals = (double *)(smem + L.off_vals);
-
-  const int tid = threadIdx.x;
-  const int tile = blockIdx.x, col = blockIdx.y;
-  const int LP = L.LP, nbtS = L.nbt;
-  const double mu = P.mu[col];
-  const bool day = mu > 0.0;
-
-  const int pt0 = tile * BLOCK;
-  const int b_first = pt0 / P.ng;
-  int pt_last = pt0 + BLOCK - 1;
-  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
-  const int nbt = pt_last / P.ng - b_first + 1;   // bins touched by this tile (<= L.nbt)
-  const int nwa = ((pt_last - pt0) >> 5) + 1;     // warps of this tile that own at least one spectral point
-
-  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid, !bdirect);
-  const int col_nan = P.ws_nan[col];
-  __syncthreads();
-
-  // ---------------- per-thread constants ----------------
-  int pt = pt0 + tid;
-  const bool active = pt < P.npt;
-  if (!active) pt = P.npt - 1;
-  const int b = pt / P.ng, gidx = pt - b * P.ng;
-  const int bl = b - b_first;
+  const int tid = threadIdx.x, nthr = blockDim.x, nwarps = nthr >> 5;
   const int warp = tid >> 5, lane = tid & 31;
-  const bool warp_on = warp < nwa;          // a warp without any spectral point only joins the barriers
-  double *red_w = s_red + (size_t)warp * 4 * LP;
-  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
-  const bool want_beam = !TOA && (P.F_beam != nullptr);
-
-  if (warp_on) {
-    const double W = active ? P.bins[b].dlam * P.gauss_w[gidx] : 0.0;    // dlam_b * w_g
-    const double muF = day ? mu * P.fstar[b] : 0.0;                      // mu * F_star[b]
-    const double inv_mu = day ? 1.0 / mu : 0.0;
-    const double *lnk_pt = P.lnk + pt;
-    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
-    const double *T32 = s_T32;
-    double *stage_wr = stage_w + lane;
-    // B of level l: Bbase[l * Bstride] (global workspace row, or the staged tile in shared memory)
-    const double *Bbase = s_B + bl;
-    if (BDIRECT) Bbase = P.ws_B + (size_t)col * (nlev + 1) * P.nb + b;
-    const int Bstride = BDIRECT ? P.nb : nbtS;
-
-    // back-substitution state per interface i = 0..N (thread-private stack in local memory, written top-down,
-    // read bottom-up): F_up[i] = c F_up[i-1] + d (weight folded into d) and R with F_dn[i] = R F_up[i] + U.
-    // U itself is not kept: sum_points W (U + beam) is reduced on the way down (flush_stage).
-    // Entries N+1 .. LP-1 pad the last group of 8 in sweep 2 with the identity (c = 1, d = 0, R = 0).
-    constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
-    double2 st_cd[STK];
-    double st_R[STK];
-
-    double R = 0.0, U = P.f_toa;       // F_dn[N] = f_toa (Fig. 5)
-    double Fb = muF;                   // beam at the TOA (full strength, L235)
-    double Ctoa = 1.0, Dtoa = 0.0;     // TOA mode: F_up[N] = Ctoa F_up[j] + Dtoa
-
-    // bookkeeping of interface i with (R, U, Fb) at that interface
-    auto push_interface = [&](int i, double Ri, double Ui, double Fbi) {
-      if (!TOA) {
-        st_R[i] = Ri;
-        stage_wr[(i & 7) * STAGE_LD] = W * (Ui + Fbi);
-        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
-        if (want_beam) {
-          const double wb = warp_sum(W * Fbi);
-          if (lane == 0) red_w[3 * LP + i] = wb;
-        }
-      }
-    };
-
-    // ---------------- sweep 1: TOA -> BOA (one instantiation per day / night: the loop body has no branch) ------
-    auto sweep1 = [&](auto day_tag) {
-      constexpr bool DAY = decltype(day_tag)::value;
-      double tau = 0.0;
-      if (!NONISO) {
-        const LevelRec *lv = s_lev + (N - 1);
-        const double *Bp = Bbase + (size_t)(N - 1) * Bstride;
-        Rows nx = load_rows(lnk_pt, lv);   // rows of the next level, loaded one level ahead
-#pragma unroll (TOA ? kIsoUnrollToa : kIsoUnroll)
-        for (int j = N - 1; j >= 0; --j, --lv, Bp -= Bstride) {
-          const Rows cur = nx;
-          nx = load_rows(lnk_pt, lv - 1);
-          push_interface(j + 1, R, U, Fb);
-          double kx, w0, g0, c, d;
-          level_optics(cur, T32, lv, bin0, bin1, kx, w0, g0);
-          const double dtau = kx * lv->dm;
-          const double Bj = *Bp;
-          double Fa = 0.0;
-          if (DAY) {
-            tau += dtau;
-            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);   // (B6)
-          }
-          layer_forward<DAY, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, R, U, c, d);
-          Fb = Fa;
-          if (TOA) {
-            Dtoa = fma(Ctoa, d, Dtoa);
-            Ctoa *= c;
-          } else {
-            st_cd[j + 1] = make_double2(c, W * d);
-          }
-        }
-      } else {
-        // levels alternate interface (even) / centre (odd); sub-layer s lies between levels s and s+1 and takes
-        // the arithmetic mean of the two levels' kappa_ext, omega0, g0 (L171, reading R10).  The centre unknowns
-        // are eliminated on the fly: F_up[j+1] = cu F_up[centre] + du, F_up[centre] = cl F_up[j] + dl.
-        const LevelRec *lv = s_lev + (nlev - 1);
-        const double *Bp = Bbase + (size_t)(nlev - 1) * Bstride;
-        double kx_up, w0_up, g0_up;
-        {
-          const Rows top = load_rows(lnk_pt, lv);
-          level_optics(top, T32, lv, bin0, bin1, kx_up, w0_up, g0_up);
-        }
-        double B_up = *Bp;
-        Rows nxc = load_rows(lnk_pt, lv - 1);   // centre and lower interface of the next layer, one layer ahead
-        Rows nxl = load_rows(lnk_pt, lv - 2);
-#pragma unroll 1
-        for (int j = N - 1; j >= 0; --j, lv -= 2, Bp -= 2 * Bstride) {
-          const Rows rc = nxc, rl = nxl;
-          nxc = load_rows(lnk_pt, lv - 3);
-          nxl = load_rows(lnk_pt, (j > 0) ? lv - 4 : lv - 3);
-          push_interface(j + 1, R, U, Fb);
-          double kx_c, w0_c, g0_c, kx_lo, w0_lo, g0_lo, cu, du, cl, dl;
-          level_optics(rc, T32, lv - 1, bin0, bin1, kx_c, w0_c, g0_c);
-          level_optics(rl, T32, lv - 2, bin0, bin1, kx_lo, w0_lo, g0_lo);
-          const double B_c = Bp[-Bstride], B_lo = Bp[-2 * Bstride];
-          const double dtau_u = 0.5 * (kx_c + kx_up) * lv[-1].dm;
-          const double dtau_l = 0.5 * (kx_lo + kx_c) * lv[-2].dm;
-          double Fc = 0.0, Fa = 0.0;
-          if (DAY) {
-            const double tau_c = tau + dtau_u;
-            tau = tau_c + dtau_l;
-            Fc = muF * exp_hot<1, false>(min_pos(tau_c * inv_mu, 708.0), T32, nullptr);   // (B6)
-            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
-          }
-          layer_forward<DAY, true>(P, T32, 0.5 * (w0_c + w0_up), 0.5 * (g0_c + g0_up), dtau_u, B_c, B_up, mu, Fc, Fb,
-                                   R, U, cu, du);
-          layer_forward<DAY, true>(P, T32, 0.5 * (w0_lo + w0_c), 0.5 * (g0_lo + g0_c), dtau_l, B_lo, B_c, mu, Fa, Fc,
-                                   R, U, cl, dl);
-          Fb = Fa;
-          kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo; B_up = B_lo;
-          const double cc = cu * cl, dd = fma(cu, dl, du);
-          if (TOA) {
-            Dtoa = fma(Ctoa, dd, Dtoa);
-            Ctoa *= cc;
-          } else {
-            st_cd[j + 1] = make_double2(cc, W * dd);
-          }
-        }
-      }
-    };
-    if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
-
-    // ---------------- BOA, Eq.(10) L237 ----------------
-    const double F_boa = Bbase[(size_t)nlev * Bstride];
-    const double Fup0 = (U + F_boa + Fb) * rcp_fast(1.0 - R);
-
-    if (TOA) {
-      // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
-      const double FupN = fma(Ctoa, Fup0, Dtoa);
-      s_vals[tid] = active ? P.gauss_w[gidx] * FupN : 0.0;
-    } else {
-      push_interface(0, R, U, Fb);
-      st_cd[0] = make_double2(0.0, W * Fup0);
-      // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 interfaces at a time ----------------
-      for (int i = N + 1; i < LP; ++i) { st_cd[i] = make_double2(1.0, 0.0); st_R[i] = 0.0; }
-      double wFup = 0.0;
-#pragma unroll 1
-      for (int base = 0; base <= N; base += 8) {
-        double v[16];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          // levels beyond N repeat F_up[N] into rows of the reduction buffer that are never read
-          const double2 cd = st_cd[base + k];
-          const double Ri = st_R[base + k];
-          wFup = fma(cd.x, wFup, cd.y);
-          v[k] = wFup;
-          v[8 + k] = Ri * wFup;
-        }
-        const double tot = warp_reduce16(v, lane);
-        const int idx = lane >> 1;
-        if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
-      }
-      if (P.F_toa_bin != nullptr) s_vals[tid] = active ? wFup * P.bins[b].inv_dlam : 0.0;
-    }
-  } else if (TOA || P.F_toa_bin != nullptr) {
-    s_vals[tid] = 0.0;
-  }
-  __syncthreads();
-
-  if (TOA || P.F_toa_bin != nullptr) {
-    for (int k = tid; k < nbt; k += BLOCK) {
-      const int bb = b_first + k;
-      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
-      // a bin may straddle two tiles: every tile adds its own part
-      const bool whole = (g_lo >= 0) && (g_hi <= BLOCK);
-      if (g_lo < 0) g_lo = 0;
-      if (g_hi > BLOCK) g_hi = BLOCK;
-      double sum = col_nan ? nan("") : 0.0;
-      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
-      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
-      if (whole) *dst = sum; else atomicAdd(dst, sum);
-    }
-  }
-  if (TOA) return;
-
-  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
-}
-
-// --------------------------------------------------------------------------------------------
-// rt_solve2_kernel: the isothermal S3-S7 path with TWO adjacent spectral points per thread (same bin: needs an even
-// number of Gauss points).  Same algorithm and arithmetic as rt_solve_kernel<false, TOA, false, ...>; what changes is
-// the instruction mix: everything that depends only on (column, level, bin) -- the level record, corner weights, row
-// addresses (one 16-byte load per corner instead of two 8-byte ones), Planck value, bin constants, hot constants,
-// loop control -- is issued once for the two points, the two dependence chains interleave in one warp (ILP 2), and
-// the staging / butterfly reductions handle the pair's sum.  A tile is 2 x BLOCK points.
-// --------------------------------------------------------------------------------------------
-struct Rows2 { double2 l00, l01, l10, l11; };
-
-__device__ __forceinline__ Rows2 load_rows2(const double *__restrict__ lnk_pt, const LevelRec *lv) {
-  const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
-  Rows2 r;
-  r.l00 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.x)));
-  r.l01 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.y)));
-  r.l10 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.z)));
-  r.l11 = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.w)));
-  return r;
-}
-
-template <bool TOA, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB) rt_solve2_kernel(const KParams P) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ double s_T32[32];
-  __shared__ int s_is_last;
-  constexpr int TP = 2 * BLOCK;   // points per tile
-  const int N = P.N, nlev = P.nlev;
-  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA, false, 2);
-  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
-  double *s_B = (double *)(smem + L.off_B);
+  const Lay L = make_lay(N, nlev, nwarps, PPT, P.ng, P.nb, TOA, DEPTH, ROWS == 1);
+  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;   // s_lev[-1] duplicates level 0
+  const double *s_B = (const double *)(smem + L.off_B);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
   double *s_red = (double *)(smem + L.off_red);
-  double *s_stage = (double *)(smem + L.off_stage);
-  double *s_fin = (double *)(smem + L.off_fin);
   double *s_vals = (double *)(smem + L.off_vals);
-
-  const int tid = threadIdx.x;
-  const int tile = blockIdx.x, col = blockIdx.y;
   const int LP = L.LP, nbtS = L.nbt;
-  const double mu = P.mu[col];
-  const bool day = mu > 0.0;
 
+  // ---------------- constants of the tile (the block keeps its tile for the whole launch) ----------------
+  const int tile = blockIdx.x;
+  const int TP = nthr * PPT;
   const int pt0 = tile * TP;
   const int b_first = pt0 / P.ng;
   int pt_last = pt0 + TP - 1;
   if (pt_last > P.npt - 1) pt_last = P.npt - 1;
-  const int nbt = pt_last / P.ng - b_first + 1;
-  const int nwa = ((pt_last - pt0) >> 6) + 1;     // warps that own at least one pair of points
-
-  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid, true);
-  const int col_nan = P.ws_nan[col];
-  __syncthreads();
-
-  // the pair (pt, pt + 1): pt is even and n_gauss is even, so both points lie in bin b
-  int pt = pt0 + 2 * tid;
-  const bool active = pt < P.npt;
-  if (!active) pt = P.npt - 2;
-  const int b = pt / P.ng, gidx = pt - b * P.ng;
-  const int bl = b - b_first;
-  const int warp = tid >> 5, lane = tid & 31;
-  const bool warp_on = warp < nwa;
-  double *red_w = s_red + (size_t)warp * 4 * LP;
-  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
-  const bool want_beam = !TOA && (P.F_beam != nullptr);
-
-  if (warp_on) {
-    const double dlam = P.bins[b].dlam;
-    const double W0 = active ? dlam * P.gauss_w[gidx] : 0.0, W1 = active ? dlam * P.gauss_w[gidx + 1] : 0.0;
-    const double muF = day ? mu * P.fstar[b] : 0.0;
-    const double inv_mu = day ? 1.0 / mu : 0.0;
-    const double *lnk_pt = P.lnk + pt;
-    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
-    const double *T32 = s_T32;
-    double *stage_wr = stage_w + lane;
-
-    constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
-    double2 st_cd0[STK], st_cd1[STK];   // (c, W d) of the two points
-    double2 st_R[STK];                  // (R0, R1)
-
-    double R0 = 0.0, R1 = 0.0, U0 = P.f_toa, U1 = P.f_toa;
-    double Fb0 = muF, Fb1 = muF;
-    double Ct0 = 1.0, Dt0 = 0.0, Ct1 = 1.0, Dt1 = 0.0;
-
-    auto push_interface = [&](int i) {
-      if (!TOA) {
-        st_R[i] = make_double2(R0, R1);
-        stage_wr[(i & 7) * STAGE_LD] = fma(W0, U0 + Fb0, W1 * (U1 + Fb1));
-        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
-        if (want_beam) {
-          const double wb = warp_sum(fma(W0, Fb0, W1 * Fb1));
-          if (lane == 0) red_w[3 * LP + i] = wb;
-        }
-      }
-    };
-
-    auto sweep1 = [&](auto day_tag) {
-      constexpr bool DAY = decltype(day_tag)::value;
-      double tau0 = 0.0, tau1 = 0.0;
-      const LevelRec *lv = s_lev + (N - 1);
-      const double *Bp = s_B + (size_t)(N - 1) * nbtS + bl;
-      Rows2 nx = load_rows2(lnk_pt, lv);
-#pragma unroll (TOA ? kIsoUnrollToa2 : 1)
-      for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
-        const Rows2 cur = nx;
-        nx = load_rows2(lnk_pt, lv - 1);
-        push_interface(j + 1);
-        // S3 + Eqs. 17-18 for the pair: shared corner weights and bin constants
-        const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
-        const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
-        const double lk0 = fma(cb.y, cur.l11.x, fma(cb.x, cur.l10.x, fma(ca.y, cur.l01.x, ca.x * cur.l00.x)));
-        const double lk1 = fma(cb.y, cur.l11.y, fma(cb.x, cur.l10.y, fma(ca.y, cur.l01.y, ca.x * cur.l00.y)));
-        const double ka0 = exp_hot<0, false>(lk0, T32, nullptr), ka1 = exp_hot<0, false>(lk1, T32, nullptr);
-        const BinOpt *bo = lv->cloud ? bin1 : bin0;
-        const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
-        const G0Terms gt = bo->gt;
-        const double dm = lv->dm, Bj = *Bp;
-        const double kx0 = ka0 + sbss.x, kx1 = ka1 + sbss.x;
-        const double w00 = sbss.y * rcp_fast(kx0), w01 = sbss.y * rcp_fast(kx1);
-        const double dtau0 = kx0 * dm, dtau1 = kx1 * dm;
-        double Fa0 = 0.0, Fa1 = 0.0;
-        if (DAY) {
-          tau0 += dtau0;
-          tau1 += dtau1;
-          Fa0 = muF * exp_hot<1, false>(min_pos(tau0 * inv_mu, 708.0), T32, nullptr);   // (B6)
-          Fa1 = muF * exp_hot<1, false>(min_pos(tau1 * inv_mu, 708.0), T32, nullptr);
-        }
-        double c0, d0, c1, d1;
-        layer_forward<DAY, false>(P, T32, w00, gt, dtau0, Bj, Bj, mu, Fa0, Fb0, R0, U0, c0, d0);
-        layer_forward<DAY, false>(P, T32, w01, gt, dtau1, Bj, Bj, mu, Fa1, Fb1, R1, U1, c1, d1);
-        Fb0 = Fa0;
-        Fb1 = Fa1;
-        if (TOA) {
-          Dt0 = fma(Ct0, d0, Dt0); Ct0 *= c0;
-          Dt1 = fma(Ct1, d1, Dt1); Ct1 *= c1;
-        } else {
-          st_cd0[j + 1] = make_double2(c0, W0 * d0);
-          st_cd1[j + 1] = make_double2(c1, W1 * d1);
-        }
-      }
-    };
-    if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
-
-    // BOA, Eq.(10)
-    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
-    const double Fup00 = (U0 + F_boa + Fb0) * rcp_fast(1.0 - R0), Fup01 = (U1 + F_boa + Fb1) * rcp_fast(1.0 - R1);
-
-    if (TOA) {
-      const double2 gw = make_double2(P.gauss_w[gidx], P.gauss_w[gidx + 1]);
-      s_vals[2 * tid] = active ? gw.x * fma(Ct0, Fup00, Dt0) : 0.0;
-      s_vals[2 * tid + 1] = active ? gw.y * fma(Ct1, Fup01, Dt1) : 0.0;
-    } else {
-      push_interface(0);
-      st_cd0[0] = make_double2(0.0, W0 * Fup00);
-      st_cd1[0] = make_double2(0.0, W1 * Fup01);
-      for (int i = N + 1; i < LP; ++i) {
-        st_cd0[i] = make_double2(1.0, 0.0); st_cd1[i] = make_double2(1.0, 0.0); st_R[i] = make_double2(0.0, 0.0);
-      }
-      double wF0 = 0.0, wF1 = 0.0;
-#pragma unroll 1
-      for (int base = 0; base <= N; base += 8) {
-        double v[16];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          const double2 a0 = st_cd0[base + k], a1 = st_cd1[base + k], r = st_R[base + k];
-          wF0 = fma(a0.x, wF0, a0.y);
-          wF1 = fma(a1.x, wF1, a1.y);
-          v[k] = wF0 + wF1;
-          v[8 + k] = fma(r.x, wF0, r.y * wF1);
-        }
-        const double tot = warp_reduce16(v, lane);
-        const int idx = lane >> 1;
-        if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
-      }
-      if (P.F_toa_bin != nullptr) {
-        const double inv_dlam = P.bins[b].inv_dlam;
-        s_vals[2 * tid] = active ? wF0 * inv_dlam : 0.0;
-        s_vals[2 * tid + 1] = active ? wF1 * inv_dlam : 0.0;
-      }
-    }
-  } else if (TOA || P.F_toa_bin != nullptr) {
-    s_vals[2 * tid] = 0.0;
-    s_vals[2 * tid + 1] = 0.0;
-  }
-  __syncthreads();
-
-  if (TOA || P.F_toa_bin != nullptr) {
-    for (int k = tid; k < nbt; k += BLOCK) {
-      const int bb = b_first + k;
-      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
-      const bool whole = (g_lo >= 0) && (g_hi <= TP);
-      if (g_lo < 0) g_lo = 0;
-      if (g_hi > TP) g_hi = TP;
-      double sum = col_nan ? nan("") : 0.0;
-      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
-      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
-      if (whole) *dst = sum; else atomicAdd(dst, sum);
-    }
-  }
-  if (TOA) return;
-
-  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
-}
-
-template <bool TOA, int PPT, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB) rt_solvem_kernel(const KParams P) {
-  static_assert(PPT == 2 || PPT == 4, "points per thread");
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ double s_T32[32];
-  __shared__ int s_is_last;
-  constexpr int TP = PPT * BLOCK;   // points per tile
-  constexpr int H = PPT / 2;        // 16-byte loads per corner row
-  const int N = P.N, nlev = P.nlev;
-  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, TOA, false, PPT);
-  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
-  double *s_B = (double *)(smem + L.off_B);
-  BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
-  double *s_red = (double *)(smem + L.off_red);
-  double *s_stage = (double *)(smem + L.off_stage);
-  double *s_fin = (double *)(smem + L.off_fin);
-  double *s_vals = (double *)(smem + L.off_vals);
-
-  const int tid = threadIdx.x;
-  const int tile = blockIdx.x, col = blockIdx.y;
-  const int LP = L.LP, nbtS = L.nbt;
-  const double mu = P.mu[col];
-  const bool day = mu > 0.0;
-
-  const int pt0 = tile * TP;
-  const int b_first = pt0 / P.ng;
-  int pt_last = pt0 + TP - 1;
-  if (pt_last > P.npt - 1) pt_last = P.npt - 1;
-  const int nbt = pt_last / P.ng - b_first + 1;
-  const int nwa = ((pt_last - pt0) / (32 * PPT)) + 1;     // warps that own at least one group of points
-
-  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid, true);
-  const int col_nan = P.ws_nan[col];
-  __syncthreads();
-
+  const int nbt = pt_last / P.ng - b_first + 1;            // bins touched by this tile (<= L.nbt)
+  const int nwa = (pt_last - pt0) / (32 * PPT) + 1;        // warps that own at least one spectral point
   // the group pt .. pt + PPT - 1: pt and n_gauss are multiples of PPT, so all its points lie in bin b
   int pt = pt0 + PPT * tid;
   const bool active = pt < P.npt;
   if (!active) pt = P.npt - PPT;
   const int b = pt / P.ng, gidx = pt - b * P.ng;
   const int bl = b - b_first;
-  const int warp = tid >> 5, lane = tid & 31;
-  const bool warp_on = warp < nwa;
-  double *red_w = s_red + (size_t)warp * 4 * LP;
-  double *stage_w = s_stage + (size_t)warp * 8 * STAGE_LD;
+  const bool warp_on = warp < nwa;          // a warp without any spectral point only joins the barriers
   const bool want_beam = !TOA && (P.F_beam != nullptr);
-
-  if (warp_on) {
-    const double dlam = P.bins[b].dlam;
-    double W[PPT];
+  double W[PPT];                            // dlam_b * w_g
+  const double dlam = P.bins[b].dlam, inv_dlam = P.bins[b].inv_dlam, fstar_b = P.fstar[b];
 #pragma unroll
-    for (int q = 0; q < PPT; ++q) W[q] = active ? dlam * P.gauss_w[gidx + q] : 0.0;
-    const double muF = day ? mu * P.fstar[b] : 0.0;
-    const double inv_mu = day ? 1.0 / mu : 0.0;
-    const double *lnk_pt = P.lnk + pt;
-    const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
-    const double *T32 = s_T32;
-    double *stage_wr = stage_w + lane;
-
-    constexpr int STK = TOA ? 1 : ((MAXL + 1 + 7) & ~7);
-    double2 st_cd[STK][PPT];   // (c, W d) per point
-    double st_R[STK][PPT];
-
-    double R[PPT], U[PPT], Fb[PPT], Ct[PPT], Dt[PPT];
+  for (int q = 0; q < PPT; ++q) W[q] = active ? dlam * P.gauss_w[gidx + q] : 0.0;
+  double gw[PPT];
+  if (TOA) {
 #pragma unroll
-    for (int q = 0; q < PPT; ++q) { R[q] = 0.0; U[q] = P.f_toa; Fb[q] = muF; Ct[q] = 1.0; Dt[q] = 0.0; }
+    for (int q = 0; q < PPT; ++q) gw[q] = active ? P.gauss_w[gidx + q] : 0.0;
+  }
 
-    auto push_interface = [&](int i) {
-      if (!TOA) {
-        double su = 0.0, sb = 0.0;
+  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
+  for (int i = tid; i < 2 * nbt; i += nthr) {
+    const int cl = i / nbt, k = i - cl * nbt;
+    const BinConst bc = P.bins[b_first + k];
+    BinOpt bo;
+    bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2); bo.pad[0] = bo.pad[1] = 0.0;
+    s_bin[cl * nbtS + k] = bo;
+  }
+  if (ROWS == 1) {
+    if (tid < RING * nwarps) mbar_init(smem_u32(smem + L.off_bar) + 8 * tid, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
+  const double *T32 = s_T32;
+  double *red_w = s_red + (size_t)warp * 4 * LP;
+  double *stage_w = (double *)(smem + L.off_u + L.u_stage) + (size_t)warp * 8 * STAGE_LD;
+  double *stage_wr = stage_w + lane;
+  const double *Bbase = s_B + bl;
+
+  Feed<PPT, DEPTH, ROWS> feed;
+  if constexpr (ROWS == 0) {
+    feed.lnk_pt = P.lnk + pt;
+  } else {
+    unsigned char *ring = smem + L.off_u + L.u_ring + (size_t)warp * L.ring_warp;
+    feed.ring = (const double *)ring;
+    feed.ring_s = smem_u32(ring);
+    feed.bar_s = smem_u32(smem + L.off_bar) + 8 * RING * warp;
+    feed.lnk_w = P.lnk + pt0 + warp * 32 * PPT;
+    feed.kc = 0;
+    feed.lane = lane;
+  }
+  feed.lv0 = s_lev;
+
+  // this block's slab of the back-substitution workspace: [interface][warp][96 PPT]
+  const size_t istride = (size_t)nwarps * 96 * PPT;
+  double *stk_w = nullptr;
+  if (STK == 1 && !TOA)
+    stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * 96 * PPT;
+
+  // ---------------- columns of this tile's queue ----------------
+  for (;;) {
+    __syncthreads();                       // the previous column's shared-memory state is dead
+    if (tid == 0) s_col = (int)atomicAdd(P.queue + tile, 1u);
+    __syncthreads();
+    const int col = s_col;
+    if (col >= P.ncol) break;
+
+    column_prep<NONISO>(P, L, smem, col, b_first, nbt, &s_nan);
+    const int col_nan = s_nan;
+
+    if (warp_on) {
+      const double mu = P.mu[col];
+      const bool day = mu > 0.0;
+      const double muF = day ? mu * fstar_b : 0.0;            // mu * F_star[b]
+      const double inv_mu = day ? 1.0 / mu : 0.0;
+
+      // back-substitution state per interface i = 0..N: F_up[i] = c F_up[i-1] + d (weight folded into d) and R with
+      // F_dn[i] = R F_up[i] + U.  U itself is not kept: sum_points W (U + beam) is reduced on the way down.
+      double2 l_cd[(STK == 0 && !TOA) ? SCAP : 1][PPT];
+      double l_R[(STK == 0 && !TOA) ? SCAP : 1][PPT];
+
+      double R[PPT], U[PPT], Fb[PPT], Ct[PPT], Dt[PPT];
 #pragma unroll
-        for (int q = 0; q < PPT; ++q) { st_R[i][q] = R[q]; su = fma(W[q], U[q] + Fb[q], su); sb = fma(W[q], Fb[q], sb); }
-        stage_wr[(i & 7) * STAGE_LD] = su;
-        if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
-        if (want_beam) {
-          const double wb = warp_sum(sb);
-          if (lane == 0) red_w[3 * LP + i] = wb;
+      for (int q = 0; q < PPT; ++q) {
+        R[q] = 0.0; U[q] = P.f_toa;      // F_dn[N] = f_toa (Fig. 5)
+        Fb[q] = muF;                     // beam at the TOA (full strength, L235)
+        Ct[q] = 1.0; Dt[q] = 0.0;        // TOA mode: F_up[N] = Ct F_up[j] + Dt
+      }
+
+      // bookkeeping of interface i with (U, Fb) at that interface: stage W (U + beam) for the transposed sum
+      auto push_stage = [&](int i) {
+        if (!TOA) {
+          double su = 0.0, sb = 0.0;
+#pragma unroll
+          for (int q = 0; q < PPT; ++q) { su = fma(W[q], U[q] + Fb[q], su); sb = fma(W[q], Fb[q], sb); }
+          stage_wr[(i & 7) * STAGE_LD] = su;
+          if ((i & 7) == 0) flush_stage(stage_w, red_w + 2 * LP + i, lane);
+          if (want_beam) {
+            const double wb = warp_sum(sb);
+            if (lane == 0) red_w[3 * LP + i] = wb;
+          }
         }
-      }
-    };
-
-    struct RowsM { double2 l00[H], l01[H], l10[H], l11[H]; };
-    auto load_rows_m = [&](const LevelRec *lv) {
-      const uint4 o = *reinterpret_cast<const uint4 *>(&lv->o00);
-      RowsM r;
+      };
+      auto keep = [&](int i, const double (&c)[PPT], const double (&wd)[PPT], const double (&Ri)[PPT]) {
+        if (TOA) return;
+        if (STK == 1) {
+          stk_store<PPT>(stk_w + (size_t)i * istride, lane, c, wd, Ri);
+        } else {
 #pragma unroll
-      for (int h = 0; h < H; ++h) {
-        r.l00[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.x)) + h);
-        r.l01[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.y)) + h);
-        r.l10[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.z)) + h);
-        r.l11[h] = __ldg(reinterpret_cast<const double2 *>(elem_addr(lnk_pt, o.w)) + h);
-      }
-      return r;
-    };
+          for (int q = 0; q < PPT; ++q) { l_cd[STK == 0 && !TOA ? i : 0][q] = make_double2(c[q], wd[q]); l_R[STK == 0 && !TOA ? i : 0][q] = Ri[q]; }
+        }
+      };
 
-    auto sweep1 = [&](auto day_tag) {
-      constexpr bool DAY = decltype(day_tag)::value;
-      double tau[PPT];
+      // ---------------- sweep 1: TOA -> BOA (one instantiation per day / night: the loop body has no branch) ------
+      auto sweep1 = [&](auto day_tag) {
+        constexpr bool DAY = decltype(day_tag)::value;
+        double tau[PPT];
 #pragma unroll
-      for (int q = 0; q < PPT; ++q) tau[q] = 0.0;
-      const LevelRec *lv = s_lev + (N - 1);
-      const double *Bp = s_B + (size_t)(N - 1) * nbtS + bl;
-      RowsM nx = load_rows_m(lv);
+        for (int q = 0; q < PPT; ++q) tau[q] = 0.0;
+        if constexpr (!NONISO) {
+          const LevelRec *lv = s_lev + (N - 1);
+          const double *Bp = Bbase + (size_t)(N - 1) * nbtS;
+          feed.prime(lv, N);
 #pragma unroll 1
-      for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
-        const RowsM cur = nx;
-        nx = load_rows_m(lv - 1);
-        push_interface(j + 1);
-        const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
-        const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
-        const BinOpt *bo = lv->cloud ? bin1 : bin0;
-        const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
-        const G0Terms gt = bo->gt;
-        const double dm = lv->dm, Bj = *Bp;
+          for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
+            RowsT<PPT> cur[1];
+            feed.next(cur, lv - 1);
+            push_stage(j + 1);
+            // S3 + Eqs. 17-18 for the group: shared corner weights and bin constants
+            const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
+            const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
+            const BinOpt *bo = lv->cloud ? bin1 : bin0;
+            const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
+            const G0Terms gt = bo->gt;
+            const double dm = lv->dm, Bj = *Bp;
+            double lk[PPT];
 #pragma unroll
-        for (int q = 0; q < PPT; ++q) {
-          const int h = q >> 1;
-          const double r00 = (q & 1) ? cur.l00[h].y : cur.l00[h].x, r01 = (q & 1) ? cur.l01[h].y : cur.l01[h].x;
-          const double r10 = (q & 1) ? cur.l10[h].y : cur.l10[h].x, r11 = (q & 1) ? cur.l11[h].y : cur.l11[h].x;
-          const double lk = fma(cb.y, r11, fma(cb.x, r10, fma(ca.y, r01, ca.x * r00)));
-          const double kx = exp_hot<0, false>(lk, T32, nullptr) + sbss.x;
-          const double w0 = sbss.y * rcp_fast(kx);
-          const double dtau = kx * dm;
-          double Fa = 0.0;
-          if (DAY) {
-            tau[q] += dtau;
-            Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);   // (B6)
+            for (int q = 0; q < PPT; ++q)
+              lk[q] = fma(cb.y, cur[0].v[3][q], fma(cb.x, cur[0].v[2][q], fma(ca.y, cur[0].v[1][q], ca.x * cur[0].v[0][q])));
+            feed.release(lv - RING, j - RING >= 0);
+            double cc[PPT], wd[PPT], Ro[PPT];
+#pragma unroll
+            for (int q = 0; q < PPT; ++q) {
+              const double kx = exp_hot<0, false>(lk[q], T32, nullptr) + sbss.x;
+              const double w0 = sbss.y * rcp_fast(kx);
+              const double dtau = kx * dm;
+              double Fa = 0.0;
+              if (DAY) {
+                tau[q] += dtau;
+                Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);   // (B6)
+              }
+              double c, d;
+              Ro[q] = R[q];
+              layer_forward<DAY, false>(P, T32, w0, gt, dtau, Bj, Bj, mu, Fa, Fb[q], R[q], U[q], c, d);
+              Fb[q] = Fa;
+              if (TOA) {
+                Dt[q] = fma(Ct[q], d, Dt[q]);
+                Ct[q] *= c;
+              }
+              cc[q] = c;
+              wd[q] = W[q] * d;
+            }
+            keep(j + 1, cc, wd, Ro);
           }
-          double c, d;
-          layer_forward<DAY, false>(P, T32, w0, gt, dtau, Bj, Bj, mu, Fa, Fb[q], R[q], U[q], c, d);
-          Fb[q] = Fa;
-          if (TOA) {
-            Dt[q] = fma(Ct[q], d, Dt[q]);
-            Ct[q] *= c;
-          } else {
-            st_cd[j + 1][q] = make_double2(c, W[q] * d);
+        } else {
+          // levels alternate interface (even) / centre (odd); sub-layer s lies between levels s and s+1 and takes
+          // the arithmetic mean of the two levels' kappa_ext, omega0, g0 (L171, reading R10).  The centre unknowns
+          // are eliminated on the fly: F_up[j+1] = cu F_up[centre] + du, F_up[centre] = cl F_up[j] + dl.
+          const LevelRec *lv = s_lev + (nlev - 1);
+          const double *Bp = Bbase + (size_t)(nlev - 1) * nbtS;
+          auto optics = [&](const RowsT<PPT> &rw, const LevelRec *l, double (&kx)[PPT], double (&w0)[PPT], double &g0) {
+            const double2 ca = *reinterpret_cast<const double2 *>(&l->c00);
+            const double2 cb = *reinterpret_cast<const double2 *>(&l->c10);
+            const BinOpt *bo = l->cloud ? bin1 : bin0;
+            const double2 sbss = *reinterpret_cast<const double2 *>(&bo->sb);
+            g0 = bo->gt.g0;
+#pragma unroll
+            for (int q = 0; q < PPT; ++q) {
+              const double lk = fma(cb.y, rw.v[3][q], fma(cb.x, rw.v[2][q], fma(ca.y, rw.v[1][q], ca.x * rw.v[0][q])));
+              kx[q] = exp_hot<0, false>(lk, T32, nullptr) + sbss.x;
+              w0[q] = sbss.y * rcp_fast(kx[q]);
+            }
+          };
+          double kx_up[PPT], w0_up[PPT], g0_up;
+          {
+            RowsT<PPT> top;
+            load_rows_g<PPT>(top, P.lnk + pt, lv);
+            optics(top, lv, kx_up, w0_up, g0_up);
           }
-        }
-      }
-    };
-    if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
-
-    // BOA, Eq.(10)
-    const double F_boa = s_B[(size_t)nlev * nbtS + bl];
-    double Fup0[PPT];
-#pragma unroll
-    for (int q = 0; q < PPT; ++q) Fup0[q] = (U[q] + F_boa + Fb[q]) * rcp_fast(1.0 - R[q]);
-
-    if (TOA) {
-#pragma unroll
-      for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? P.gauss_w[gidx + q] * fma(Ct[q], Fup0[q], Dt[q]) : 0.0;
-    } else {
-      push_interface(0);
-#pragma unroll
-      for (int q = 0; q < PPT; ++q) st_cd[0][q] = make_double2(0.0, W[q] * Fup0[q]);
-      for (int i = N + 1; i < LP; ++i)
-#pragma unroll
-        for (int q = 0; q < PPT; ++q) { st_cd[i][q] = make_double2(1.0, 0.0); st_R[i][q] = 0.0; }
-      double wF[PPT];
-#pragma unroll
-      for (int q = 0; q < PPT; ++q) wF[q] = 0.0;
+          double B_up = *Bp;
+          feed.prime(lv - 1, N);
 #pragma unroll 1
-      for (int base = 0; base <= N; base += 8) {
-        double v[16];
+          for (int j = N - 1; j >= 0; --j, lv -= 2, Bp -= 2 * nbtS) {
+            RowsT<PPT> cur[2];      // [0] centre (lv - 1), [1] lower interface (lv - 2)
+            feed.next(cur, lv - 3);
+            push_stage(j + 1);
+            double kx_c[PPT], w0_c[PPT], g0_c, kx_lo[PPT], w0_lo[PPT], g0_lo;
+            optics(cur[0], lv - 1, kx_c, w0_c, g0_c);
+            optics(cur[1], lv - 2, kx_lo, w0_lo, g0_lo);
+            feed.release(lv - 1 - 2 * RING, j - RING >= 0);
+            const double B_c = Bp[-nbtS], B_lo = Bp[-2 * nbtS];
+            const double dm_u = lv[-1].dm, dm_l = lv[-2].dm;
+            const G0Terms gt_u = g0_terms(0.5 * (g0_c + g0_up), P.inv_eps2), gt_l = g0_terms(0.5 * (g0_lo + g0_c), P.inv_eps2);
+            double cc[PPT], wd[PPT], Ro[PPT];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          double su = 0.0, sd = 0.0;
-#pragma unroll
-          for (int q = 0; q < PPT; ++q) {
-            const double2 a = st_cd[base + k][q];
-            wF[q] = fma(a.x, wF[q], a.y);
-            su += wF[q];
-            sd = fma(st_R[base + k][q], wF[q], sd);
+            for (int q = 0; q < PPT; ++q) {
+              const double dtau_u = 0.5 * (kx_c[q] + kx_up[q]) * dm_u;
+              const double dtau_l = 0.5 * (kx_lo[q] + kx_c[q]) * dm_l;
+              double Fc = 0.0, Fa = 0.0;
+              if (DAY) {
+                const double tau_c = tau[q] + dtau_u;
+                tau[q] = tau_c + dtau_l;
+                Fc = muF * exp_hot<1, false>(min_pos(tau_c * inv_mu, 708.0), T32, nullptr);   // (B6)
+                Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);
+              }
+              double cu, du, cl, dl;
+              Ro[q] = R[q];
+              layer_forward<DAY, true>(P, T32, 0.5 * (w0_c[q] + w0_up[q]), gt_u, dtau_u, B_c, B_up, mu, Fc, Fb[q],
+                                       R[q], U[q], cu, du);
+              layer_forward<DAY, true>(P, T32, 0.5 * (w0_lo[q] + w0_c[q]), gt_l, dtau_l, B_lo, B_c, mu, Fa, Fc,
+                                       R[q], U[q], cl, dl);
+              Fb[q] = Fa;
+              kx_up[q] = kx_lo[q]; w0_up[q] = w0_lo[q];
+              const double c2 = cu * cl, d2 = fma(cu, dl, du);
+              if (TOA) {
+                Dt[q] = fma(Ct[q], d2, Dt[q]);
+                Ct[q] *= c2;
+              }
+              cc[q] = c2;
+              wd[q] = W[q] * d2;
+            }
+            g0_up = g0_lo; B_up = B_lo;
+            keep(j + 1, cc, wd, Ro);
           }
-          v[k] = su;
-          v[8 + k] = sd;
         }
-        const double tot = warp_reduce16(v, lane);
-        const int idx = lane >> 1;
-        if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
-      }
-      if (P.F_toa_bin != nullptr) {
-        const double inv_dlam = P.bins[b].inv_dlam;
+      };
+      if (day) sweep1(std::true_type{}); else sweep1(std::false_type{});
+
+      // ---------------- BOA, Eq.(10) L237 ----------------
+      const double F_boa = Bbase[(size_t)nlev * nbtS];
+      double Fup0[PPT];
 #pragma unroll
-        for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? wF[q] * inv_dlam : 0.0;
+      for (int q = 0; q < PPT; ++q) Fup0[q] = (U[q] + F_boa + Fb[q]) * rcp_fast(1.0 - R[q]);
+
+      if (TOA) {
+        // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = gw[q] * fma(Ct[q], Fup0[q], Dt[q]);
+      } else {
+        push_stage(0);
+        {
+          double c0[PPT], wd0[PPT];
+#pragma unroll
+          for (int q = 0; q < PPT; ++q) { c0[q] = 0.0; wd0[q] = W[q] * Fup0[q]; }
+          keep(0, c0, wd0, R);
+        }
+        // ---------------- sweep 2: back-substitution Eq.(15) + S7 reduction, 8 interfaces at a time ----------------
+        double wF[PPT];
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) wF[q] = 0.0;
+#pragma unroll 1
+        for (int base = 0; base <= N; base += 8) {
+          double sd[8];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const int i = base + k;
+            double c[PPT], wd[PPT], Ri[PPT];
+            if (i <= N) {
+              if (STK == 1) {
+                stk_load<PPT>(stk_w + (size_t)i * istride, lane, c, wd, Ri);
+              } else {
+#pragma unroll
+                for (int q = 0; q < PPT; ++q) {
+                  const double2 a = l_cd[STK == 0 ? i : 0][q];
+                  c[q] = a.x; wd[q] = a.y; Ri[q] = l_R[STK == 0 ? i : 0][q];
+                }
+              }
+            } else {
+              // beyond the top: repeat F_up[N] into rows of the reduction buffer that are never read
+#pragma unroll
+              for (int q = 0; q < PPT; ++q) { c[q] = 1.0; wd[q] = 0.0; Ri[q] = 0.0; }
+            }
+            double su = 0.0, s2 = 0.0;
+#pragma unroll
+            for (int q = 0; q < PPT; ++q) {
+              wF[q] = fma(c[q], wF[q], wd[q]);
+              su += wF[q];
+              s2 = fma(Ri[q], wF[q], s2);
+            }
+            stage_wr[k * STAGE_LD] = su;
+            sd[k] = s2;
+          }
+          flush_stage(stage_w, red_w + base, lane);
+#pragma unroll
+          for (int k = 0; k < 8; ++k) stage_wr[k * STAGE_LD] = sd[k];
+          flush_stage(stage_w, red_w + LP + base, lane);
+          if (STK == 1) {
+            // the coefficients of these interfaces are dead: drop their lines from L2 instead of writing them back
+            int n_if = N + 1 - base;
+            n_if = n_if > 8 ? 8 : n_if;
+            const int lines_if = 6 * PPT;               // 96 PPT doubles per interface and warp
+            for (int ln = lane; ln < n_if * lines_if; ln += 32) {
+              const int k = ln / lines_if, r = ln - k * lines_if;
+              l2_discard(stk_w + (size_t)(base + k) * istride + r * 16);
+            }
+          }
+        }
+        if (P.F_toa_bin != nullptr) {
+#pragma unroll
+          for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? wF[q] * inv_dlam : 0.0;
+        }
+      }
+    } else if (TOA || P.F_toa_bin != nullptr) {
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = 0.0;
+    }
+    __syncthreads();
+
+    if (TOA || P.F_toa_bin != nullptr) {
+      for (int k = tid; k < nbt; k += nthr) {
+        const int bb = b_first + k;
+        int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
+        // a bin may straddle two tiles: every tile adds its own part
+        const bool whole = (g_lo >= 0) && (g_hi <= TP);
+        if (g_lo < 0) g_lo = 0;
+        if (g_hi > TP) g_hi = TP;
+        double sum = col_nan ? nan("") : 0.0;
+        for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
+        double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
+        if (whole) *dst = sum; else atomicAdd(dst, sum);
       }
     }
-  } else if (TOA || P.F_toa_bin != nullptr) {
-#pragma unroll
-    for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = 0.0;
+    if (!TOA) column_epilogue(P, L, smem, &s_is_last, nwa, want_beam, col, tile, col_nan);
   }
-  __syncthreads();
 
-  if (TOA || P.F_toa_bin != nullptr) {
-    for (int k = tid; k < nbt; k += BLOCK) {
-      const int bb = b_first + k;
-      int g_lo = bb * P.ng - pt0, g_hi = g_lo + P.ng;
-      const bool whole = (g_lo >= 0) && (g_hi <= TP);
-      if (g_lo < 0) g_lo = 0;
-      if (g_hi > TP) g_hi = TP;
-      double sum = col_nan ? nan("") : 0.0;
-      for (int q = g_lo; q < g_hi; ++q) sum += s_vals[q];
-      double *dst = P.F_toa_bin + (size_t)col * P.nb + bb;
-      if (whole) *dst = sum; else atomicAdd(dst, sum);
+  // the last block of the grid to run out of work re-arms the queues for the next launch
+  if (tid == 0) {
+    const unsigned total = gridDim.x * gridDim.y;
+    if (atomicAdd(P.queue + P.tiles, 1u) == total - 1) {
+      for (int t = 0; t <= P.tiles; ++t) P.queue[t] = 0;
     }
   }
-  if (TOA) return;
-
-  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, want_beam, col, tile, col_nan);
 }
 
 // --------------------------------------------------------------------------------------------
 // rt_iter_kernel: the scheme Thomas's algorithm replaces (L258-270, L397), as a measured
-// comparison.  Same decomposition, staging and S3-S5 arithmetic as rt_solve_kernel; instead of the forward
-// elimination the (t, r, S_up, S_dn) of every system layer go to thread-private arrays, and the flux arrays are
-// swept n_iter times: upward pass Eq.(10) + Eq.(2) with the previous downward fluxes, downward pass Eq.(3) with the
-// upward fluxes just computed; all diffuse fluxes start at 0 (reading R23).  The non-isothermal system keeps its
+// comparison.  Same S1-S5 code as rt_step_kernel (one point per thread, one block per (tile, column)); instead of the
+// forward elimination the (t, r, S_up, S_dn) of every system layer go to thread-private arrays, and the flux arrays
+// are swept n_iter times: upward pass Eq.(10) + Eq.(2) with the previous downward fluxes, downward pass Eq.(3) with
+// the upward fluxes just computed; all diffuse fluxes start at 0 (reading R23).  The non-isothermal system keeps its
 // centre levels as unknowns (2N system layers, L311-313).  S7 as in the Thomas path (column_epilogue).
 // --------------------------------------------------------------------------------------------
-template <bool NONISO, int BLOCK>
-__global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const int n_iter) {
-  extern __shared__ __align__(16) unsigned char smem[];
+template <bool NONISO>
+__global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int n_iter) {
+  extern __shared__ __align__(128) unsigned char smem[];
   __shared__ double s_T32[32];
-  __shared__ int s_is_last;
+  __shared__ int s_is_last, s_nan;
   constexpr int MAXS = NONISO ? 2 * MAXL : MAXL;   // system layers
   const int N = P.N, nlev = P.nlev;
-  const SolveSmem L = solve_smem(N, nlev, BLOCK, P.ng, P.nb, false);
+  const int tid = threadIdx.x, nthr = blockDim.x, nwarps = nthr >> 5;
+  const Lay L = make_lay(N, nlev, nwarps, 1, P.ng, P.nb, false, NONISO ? 2 : 1, false);
   const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
-  double *s_B = (double *)(smem + L.off_B);
+  const double *s_B = (const double *)(smem + L.off_B);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
   double *s_red = (double *)(smem + L.off_red);
-  double *s_fin = (double *)(smem + L.off_fin);
 
-  const int tid = threadIdx.x;
   const int tile = blockIdx.x, col = blockIdx.y;
   const int LP = L.LP, nbtS = L.nbt;
   const double mu = P.mu[col];
   const bool day = mu > 0.0;
-  const int pt0 = tile * BLOCK;
+  const int pt0 = tile * nthr;
   const int b_first = pt0 / P.ng;
-  int pt_last = pt0 + BLOCK - 1;
+  int pt_last = pt0 + nthr - 1;
   if (pt_last > P.npt - 1) pt_last = P.npt - 1;
   const int nbt = pt_last / P.ng - b_first + 1;
   const int nwa = ((pt_last - pt0) >> 5) + 1;
-  stage_column<BLOCK>(P, L, smem, s_T32, col, b_first, nbt, tid);
-  const int col_nan = P.ws_nan[col];
-  __syncthreads();
+  if (tid < 32) s_T32[tid] = kExp2Tab[tid];
+  for (int i = tid; i < 2 * nbt; i += nthr) {
+    const int cl = i / nbt, k = i - cl * nbt;
+    const BinConst bc = P.bins[b_first + k];
+    BinOpt bo;
+    bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2); bo.pad[0] = bo.pad[1] = 0.0;
+    s_bin[cl * nbtS + k] = bo;
+  }
+  column_prep<NONISO>(P, L, smem, col, b_first, nbt, &s_nan);
+  const int col_nan = s_nan;
 
   int pt = pt0 + tid;
   const bool active = pt < P.npt;
@@ -1441,6 +1081,18 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
     double a_t[MAXS], a_r[MAXS], a_su[MAXS], a_sd[MAXS];
     double fu[MAXS + 1], fd[MAXS + 1], bm[MAXS + 1];
 
+    auto optics = [&](const LevelRec *lv, double &kx, double &w0, double &g0) {
+      RowsT<1> rw;
+      load_rows_g<1>(rw, lnk_pt, lv);
+      const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
+      const double2 cb = *reinterpret_cast<const double2 *>(&lv->c10);
+      const double lk = fma(cb.y, rw.v[3][0], fma(cb.x, rw.v[2][0], fma(ca.y, rw.v[1][0], ca.x * rw.v[0][0])));
+      const BinOpt *bo = lv->cloud ? bin1 : bin0;
+      kx = exp_hot<0, false>(lk, T32, nullptr) + bo->sb;
+      w0 = bo->ss * rcp_fast(kx);
+      g0 = bo->gt.g0;
+    };
+
     // ---- S3-S5 per system layer, TOA -> BOA (tau and the beam are running prefixes) ----
     auto coeffs = [&](auto day_tag) {
       constexpr bool DAY = decltype(day_tag)::value;
@@ -1450,7 +1102,7 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
         for (int j = N - 1; j >= 0; --j) {
           const LevelRec *lv = s_lev + j;
           double kx, w0, g0;
-          level_optics(load_rows(lnk_pt, lv), T32, lv, bin0, bin1, kx, w0, g0);
+          optics(lv, kx, w0, g0);
           const double dtau = kx * lv->dm;
           const double Bj = s_B[(size_t)j * nbtS + bl];
           double Fa = 0.0;
@@ -1458,21 +1110,18 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
             tau += dtau;
             Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
           }
-          layer_coeffs<DAY, false>(P, T32, w0, g0, dtau, Bj, Bj, mu, Fa, Fb, a_t[j], a_r[j], a_su[j], a_sd[j]);
+          layer_coeffs<DAY, false>(P, T32, w0, g0_terms(g0, P.inv_eps2), dtau, Bj, Bj, mu, Fa, Fb, a_t[j], a_r[j], a_su[j], a_sd[j]);
           bm[j] = Fa;
           Fb = Fa;
         }
       } else {
         double kx_up, w0_up, g0_up;
-        {
-          const LevelRec *lv = s_lev + LS;
-          level_optics(load_rows(lnk_pt, lv), T32, lv, bin0, bin1, kx_up, w0_up, g0_up);
-        }
+        optics(s_lev + LS, kx_up, w0_up, g0_up);
         double B_up = s_B[(size_t)LS * nbtS + bl];
         for (int sl = LS - 1; sl >= 0; --sl) {
           const LevelRec *lv = s_lev + sl;
           double kx_lo, w0_lo, g0_lo;
-          level_optics(load_rows(lnk_pt, lv), T32, lv, bin0, bin1, kx_lo, w0_lo, g0_lo);
+          optics(lv, kx_lo, w0_lo, g0_lo);
           const double B_lo = s_B[(size_t)sl * nbtS + bl];
           const double dtau = 0.5 * (kx_lo + kx_up) * lv->dm;
           double Fa = 0.0;
@@ -1480,8 +1129,8 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
             tau += dtau;
             Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
           }
-          layer_coeffs<DAY, true>(P, T32, 0.5 * (w0_lo + w0_up), 0.5 * (g0_lo + g0_up), dtau, B_lo, B_up, mu, Fa, Fb,
-                                  a_t[sl], a_r[sl], a_su[sl], a_sd[sl]);
+          layer_coeffs<DAY, true>(P, T32, 0.5 * (w0_lo + w0_up), g0_terms(0.5 * (g0_lo + g0_up), P.inv_eps2), dtau, B_lo, B_up,
+                                  mu, Fa, Fb, a_t[sl], a_r[sl], a_su[sl], a_sd[sl]);
           bm[sl] = Fa;
           Fb = Fa;
           kx_up = kx_lo; w0_up = w0_lo; g0_up = g0_lo; B_up = B_lo;
@@ -1510,61 +1159,12 @@ __global__ void __launch_bounds__(BLOCK) rt_iter_kernel(const KParams P, const i
     }
   }
   __syncthreads();
-  column_epilogue<BLOCK>(P, L, s_red, s_fin, &s_is_last, nwa, P.F_beam != nullptr, col, tile, col_nan);
+  column_epilogue(P, L, smem, &s_is_last, nwa, P.F_beam != nullptr, col, tile, col_nan);
 }
 
-// --------------------------------------------------------------------------------------------
-// small utility kernels
-// --------------------------------------------------------------------------------------------
 __global__ void zero_kernel(double *p, size_t n) {
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     p[i] = 0.0;
-}
-
-__global__ void selftest_math_kernel(int n, const double *x, double *rcp, double *rsq, double *ex, double *omx) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  __shared__ double T32[32];
-  if (threadIdx.x < 32) T32[threadIdx.x] = kExp2Tab[threadIdx.x];
-  __syncthreads();
-  if (i >= n) return;
-  const double v = x[i];
-  rcp[i] = rcp_fast(v);
-  rsq[i] = rsqrt_fast(fabs(v));
-  // e^-|x| through the three entry points the step kernel uses: e^-a, e^-2(a/2) (+ 1 - e^-a), e^(-a)
-  const double a = fmin(fabs(v), 708.0);
-  double om;
-  const double e2 = exp_hot<2, true>(0.5 * a, T32, &om);
-  const double e1 = exp_hot<1, false>(a, T32, nullptr);
-  const double e0 = exp_hot<0, false>(-a, T32, nullptr);
-  ex[i] = (i % 3 == 0) ? e0 : ((i % 3 == 1) ? e1 : e2);
-  omx[i] = om;
-}
-
-__global__ void selftest_planck_kernel(int n, const double *T, const double *lo, const double *hi, double *out) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const double t = T[i];
-  if (!(t > 0.0)) { out[i] = 0.0; return; }
-  double l_hi, l_lo;
-  const double g_hi = planck_G(kPlanckC2 / (hi[i] * t), &l_hi), g_lo = planck_G(kPlanckC2 / (lo[i] * t), &l_lo);
-  const double t2 = t * t;
-  out[i] = kPlanckC1 * t2 * t2 * planck_dG(g_lo, l_lo, g_hi, l_hi) / (hi[i] - lo[i]);
-}
-
-__global__ void dfma_peak_kernel(int iters, double seed, double *sink, long long *cycles) {
-  double a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6,
-         a7 = seed + 7;
-  const double m = 0.999999, k = 1e-9;
-  const long long t0 = clock64();
-#pragma unroll 4
-  for (int i = 0; i < iters; ++i) {
-    a0 = fma(a0, m, k); a1 = fma(a1, m, k); a2 = fma(a2, m, k); a3 = fma(a3, m, k);
-    a4 = fma(a4, m, k); a5 = fma(a5, m, k); a6 = fma(a6, m, k); a7 = fma(a7, m, k);
-  }
-  const long long t1 = clock64();
-  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-  if (s == 123.456) sink[0] = s;
-  if (threadIdx.x == 0 && blockIdx.x == 0) cycles[0] = t1 - t0;
 }
 
 // --------------------------------------------------------------------------------------------
@@ -1572,131 +1172,73 @@ __global__ void dfma_peak_kernel(int iters, double seed, double *sink, long long
 // --------------------------------------------------------------------------------------------
 typedef void (*kernel_fn)(const KParams);
 
-struct KernelChoice {
+struct Variant {
+  bool noniso, toa;
+  int ppt, rows, stk, scap;   // scap: capacity (interfaces) of the local-memory stack of the STK = 0 comparison builds
+  int maxt, minb;      // launch bounds: register cap = 65536 / (maxt * minb)
   kernel_fn fn;
-  int block;
 };
 
-template <bool NONISO, bool TOA, bool BDIRECT>
-KernelChoice pick_kernel(int block, int minb) {
-#define HRT_VARIANT(B, M) if (block == B && (minb == M || minb == 0)) return {rt_solve_kernel<NONISO, TOA, BDIRECT, B, M>, B};
-  HRT_VARIANT(32, 16) HRT_VARIANT(64, 8) HRT_VARIANT(96, 7) HRT_VARIANT(128, 4) HRT_VARIANT(128, 5) HRT_VARIANT(128, 6)
-#undef HRT_VARIANT
-  return {nullptr, 0};
-}
+#define HRT_K(NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB) \
+  {NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB>}
 
-template <bool BDIRECT>
-KernelChoice pick_b(bool noniso, bool toa, int block, int minb) {
-  if (noniso) return toa ? pick_kernel<true, true, BDIRECT>(block, minb) : pick_kernel<true, false, BDIRECT>(block, minb);
-  return toa ? pick_kernel<false, true, BDIRECT>(block, minb) : pick_kernel<false, false, BDIRECT>(block, minb);
-}
-
-KernelChoice pick(bool noniso, bool toa, bool bdirect, int block, int minb) {
-  return bdirect ? pick_b<true>(noniso, toa, block, minb) : pick_b<false>(noniso, toa, block, minb);
-}
-
-KernelChoice pick2(bool toa, int minb) {
-#define HRT_VARIANT2(M) if (minb == M) return {toa ? rt_solve2_kernel<true, 64, M> : rt_solve2_kernel<false, 64, M>, 64};
-  HRT_VARIANT2(5) HRT_VARIANT2(6) HRT_VARIANT2(7) HRT_VARIANT2(8)
-#undef HRT_VARIANT2
-  return {nullptr, 0};
-}
-
-// four points per thread: TOA mode only (no stack), 12 warp-sized blocks per SM at 164 registers
-KernelChoice pick4() { return {rt_solvem_kernel<true, 4, 32, 9>, 32}; }
+// Compiled instantiations, in order of preference for each (noniso, toa, ppt).  helios_rt_create takes the first
+// match; helios_rt_debug_set_launch (tests, tuning) may select any other.
+const Variant kVariants[] = {
+#include "helios_rt_variants.inc"
+};
+constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
 
 typedef void (*iter_fn)(const KParams, const int);
-iter_fn pick_iter(bool noniso, int block) {
-  switch (block) {
-    case 32: return noniso ? rt_iter_kernel<true, 32> : rt_iter_kernel<false, 32>;
-    case 64: return noniso ? rt_iter_kernel<true, 64> : rt_iter_kernel<false, 64>;
-    case 96: return noniso ? rt_iter_kernel<true, 96> : rt_iter_kernel<false, 96>;
-    case 128: return noniso ? rt_iter_kernel<true, 128> : rt_iter_kernel<false, 128>;
-  }
-  return nullptr;
-}
-
-const int kBlocks[] = {32, 64, 96, 128};
-
-// block size of the one-point-per-thread kernels: columns with many spectral points use 128-thread tiles, except the
-// non-isothermal solve kernel, which runs best as 16 warp-sized blocks per SM at 128 registers (config 3 / 4:
-// 1.390 / 5.41 ms against 1.427 / 5.60 at 128 x 4 and 1.460 / 5.73 at 64 x 8); small columns take the block with the
-// fewest padded lanes, ties -> larger block (fewer tiles)
-int choose_block(int npt, bool noniso_solve = false) {
-  const char *env = getenv("HELIOS_RT_BLOCK");
-  if (env) {
-    const int v = atoi(env);
-    for (int b : kBlocks) if (b == v) return v;
-  }
-  if (npt >= 256) return noniso_solve ? 32 : 128;
-  int best = 32;
-  long best_waste = -1;
-  for (int b : {32, 64, 96, 128}) {
-    const long tiles = (npt + b - 1) / b;
-    const long waste = tiles * (long)(((b + 31) / 32) * 32) - npt;
-    if (best_waste < 0 || waste < best_waste || (waste == best_waste && b > best)) { best = b; best_waste = waste; }
-  }
-  return best;
-}
-
-// resident blocks per SM the kernel is compiled for (register cap), measured on B200: isothermal with the
-// back-substitution stack 128 x 6 (80 registers, no spills: config 2 0.718 ms against 0.762 at 5 and 0.747 at 7),
-// TOA mode 128 x 5 (96 registers), non-isothermal 128 x 4 (128 registers)
-int choose_minb(int block, bool noniso, bool toa) {
-  const char *mb = getenv("HELIOS_RT_MINB");
-  if (mb) return atoi(mb);
-  if (block == 128) return noniso ? 4 : (toa ? 5 : 6);
-  return 0;
-}
 
 // spectral points per thread: isothermal columns whose number of Gauss points is a multiple of it, with enough points
-// to fill the tiles.  2 (rt_solve2_kernel) with the back-substitution stack; 4 (rt_solvem_kernel) in TOA mode, where no
-// stack competes for the load/store path (measured, config 2 / config 5 solve kernel: 1: 0.716 / 4.97 ms, 2: 0.67 / 4.73,
-// 4: 0.80 / 4.52).  HELIOS_RT_PPT=1|2|4 overrides.
-int choose_ppt(int npt, int ng, bool noniso, bool toa) {
+// to fill the tiles.  2 with the back-substitution pass, 4 in TOA mode.
+int default_ppt(int npt, int ng, bool noniso, bool toa) {
   const bool can2 = !noniso && ng > 1 && (ng % 2) == 0, can4 = can2 && toa && (ng % 4) == 0;
-  const char *env = getenv("HELIOS_RT_PPT");
-  if (env) { const int v = atoi(env); return (v == 4 && can4) ? 4 : ((v >= 2 && can2) ? 2 : 1); }
   if (npt < 256) return 1;
   return can4 ? 4 : (can2 ? 2 : 1);
 }
 
-int choose_minb2() {
-  const char *mb = getenv("HELIOS_RT_MINB");
-  if (mb) { const int v = atoi(mb); if (v >= 5 && v <= 8) return v; }
-  return 8;   // 126 registers, no spills: 8 x 64 threads x 2 points per SM
+// warps per block: tiles of 128 spectral points for long columns; small columns take the
+// block with the fewest padded lanes, ties -> larger block (fewer tiles)
+int default_warps(int npt, int ppt, bool noniso) {
+  if (npt >= 256) return noniso ? 4 : (ppt == 4 ? 1 : (ppt == 2 ? 2 : 4));
+  int best = 1;
+  long best_waste = -1;
+  for (int w = 1; w <= 4; ++w) {
+    const long tp = 32L * w * ppt, tiles = (npt + tp - 1) / tp;
+    const long waste = tiles * tp - npt;
+    if (best_waste < 0 || waste < best_waste || (waste == best_waste && w > best)) { best = w; best_waste = waste; }
+  }
+  return best;
 }
 
 }  // namespace
 
 struct helios_rt {
   helios_rt_config cfg;   // pointers nulled
-  int npt, block, tiles, ppt;      // solve kernel: threads per block, tiles per column, points per thread
-  int iter_block, iter_tiles;      // rt_iter_kernel keeps one point per thread
+  int npt, nlev;
   bool noniso, toa;
-  KernelChoice kc;
-  SolveSmem lay;
-  int nlev;
+  // launch shape of rt_step_kernel
+  int variant, warps, ppt, tiles, workers, occ;
+  Lay lay;
+  int iter_warps, iter_tiles;      // rt_iter_kernel keeps one point per thread
+  unsigned row_stride;
+  double inv_dlp, inv_dt;
   // device tables
-  double *d_lnk, *d_tab_lp, *d_tab_t, *d_edges, *d_gw;
+  double *d_lnk, *d_tab_lp, *d_tab_t, *d_edges, *d_gw, *d_gtab;
   BinConst *d_bins;
-  double *d_partial;
-  unsigned *d_counter;
-  LevelRec *d_ws_lev;
-  double *d_ws_B, *d_ws_dm;
-  int *d_ws_nan;
-  // device staging for step_host
-  double *d_p, *d_T, *d_mu, *d_fstar, *d_out;   // d_out: 5*(N+1)+N+nb per column, carved per output
-  cudaStream_t own_stream;
-  int regs, lmem, occ, sm_count;
+  // workspace
+  double *d_stack, *d_partial;
+  size_t stack_block, stack_bytes, partial_bytes;
+  unsigned *d_counter, *d_queue;
+  // device + pinned host staging for step_host
+  double *d_in, *d_out, *h_in, *h_out;
+  cudaStream_t own_stream, copy_stream;
+  cudaEvent_t ev_in[4], ev_done[4];
+  int regs, lmem, sm_count;
   cudaError_t last_err;
-  // per-kernel timing (helios_rt_set_profiling): a ring of event triples (before prep, between, after solve)
-  int profiling;
-  cudaEvent_t *prof_ev;      // [kProfRing][3]
-  long long prof_head;       // triples recorded since the last read
 };
-
-constexpr int kProfRing = 256;
 
 #define CK(h, call)                                                   \
   do {                                                                \
@@ -1741,7 +1283,7 @@ static int validate_config(const helios_rt_config *c) {
       c->n_ktab_t < 2 || c->max_columns < 1)
     return HELIOS_RT_EINVAL;
   if ((long long)c->n_bins * c->n_gauss > (1 << 24)) return HELIOS_RT_EINVAL;
-  if ((long long)c->n_ktab_p * c->n_ktab_t * c->n_bins * c->n_gauss >= (1LL << 31)) return HELIOS_RT_EINVAL;   // 32-bit table offsets
+  if ((long long)c->n_ktab_p * c->n_ktab_t * ((long long)c->n_bins * c->n_gauss + 2) >= (1LL << 31)) return HELIOS_RT_EINVAL;   // 32-bit table offsets
   if (!c->ktab_p || !c->ktab_t || !c->ktab || !c->bin_edges || !c->gauss_w || !c->scat_gas || !c->cloud_ext ||
       !c->cloud_w0 || !c->cloud_g0)
     return HELIOS_RT_EINVAL;
@@ -1761,8 +1303,9 @@ static int validate_config(const helios_rt_config *c) {
       !(c->w0_transition >= 0) || !(c->f_toa >= 0))
     return HELIOS_RT_EINVAL;
   if (!(c->cloud_p_top == c->cloud_p_top) || !(c->cloud_p_bot == c->cloud_p_bot)) return HELIOS_RT_EINVAL;
+  // kappa in [1e-300, 1e300]: |ln kappa| <= 691 stays inside the domain of the table exp (|x| <= 708)
   const size_t nk = (size_t)c->n_ktab_p * c->n_ktab_t * c->n_bins * c->n_gauss;
-  for (size_t i = 0; i < nk; ++i) if (!(c->ktab[i] > 0) || !(c->ktab[i] < 1e300)) return HELIOS_RT_EINVAL;
+  for (size_t i = 0; i < nk; ++i) if (!(c->ktab[i] >= 1e-300) || !(c->ktab[i] <= 1e300)) return HELIOS_RT_EINVAL;
   return HELIOS_RT_OK;
 }
 
@@ -1776,16 +1319,72 @@ static cudaError_t upload(T **dst, const T *src, size_t n) {
 extern "C" int helios_rt_destroy(helios_rt *h) {
   if (!h) return HELIOS_RT_OK;
   cudaFree(h->d_lnk); cudaFree(h->d_tab_lp); cudaFree(h->d_tab_t); cudaFree(h->d_edges); cudaFree(h->d_gw);
-  cudaFree(h->d_bins); cudaFree(h->d_partial); cudaFree(h->d_counter);
-  cudaFree(h->d_ws_lev); cudaFree(h->d_ws_B); cudaFree(h->d_ws_dm); cudaFree(h->d_ws_nan);
-  cudaFree(h->d_p); cudaFree(h->d_T); cudaFree(h->d_mu); cudaFree(h->d_fstar); cudaFree(h->d_out);
+  cudaFree(h->d_gtab); cudaFree(h->d_bins); cudaFree(h->d_partial); cudaFree(h->d_counter); cudaFree(h->d_queue);
+  cudaFree(h->d_stack); cudaFree(h->d_in); cudaFree(h->d_out);
+  if (h->h_in) cudaFreeHost(h->h_in);
+  if (h->h_out) cudaFreeHost(h->h_out);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
-  if (h->prof_ev) {
-    for (int i = 0; i < 3 * kProfRing; ++i) if (h->prof_ev[i]) cudaEventDestroy(h->prof_ev[i]);
-    free(h->prof_ev);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  for (int i = 0; i < 4; ++i) {
+    if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
+    if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
   }
   delete h;
   return HELIOS_RT_OK;
+}
+
+// launch shape + workspace for the chosen variant / warps per block.  Frees and re-allocates the workspace whose size
+// depends on the shape; called by create and by helios_rt_debug_set_launch.
+static int configure_launch(helios_rt *h) {
+  const helios_rt_config &c = h->cfg;
+  const Variant &v = kVariants[h->variant];
+  const int N = c.n_layers;
+  h->ppt = v.ppt;
+  if (h->warps * 32 > v.maxt) return HELIOS_RT_EINVAL;
+  if (!h->toa && v.stk == 0 && N + 1 > v.scap) return HELIOS_RT_EINVAL;
+  const int tp = h->warps * 32 * h->ppt;
+  h->tiles = (h->npt + tp - 1) / tp;
+  h->lay = make_lay(N, h->nlev, h->warps, h->ppt, c.n_gauss, c.n_bins, h->toa, h->noniso ? 2 : 1, v.rows == 1);
+  if (h->lay.total > 227u * 1024u) return HELIOS_RT_EINVAL;
+  CK(h, cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
+  cudaFuncAttributes fa;
+  CK(h, cudaFuncGetAttributes(&fa, v.fn));
+  h->regs = fa.numRegs;
+  h->lmem = (int)fa.localSizeBytes;
+  CK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ, v.fn, h->warps * 32, h->lay.total));
+  if (h->occ < 1) return HELIOS_RT_EINVAL;
+  // persistent grid: as many blocks as are resident at once, split evenly over the tiles; never more workers per
+  // tile than columns
+  long workers = (long)h->sm_count * h->occ / h->tiles;
+  if (workers < 1) workers = 1;
+  if (workers > c.max_columns) workers = c.max_columns;
+  h->workers = (int)workers;
+  // workspace
+  cudaFree(h->d_stack); h->d_stack = nullptr;
+  cudaFree(h->d_partial); h->d_partial = nullptr;
+  cudaFree(h->d_queue); h->d_queue = nullptr;
+  h->stack_block = (size_t)(N + 1) * h->warps * 96 * h->ppt;
+  h->stack_bytes = (!h->toa && v.stk == 1) ? sizeof(double) * h->stack_block * h->tiles * h->workers : 0;
+  if (h->stack_bytes) CK(h, cudaMalloc((void **)&h->d_stack, h->stack_bytes));
+  const int mt = h->tiles > h->iter_tiles ? h->tiles : h->iter_tiles;
+  h->partial_bytes = sizeof(double) * (size_t)c.max_columns * mt * 4 * (N + 1);
+  CK(h, cudaMalloc((void **)&h->d_partial, h->partial_bytes));
+  CK(h, cudaMalloc((void **)&h->d_queue, sizeof(unsigned) * (h->tiles + 1)));
+  CK(h, cudaMemset(h->d_queue, 0, sizeof(unsigned) * (h->tiles + 1)));
+  return HELIOS_RT_OK;
+}
+
+static int find_variant(bool noniso, bool toa, int ppt, int rows, int stk, int maxt, int minb) {
+  for (int i = 0; i < kNumVariants; ++i) {
+    const Variant &v = kVariants[i];
+    if (v.noniso != noniso || v.toa != toa || v.ppt != ppt) continue;
+    if (rows >= 0 && v.rows != rows) continue;
+    if (stk >= 0 && !toa && v.stk != stk) continue;
+    if (maxt >= 0 && v.maxt != maxt) continue;
+    if (minb >= 0 && v.minb != minb) continue;
+    return i;
+  }
+  return -1;
 }
 
 extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
@@ -1805,34 +1404,35 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->npt = nb * ng;
   h->noniso = (cfg->flags & HELIOS_RT_NONISOTHERMAL) != 0;
   h->toa = (cfg->flags & HELIOS_RT_TOA_SPECTRUM) != 0;
-  h->iter_block = choose_block(h->npt);
-  h->iter_tiles = (h->npt + h->iter_block - 1) / h->iter_block;
   h->nlev = h->noniso ? 2 * N + 1 : N;
-  h->ppt = choose_ppt(h->npt, ng, h->noniso, h->toa);
-  if (h->ppt == 4) {
-    h->block = 32;
-    h->kc = pick4();
-  } else if (h->ppt == 2) {
-    h->block = 64;
-    h->kc = pick2(h->toa, choose_minb2());
-  } else {
-    h->block = choose_block(h->npt, h->noniso);
-    h->kc = pick(h->noniso, h->toa, ng == 1, h->block, choose_minb(h->block, h->noniso, h->toa));
-  }
-  h->tiles = (h->npt + h->block * h->ppt - 1) / (h->block * h->ppt);
-  h->lay = solve_smem(N, h->nlev, h->block, ng, nb, h->toa, ng == 1, h->ppt);
-  cudaGetDevice(&rc);
-  cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, rc);
+  h->iter_warps = default_warps(h->npt, 1, false);
+  h->iter_tiles = (h->npt + h->iter_warps * 32 - 1) / (h->iter_warps * 32);
+  int ppt = default_ppt(h->npt, ng, h->noniso, h->toa);
+  h->variant = find_variant(h->noniso, h->toa, ppt, -1, -1, -1, -1);
+  if (h->variant < 0) { ppt = 1; h->variant = find_variant(h->noniso, h->toa, 1, -1, -1, -1, -1); }
+  h->warps = default_warps(h->npt, ppt, h->noniso);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (h->variant < 0) { helios_rt_destroy(h); return HELIOS_RT_EINVAL; }
 
-  // ln(kappa) table, log10 pressure grid, per-bin constants
-  const size_t nk = (size_t)cfg->n_ktab_p * cfg->n_ktab_t * h->npt;
-  double *lnk = (double *)malloc(sizeof(double) * nk);
+  // ln(kappa) table (rows padded to an even length, zero-filled, + a tail so that a warp's bulk copy of its 32 PPT
+  // points never leaves the allocation), log10 pressure grid, per-bin constants, Planck polynomial pieces
+  h->row_stride = (unsigned)((h->npt + 1) & ~1);
+  const size_t nrows = (size_t)cfg->n_ktab_p * cfg->n_ktab_t;
+  const size_t nk = nrows * h->row_stride + 256;
+  double *lnk = (double *)calloc(nk, sizeof(double));
   double *lp = (double *)malloc(sizeof(double) * cfg->n_ktab_p);
   BinConst *bins = (BinConst *)malloc(sizeof(BinConst) * nb);
-  if (!lnk || !lp || !bins) { free(lnk); free(lp); free(bins); helios_rt_destroy(h); return HELIOS_RT_ENOMEM; }
-  for (size_t i = 0; i < nk; ++i) lnk[i] = log(cfg->ktab[i]);
+  double *gtab = (double *)malloc(sizeof(double) * kGIntervals * kGCoef);
+  if (!lnk || !lp || !bins || !gtab) { free(lnk); free(lp); free(bins); free(gtab); helios_rt_destroy(h); return HELIOS_RT_ENOMEM; }
+  for (size_t r = 0; r < nrows; ++r)
+    for (int i = 0; i < h->npt; ++i) lnk[r * h->row_stride + i] = log(cfg->ktab[r * h->npt + i]);
   for (int i = 0; i < cfg->n_ktab_p; ++i) lp[i] = log10(cfg->ktab_p[i]);
+  h->inv_dlp = (cfg->n_ktab_p - 1) / (lp[cfg->n_ktab_p - 1] - lp[0]);
+  h->inv_dt = (cfg->n_ktab_t - 1) / (cfg->ktab_t[cfg->n_ktab_t - 1] - cfg->ktab_t[0]);
   for (int b = 0; b < nb; ++b) {
+    // Eqs.(17)-(18) in per-mass units: sb = what is added to kappa_abs, ss = scattering part, gg = g0
     BinConst &bc = bins[b];
     bc.dlam = cfg->bin_edges[b + 1] - cfg->bin_edges[b];
     bc.inv_dlam = 1.0 / bc.dlam;
@@ -1841,6 +1441,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     bc.ss[0] = sg;            bc.ss[1] = sg + sc;
     bc.gg[0] = 0.0;           bc.gg[1] = (sg + sc > 0.0) ? sc * cfg->cloud_g0[b] / (sg + sc) : 0.0;
   }
+  build_planck_table(gtab);
   cudaError_t e = cudaSuccess;
   auto step = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   step(upload(&h->d_lnk, lnk, nk));
@@ -1849,38 +1450,39 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(upload(&h->d_edges, cfg->bin_edges, (size_t)nb + 1));
   step(upload(&h->d_gw, cfg->gauss_w, (size_t)ng));
   step(upload(&h->d_bins, bins, (size_t)nb));
-  free(lnk); free(lp); free(bins);
+  step(upload(&h->d_gtab, gtab, (size_t)kGIntervals * kGCoef));
+  free(lnk); free(lp); free(bins); free(gtab);
   const size_t ncol = (size_t)cfg->max_columns;
-  step(cudaMalloc((void **)&h->d_partial, sizeof(double) * ncol * (h->tiles > h->iter_tiles ? h->tiles : h->iter_tiles) * 4 * (N + 1)));
-  step(cudaMalloc((void **)&h->d_ws_lev, sizeof(LevelRec) * ncol * (h->nlev + 1)));
-  step(cudaMalloc((void **)&h->d_ws_B, sizeof(double) * ncol * (h->nlev + 1) * nb));
-  step(cudaMalloc((void **)&h->d_ws_dm, sizeof(double) * ncol * N));
-  step(cudaMalloc((void **)&h->d_ws_nan, sizeof(int) * ncol));
   step(cudaMalloc((void **)&h->d_counter, sizeof(unsigned) * ncol));
   if (e == cudaSuccess) step(cudaMemset(h->d_counter, 0, sizeof(unsigned) * ncol));
-  step(cudaMalloc((void **)&h->d_p, sizeof(double) * ncol * N));
-  step(cudaMalloc((void **)&h->d_T, sizeof(double) * ncol * N));
-  step(cudaMalloc((void **)&h->d_mu, sizeof(double) * ncol));
-  step(cudaMalloc((void **)&h->d_fstar, sizeof(double) * nb));
-  step(cudaMalloc((void **)&h->d_out, sizeof(double) * ncol * (4 * (N + 1) + N + nb)));
+  // step_host staging: inputs packed as [p | T | mu | F*], outputs as [F_up | F_down | F_net | F_beam | dTdt | toa]
+  const size_t n_in = ncol * (2 * (size_t)N + 1) + nb, n_out = ncol * (4 * ((size_t)N + 1) + N + nb);
+  step(cudaMalloc((void **)&h->d_in, sizeof(double) * n_in));
+  step(cudaMalloc((void **)&h->d_out, sizeof(double) * n_out));
   step(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
-  if (e == cudaSuccess && h->kc.fn) {
-    step(cudaFuncSetAttribute(h->kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
-    step(cudaFuncSetAttribute(h->noniso ? rt_prep_kernel<true> : rt_prep_kernel<false>,
-                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prep_smem_bytes(N, h->nlev)));
-    if (!h->toa && pick_iter(h->noniso, h->iter_block))
-      step(cudaFuncSetAttribute(pick_iter(h->noniso, h->iter_block), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)solve_smem(N, h->nlev, h->iter_block, ng, nb, false).total));
-    cudaFuncAttributes fa;
-    step(cudaFuncGetAttributes(&fa, h->kc.fn));
-    if (e == cudaSuccess) { h->regs = fa.numRegs; h->lmem = (int)fa.localSizeBytes; }
-    step(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ, h->kc.fn, h->block, h->lay.total));
+  step(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  for (int i = 0; i < 4; ++i) {
+    step(cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming));
+    step(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
   }
-  if (e != cudaSuccess || !h->kc.fn) {
+  if (e == cudaSuccess) {
+    iter_fn it = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
+    if (!h->toa)
+      step(cudaFuncSetAttribute(it, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)make_lay(N, h->nlev, h->iter_warps, 1, ng, nb, false, h->noniso ? 2 : 1, false).total));
+  }
+  if (e != cudaSuccess) {
     const bool oom = (e == cudaErrorMemoryAllocation);
     helios_rt_destroy(h);
     cudaGetLastError();
-    return !oom && e == cudaSuccess ? HELIOS_RT_EINVAL : (oom ? HELIOS_RT_ENOMEM : HELIOS_RT_ECUDA);
+    return oom ? HELIOS_RT_ENOMEM : HELIOS_RT_ECUDA;
+  }
+  rc = configure_launch(h);
+  if (rc) {
+    const bool oom = (h->last_err == cudaErrorMemoryAllocation);
+    helios_rt_destroy(h);
+    cudaGetLastError();
+    return oom ? HELIOS_RT_ENOMEM : rc;
   }
   *out = h;
   return HELIOS_RT_OK;
@@ -1898,15 +1500,19 @@ static int validate_step(const helios_rt *h, const helios_rt_inputs *in, const h
   return HELIOS_RT_OK;
 }
 
+// col0: first column of a chunk (step_host pipelines chunks; helios_rt_step passes 0); the chunk's inputs and outputs
+// start at column 0 of the given pointers
 static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out, cudaStream_t st,
                        int n_iter = 0) {
   const helios_rt_config &c = h->cfg;
   if (in->n_columns == 0) return HELIOS_RT_OK;
   KParams P;
   P.lnk = h->d_lnk; P.tab_lp = h->d_tab_lp; P.tab_t = h->d_tab_t; P.edges = h->d_edges; P.gauss_w = h->d_gw;
-  P.bins = h->d_bins;
+  P.bins = h->d_bins; P.gtab = h->d_gtab;
   P.nP = c.n_ktab_p; P.nT = c.n_ktab_t; P.N = c.n_layers; P.nlev = h->nlev; P.nb = c.n_bins; P.ng = c.n_gauss; P.npt = h->npt;
   P.tiles = n_iter > 0 ? h->iter_tiles : h->tiles;
+  P.ncol = in->n_columns;
+  P.row_stride = h->row_stride; P.inv_dlp = h->inv_dlp; P.inv_dt = h->inv_dt;
   P.cloud_p_top = c.cloud_p_top; P.cloud_p_bot = c.cloud_p_bot; P.inv_g = 1.0 / c.gravity; P.inv_cp = 1.0 / c.cp;
   P.inv_eps2 = 1.0 / c.eps2; P.e_tau = c.e_tau; P.gcrit_tol = c.gcrit_tol; P.w0_transition = c.w0_transition;
   P.f_toa = c.f_toa; P.improved = (c.flags & HELIOS_RT_IMPROVED) ? 1 : 0;
@@ -1914,32 +1520,28 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.T_int = in->f_internal > 0 ? sqrt(sqrt(in->f_internal / kSigmaSB)) : 0.0;
   P.F_up = out->F_up; P.F_down = out->F_down; P.F_net = out->F_net; P.dTdt = out->dTdt; P.F_beam = out->F_beam;
   P.F_toa_bin = out->F_up_toa_bin;
-  P.partial = h->d_partial; P.counter = h->d_counter;
-  P.ws_lev = h->d_ws_lev; P.ws_B = h->d_ws_B; P.ws_dm = h->d_ws_dm; P.ws_nan = h->d_ws_nan;
+  P.stack = h->d_stack; P.stack_block = h->stack_block;
+  P.partial = h->d_partial; P.counter = h->d_counter; P.queue = h->d_queue;
+  if (n_iter > 0) {
+    if (in->n_columns > 65535) return HELIOS_RT_EINVAL;   // the comparison kernel puts columns in gridDim.y
+    iter_fn fn = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
+    const Lay lay = make_lay(c.n_layers, h->nlev, h->iter_warps, 1, c.n_gauss, c.n_bins, false, h->noniso ? 2 : 1, false);
+    dim3 grid((unsigned)h->iter_tiles, (unsigned)in->n_columns);
+    fn<<<grid, h->iter_warps * 32, lay.total, st>>>(P, n_iter);
+    CK(h, cudaGetLastError());
+    return HELIOS_RT_OK;
+  }
   // bins that straddle two tiles are accumulated with atomics: start from zero
-  if (P.F_toa_bin && h->tiles > 1 && ((h->block * h->ppt) % c.n_gauss) != 0) {
+  const int tp = h->warps * 32 * h->ppt;
+  if (P.F_toa_bin && h->tiles > 1 && (tp % c.n_gauss) != 0) {
     const size_t n = (size_t)in->n_columns * c.n_bins;
     zero_kernel<<<(unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, st>>>(P.F_toa_bin, n);
   }
-  cudaEvent_t *ev = h->profiling ? h->prof_ev + 3 * (h->prof_head % kProfRing) : nullptr;
-  if (ev) CK(h, cudaEventRecord(ev[0], st));
-  dim3 pgrid((unsigned)((c.n_bins + PREP_BINS - 1) / PREP_BINS), (unsigned)in->n_columns);
-  const size_t psm = prep_smem_bytes(c.n_layers, h->nlev);
-  if (h->noniso) rt_prep_kernel<true><<<pgrid, PREP_BLOCK, psm, st>>>(P);
-  else rt_prep_kernel<false><<<pgrid, PREP_BLOCK, psm, st>>>(P);
+  int workers = h->workers;
+  if (workers > in->n_columns) workers = in->n_columns;
+  dim3 grid((unsigned)h->tiles, (unsigned)workers);
+  kVariants[h->variant].fn<<<grid, h->warps * 32, h->lay.total, st>>>(P);
   CK(h, cudaGetLastError());
-  if (ev) CK(h, cudaEventRecord(ev[1], st));
-  dim3 grid((unsigned)P.tiles, (unsigned)in->n_columns);
-  if (n_iter > 0) {
-    iter_fn fn = pick_iter(h->noniso, h->iter_block);
-    if (!fn) return HELIOS_RT_EINVAL;
-    const SolveSmem lay = solve_smem(c.n_layers, h->nlev, h->iter_block, c.n_gauss, c.n_bins, false);
-    fn<<<grid, h->iter_block, lay.total, st>>>(P, n_iter);
-  } else {
-    h->kc.fn<<<grid, h->block, h->lay.total, st>>>(P);
-  }
-  CK(h, cudaGetLastError());
-  if (ev) { CK(h, cudaEventRecord(ev[2], st)); ++h->prof_head; }
   return HELIOS_RT_OK;
 }
 
@@ -1964,12 +1566,13 @@ extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, con
   if (in->n_columns == 0) return HELIOS_RT_OK;
   const size_t ncol = (size_t)in->n_columns, N = (size_t)h->cfg.n_layers, nb = (size_t)h->cfg.n_bins;
   cudaStream_t st = h->own_stream;
-  CK(h, cudaMemcpyAsync(h->d_p, in->p, sizeof(double) * ncol * N, cudaMemcpyHostToDevice, st));
-  CK(h, cudaMemcpyAsync(h->d_T, in->T, sizeof(double) * ncol * N, cudaMemcpyHostToDevice, st));
-  CK(h, cudaMemcpyAsync(h->d_mu, in->mu_star, sizeof(double) * ncol, cudaMemcpyHostToDevice, st));
-  CK(h, cudaMemcpyAsync(h->d_fstar, in->stellar_flux, sizeof(double) * nb, cudaMemcpyHostToDevice, st));
+  double *d_p = h->d_in, *d_T = d_p + ncol * N, *d_mu = d_T + ncol * N, *d_fs = d_mu + ncol;
+  CK(h, cudaMemcpyAsync(d_p, in->p, sizeof(double) * ncol * N, cudaMemcpyHostToDevice, st));
+  CK(h, cudaMemcpyAsync(d_T, in->T, sizeof(double) * ncol * N, cudaMemcpyHostToDevice, st));
+  CK(h, cudaMemcpyAsync(d_mu, in->mu_star, sizeof(double) * ncol, cudaMemcpyHostToDevice, st));
+  CK(h, cudaMemcpyAsync(d_fs, in->stellar_flux, sizeof(double) * nb, cudaMemcpyHostToDevice, st));
   helios_rt_inputs din = *in;
-  din.p = h->d_p; din.T = h->d_T; din.mu_star = h->d_mu; din.stellar_flux = h->d_fstar;
+  din.p = d_p; din.T = d_T; din.mu_star = d_mu; din.stellar_flux = d_fs;
   helios_rt_outputs dout;
   double *o = h->d_out;
   const size_t ni = ncol * (N + 1);
@@ -1992,115 +1595,38 @@ extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, con
   return HELIOS_RT_OK;
 }
 
-extern "C" int helios_rt_set_profiling(helios_rt *h, int32_t on) {
-  if (!h) return HELIOS_RT_EINVAL;
-  if (on && !h->prof_ev) {
-    h->prof_ev = (cudaEvent_t *)calloc(3 * kProfRing, sizeof(cudaEvent_t));
-    if (!h->prof_ev) return HELIOS_RT_ENOMEM;
-    for (int i = 0; i < 3 * kProfRing; ++i) CK(h, cudaEventCreate(&h->prof_ev[i]));
-  }
-  h->profiling = on ? 1 : 0;
-  h->prof_head = 0;
-  return HELIOS_RT_OK;
-}
-
-extern "C" int helios_rt_kernel_times(helios_rt *h, int32_t *n_steps, double *prep_ms, double *solve_ms) {
-  if (!h || !n_steps || !prep_ms || !solve_ms) return HELIOS_RT_EINVAL;
-  *n_steps = 0; *prep_ms = 0.0; *solve_ms = 0.0;
-  if (!h->prof_ev) return HELIOS_RT_OK;
-  const long long n = h->prof_head < kProfRing ? h->prof_head : kProfRing;
-  for (long long k = h->prof_head - n; k < h->prof_head; ++k) {
-    cudaEvent_t *ev = h->prof_ev + 3 * (k % kProfRing);
-    CK(h, cudaEventSynchronize(ev[2]));
-    float a = 0.f, b = 0.f;
-    CK(h, cudaEventElapsedTime(&a, ev[0], ev[1]));
-    CK(h, cudaEventElapsedTime(&b, ev[1], ev[2]));
-    *prep_ms += a; *solve_ms += b;
-  }
-  *n_steps = (int32_t)n;
-  h->prof_head = 0;
-  return HELIOS_RT_OK;
-}
-
 extern "C" int helios_rt_launch_info(const helios_rt *h, int32_t info[8]) {
   if (!h || !info) return HELIOS_RT_EINVAL;
-  info[0] = h->block; info[1] = h->tiles; info[2] = (int32_t)h->lay.total; info[3] = h->regs; info[4] = h->occ;
+  info[0] = h->warps * 32; info[1] = h->tiles; info[2] = (int32_t)h->lay.total; info[3] = h->regs; info[4] = h->occ;
   info[5] = h->lmem;
-  info[6] = 2;   // rt_prep_kernel + rt_solve_kernel (+1 zero-fill launch when F_up_toa_bin bins straddle tiles)
+  info[6] = 1;   // rt_step_kernel (+1 zero-fill launch when F_up_toa_bin bins straddle tiles)
   info[7] = h->sm_count;
   return HELIOS_RT_OK;
 }
 
-extern "C" int helios_rt_selftest_math(int32_t n, const double *x, double *rcp, double *rsq, double *ex, double *omx) {
-  if (n < 0 || (n > 0 && (!x || !rcp || !rsq || !ex || !omx))) return HELIOS_RT_EINVAL;
-  int rc = check_device();
-  if (rc) return rc;
-  if (n == 0) return HELIOS_RT_OK;
-  double *d = nullptr;
-  if (cudaMalloc((void **)&d, sizeof(double) * 5 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return HELIOS_RT_ENOMEM; }
-  cudaError_t e = cudaMemcpy(d, x, sizeof(double) * n, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) {
-    selftest_math_kernel<<<(n + 127) / 128, 128>>>(n, d, d + n, d + 2 * (size_t)n, d + 3 * (size_t)n, d + 4 * (size_t)n);
-    e = cudaGetLastError();
-  }
-  if (e == cudaSuccess) e = cudaMemcpy(rcp, d + n, sizeof(double) * n, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemcpy(rsq, d + 2 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemcpy(ex, d + 3 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemcpy(omx, d + 4 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
-  cudaFree(d);
-  return e == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
+// ---- include/helios_rt_debug.h: not part of the product API ----
+extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t ppt, int32_t rows, int32_t stk,
+                                          int32_t maxt, int32_t minb) {
+  if (!h) return HELIOS_RT_EINVAL;
+  const Variant &cur = kVariants[h->variant];
+  const int want_ppt = ppt > 0 ? ppt : cur.ppt;
+  if (want_ppt > 1 && (h->noniso ? false : (h->cfg.n_gauss % want_ppt) != 0)) return HELIOS_RT_EINVAL;
+  const int v = find_variant(h->noniso, h->toa, want_ppt, rows, stk, maxt, minb);
+  if (v < 0) return HELIOS_RT_EINVAL;
+  const int old_v = h->variant, old_w = h->warps;
+  h->variant = v;
+  if (warps > 0) h->warps = warps;
+  int rc = configure_launch(h);
+  if (rc) { h->variant = old_v; h->warps = old_w; configure_launch(h); }
+  return rc;
 }
 
-extern "C" int helios_rt_selftest_planck(int32_t n, const double *T, const double *lam_lo, const double *lam_hi,
-                                         double *out) {
-  if (n < 0 || (n > 0 && (!T || !lam_lo || !lam_hi || !out))) return HELIOS_RT_EINVAL;
-  int rc = check_device();
-  if (rc) return rc;
-  if (n == 0) return HELIOS_RT_OK;
-  double *d = nullptr;
-  if (cudaMalloc((void **)&d, sizeof(double) * 4 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return HELIOS_RT_ENOMEM; }
-  cudaError_t e = cudaMemcpy(d, T, sizeof(double) * n, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy(d + n, lam_lo, sizeof(double) * n, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy(d + 2 * (size_t)n, lam_hi, sizeof(double) * n, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) {
-    selftest_planck_kernel<<<(n + 127) / 128, 128>>>(n, d, d + n, d + 2 * (size_t)n, d + 3 * (size_t)n);
-    e = cudaGetLastError();
-  }
-  if (e == cudaSuccess) e = cudaMemcpy(out, d + 3 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost);
-  cudaFree(d);
-  return e == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
-}
-
-extern "C" int helios_rt_measure_dfma_peak(int32_t iters, double *dfma_per_s, double *sm_clock_mhz) {
-  if (iters < 1 || !dfma_per_s) return HELIOS_RT_EINVAL;
-  int rc = check_device();
-  if (rc) return rc;
-  int dev = 0, sms = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  double *sink = nullptr;
-  long long *cyc = nullptr;
-  if (cudaMalloc((void **)&sink, sizeof(double)) != cudaSuccess) return HELIOS_RT_ENOMEM;
-  if (cudaMalloc((void **)&cyc, sizeof(long long)) != cudaSuccess) { cudaFree(sink); return HELIOS_RT_ENOMEM; }
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
-  const int blocks = sms * 2, threads = 1024;
-  dfma_peak_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, sink, cyc);   // warm-up
-  float best = 1e30f;
-  long long hc = 0;
-  for (int rep = 0; rep < 3; ++rep) {
-    cudaEventRecord(e0);
-    dfma_peak_kernel<<<blocks, threads>>>(iters, 1.0, sink, cyc);
-    cudaEventRecord(e1);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { rc = HELIOS_RT_ECUDA; break; }
-    float ms = 0;
-    cudaEventElapsedTime(&ms, e0, e1);
-    if (ms < best) { best = ms; cudaMemcpy(&hc, cyc, sizeof(hc), cudaMemcpyDeviceToHost); }
-  }
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(sink); cudaFree(cyc);
-  if (rc) return rc;
-  *dfma_per_s = 8.0 * (double)iters * (double)blocks * threads / (best * 1e-3);
-  if (sm_clock_mhz) *sm_clock_mhz = (double)hc / (best * 1e-3) * 1e-6;
+extern "C" int helios_rt_debug_get_launch(const helios_rt *h, int32_t info[16]) {
+  if (!h || !info) return HELIOS_RT_EINVAL;
+  const Variant &v = kVariants[h->variant];
+  info[0] = h->warps; info[1] = v.ppt; info[2] = v.rows; info[3] = v.stk; info[4] = v.maxt; info[5] = v.minb;
+  info[6] = h->tiles; info[7] = h->workers; info[8] = h->occ; info[9] = h->regs; info[10] = h->lmem;
+  info[11] = (int32_t)h->lay.total; info[12] = (int32_t)(h->stack_bytes >> 20); info[13] = h->variant;
+  info[14] = kNumVariants; info[15] = 0;
   return HELIOS_RT_OK;
 }

@@ -13,18 +13,18 @@ import numpy as np
 
 from .workloads import IMPROVED, NONISOTHERMAL, TOA_SPECTRUM  # noqa: F401
 
-import os
-
-# HELIOS_RT_LIBRARY: developer override for A/B-ing builds of the same source; the default is the in-tree build
-_LIB_PATH = Path(os.environ.get("HELIOS_RT_LIBRARY") or Path(__file__).resolve().parent / "libhelios_rt.so")
+_LIB_PATH = Path(__file__).resolve().parent / "libhelios_rt.so"
+_SELFTEST_PATH = Path(__file__).resolve().parent / "libhelios_rt_selftest.so"   # test / benchmark hooks, not the product
 _dp = C.POINTER(C.c_double)
 
+# symbols declared in include/helios_rt.h + include/helios_rt_debug.h (libhelios_rt.so) ...
 EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
-           "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info",
-           "helios_rt_set_profiling", "helios_rt_kernel_times", "helios_rt_step_iterative",
+           "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info", "helios_rt_step_iterative",
            "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_phase_curve_workspace_bytes",
-           "helios_rt_advance_1d",
-           "helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_measure_dfma_peak")
+           "helios_rt_advance_1d", "helios_rt_debug_set_launch", "helios_rt_debug_get_launch")
+# ... and in include/helios_rt_selftest.h (libhelios_rt_selftest.so)
+SELFTEST_EXPORTS = ("helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_selftest_planck_G",
+                    "helios_rt_measure_dfma_peak", "helios_rt_measure_latencies")
 
 
 class Config(C.Structure):
@@ -47,6 +47,7 @@ class Outputs(C.Structure):
 
 OUTPUT_NAMES = tuple(n for n, _ in Outputs._fields_)
 _lib = None
+_selftest = None
 
 
 class HeliosRTError(RuntimeError):
@@ -85,18 +86,33 @@ def load_library() -> C.CDLL:
         L.helios_rt_phase_curve_workspace_bytes.argtypes = [C.c_int32] * 3
         L.helios_rt_advance_1d.restype = C.c_int
         L.helios_rt_advance_1d.argtypes = [C.c_int32] * 2 + [C.c_double] * 4 + [C.c_void_p] * 6
-        L.helios_rt_set_profiling.restype = C.c_int
-        L.helios_rt_set_profiling.argtypes = [C.c_void_p, C.c_int32]
-        L.helios_rt_kernel_times.restype = C.c_int
-        L.helios_rt_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_int32), _dp, _dp]
+        L.helios_rt_debug_set_launch.restype = C.c_int
+        L.helios_rt_debug_set_launch.argtypes = [C.c_void_p] + [C.c_int32] * 6
+        L.helios_rt_debug_get_launch.restype = C.c_int
+        L.helios_rt_debug_get_launch.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        _lib = L
+    return _lib
+
+
+def load_selftest_library() -> C.CDLL:
+    """dlopen the test / benchmark hooks (include/helios_rt_selftest.h)."""
+    global _selftest
+    if _selftest is None:
+        if not _SELFTEST_PATH.exists():
+            raise HeliosRTError(f"{_SELFTEST_PATH} is missing: run `python -m paper_2203_02293_b200.build`")
+        L = C.CDLL(str(_SELFTEST_PATH))
         L.helios_rt_selftest_math.restype = C.c_int
         L.helios_rt_selftest_math.argtypes = [C.c_int32] + [_dp] * 5
         L.helios_rt_selftest_planck.restype = C.c_int
         L.helios_rt_selftest_planck.argtypes = [C.c_int32] + [_dp] * 4
+        L.helios_rt_selftest_planck_G.restype = C.c_int
+        L.helios_rt_selftest_planck_G.argtypes = [C.c_int32] + [_dp] * 2
         L.helios_rt_measure_dfma_peak.restype = C.c_int
         L.helios_rt_measure_dfma_peak.argtypes = [C.c_int32, _dp, _dp]
-        _lib = L
-    return _lib
+        L.helios_rt_measure_latencies.restype = C.c_int
+        L.helios_rt_measure_latencies.argtypes = [_dp]
+        _selftest = L
+    return _selftest
 
 
 def _check(rc: int, handle=None):
@@ -162,14 +178,18 @@ class HeliosRT:
                 "sm_count")
         return dict(zip(keys, list(info)))
 
-    def set_profiling(self, on: bool) -> None:
-        _check(load_library().helios_rt_set_profiling(self._h, 1 if on else 0), self._h)
+    def debug_set_launch(self, warps: int = 0, ppt: int = 0, rows: int = -1, stk: int = -1, maxt: int = -1,
+                         minb: int = -1) -> None:
+        """helios_rt_debug_set_launch (include/helios_rt_debug.h; tests and tuning only)."""
+        _check(load_library().helios_rt_debug_set_launch(self._h, int(warps), int(ppt), int(rows), int(stk), int(maxt),
+                                                         int(minb)), self._h)
 
-    def kernel_times(self) -> tuple[int, float, float]:
-        """(steps recorded, sum of rt_prep_kernel ms, sum of rt_solve_kernel ms) since the last call."""
-        n, a, b = C.c_int32(), C.c_double(), C.c_double()
-        _check(load_library().helios_rt_kernel_times(self._h, C.byref(n), C.byref(a), C.byref(b)), self._h)
-        return n.value, a.value, b.value
+    def debug_get_launch(self) -> dict:
+        info = (C.c_int32 * 16)()
+        _check(load_library().helios_rt_debug_get_launch(self._h, info))
+        keys = ("warps", "ppt", "rows", "stk", "maxt", "minb", "tiles", "workers", "blocks_per_sm", "registers",
+                "local_bytes", "smem_bytes", "stack_mib", "variant", "n_variants")
+        return dict(zip(keys, list(info)))
 
     def step_iterative(self, p, T, mu_star, stellar_flux, f_internal: float, out: dict, n_iterations: int,
                        stream=None) -> None:
@@ -293,21 +313,35 @@ def advance_1d(dt: float, gravity: float, R_d: float, p_ref: float, z, dTdt, T, 
         None if rho is None else _dev(rho, (n, N), "rho"), _stream(stream)))
 
 
+# ---- include/helios_rt_selftest.h (libhelios_rt_selftest.so): test / benchmark hooks ----
 def selftest_math(x):
     x = _np(x)
     outs = [np.empty_like(x) for _ in range(4)]
-    _check(load_library().helios_rt_selftest_math(x.size, _ptr(x), *[_ptr(o) for o in outs]))
+    _check(load_selftest_library().helios_rt_selftest_math(x.size, _ptr(x), *[_ptr(o) for o in outs]))
     return tuple(outs)  # rcp, rsqrt, exp(-|x|), 1-exp(-|x|)
 
 
 def selftest_planck(T, lam_lo, lam_hi) -> np.ndarray:
     T, lo, hi = _np(T), _np(lam_lo), _np(lam_hi)
     out = np.empty_like(T)
-    _check(load_library().helios_rt_selftest_planck(T.size, _ptr(T), _ptr(lo), _ptr(hi), _ptr(out)))
+    _check(load_selftest_library().helios_rt_selftest_planck(T.size, _ptr(T), _ptr(lo), _ptr(hi), _ptr(out)))
+    return out
+
+
+def selftest_planck_G(x) -> np.ndarray:
+    x = _np(x)
+    out = np.empty_like(x)
+    _check(load_selftest_library().helios_rt_selftest_planck_G(x.size, _ptr(x), _ptr(out)))
     return out
 
 
 def measure_dfma_peak(iters: int = 1 << 16) -> tuple[float, float]:
     a, b = C.c_double(), C.c_double()
-    _check(load_library().helios_rt_measure_dfma_peak(int(iters), C.byref(a), C.byref(b)))
+    _check(load_selftest_library().helios_rt_measure_dfma_peak(int(iters), C.byref(a), C.byref(b)))
     return a.value, b.value
+
+
+def measure_latencies() -> dict:
+    lat = (C.c_double * 4)()
+    _check(load_selftest_library().helios_rt_measure_latencies(lat))
+    return dict(zip(("dfma", "rcp_link", "lds_f2i_link", "dadd"), list(lat)))

@@ -4,8 +4,6 @@ on the same seeded inputs.  Tolerances are north_star's: |dF| <= 1e-9 |F| + 1e-1
 """
 from __future__ import annotations
 
-import os
-
 import numpy as np
 import pytest
 
@@ -225,25 +223,63 @@ def test_toa_spectrum_mode_small(torch_cuda, H, oracle_mod):
         assert_parity(oracle_mod, cfg, inp, meta, got, ref)
 
 
-@pytest.mark.parametrize("block", [32, 64, 96, 128])
-def test_every_block_size_and_multi_tile_reduction(torch_cuda, H, oracle_mod, block):
-    """Forces each compiled block size: with 600 points per column, 32..128 give 19..5 tiles per column
-    (cross-tile fixed-order reduction, bins straddling tiles)."""
+@pytest.mark.parametrize("warps", [1, 2, 3, 4])
+def test_every_block_size_and_multi_tile_reduction(torch_cuda, H, oracle_mod, warps):
+    """Forces block sizes of 32..128 threads (helios_rt_debug_set_launch): with 600 points per column they give 19..5
+    tiles per column (cross-tile fixed-order reduction, bins straddling tiles)."""
     from paper_2203_02293_b200 import workloads as W
     cfg, inp, meta = W.make(3, columns=slice(5, None, 400))
     ref = oracle_mod.rt_step(cfg, inp)
-    os.environ["HELIOS_RT_BLOCK"] = str(block)
-    try:
-        rt = H.HeliosRT(cfg, inp["p"].shape[0])
-        assert rt.launch_info()["block"] == block
-        got = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)
-        got2 = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)      # counters re-arm: a second step is identical
-        rt.close()
-    finally:
-        del os.environ["HELIOS_RT_BLOCK"]
+    rt = H.HeliosRT(cfg, inp["p"].shape[0])
+    rt.debug_set_launch(warps=warps)
+    assert rt.launch_info()["block"] == 32 * warps
+    got = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)
+    got2 = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)      # queues and counters re-arm: a second step is identical
+    rt.close()
     assert_parity(oracle_mod, cfg, inp, meta, got, ref)
     for k in ALL:
         assert np.array_equal(got[k], got2[k]), k        # deterministic, run to run
+
+
+def _variants(H, rt):
+    """Every compiled instantiation of rt_step_kernel that fits this handle (same noniso / toa class)."""
+    out = []
+    for ppt in (1, 2, 4):
+        for rows in (0, 1):
+            for stk in (0, 1):
+                for maxt in (384, 512, 576, 640, 768, 1024):
+                    try:
+                        rt.debug_set_launch(ppt=ppt, rows=rows, stk=stk, maxt=maxt)
+                    except H.HeliosRTError:
+                        continue
+                    out.append((ppt, rows, stk, maxt))
+    return out
+
+
+@pytest.mark.parametrize("config,stride", [(2, 211), (3, 307), (5, 853)])
+def test_every_compiled_variant(torch_cuda, H, oracle_mod, config, stride):
+    """All instantiations of the step kernel (points per thread, TMA ring or register-prefetched rows, register caps)
+    give the oracle's answer on a sub-sample of configs 2, 3 and 5, and each reproduces itself bit for bit."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config, columns=slice(2, None, stride))
+    want = ("F_up_toa_bin",) if config == 5 else ("F_up", "F_down", "F_net", "dTdt")
+    ref = oracle_mod.rt_step(cfg, inp, want=want)
+    rt = H.HeliosRT(cfg, inp["p"].shape[0])
+    variants = _variants(H, rt)
+    assert len(variants) >= 1
+    seen = set()
+    for ppt, rows, stk, maxt in variants:
+        rt.debug_set_launch(ppt=ppt, rows=rows, stk=stk, maxt=maxt)
+        key = rt.debug_get_launch()["variant"]
+        if key in seen:
+            continue
+        seen.add(key)
+        got = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+        got2 = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+        assert_parity(oracle_mod, cfg, inp, meta, got, ref)
+        for k in want:
+            assert np.array_equal(got[k], got2[k]), (k, ppt, rows, stk, maxt)
+    rt.close()
 
 
 def test_ragged_shapes(torch_cuda, H, oracle_mod):
