@@ -45,6 +45,13 @@ using namespace hrt;
 
 constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
 
+// unroll factor of the isothermal sweep-1 loop (1: measured best; comparison builds override it)
+#ifndef HRT_UNROLL_ISO
+#define HRT_UNROLL_ISO 1
+#endif
+#define HRT_PRAGMA(x) _Pragma(#x)
+#define HRT_UNROLL(n) HRT_PRAGMA(unroll n)
+
 // --------------------------------------------------------------------------------------------
 // kernel parameters
 // --------------------------------------------------------------------------------------------
@@ -56,7 +63,11 @@ struct BinConst {   // per bin, built at create time from scat_gas / cloud_* (Eq
   double gg[2];     // g0 at a clear / cloudy level
 };
 
-// S1 result per (column, level), built by the block in shared memory
+// phase A, per bin: where its Planck value goes (slots in doubles from the row's start; s1 = -1: one tile only,
+// s1 = -2: more than two tiles own points of the bin -- the CSR lists them all) and 1 / (lam_hi - lam_lo)
+struct __align__(16) BinSlot { int s0, s1; double inv_dlam; };
+
+// S1 result per (column, level), built by phase A in the workspace
 struct __align__(16) LevelRec {
   double c00, c01, c10, c11;  // bilinear weights of the corners (iP,iT), (iP,iT+1), (iP+1,iT), (iP+1,iT+1)
   unsigned o00, o01, o10, o11;  // offsets of the four corner rows (spectral point 0) in the ln(kappa) table, doubles
@@ -75,6 +86,7 @@ struct KParams {
   const double *gauss_w;  // [ng]
   const BinConst *bins;   // [nb]
   const double *gtab;     // Planck polynomial pieces (build_planck_table)
+  const double *c2lam;    // [nb+1] h c / (k lam_edge): x = c2lam / T
   int nP, nT, N, nlev, nb, ng, npt, tiles, ncol;
   unsigned row_stride;
   double inv_dlp, inv_dt;   // 1 / mean spacing of the table grids: first guess of the cell search
@@ -85,11 +97,20 @@ struct KParams {
   double T_int;
   double *F_up, *F_down, *F_net, *dTdt, *F_beam, *F_toa_bin;
   // workspace
+  unsigned char *ws_rec;  // [ncol] per-column record block (Lay::rec_bytes): LevelRec[nlev+1] | layer masses [N] | NaN flag
+  unsigned char *ws_B;    // [ncol][tiles] per-(column, tile) band Planck block (Lay::b_bytes): [nlev+1][nbt], last row pi B(T_int)
+  unsigned *flags;        // [ncol] levels of the column whose phase-A item is published (nlev + 1 = ready); zeroed
+                          // again by the last block of the launch
+  const int *slot_ptr;    // [nb+1] CSR: bin b's value goes to slots[slot_ptr[b] .. slot_ptr[b+1]) ...
+  const int *slots;       // ... = (tile t) (b_bytes/8) + (b - first bin of tile t), for every tile t that owns points of b
+  const BinSlot *bslot;   // [nb] the first two slots and 1/dlam of each bin in one 16-byte record
+  int fused_prep;         // 1: rt_step_kernel runs phase A itself (cooperative launch: the whole grid is resident)
   double *stack;          // [blocks of the grid][N+1][warps][96 PPT] back-substitution coefficients
   size_t stack_block;     // doubles per block
   double *partial;        // [ncol][tiles][4][N+1]
   unsigned *counter;      // [ncol]   tiles of the column that have published their partial sums
-  unsigned *queue;        // [tiles]  next column of each tile's queue;  queue[tiles] = blocks that have finished
+  unsigned *queue;        // [tiles]  next column of each tile's queue;  queue[tiles] = blocks that have finished;
+                          // queue[tiles + 1] = blocks that have finished phase A
 };
 
 // --------------------------------------------------------------------------------------------
@@ -194,6 +215,33 @@ __device__ __forceinline__ void layer_forward(const KParams &P, const double *__
   U = Un;
 }
 
+// Sum each of the 16 values v[0..15] over the 32 lanes of the warp by recursive halving: 16 shuffle+add
+// steps instead of 16 x 5.  Returns, in lanes L and L^1, the total of v[L >> 1].  Fixed order: deterministic.
+__device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
+  const unsigned full = 0xffffffffu;
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const double send = b4 ? v[i] : v[i + 8], keep = b4 ? v[i + 8] : v[i];
+    v[i] = keep + __shfl_xor_sync(full, send, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const double send = b3 ? v[i] : v[i + 4], keep = b3 ? v[i + 4] : v[i];
+    v[i] = keep + __shfl_xor_sync(full, send, 8);
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const double send = b2 ? v[i] : v[i + 2], keep = b2 ? v[i + 2] : v[i];
+    v[i] = keep + __shfl_xor_sync(full, send, 4);
+  }
+  {
+    const double send = b1 ? v[0] : v[1], keep = b1 ? v[1] : v[0];
+    v[0] = keep + __shfl_xor_sync(full, send, 2);
+  }
+  return v[0] + __shfl_xor_sync(full, v[0], 1);
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -213,47 +261,44 @@ static_assert(sizeof(BinOpt) == 64, "BinOpt layout");
 struct Lay {
   int nbt;         // max bins per tile
   int LP;          // N + 1 rounded up to a multiple of 8 (the reductions handle 8 interfaces at a time)
-  unsigned off_lev, off_B, off_bin, off_dm, off_red, off_fin, off_vals, off_bar, off_u, total;
-  unsigned u_lnp, u_pint, u_tint, u_tlev, u_G, u_Glow;   // S1/S2 view of the union at off_u
+  unsigned rec_bytes, b_bytes;     // sizes of the per-column record block and of the per-(column, tile) Planck block
+  unsigned off_rec[2], off_Bt[2];  // both double-buffered: the next column's blocks arrive while this one is swept
+  unsigned off_bin, off_red, off_fin, off_vals, off_bar, off_u, total;   // off_u: per-warp sweep scratch
   unsigned u_stage, u_ring, ring_warp;                   // sweep view: [warp] staging tile; [warp] row ring
 };
 
-// ppt: spectral points per thread; depth: levels per sweep iteration (1 isothermal, 2 non-isothermal); ring: TMA rows
-__host__ __device__ inline Lay make_lay(int N, int nlev, int warps, int ppt, int ng, int nb, bool toa, int depth, bool ring) {
+// ppt: spectral points per thread; depth: levels per sweep iteration (1 isothermal, 2 non-isothermal); rows: 1 TMA ring,
+// 2 per-lane cp.async buffer;
+// bdirect: one Gauss point per bin -- the Planck block is read from the workspace, not staged
+__host__ __device__ inline Lay make_lay(int N, int nlev, int warps, int ppt, int ng, int nb, bool toa, int depth, int rows,
+                                        bool bdirect) {
   Lay L;
   const int tp = warps * 32 * ppt;
   const int nbt = (tp + ng - 1) / ng + 1;
   L.nbt = nbt < nb ? nbt : nb;
   L.LP = (N + 1 + 7) & ~7;
+  L.rec_bytes = (unsigned)((sizeof(LevelRec) * (nlev + 1) + sizeof(double) * (N + 1) + 15) & ~size_t(15));   // LevelRec[nlev+1] | dm[N] | mu
+  L.b_bytes = (unsigned)((sizeof(double) * (nlev + 1) * L.nbt + 15) & ~size_t(15));
   unsigned o = 0;
   auto take = [&](size_t bytes) { unsigned r = o; o += (unsigned)((bytes + 127) & ~size_t(127)); return r; };
-  L.off_lev = take(sizeof(LevelRec) * (nlev + 1));
-  L.off_B = take(sizeof(double) * (nlev + 1) * L.nbt);
+  L.off_rec[0] = take(L.rec_bytes);
+  L.off_rec[1] = take(L.rec_bytes);
+  L.off_Bt[0] = take(bdirect ? 0 : L.b_bytes);
+  L.off_Bt[1] = take(bdirect ? 0 : L.b_bytes);
   L.off_bin = take(sizeof(BinOpt) * 2 * L.nbt);
-  L.off_dm = take(sizeof(double) * N);
   L.off_red = take(toa ? 0 : sizeof(double) * warps * 4 * L.LP);       // F_up, R F_up, U + beam, beam
   L.off_fin = take(toa ? 0 : sizeof(double) * 4 * (N + 1));
   L.off_vals = take(sizeof(double) * tp);
-  L.off_bar = take(8 * RING * warps);
+  L.off_bar = take(8 * (RING * warps + 2));                            // row-ring barriers, then the two record barriers
   L.off_u = o;
-  // S1 / S2 scratch
   unsigned u = 0;
   auto utake = [&](size_t bytes) { unsigned r = u; u += (unsigned)((bytes + 15) & ~size_t(15)); return r; };
-  L.u_lnp = utake(sizeof(double) * N);
-  L.u_pint = utake(sizeof(double) * (N + 1));
-  L.u_tint = utake(sizeof(double) * (N + 1));
-  L.u_tlev = utake(sizeof(double) * (nlev + 1));
-  L.u_G = utake(sizeof(double) * (L.nbt + 1) * (nlev + 1));
-  L.u_Glow = utake(sizeof(double) * (L.nbt + 1) * (nlev + 1));
-  const unsigned prep_bytes = u;
   // sweep scratch
-  u = 0;
   L.u_stage = utake(toa ? 0 : sizeof(double) * warps * 8 * STAGE_LD);
   u = (u + 127) & ~127u;
-  L.ring_warp = ring ? (unsigned)(RING * depth * 4 * 32 * ppt * 8) : 0;
+  L.ring_warp = rows == 1 ? (unsigned)(RING * depth * 4 * 32 * ppt * 8) : (rows == 2 ? (unsigned)(depth * 4 * 32 * ppt * 8) : 0);
   L.u_ring = utake((size_t)L.ring_warp * warps);
-  const unsigned sweep_bytes = u;
-  L.total = L.off_u + (prep_bytes > sweep_bytes ? prep_bytes : sweep_bytes);
+  L.total = L.off_u + u;
   return L;
 }
 
@@ -411,6 +456,66 @@ template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 1> {
   }
 };
 
+// ROWS = 2: per-lane asynchronous copies (cp.async, SASS LDGSTS): every lane copies its own PPT values of each corner
+// row of the NEXT iteration's levels into its own slots of a one-stage per-warp buffer, right after it has consumed
+// this iteration's rows; no other lane touches those slots, so no barrier is involved -- only cp.async.wait_group.
+// Against ROWS = 0 this frees the 8 PPT DEPTH prefetch registers and the moves that rotate them.
+template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 2> {
+  const double *slot;      // this lane's first slot (generic address); row r of level d at slot + (d * 4 + r) * 32 * PPT
+  uint32_t slot_s;
+  const double *lnk_pt;
+  const LevelRec *lv0, *lv_pending;
+  __device__ __forceinline__ void issue(const LevelRec *lv) {
+#pragma unroll
+    for (int d = 0; d < DEPTH; ++d) {
+      const LevelRec *q = lv - d;
+      q = q < lv0 ? lv0 : q;
+      const uint4 o = *reinterpret_cast<const uint4 *>(&q->o00);
+      const unsigned off[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const double *src = elem_addr(lnk_pt, off[c]);
+        const uint32_t dst = slot_s + (uint32_t)((d * 4 + c) * 32 * PPT * 8);
+        if (PPT == 1) {
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+        } else {
+#pragma unroll
+          for (int h = 0; h < PPT / 2; ++h)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 16 * h), "l"(src + 2 * h) : "memory");
+        }
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  __device__ __forceinline__ void prime(const LevelRec *lv, int) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");   // the previous column's last (unused) prefetch has landed
+    issue(lv);
+  }
+  __device__ __forceinline__ void next(RowsT<PPT> (&cur)[DEPTH], const LevelRec *lv_next) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+    for (int d = 0; d < DEPTH; ++d) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const double *a = slot + (d * 4 + c) * 32 * PPT;
+        if (PPT == 1) {
+          cur[d].v[c][0] = *a;
+        } else {
+#pragma unroll
+          for (int h = 0; h < PPT / 2; ++h) {
+            const double2 t = reinterpret_cast<const double2 *>(a)[h];
+            cur[d].v[c][2 * h] = t.x;
+            cur[d].v[c][2 * h + 1] = t.y;
+          }
+        }
+      }
+    }
+    lv_pending = lv_next;
+  }
+  // call once this iteration's rows have been used (their shared-memory loads have completed)
+  __device__ __forceinline__ void release(const LevelRec *, bool) { issue(lv_pending); }
+};
+
 // sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
 // base + k.  Lane L sums 8 entries of row L >> 2, two shuffle steps finish the row.  Fixed order.
 __device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, double *__restrict__ dst, int lane) {
@@ -458,145 +563,155 @@ __device__ __forceinline__ void stk_load(const double *w, int lane, double (&c)[
 }
 
 // --------------------------------------------------------------------------------------------
-// S1 + S2 for one column, by the whole block, into shared memory.
-//   S1 (L171, R9, R7): ln p, interface p/T, layer masses, and per level a LevelRec: the four bilinear corner weights
-//       (1-w_p)(1-w_T) ..., the four k-table row offsets, the (sub-)layer column mass and the cloud flag.
-//   S2 (L171, L239, R8): planck_G at every (level, bin edge of the tile) -- consecutive lanes take consecutive levels
-//       of one edge, so a warp's arguments x = hc/(lam k T) stay close and its lanes take the same branch -- then B_b
-//       per (level, bin); the extra level nlev carries T_int and yields F_BOA,b = pi B_b(T_int).
-// Ends with a block barrier; the S1/S2 scratch (union) is dead afterwards.
+// Phase A: S1 + S2.  One work item = one (column, level); items are independent (a thread recomputes the two or
+// three ln p of its neighbours instead of sharing them), so they are spread over all threads of the grid with no
+// barrier.  Results go to the workspace, read back by the sweeping blocks through bulk async copies.
+//   S1 (L171, R9, R7): the level's p, T (interfaces by linear interpolation in ln p; ends extrapolated half a step
+//       with T held), its LevelRec -- the four bilinear corner weights (1-w_p)(1-w_T) ..., the four k-table row
+//       offsets, the (sub-)layer column mass, the cloud flag, a NaN flag (R19) -- and the layer mass for R14.
+//   S2 (L171, L239, R8): the level's row of band Planck values: the thread walks the bin edges keeping the previous
+//       edge's G (two edges per trip for instruction-level parallelism; consecutive lanes = consecutive levels of one
+//       column, so a warp's x = hc/(lam k T) stay close and its lanes take the same branch of planck_G); every bin's
+//       B_b goes to the Planck block of each tile that owns points of the bin (slots CSR).  The extra level nlev
+//       carries T_int and yields F_BOA,b = pi B_b(T_int).
 // --------------------------------------------------------------------------------------------
 template <bool NONISO>
-__device__ __forceinline__ void column_prep(const KParams &P, const Lay &L, unsigned char *smem, int col, int b_first,
-                                            int nbt, int *s_nan) {
-  const int N = P.N, nlev = P.nlev, tid = threadIdx.x, nthr = blockDim.x;
-  unsigned char *un = smem + L.off_u;
-  double *s_lnp = (double *)(un + L.u_lnp), *s_pint = (double *)(un + L.u_pint), *s_tint = (double *)(un + L.u_tint);
-  double *s_tlev = (double *)(un + L.u_tlev), *s_G = (double *)(un + L.u_G), *s_Glow = (double *)(un + L.u_Glow);
-  LevelRec *s_rec = (LevelRec *)(smem + L.off_lev);   // record 0 duplicates level 0 (prefetch pad); level l at [l + 1]
-  double *s_B = (double *)(smem + L.off_B), *s_dm = (double *)(smem + L.off_dm);
+__device__ __forceinline__ void prep_item(const KParams &P, const Lay &L, const double *__restrict__ T32, int col, int l) {
+  const int N = P.N, nlev = P.nlev;
   const double *pc = P.p + (size_t)col * N;
   const double *Tc = P.T + (size_t)col * N;
-
-  // NaN in p, T or mu of this column poisons the column's outputs (and only them): the clamps and
-  // selects below would otherwise swallow it (R19).
-  if (tid == 0) { const double mu = P.mu[col]; *s_nan = (mu != mu) ? 1 : 0; }
-  __syncthreads();
-  for (int j = tid; j < N; j += nthr) {
-    const double pj = pc[j], tj = Tc[j];
-    if (pj != pj || tj != tj) *s_nan = 1;
-    s_lnp[j] = log(pj);
-  }
-  __syncthreads();
-  for (int i = tid; i <= N; i += nthr) {
-    double lp, ti;
-    if (N == 1) {
-      lp = s_lnp[0] + (i == 0 ? 0.5 : -0.5) * 2.302585092994045684;
-      ti = Tc[0];
-    } else if (i == 0) {
-      lp = s_lnp[0] + 0.5 * (s_lnp[0] - s_lnp[1]);
-      ti = Tc[0];
-    } else if (i == N) {
-      lp = s_lnp[N - 1] - 0.5 * (s_lnp[N - 2] - s_lnp[N - 1]);
-      ti = Tc[N - 1];
-    } else {
-      lp = 0.5 * (s_lnp[i - 1] + s_lnp[i]);
-      ti = 0.5 * (Tc[i - 1] + Tc[i]);
-    }
-    s_pint[i] = exp(lp);
-    s_tint[i] = ti;
-  }
-  __syncthreads();
-  auto p_level = [&](int l) -> double {
-    if (NONISO) return (l & 1) ? pc[l >> 1] : s_pint[l >> 1];
-    return pc[l];
+  unsigned char *rec = P.ws_rec + (size_t)col * L.rec_bytes;
+  LevelRec *g_rec = (LevelRec *)rec;    // record 0 duplicates level 0 (prefetch pad); level l at [l + 1]
+  double *g_dm = (double *)(rec + sizeof(LevelRec) * (nlev + 1));
+  // ln p at interface i of the column (R9)
+  auto lnp_int = [&](int i) -> double {
+    if (N == 1) return log(pc[0]) + (i == 0 ? 0.5 : -0.5) * 2.302585092994045684;
+    if (i == 0) { const double a = log(pc[0]); return a + 0.5 * (a - log(pc[1])); }
+    if (i == N) { const double a = log(pc[N - 1]); return a - 0.5 * (log(pc[N - 2]) - a); }
+    return 0.5 * (log(pc[i - 1]) + log(pc[i]));
   };
-  for (int l = tid; l <= nlev; l += nthr) {
-    if (l == nlev) { s_tlev[l] = P.T_int; continue; }
-    const double pl = p_level(l);
-    const double tl = NONISO ? ((l & 1) ? Tc[l >> 1] : s_tint[l >> 1]) : Tc[l];
-    s_tlev[l] = tl;
-    LevelRec rec;
-    rec.cloud = (pl >= P.cloud_p_top && pl <= P.cloud_p_bot) ? 1 : 0;
+  auto T_int_face = [&](int i) -> double {
+    if (N == 1 || i == 0) return Tc[0];
+    if (i == N) return Tc[N - 1];
+    return 0.5 * (Tc[i - 1] + Tc[i]);
+  };
+  double Tl;
+  if (l < nlev) {
+    double pl, lnpl, dm;
+    if (!NONISO) {
+      pl = pc[l]; Tl = Tc[l]; lnpl = log(pl);
+      dm = (exp(lnp_int(l)) - exp(lnp_int(l + 1))) * P.inv_g;     // the layer between its two interfaces
+      g_dm[l] = dm;
+    } else if (l & 1) {
+      const int i = l >> 1;                                      // centre of layer i; above it: interface i + 1
+      pl = pc[i]; Tl = Tc[i]; lnpl = log(pl);
+      const double p_up = exp(lnp_int(i + 1));
+      dm = (pl - p_up) * P.inv_g;
+      g_dm[i] = (exp(lnp_int(i)) - p_up) * P.inv_g;
+    } else {
+      const int i = l >> 1;                                      // interface i; above it: centre of layer i
+      lnpl = lnp_int(i); pl = exp(lnpl); Tl = T_int_face(i);
+      dm = (l < nlev - 1) ? (pl - pc[i]) * P.inv_g : 0.0;
+    }
+    LevelRec r;
+    r.dm = dm;
+    r.cloud = (pl >= P.cloud_p_top && pl <= P.cloud_p_bot) ? 1 : 0;
+    r.pad = (pl != pl || Tl != Tl) ? 1 : 0;                       // NaN in the column's p or T
     // table cell + weights: bilinear in (log10 p, T), clamped (R7).  Cell = the one with grid[i] < x <= grid[i+1]
     // (x at or below the first node: cell 0); found from a uniform-grid guess corrected by a walk.
-    double xp = log10(pl);
+    double xp = lnpl * 0.43429448190325182765;
     xp = fmin(fmax(xp, P.tab_lp[0]), P.tab_lp[P.nP - 1]);
     int ip = (int)((xp - P.tab_lp[0]) * P.inv_dlp);
     ip = ip < 0 ? 0 : (ip > P.nP - 2 ? P.nP - 2 : ip);
     while (ip > 0 && !(xp > P.tab_lp[ip])) --ip;
     while (ip < P.nP - 2 && xp > P.tab_lp[ip + 1]) ++ip;
     const double wp = (xp - P.tab_lp[ip]) / (P.tab_lp[ip + 1] - P.tab_lp[ip]);
-    const double xt = fmin(fmax(tl, P.tab_t[0]), P.tab_t[P.nT - 1]);
+    const double xt = fmin(fmax(Tl, P.tab_t[0]), P.tab_t[P.nT - 1]);
     int it = (int)((xt - P.tab_t[0]) * P.inv_dt);
     it = it < 0 ? 0 : (it > P.nT - 2 ? P.nT - 2 : it);
     while (it > 0 && !(xt > P.tab_t[it])) --it;
     while (it < P.nT - 2 && xt > P.tab_t[it + 1]) ++it;
     const double wt = (xt - P.tab_t[it]) / (P.tab_t[it + 1] - P.tab_t[it]);
-    rec.c00 = (1.0 - wp) * (1.0 - wt);
-    rec.c01 = (1.0 - wp) * wt;
-    rec.c10 = wp * (1.0 - wt);
-    rec.c11 = wp * wt;
-    rec.o00 = (unsigned)(ip * P.nT + it) * P.row_stride;
-    rec.o01 = rec.o00 + P.row_stride;
-    rec.o10 = rec.o00 + (unsigned)P.nT * P.row_stride;
-    rec.o11 = rec.o10 + P.row_stride;
-    rec.pad = 0;
-    // column mass below this level down to the next level: full layer (isothermal: level = layer centre,
-    // mass between its two interfaces) or sub-layer (non-isothermal: levels alternate interface / centre)
-    if (NONISO) rec.dm = (l < nlev - 1) ? (pl - p_level(l + 1)) * P.inv_g : 0.0;
-    else rec.dm = (s_pint[l] - s_pint[l + 1]) * P.inv_g;
-    s_rec[1 + l] = rec;
-    if (l == 0) s_rec[0] = rec;
+    r.c00 = (1.0 - wp) * (1.0 - wt);
+    r.c01 = (1.0 - wp) * wt;
+    r.c10 = wp * (1.0 - wt);
+    r.c11 = wp * wt;
+    r.o00 = (unsigned)(ip * P.nT + it) * P.row_stride;
+    r.o01 = r.o00 + P.row_stride;
+    r.o10 = r.o00 + (unsigned)P.nT * P.row_stride;
+    r.o11 = r.o10 + P.row_stride;
+    g_rec[1 + l] = r;
+    if (l == 0) g_rec[0] = r;
+  } else {
+    Tl = P.T_int;
+    const double mu = P.mu[col];
+    g_dm[N] = mu;                                                 // mu rides along with the records
   }
-  for (int j = tid; j < N; j += nthr) s_dm[j] = (s_pint[j] - s_pint[j + 1]) * P.inv_g;
-  __syncthreads();
 
   // ---------------- S2 ----------------
-  const int nedge = nbt + 1, nlevp = nlev + 1;
-  for (int idx = tid; idx < nedge * nlevp; idx += nthr) {
-    const int e = idx / nlevp, l = idx - e * nlevp;
-    const double Tl = s_tlev[l];
-    double low = 0.0, G = 0.0;
-    if (Tl > 0.0) G = planck_G(kPlanckC2 / (P.edges[b_first + e] * Tl), P.gtab, &low);
-    s_G[idx] = G;
-    s_Glow[idx] = low;
+  double *Brow = (double *)(P.ws_B + (size_t)col * P.tiles * L.b_bytes) + (size_t)l * L.nbt;
+  const bool hot = Tl > 0.0;
+  const double invT = hot ? 1.0 / Tl : 0.0;
+  const double T2 = Tl * Tl;
+  const double scale = hot ? ((l == nlev) ? kPlanckC1 * kPi : kPlanckC1) * T2 * T2 : 0.0;   // row nlev: F_BOA = pi B(T_int), L239
+  double low_p = 0.0, G_p = planck_G(__ldg(P.c2lam) * invT, P.gtab, T32, &low_p);
+#pragma unroll 4
+  for (int e = 0; e < P.nb; ++e) {
+    double low_a;
+    const double G_a = planck_G(__ldg(P.c2lam + e + 1) * invT, P.gtab, T32, &low_a);
+    const int4 raw = __ldg(reinterpret_cast<const int4 *>(P.bslot + e));
+    const double inv_dlam = __hiloint2double(raw.w, raw.z);
+    const double B = scale * planck_dG(G_p, low_p, G_a, low_a) * inv_dlam;
+    Brow[raw.x] = B;
+    if (raw.y >= 0) Brow[raw.y] = B;
+    else if (raw.y == -2)
+      for (int k = __ldg(P.slot_ptr + e) + 1; k < __ldg(P.slot_ptr + e + 1); ++k) Brow[__ldg(P.slots + k)] = B;
+    G_p = G_a; low_p = low_a;
   }
-  __syncthreads();
-  for (int idx = tid; idx < nbt * nlevp; idx += nthr) {
-    const int k = idx / nlevp, l = idx - k * nlevp;
-    const double Tl = s_tlev[l];
-    const double T2 = Tl * Tl;
-    const int g0i = k * nlevp + l, g1i = g0i + nlevp;
-    double B = kPlanckC1 * T2 * T2 * planck_dG(s_G[g0i], s_Glow[g0i], s_G[g1i], s_Glow[g1i]) * P.bins[b_first + k].inv_dlam;
-    if (l == nlev) B *= kPi;   // F_BOA = pi B(T_int), L239
-    s_B[l * L.nbt + k] = (Tl > 0.0) ? B : 0.0;
+}
+
+// phase A over the whole grid: item = (column, level) in column-major order
+template <bool NONISO>
+__device__ __forceinline__ void phase_a(const KParams &P, const Lay &L, const double *__restrict__ T32, long gtid, long gthreads,
+                                        bool count) {
+  const int nlevp = P.nlev + 1;
+  const long nitems = (long)P.ncol * nlevp;
+  for (long item = gtid; item < nitems; item += gthreads) {
+    const int col = (int)(item / nlevp), l = (int)(item - (long)col * nlevp);
+    prep_item<NONISO>(P, L, T32, col, l);
+    if (count) {
+      // count the warp's items of each column with one fence + one atomic (the warp barrier + the leader's fence
+      // order every lane's stores before the count)
+      const unsigned act = __activemask();
+      const unsigned same = __match_any_sync(act, col);
+      __syncwarp(act);
+      if ((threadIdx.x & 31) == __ffs(same) - 1) {
+        __threadfence();
+        atomicAdd(P.flags + col, (unsigned)__popc(same));
+      }
+    }
   }
-  __syncthreads();
 }
 
 // cross-warp sum of the per-warp interface sums (s_red: [warp][4][LP] = F_up, diffuse F_dn part 1, part 2 (+ beam),
 // beam), tile partials in fixed order, and the column's outputs written by its last tile.  A tile publishes its
 // partial sums with a release atomic (no L1 invalidation); only the column's last tile takes the acquire fence.
-__device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, unsigned char *smem, int *s_is_last_p,
-                                                int nwa, bool want_beam, int col, int tile, int col_nan) {
+__device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, unsigned char *smem, const double *s_dm,
+                                                int *s_is_last_p, int nwa, bool want_beam, int col, int tile, int col_nan) {
   const int N = P.N, LP = L.LP, tid = threadIdx.x, nthr = blockDim.x;
   double *s_red = (double *)(smem + L.off_red), *s_fin = (double *)(smem + L.off_fin);
-  const double *s_dm = (const double *)(smem + L.off_dm);
   int &s_is_last = *s_is_last_p;
   const int nq = want_beam ? 4 : 3;
   const int nred = nq * (N + 1);
-  for (int k = tid; k < nred; k += nthr) {
-    const int q = k / (N + 1), lev = k - q * (N + 1);
-    double sum = 0.0;
-    for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
-    s_fin[k] = sum;
-  }
-  __syncthreads();
-
   if (P.tiles > 1) {
+    // cross-warp sum in fixed order, published straight to this tile's partial-sum slot
     double *part = P.partial + ((size_t)col * P.tiles + tile) * 4 * (N + 1);
-    for (int k = tid; k < nred; k += nthr) __stcg(part + k, s_fin[k]);
+    for (int k = tid; k < nred; k += nthr) {
+      const int q = k / (N + 1), lev = k - q * (N + 1);
+      double sum = 0.0;
+      for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
+      __stcg(part + k, sum);
+    }
     __syncthreads();
     if (tid == 0) {
       unsigned prev;
@@ -609,10 +724,19 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, 
     }
     __syncthreads();
     if (!s_is_last) return;
+    // the column's last tile sums the partial sums in tile order
     const double *pall = P.partial + (size_t)col * P.tiles * 4 * (N + 1);
     for (int k = tid; k < nred; k += nthr) {
       double sum = 0.0;
       for (int t = 0; t < P.tiles; ++t) sum += __ldcg(pall + (size_t)t * 4 * (N + 1) + k);
+      s_fin[k] = sum;
+    }
+    __syncthreads();
+  } else {
+    for (int k = tid; k < nred; k += nthr) {
+      const int q = k / (N + 1), lev = k - q * (N + 1);
+      double sum = 0.0;
+      for (int w = 0; w < nwa; ++w) sum += s_red[(size_t)w * 4 * LP + q * LP + lev];
       s_fin[k] = sum;
     }
     __syncthreads();
@@ -647,21 +771,22 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, 
 //   ROWS    0: k-table rows by register-prefetched loads; 1: by bulk async copies (TMA) into the per-warp ring
 //   STK     back-substitution coefficients: 1 = per-block slab of the global workspace (L2), 0 = thread-private
 //           local memory (kept for comparison builds; SCAP = its capacity in interfaces)
+//   BDIRECT one Gauss point per bin (opacity sampling, L385): every thread has its own bin, so the Planck values are
+//           read coalesced from the workspace instead of being staged (64 KB per block otherwise); PPT = 1
 //   MAXT, MINB  launch bounds (register cap = 65536 / (MAXT MINB)); any block of <= MAXT threads may be launched
 // --------------------------------------------------------------------------------------------
-template <bool NONISO, bool TOA, int PPT, int ROWS, int STK, int SCAP, int MAXT, int MINB>
+template <bool NONISO, bool TOA, int PPT, int ROWS, int STK, int SCAP, bool BDIRECT, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   static_assert(PPT == 1 || PPT == 2 || PPT == 4, "points per thread");
+  static_assert(!BDIRECT || PPT == 1, "one Gauss point per bin: one point per thread");
   constexpr int DEPTH = NONISO ? 2 : 1;
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ double s_T32[32];
-  __shared__ int s_is_last, s_nan, s_col;
+  __shared__ int s_is_last, s_col[2];
   const int N = P.N, nlev = P.nlev;
   const int tid = threadIdx.x, nthr = blockDim.x, nwarps = nthr >> 5;
   const int warp = tid >> 5, lane = tid & 31;
-  const Lay L = make_lay(N, nlev, nwarps, PPT, P.ng, P.nb, TOA, DEPTH, ROWS == 1);
-  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;   // s_lev[-1] duplicates level 0
-  const double *s_B = (const double *)(smem + L.off_B);
+  const Lay L = make_lay(N, nlev, nwarps, PPT, P.ng, P.nb, TOA, DEPTH, ROWS, BDIRECT);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
   double *s_red = (double *)(smem + L.off_red);
   double *s_vals = (double *)(smem + L.off_vals);
@@ -685,13 +810,11 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   const bool warp_on = warp < nwa;          // a warp without any spectral point only joins the barriers
   const bool want_beam = !TOA && (P.F_beam != nullptr);
   double W[PPT];                            // dlam_b * w_g
-  const double dlam = P.bins[b].dlam, inv_dlam = P.bins[b].inv_dlam, fstar_b = P.fstar[b];
+  const double fstar_b = P.fstar[b];
+  {
+    const double dlam = P.bins[b].dlam;
 #pragma unroll
-  for (int q = 0; q < PPT; ++q) W[q] = active ? dlam * P.gauss_w[gidx + q] : 0.0;
-  double gw[PPT];
-  if (TOA) {
-#pragma unroll
-    for (int q = 0; q < PPT; ++q) gw[q] = active ? P.gauss_w[gidx + q] : 0.0;
+    for (int q = 0; q < PPT; ++q) W[q] = active ? dlam * P.gauss_w[gidx + q] : 0.0;
   }
 
   if (tid < 32) s_T32[tid] = kExp2Tab[tid];
@@ -699,22 +822,42 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
     const int cl = i / nbt, k = i - cl * nbt;
     const BinConst bc = P.bins[b_first + k];
     BinOpt bo;
-    bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2); bo.pad[0] = bo.pad[1] = 0.0;
+    bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2);
+    bo.pad[0] = bo.pad[1] = 0.0;
     s_bin[cl * nbtS + k] = bo;
   }
-  if (ROWS == 1) {
-    if (tid < RING * nwarps) mbar_init(smem_u32(smem + L.off_bar) + 8 * tid, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
+  if (tid < RING * nwarps + 2) mbar_init(smem_u32(smem + L.off_bar) + 8 * tid, 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  const uint32_t rec_bar = smem_u32(smem + L.off_bar) + 8 * RING * nwarps;   // two barriers: one per record buffer
   const BinOpt *bin0 = s_bin + bl, *bin1 = s_bin + nbtS + bl;
   const double *T32 = s_T32;
   double *red_w = s_red + (size_t)warp * 4 * LP;
   double *stage_w = (double *)(smem + L.off_u + L.u_stage) + (size_t)warp * 8 * STAGE_LD;
   double *stage_wr = stage_w + lane;
-  const double *Bbase = s_B + bl;
+
+  // ---------------- phase A: this block's share of the (column, level) items of S1 + S2 ----------------
+#ifdef HRT_DIAG_SKIP_PHASE_A   /* timing-only diagnostic build (_work/): phase A on the handle's first launch only */
+  if (P.fused_prep == 1) {
+#else
+  if (P.fused_prep) {
+#endif
+    __syncthreads();                       // s_T32
+    const long nblk = (long)gridDim.x * gridDim.y;
+    phase_a<NONISO>(P, L, s_T32, ((long)blockIdx.y * gridDim.x + blockIdx.x) * nthr + tid, nblk * nthr, true);
+    __syncthreads();
+    if (tid == 0) {
+      unsigned prev;
+      asm volatile("atom.add.release.gpu.global.u32 %0, [%1], 1;" : "=r"(prev) : "l"(P.queue + P.tiles + 1) : "memory");
+    }
+  }
 
   Feed<PPT, DEPTH, ROWS> feed;
   if constexpr (ROWS == 0) {
+    feed.lnk_pt = P.lnk + pt;
+  } else if constexpr (ROWS == 2) {
+    unsigned char *slot = smem + L.off_u + L.u_ring + (size_t)warp * L.ring_warp + (size_t)lane * PPT * 8;
+    feed.slot = (const double *)slot;
+    feed.slot_s = smem_u32(slot);
     feed.lnk_pt = P.lnk + pt;
   } else {
     unsigned char *ring = smem + L.off_u + L.u_ring + (size_t)warp * L.ring_warp;
@@ -725,7 +868,6 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
     feed.kc = 0;
     feed.lane = lane;
   }
-  feed.lv0 = s_lev;
 
   // this block's slab of the back-substitution workspace: [interface][warp][96 PPT]
   const size_t istride = (size_t)nwarps * 96 * PPT;
@@ -733,19 +875,67 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   if (STK == 1 && !TOA)
     stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * 96 * PPT;
 
-  // ---------------- columns of this tile's queue ----------------
-  for (;;) {
-    __syncthreads();                       // the previous column's shared-memory state is dead
-    if (tid == 0) s_col = (int)atomicAdd(P.queue + tile, 1u);
-    __syncthreads();
-    const int col = s_col;
+  // ---------------- phase B: columns of this tile's queue ----------------
+  // The record block and the tile's Planck block of the NEXT column are fetched by bulk async copies (TMA) into the
+  // other shared-memory buffer while this column is swept; thread 0 first waits for the column's publication flag.
+  bool all_published = false;               // thread 0: every block has finished phase A -- no more flag polls
+#ifdef HRT_DIAG_SKIP_PHASE_A
+  if (P.fused_prep == 2) all_published = true;
+#endif
+  auto fetch_column = [&](int c, int buf) {   // thread 0
+    // (the whole grid is resident -- cooperative launch -- and phase A waits for nothing, so this terminates; the
+    // poll count is bounded all the same: a wedged GPU is worse than a wrong column)
+    if (!all_published) {
+      unsigned n;
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(n) : "l"(P.queue + P.tiles + 1) : "memory");
+      all_published = (n == gridDim.x * gridDim.y);
+      if (!all_published) {
+        unsigned f, polls = 0;
+        do {
+          asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(P.flags + c) : "memory");
+        } while (f != (unsigned)(nlev + 1) && ++polls < (1u << 26));
+      }
+      asm volatile("fence.proxy.async.global;" ::: "memory");
+    }
+    const uint32_t bar = rec_bar + 8 * buf;
+    mbar_expect_tx(bar, L.rec_bytes + (BDIRECT ? 0u : L.b_bytes));
+    bulk_g2s(smem_u32(smem + L.off_rec[buf]), P.ws_rec + (size_t)c * L.rec_bytes, L.rec_bytes, bar);
+    if (!BDIRECT)
+      bulk_g2s(smem_u32(smem + L.off_Bt[buf]), P.ws_B + ((size_t)c * P.tiles + tile) * L.b_bytes, L.b_bytes, bar);
+  };
+  __syncthreads();                         // tile constants and barriers are set up; phase A scratch is dead
+  int pend = 0;                            // thread 0: the queue entry after the next one, fetched one column early
+  if (tid == 0) {
+    const int c = (int)atomicAdd(P.queue + tile, 1u);
+    pend = (int)atomicAdd(P.queue + tile, 1u);
+    s_col[0] = c;
+    if (c < P.ncol) fetch_column(c, 0);
+  }
+  __syncthreads();
+  for (unsigned it = 0;; ++it) {
+    const int buf = it & 1;
+    const int col = s_col[buf];
     if (col >= P.ncol) break;
-
-    column_prep<NONISO>(P, L, smem, col, b_first, nbt, &s_nan);
-    const int col_nan = s_nan;
+    if (tid == 0) {
+      const int c = pend;
+      pend = (int)atomicAdd(P.queue + tile, 1u);   // consumed at the top of the next column: its latency is hidden
+      s_col[buf ^ 1] = c;
+      if (c < P.ncol) fetch_column(c, buf ^ 1);    // the other buffer is free since the barrier that ended the last column
+    }
+    mbar_wait(rec_bar + 8 * buf, (it >> 1) & 1u);
+    const LevelRec *s_lev = (const LevelRec *)(smem + L.off_rec[buf]) + 1;   // s_lev[-1] duplicates level 0
+    const double *s_dm = (const double *)(smem + L.off_rec[buf] + sizeof(LevelRec) * (nlev + 1));
+    // NaN in p, T or mu of this column poisons the column's outputs (and only them): the clamps and selects of the
+    // sweeps would otherwise swallow it (R19).  Level flags from phase A; reduced at the barrier after the sweeps.
+    int my_nan = 0;
+    for (int l = tid; l < nlev; l += nthr) my_nan |= s_lev[l].pad;
+    // B of level l: Bbase[l * Bstride] (the staged block, or the workspace block when every thread has its own bin)
+    const double *Bbase = BDIRECT ? (const double *)(P.ws_B + ((size_t)col * P.tiles + tile) * L.b_bytes) + bl
+                                  : (const double *)(smem + L.off_Bt[buf]) + bl;
+    feed.lv0 = s_lev;
 
     if (warp_on) {
-      const double mu = P.mu[col];
+      const double mu = s_dm[N];
       const bool day = mu > 0.0;
       const double muF = day ? mu * fstar_b : 0.0;            // mu * F_star[b]
       const double inv_mu = day ? 1.0 / mu : 0.0;
@@ -797,7 +987,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
           const LevelRec *lv = s_lev + (N - 1);
           const double *Bp = Bbase + (size_t)(N - 1) * nbtS;
           feed.prime(lv, N);
-#pragma unroll 1
+          HRT_UNROLL(HRT_UNROLL_ISO)
           for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
             RowsT<PPT> cur[1];
             feed.next(cur, lv - 1);
@@ -921,7 +1111,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
       if (TOA) {
         // S7 (spectrum shape): F_up_toa_bin[b] = sum_g w_g F_up[N]
 #pragma unroll
-        for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = gw[q] * fma(Ct[q], Fup0[q], Dt[q]);
+        for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? P.gauss_w[gidx + q] * fma(Ct[q], Fup0[q], Dt[q]) : 0.0;
       } else {
         push_stage(0);
         {
@@ -934,42 +1124,87 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         double wF[PPT];
 #pragma unroll
         for (int q = 0; q < PPT; ++q) wF[q] = 0.0;
+        // The coefficients come back from L2 (several hundred cycles).  Comparison builds (HRT_S2_PF=1) load a group
+        // of 4 interfaces while the previous group is used (two register buffers); it costs registers in sweep 1 and
+        // loses, so 8 interfaces are loaded at a time.
+        constexpr int G = 4;
+#ifndef HRT_S2_PF
+#define HRT_S2_PF 0   /* measured (config 2, same box): 0.739 ms without, 0.784 ms with the two-buffer prefetch */
+#endif
+        constexpr bool PF = (PPT <= 2) && (HRT_S2_PF != 0);
+        double gc[PF ? 2 : 1][PF ? G : 8][PPT], gwd[PF ? 2 : 1][PF ? G : 8][PPT], gR[PF ? 2 : 1][PF ? G : 8][PPT];
+        auto load_one = [&](int bsel, int k, int i) {
+          if (i <= N) {
+            if (STK == 1) {
+              stk_load<PPT>(stk_w + (size_t)i * istride, lane, gc[bsel][k], gwd[bsel][k], gR[bsel][k]);
+            } else {
+#pragma unroll
+              for (int q = 0; q < PPT; ++q) {
+                const double2 a = l_cd[STK == 0 ? i : 0][q];
+                gc[bsel][k][q] = a.x; gwd[bsel][k][q] = a.y; gR[bsel][k][q] = l_R[STK == 0 ? i : 0][q];
+              }
+            }
+          } else {
+            // beyond the top: repeat F_up[N] into rows of the reduction buffer that are never read
+#pragma unroll
+            for (int q = 0; q < PPT; ++q) { gc[bsel][k][q] = 1.0; gwd[bsel][k][q] = 0.0; gR[bsel][k][q] = 0.0; }
+          }
+        };
+#ifdef HRT_S2_BUTTERFLY
+        double v16[16];     // sums over the thread's points of W F_up (rows 0..7) and of W R F_up (rows 8..15)
+#else
+        double sd[8];
+#endif
+        auto use_one = [&](int bsel, int k, int row) {
+          double su = 0.0, s2 = 0.0;
+#pragma unroll
+          for (int q = 0; q < PPT; ++q) {
+            wF[q] = fma(gc[bsel][k][q], wF[q], gwd[bsel][k][q]);
+            su += wF[q];
+            s2 = fma(gR[bsel][k][q], wF[q], s2);
+          }
+#ifdef HRT_S2_BUTTERFLY
+          v16[row] = su;
+          v16[8 + row] = s2;
+#else
+          stage_wr[row * STAGE_LD] = su;
+          sd[row] = s2;
+#endif
+        };
+        if (PF) {
+#pragma unroll
+          for (int k = 0; k < G; ++k) load_one(0, k, k);
+        }
 #pragma unroll 1
         for (int base = 0; base <= N; base += 8) {
-          double sd[8];
+          if (PF) {
 #pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            const int i = base + k;
-            double c[PPT], wd[PPT], Ri[PPT];
-            if (i <= N) {
-              if (STK == 1) {
-                stk_load<PPT>(stk_w + (size_t)i * istride, lane, c, wd, Ri);
-              } else {
+            for (int k = 0; k < G; ++k) load_one(1, k, base + G + k);
 #pragma unroll
-                for (int q = 0; q < PPT; ++q) {
-                  const double2 a = l_cd[STK == 0 ? i : 0][q];
-                  c[q] = a.x; wd[q] = a.y; Ri[q] = l_R[STK == 0 ? i : 0][q];
-                }
-              }
-            } else {
-              // beyond the top: repeat F_up[N] into rows of the reduction buffer that are never read
+            for (int k = 0; k < G; ++k) use_one(0, k, k);
 #pragma unroll
-              for (int q = 0; q < PPT; ++q) { c[q] = 1.0; wd[q] = 0.0; Ri[q] = 0.0; }
-            }
-            double su = 0.0, s2 = 0.0;
+            for (int k = 0; k < G; ++k) load_one(0, k, base + 2 * G + k);
 #pragma unroll
-            for (int q = 0; q < PPT; ++q) {
-              wF[q] = fma(c[q], wF[q], wd[q]);
-              su += wF[q];
-              s2 = fma(Ri[q], wF[q], s2);
-            }
-            stage_wr[k * STAGE_LD] = su;
-            sd[k] = s2;
+            for (int k = 0; k < G; ++k) use_one(1, k, G + k);
+          } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) load_one(0, k, base + k);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) use_one(0, k, k);
           }
+#ifdef HRT_S2_BUTTERFLY
+          {
+            // one recursive-halving butterfly for the 16 values of the 8 interfaces
+            const double tot = warp_reduce16(v16, lane);
+            const int idx = lane >> 1;
+            if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
+          }
+#else
           flush_stage(stage_w, red_w + base, lane);
 #pragma unroll
           for (int k = 0; k < 8; ++k) stage_wr[k * STAGE_LD] = sd[k];
           flush_stage(stage_w, red_w + LP + base, lane);
+#endif
           if (STK == 1) {
             // the coefficients of these interfaces are dead: drop their lines from L2 instead of writing them back
             int n_if = N + 1 - base;
@@ -983,14 +1218,14 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         }
         if (P.F_toa_bin != nullptr) {
 #pragma unroll
-          for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? wF[q] * inv_dlam : 0.0;
+          for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? wF[q] * P.bins[b].inv_dlam : 0.0;
         }
       }
     } else if (TOA || P.F_toa_bin != nullptr) {
 #pragma unroll
       for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = 0.0;
     }
-    __syncthreads();
+    const int col_nan = __syncthreads_or(my_nan | (s_dm[N] != s_dm[N]));
 
     if (TOA || P.F_toa_bin != nullptr) {
       for (int k = tid; k < nbt; k += nthr) {
@@ -1006,15 +1241,19 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         if (whole) *dst = sum; else atomicAdd(dst, sum);
       }
     }
-    if (!TOA) column_epilogue(P, L, smem, &s_is_last, nwa, want_beam, col, tile, col_nan);
+    if (!TOA) column_epilogue(P, L, smem, s_dm, &s_is_last, nwa, want_beam, col, tile, col_nan);
+    __syncthreads();                       // this column's shared-memory state, record buffer included, is dead
   }
 
-  // the last block of the grid to run out of work re-arms the queues for the next launch
+  // the last block of the grid to run out of work re-arms the queues and the publication counts for the next launch
   if (tid == 0) {
     const unsigned total = gridDim.x * gridDim.y;
-    if (atomicAdd(P.queue + P.tiles, 1u) == total - 1) {
-      for (int t = 0; t <= P.tiles; ++t) P.queue[t] = 0;
-    }
+    s_is_last = (atomicAdd(P.queue + P.tiles, 1u) == total - 1);
+  }
+  __syncthreads();
+  if (s_is_last) {
+    for (int c = tid; c < P.ncol; c += nthr) P.flags[c] = 0;
+    for (int t = tid; t <= P.tiles + 1; t += nthr) P.queue[t] = 0;
   }
 }
 
@@ -1030,13 +1269,13 @@ template <bool NONISO>
 __global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int n_iter) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ double s_T32[32];
-  __shared__ int s_is_last, s_nan;
+  __shared__ int s_is_last;
   constexpr int MAXS = NONISO ? 2 * MAXL : MAXL;   // system layers
   const int N = P.N, nlev = P.nlev;
   const int tid = threadIdx.x, nthr = blockDim.x, nwarps = nthr >> 5;
-  const Lay L = make_lay(N, nlev, nwarps, 1, P.ng, P.nb, false, NONISO ? 2 : 1, false);
-  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_lev) + 1;
-  const double *s_B = (const double *)(smem + L.off_B);
+  const Lay L = make_lay(N, nlev, nwarps, 1, P.ng, P.nb, false, NONISO ? 2 : 1, 0, false);
+  const LevelRec *s_lev = (const LevelRec *)(smem + L.off_rec[0]) + 1;
+  const double *s_B = (const double *)(smem + L.off_Bt[0]);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
   double *s_red = (double *)(smem + L.off_red);
 
@@ -1058,8 +1297,19 @@ __global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int
     bo.sb = bc.sb[cl]; bo.ss = bc.ss[cl]; bo.gt = g0_terms(bc.gg[cl], P.inv_eps2); bo.pad[0] = bo.pad[1] = 0.0;
     s_bin[cl * nbtS + k] = bo;
   }
-  column_prep<NONISO>(P, L, smem, col, b_first, nbt, &s_nan);
-  const int col_nan = s_nan;
+  // S1 / S2 blocks of the column from the workspace (written by rt_prep_kernel, the launch before this one)
+  {
+    const double *src = (const double *)(P.ws_rec + (size_t)col * L.rec_bytes);
+    double *dst = (double *)(smem + L.off_rec[0]);
+    for (int i = tid; i < (int)(L.rec_bytes / 8); i += nthr) dst[i] = src[i];
+    src = (const double *)(P.ws_B + ((size_t)col * P.tiles + tile) * L.b_bytes);
+    dst = (double *)(smem + L.off_Bt[0]);
+    for (int i = tid; i < (int)(L.b_bytes / 8); i += nthr) dst[i] = src[i];
+  }
+  __syncthreads();
+  const double *s_dm = (const double *)(smem + L.off_rec[0] + sizeof(LevelRec) * (nlev + 1));
+  int col_nan = (mu != mu) ? 1 : 0;
+  for (int l = 0; l < nlev; ++l) col_nan |= s_lev[l].pad;
 
   int pt = pt0 + tid;
   const bool active = pt < P.npt;
@@ -1159,7 +1409,19 @@ __global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int
     }
   }
   __syncthreads();
-  column_epilogue(P, L, smem, &s_is_last, nwa, P.F_beam != nullptr, col, tile, col_nan);
+  column_epilogue(P, L, smem, s_dm, &s_is_last, nwa, P.F_beam != nullptr, col, tile, col_nan);
+}
+
+// phase A as a launch of its own: for the comparison path (rt_iter_kernel; tp = spectral points per tile of that kernel,
+// count = 0) and for rt_step_kernel when the device cannot host its grid at once (count = 1)
+template <bool NONISO>
+__global__ void __launch_bounds__(128) rt_prep_kernel(const KParams P, const int tp, const int count) {
+  __shared__ double s_T32[32];
+  // only the block sizes of the layout are used here
+  const Lay L = make_lay(P.N, P.nlev, tp / 32, 1, P.ng, P.nb, true, NONISO ? 2 : 1, 0, true);
+  if (threadIdx.x < 32) s_T32[threadIdx.x] = kExp2Tab[threadIdx.x];
+  __syncthreads();
+  phase_a<NONISO>(P, L, s_T32, (long)blockIdx.x * blockDim.x + threadIdx.x, (long)gridDim.x * blockDim.x, count != 0);
 }
 
 __global__ void zero_kernel(double *p, size_t n) {
@@ -1173,14 +1435,17 @@ __global__ void zero_kernel(double *p, size_t n) {
 typedef void (*kernel_fn)(const KParams);
 
 struct Variant {
-  bool noniso, toa;
+  bool noniso, toa, bdirect;
   int ppt, rows, stk, scap;   // scap: capacity (interfaces) of the local-memory stack of the STK = 0 comparison builds
   int maxt, minb;      // launch bounds: register cap = 65536 / (maxt * minb)
   kernel_fn fn;
 };
 
 #define HRT_K(NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB) \
-  {NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB>}
+  {NI, TOA, false, PPT, ROWS, STK, SCAP, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, STK, SCAP, false, MAXT, MINB>}
+// one Gauss point per bin (opacity sampling): Planck values read from the workspace; one point per thread
+#define HRT_KB(NI, TOA, ROWS, MAXT, MINB) \
+  {NI, TOA, true, 1, ROWS, 1, 1, MAXT, MINB, rt_step_kernel<NI, TOA, 1, ROWS, 1, 1, true, MAXT, MINB>}
 
 // Compiled instantiations, in order of preference for each (noniso, toa, ppt).  helios_rt_create takes the first
 // match; helios_rt_debug_set_launch (tests, tuning) may select any other.
@@ -1226,12 +1491,18 @@ struct helios_rt {
   unsigned row_stride;
   double inv_dlp, inv_dt;
   // device tables
-  double *d_lnk, *d_tab_lp, *d_tab_t, *d_edges, *d_gw, *d_gtab;
+  double *d_lnk, *d_tab_lp, *d_tab_t, *d_edges, *d_gw, *d_gtab, *d_c2lam;
   BinConst *d_bins;
   // workspace
   double *d_stack, *d_partial;
-  size_t stack_block, stack_bytes, partial_bytes;
-  unsigned *d_counter, *d_queue;
+  unsigned char *d_ws_rec, *d_ws_B;
+  size_t stack_block, stack_bytes, partial_bytes, ws_bytes;
+  unsigned *d_counter, *d_queue, *d_flags;
+  BinSlot *d_bslot, *d_bslot_iter;
+  int *d_slot_ptr, *d_slots, *d_slot_ptr_iter, *d_slots_iter;   // bin -> Planck-block slots (step tiling / comparison tiling)
+  unsigned epoch;
+  Lay iter_lay;
+  double *inv_dlam;          // host copy, [n_bins]
   // device + pinned host staging for step_host
   double *d_in, *d_out, *h_in, *h_out;
   cudaStream_t own_stream, copy_stream;
@@ -1319,8 +1590,12 @@ static cudaError_t upload(T **dst, const T *src, size_t n) {
 extern "C" int helios_rt_destroy(helios_rt *h) {
   if (!h) return HELIOS_RT_OK;
   cudaFree(h->d_lnk); cudaFree(h->d_tab_lp); cudaFree(h->d_tab_t); cudaFree(h->d_edges); cudaFree(h->d_gw);
-  cudaFree(h->d_gtab); cudaFree(h->d_bins); cudaFree(h->d_partial); cudaFree(h->d_counter); cudaFree(h->d_queue);
+  cudaFree(h->d_gtab); cudaFree(h->d_c2lam); cudaFree(h->d_bins); cudaFree(h->d_partial); cudaFree(h->d_counter); cudaFree(h->d_queue);
   cudaFree(h->d_stack); cudaFree(h->d_in); cudaFree(h->d_out);
+  cudaFree(h->d_ws_rec); cudaFree(h->d_ws_B); cudaFree(h->d_flags);
+  cudaFree(h->d_slot_ptr); cudaFree(h->d_slots); cudaFree(h->d_slot_ptr_iter); cudaFree(h->d_slots_iter);
+  cudaFree(h->d_bslot); cudaFree(h->d_bslot_iter);
+  free(h->inv_dlam);
   if (h->h_in) cudaFreeHost(h->h_in);
   if (h->h_out) cudaFreeHost(h->h_out);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
@@ -1330,6 +1605,40 @@ extern "C" int helios_rt_destroy(helios_rt *h) {
     if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
   }
   delete h;
+  return HELIOS_RT_OK;
+}
+
+// bin -> slots of the per-(column, tile) Planck blocks: bin b is stored once in the block of every tile that owns
+// points of it, at row offset (b - first bin of the tile)
+static int build_slots(helios_rt *h, int tp, const Lay &lay, const double *inv_dlam, int **d_ptr, int **d_slots,
+                       BinSlot **d_bslot) {
+  const int nb = h->cfg.n_bins, ng = h->cfg.n_gauss;
+  int *ptr = (int *)malloc(sizeof(int) * (nb + 1));
+  int total = 0;
+  if (!ptr) return HELIOS_RT_ENOMEM;
+  for (int b = 0; b < nb; ++b) { ptr[b] = total; total += ((b + 1) * ng - 1) / tp - (b * ng) / tp + 1; }
+  ptr[nb] = total;
+  int *sl = (int *)malloc(sizeof(int) * (total > 0 ? total : 1));
+  if (!sl) { free(ptr); return HELIOS_RT_ENOMEM; }
+  for (int b = 0, k = 0; b < nb; ++b)
+    for (int t = (b * ng) / tp; t <= ((b + 1) * ng - 1) / tp; ++t) sl[k++] = t * (int)(lay.b_bytes / 8) + (b - (t * tp) / ng);
+  BinSlot *bs = (BinSlot *)malloc(sizeof(BinSlot) * nb);
+  if (!bs) { free(ptr); free(sl); return HELIOS_RT_ENOMEM; }
+  for (int b = 0; b < nb; ++b) {
+    const int n = ptr[b + 1] - ptr[b];
+    bs[b].s0 = sl[ptr[b]];
+    bs[b].s1 = n == 1 ? -1 : (n == 2 ? sl[ptr[b] + 1] : -2);
+    bs[b].inv_dlam = inv_dlam[b];
+  }
+  cudaError_t e = cudaMalloc((void **)d_ptr, sizeof(int) * (nb + 1));
+  if (e == cudaSuccess) e = cudaMemcpy(*d_ptr, ptr, sizeof(int) * (nb + 1), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMalloc((void **)d_bslot, sizeof(BinSlot) * nb);
+  if (e == cudaSuccess) e = cudaMemcpy(*d_bslot, bs, sizeof(BinSlot) * nb, cudaMemcpyHostToDevice);
+  free(bs);
+  if (e == cudaSuccess) e = cudaMalloc((void **)d_slots, sizeof(int) * (total > 0 ? total : 1));
+  if (e == cudaSuccess) e = cudaMemcpy(*d_slots, sl, sizeof(int) * (total > 0 ? total : 1), cudaMemcpyHostToDevice);
+  free(ptr); free(sl);
+  if (e != cudaSuccess) { h->last_err = e; return e == cudaErrorMemoryAllocation ? HELIOS_RT_ENOMEM : HELIOS_RT_ECUDA; }
   return HELIOS_RT_OK;
 }
 
@@ -1344,7 +1653,8 @@ static int configure_launch(helios_rt *h) {
   if (!h->toa && v.stk == 0 && N + 1 > v.scap) return HELIOS_RT_EINVAL;
   const int tp = h->warps * 32 * h->ppt;
   h->tiles = (h->npt + tp - 1) / tp;
-  h->lay = make_lay(N, h->nlev, h->warps, h->ppt, c.n_gauss, c.n_bins, h->toa, h->noniso ? 2 : 1, v.rows == 1);
+  h->lay = make_lay(N, h->nlev, h->warps, h->ppt, c.n_gauss, c.n_bins, h->toa, h->noniso ? 2 : 1, v.rows, v.bdirect);
+  h->iter_lay = make_lay(N, h->nlev, h->iter_warps, 1, c.n_gauss, c.n_bins, false, h->noniso ? 2 : 1, 0, false);
   if (h->lay.total > 227u * 1024u) return HELIOS_RT_EINVAL;
   CK(h, cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->lay.total));
   cudaFuncAttributes fa;
@@ -1363,21 +1673,44 @@ static int configure_launch(helios_rt *h) {
   cudaFree(h->d_stack); h->d_stack = nullptr;
   cudaFree(h->d_partial); h->d_partial = nullptr;
   cudaFree(h->d_queue); h->d_queue = nullptr;
+  cudaFree(h->d_ws_rec); h->d_ws_rec = nullptr;
+  cudaFree(h->d_ws_B); h->d_ws_B = nullptr;
+  {
+    // S1/S2 blocks of every column: sized for the step kernel's tiling and for the comparison kernel's
+    size_t bB = (size_t)h->tiles * h->lay.b_bytes;
+    if (!h->toa && (size_t)h->iter_tiles * h->iter_lay.b_bytes > bB) bB = (size_t)h->iter_tiles * h->iter_lay.b_bytes;
+    const size_t bR = h->lay.rec_bytes;   // the same for both (depends on N and nlev only)
+    h->ws_bytes = (size_t)c.max_columns * (bB + bR);
+    CK(h, cudaMalloc((void **)&h->d_ws_rec, (size_t)c.max_columns * bR));
+    CK(h, cudaMalloc((void **)&h->d_ws_B, (size_t)c.max_columns * bB));
+  }
+  cudaFree(h->d_slot_ptr); h->d_slot_ptr = nullptr;
+  cudaFree(h->d_slots); h->d_slots = nullptr;
+  cudaFree(h->d_slot_ptr_iter); h->d_slot_ptr_iter = nullptr;
+  cudaFree(h->d_slots_iter); h->d_slots_iter = nullptr;
+  cudaFree(h->d_bslot); h->d_bslot = nullptr;
+  cudaFree(h->d_bslot_iter); h->d_bslot_iter = nullptr;
+  {
+    int rc = build_slots(h, tp, h->lay, h->inv_dlam, &h->d_slot_ptr, &h->d_slots, &h->d_bslot);
+    if (rc == HELIOS_RT_OK && !h->toa)
+      rc = build_slots(h, h->iter_warps * 32, h->iter_lay, h->inv_dlam, &h->d_slot_ptr_iter, &h->d_slots_iter, &h->d_bslot_iter);
+    if (rc) return rc;
+  }
   h->stack_block = (size_t)(N + 1) * h->warps * 96 * h->ppt;
   h->stack_bytes = (!h->toa && v.stk == 1) ? sizeof(double) * h->stack_block * h->tiles * h->workers : 0;
   if (h->stack_bytes) CK(h, cudaMalloc((void **)&h->d_stack, h->stack_bytes));
   const int mt = h->tiles > h->iter_tiles ? h->tiles : h->iter_tiles;
   h->partial_bytes = sizeof(double) * (size_t)c.max_columns * mt * 4 * (N + 1);
   CK(h, cudaMalloc((void **)&h->d_partial, h->partial_bytes));
-  CK(h, cudaMalloc((void **)&h->d_queue, sizeof(unsigned) * (h->tiles + 1)));
-  CK(h, cudaMemset(h->d_queue, 0, sizeof(unsigned) * (h->tiles + 1)));
+  CK(h, cudaMalloc((void **)&h->d_queue, sizeof(unsigned) * (h->tiles + 2)));
+  CK(h, cudaMemset(h->d_queue, 0, sizeof(unsigned) * (h->tiles + 2)));
   return HELIOS_RT_OK;
 }
 
-static int find_variant(bool noniso, bool toa, int ppt, int rows, int stk, int maxt, int minb) {
+static int find_variant(bool noniso, bool toa, bool bdirect, int ppt, int rows, int stk, int maxt, int minb) {
   for (int i = 0; i < kNumVariants; ++i) {
     const Variant &v = kVariants[i];
-    if (v.noniso != noniso || v.toa != toa || v.ppt != ppt) continue;
+    if (v.noniso != noniso || v.toa != toa || v.bdirect != bdirect || v.ppt != ppt) continue;
     if (rows >= 0 && v.rows != rows) continue;
     if (stk >= 0 && !toa && v.stk != stk) continue;
     if (maxt >= 0 && v.maxt != maxt) continue;
@@ -1408,8 +1741,8 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->iter_warps = default_warps(h->npt, 1, false);
   h->iter_tiles = (h->npt + h->iter_warps * 32 - 1) / (h->iter_warps * 32);
   int ppt = default_ppt(h->npt, ng, h->noniso, h->toa);
-  h->variant = find_variant(h->noniso, h->toa, ppt, -1, -1, -1, -1);
-  if (h->variant < 0) { ppt = 1; h->variant = find_variant(h->noniso, h->toa, 1, -1, -1, -1, -1); }
+  h->variant = find_variant(h->noniso, h->toa, ng == 1, ppt, -1, -1, -1, -1);
+  if (h->variant < 0) { ppt = 1; h->variant = find_variant(h->noniso, h->toa, ng == 1, 1, -1, -1, -1, -1); }
   h->warps = default_warps(h->npt, ppt, h->noniso);
   int dev = 0;
   cudaGetDevice(&dev);
@@ -1442,6 +1775,9 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     bc.gg[0] = 0.0;           bc.gg[1] = (sg + sc > 0.0) ? sc * cfg->cloud_g0[b] / (sg + sc) : 0.0;
   }
   build_planck_table(gtab);
+  h->inv_dlam = (double *)malloc(sizeof(double) * nb);
+  if (!h->inv_dlam) { free(lnk); free(lp); free(bins); free(gtab); helios_rt_destroy(h); return HELIOS_RT_ENOMEM; }
+  for (int b = 0; b < nb; ++b) h->inv_dlam[b] = bins[b].inv_dlam;
   cudaError_t e = cudaSuccess;
   auto step = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   step(upload(&h->d_lnk, lnk, nk));
@@ -1451,10 +1787,21 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(upload(&h->d_gw, cfg->gauss_w, (size_t)ng));
   step(upload(&h->d_bins, bins, (size_t)nb));
   step(upload(&h->d_gtab, gtab, (size_t)kGIntervals * kGCoef));
+  {
+    double *c2l = (double *)malloc(sizeof(double) * (nb + 1));
+    if (!c2l) step(cudaErrorMemoryAllocation);
+    else {
+      for (int i = 0; i <= nb; ++i) c2l[i] = kPlanckC2 / cfg->bin_edges[i];
+      step(upload(&h->d_c2lam, c2l, (size_t)nb + 1));
+      free(c2l);
+    }
+  }
   free(lnk); free(lp); free(bins); free(gtab);
   const size_t ncol = (size_t)cfg->max_columns;
   step(cudaMalloc((void **)&h->d_counter, sizeof(unsigned) * ncol));
   if (e == cudaSuccess) step(cudaMemset(h->d_counter, 0, sizeof(unsigned) * ncol));
+  step(cudaMalloc((void **)&h->d_flags, sizeof(unsigned) * ncol));
+  if (e == cudaSuccess) step(cudaMemset(h->d_flags, 0, sizeof(unsigned) * ncol));
   // step_host staging: inputs packed as [p | T | mu | F*], outputs as [F_up | F_down | F_net | F_beam | dTdt | toa]
   const size_t n_in = ncol * (2 * (size_t)N + 1) + nb, n_out = ncol * (4 * ((size_t)N + 1) + N + nb);
   step(cudaMalloc((void **)&h->d_in, sizeof(double) * n_in));
@@ -1469,7 +1816,7 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     iter_fn it = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
     if (!h->toa)
       step(cudaFuncSetAttribute(it, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)make_lay(N, h->nlev, h->iter_warps, 1, ng, nb, false, h->noniso ? 2 : 1, false).total));
+                                (int)make_lay(N, h->nlev, h->iter_warps, 1, ng, nb, false, h->noniso ? 2 : 1, 0, false).total));
   }
   if (e != cudaSuccess) {
     const bool oom = (e == cudaErrorMemoryAllocation);
@@ -1508,7 +1855,7 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   if (in->n_columns == 0) return HELIOS_RT_OK;
   KParams P;
   P.lnk = h->d_lnk; P.tab_lp = h->d_tab_lp; P.tab_t = h->d_tab_t; P.edges = h->d_edges; P.gauss_w = h->d_gw;
-  P.bins = h->d_bins; P.gtab = h->d_gtab;
+  P.bins = h->d_bins; P.gtab = h->d_gtab; P.c2lam = h->d_c2lam;
   P.nP = c.n_ktab_p; P.nT = c.n_ktab_t; P.N = c.n_layers; P.nlev = h->nlev; P.nb = c.n_bins; P.ng = c.n_gauss; P.npt = h->npt;
   P.tiles = n_iter > 0 ? h->iter_tiles : h->tiles;
   P.ncol = in->n_columns;
@@ -1520,12 +1867,22 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.T_int = in->f_internal > 0 ? sqrt(sqrt(in->f_internal / kSigmaSB)) : 0.0;
   P.F_up = out->F_up; P.F_down = out->F_down; P.F_net = out->F_net; P.dTdt = out->dTdt; P.F_beam = out->F_beam;
   P.F_toa_bin = out->F_up_toa_bin;
+  P.ws_rec = h->d_ws_rec; P.ws_B = h->d_ws_B; P.flags = h->d_flags;
+  P.slot_ptr = h->d_slot_ptr; P.slots = h->d_slots; P.bslot = h->d_bslot;
+  ++h->epoch;
+  P.fused_prep = 0;
   P.stack = h->d_stack; P.stack_block = h->stack_block;
   P.partial = h->d_partial; P.counter = h->d_counter; P.queue = h->d_queue;
   if (n_iter > 0) {
     if (in->n_columns > 65535) return HELIOS_RT_EINVAL;   // the comparison kernel puts columns in gridDim.y
     iter_fn fn = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
-    const Lay lay = make_lay(c.n_layers, h->nlev, h->iter_warps, 1, c.n_gauss, c.n_bins, false, h->noniso ? 2 : 1, false);
+    const Lay &lay = h->iter_lay;
+    const long items = (long)in->n_columns * (h->nlev + 1);
+    const int pblocks = (int)((items + 127) / 128 < 16L * h->sm_count ? (items + 127) / 128 : 16L * h->sm_count);
+    P.slot_ptr = h->d_slot_ptr_iter; P.slots = h->d_slots_iter; P.bslot = h->d_bslot_iter;
+    if (h->noniso) rt_prep_kernel<true><<<pblocks, 128, 0, st>>>(P, h->iter_warps * 32, 0);
+    else rt_prep_kernel<false><<<pblocks, 128, 0, st>>>(P, h->iter_warps * 32, 0);
+    CK(h, cudaGetLastError());
     dim3 grid((unsigned)h->iter_tiles, (unsigned)in->n_columns);
     fn<<<grid, h->iter_warps * 32, lay.total, st>>>(P, n_iter);
     CK(h, cudaGetLastError());
@@ -1539,9 +1896,43 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   }
   int workers = h->workers;
   if (workers > in->n_columns) workers = in->n_columns;
-  dim3 grid((unsigned)h->tiles, (unsigned)workers);
-  kVariants[h->variant].fn<<<grid, h->warps * 32, h->lay.total, st>>>(P);
-  CK(h, cudaGetLastError());
+  // One cooperative launch: phase A (S1 + S2 of all columns, spread over the grid) and phase B (the sweeps) in the same
+  // kernel; blocks of phase B wait on per-column publication flags, which is safe because the cooperative launch
+  // guarantees that the whole grid is resident.  If the device cannot host the grid at once (another context's kernels
+  // hold SMs), phase A runs as a launch of its own instead.
+  cudaLaunchConfig_t lc;
+  memset(&lc, 0, sizeof(lc));
+  lc.gridDim = dim3((unsigned)h->tiles, (unsigned)workers);
+  lc.blockDim = dim3((unsigned)(h->warps * 32));
+  lc.dynamicSmemBytes = h->lay.total;
+  lc.stream = st;
+  cudaLaunchAttribute attr;
+  attr.id = cudaLaunchAttributeCooperative;
+  attr.val.cooperative = 1;
+  lc.attrs = &attr;
+  lc.numAttrs = 1;
+  P.fused_prep = h->epoch == 1 ? 1 : 2;   // (2: a later launch of the handle; only diagnostic builds care)
+#ifdef HRT_DIAG_NOCOOP         /* diagnostic builds (_work/): plain launch / phase A as its own launch */
+  lc.numAttrs = 0;
+#endif
+#ifdef HRT_DIAG_TWO_LAUNCH
+  cudaError_t e = cudaErrorNotSupported;
+#else
+  cudaError_t e = cudaLaunchKernelEx(&lc, kVariants[h->variant].fn, P);
+#endif
+  if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) {
+    cudaGetLastError();
+    P.fused_prep = 0;
+    const long items = (long)in->n_columns * (h->nlev + 1);
+    const int pblocks = (int)((items + 127) / 128 < 16L * h->sm_count ? (items + 127) / 128 : 16L * h->sm_count);
+    const int tp2 = h->warps * 32 * h->ppt;
+    if (h->noniso) rt_prep_kernel<true><<<pblocks, 128, 0, st>>>(P, tp2, 1);
+    else rt_prep_kernel<false><<<pblocks, 128, 0, st>>>(P, tp2, 1);
+    CK(h, cudaGetLastError());
+    lc.numAttrs = 0;
+    e = cudaLaunchKernelEx(&lc, kVariants[h->variant].fn, P);
+  }
+  CK(h, e);
   return HELIOS_RT_OK;
 }
 
@@ -1611,7 +2002,7 @@ extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t p
   const Variant &cur = kVariants[h->variant];
   const int want_ppt = ppt > 0 ? ppt : cur.ppt;
   if (want_ppt > 1 && (h->noniso ? false : (h->cfg.n_gauss % want_ppt) != 0)) return HELIOS_RT_EINVAL;
-  const int v = find_variant(h->noniso, h->toa, want_ppt, rows, stk, maxt, minb);
+  const int v = find_variant(h->noniso, h->toa, cur.bdirect, want_ppt, rows, stk, maxt, minb);
   if (v < 0) return HELIOS_RT_EINVAL;
   const int old_v = h->variant, old_w = h->warps;
   h->variant = v;

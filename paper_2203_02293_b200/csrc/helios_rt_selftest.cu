@@ -43,20 +43,27 @@ __global__ void selftest_math_kernel(int n, const double *x, double *rcp, double
 __global__ void selftest_planck_kernel(int n, const double *gtab, const double *T, const double *lo, const double *hi,
                                        double *out) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ double T32[32];
+  if (threadIdx.x < 32) T32[threadIdx.x] = kExp2Tab[threadIdx.x];
+  __syncthreads();
   if (i >= n) return;
   const double t = T[i];
   if (!(t > 0.0)) { out[i] = 0.0; return; }
   double l_hi, l_lo;
-  const double g_hi = planck_G(kPlanckC2 / (hi[i] * t), gtab, &l_hi), g_lo = planck_G(kPlanckC2 / (lo[i] * t), gtab, &l_lo);
+  const double g_hi = planck_G((kPlanckC2 / hi[i]) * (1.0 / t), gtab, T32, &l_hi),
+               g_lo = planck_G((kPlanckC2 / lo[i]) * (1.0 / t), gtab, T32, &l_lo);   // x formed as S2 forms it
   const double t2 = t * t;
   out[i] = kPlanckC1 * t2 * t2 * planck_dG(g_lo, l_lo, g_hi, l_hi) / (hi[i] - lo[i]);
 }
 
 __global__ void selftest_G_kernel(int n, const double *gtab, const double *x, double *G) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ double T32[32];
+  if (threadIdx.x < 32) T32[threadIdx.x] = kExp2Tab[threadIdx.x];
+  __syncthreads();
   if (i >= n) return;
   double low;
-  G[i] = planck_G(x[i], gtab, &low);
+  G[i] = planck_G(x[i], gtab, T32, &low);
 }
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
