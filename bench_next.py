@@ -1,11 +1,12 @@
-"""Measurements of the NEXT rows on one B200: `python -m paper_2203_02293_b200.bench_next
+"""Measurements of the NEXT rows on one B200: `python bench_next.py
 [--what postproc|onedim|iterative|all] [--steps K]`.  One JSON line per row; CUDA-event times on the launching
 stream after warm-up, inputs resident on the device, L2 flushed between timed repetitions.
 
   postproc   config 6: helios_rt_extend_top -> helios_rt_step (R=500 opacity sampling, 3255 wavelengths, 60 layers,
              TOA spectrum) -> helios_rt_phase_curve (64 phases + HST-WFC3 band), Eqs. 23-26
   onedim     Sec. 3 "1-D mode": (helios_rt_step -> helios_rt_advance_1d) per time step, plain launches and one
-             CUDA graph of the pair replayed; 4 zenith angles (config-1 sized columns) and the config-2 grid
+             CUDA graph of the pair replayed; 4 zenith angles (config-1 sized columns) and the config-2 grid; then the
+             four zenith angles run to radiative equilibrium (12000 / 36000 replays), residuals reported
   iterative  helios_rt_step_iterative (the scheme Thomas replaces, L258-270) against helios_rt_step on config 2:
              the paper's "about 2 orders of magnitude" (L13, L397) re-measured on B200
 """
@@ -18,7 +19,7 @@ from pathlib import Path
 
 import numpy as np
 
-ROOT = Path(__file__).resolve().parent.parent
+ROOT = Path(__file__).resolve().parent
 if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
@@ -156,6 +157,56 @@ def bench_onedim(torch, H, W, steps):
     return out
 
 
+def bench_steady_state(torch, H, W):
+    """NEXT-3: the Sec. 3 experiment -- the four zenith angles run to radiative equilibrium by replaying one captured time
+    step (RT step + T update + Eq. 20); residuals at the end and time steps per second."""
+    import time
+    dev = torch.device("cuda", 0)
+    t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
+    out = []
+    for zenith, cp, K in (((0.0, 30.0, 60.0), 2000.0, 12000), ((89.0,), 500.0, 36000)):
+        cfg, inp, meta, ex = W.make_one_d(zenith, cp)
+        n, N = inp["T"].shape
+        g = cfg["gravity"]
+        rt = H.HeliosRT(cfg, n)
+        dT, dz, dmu, dfs = t(inp["T"]), t(ex["z"]), t(inp["mu_star"]), t(inp["stellar_flux"])
+        dp = torch.empty((n, N), dtype=torch.float64, device=dev)
+        dh = torch.empty((n, N), dtype=torch.float64, device=dev)
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            H.advance_1d(0.0, g, ex["R_d"], ex["p_ref"], dz, None, dT, dp, None, stream=s)
+
+            def pair():
+                rt.step(dp, dT, dmu, dfs, inp["f_internal"], {"dTdt": dh}, stream=s)
+                H.advance_1d(ex["dt"], g, ex["R_d"], ex["p_ref"], dz, dh, dT, dp, None, stream=s)
+            pair()
+            s.synchronize()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr, stream=s):
+                pair()
+            t0 = time.perf_counter()
+            for _ in range(K - 1):
+                gr.replay()
+            s.synchronize()
+            wall = time.perf_counter() - t0
+            res = {k: torch.empty((n, N + 1) if k != "dTdt" else (n, N), dtype=torch.float64, device=dev) for k in ("F_net", "dTdt")}
+            rt.step(dp, dT, dmu, dfs, inp["f_internal"], res, stream=s)
+        torch.cuda.synchronize()
+        F_net, dTdt = res["F_net"].cpu().numpy(), res["dTdt"].cpu().numpy()
+        absorbed = inp["mu_star"] * meta["F_star_tot"]
+        out.append({"row": "NEXT-3 steady state", "metric": "one_d_time_steps_per_s", "value": (K - 1) / wall, "unit": "steps/s",
+                    "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+                    "config": {"workload": f"1-D mode, zenith angles {list(zenith)} deg, config-1 column shape, c_P = {cp:.0f} "
+                                           f"(pseudo-time acceleration), dt = {ex['dt']:.0f} s, {K} time steps replayed from one "
+                                           "CUDA graph"},
+                    "max_abs_dTdt_times_dt_K": float(np.abs(dTdt).max() * ex["dt"]),
+                    "max_F_net_spread_over_absorbed": float(np.max(np.abs(F_net - F_net[:, :1]) / absorbed[:, None])),
+                    "F_net_boa": [float(x) for x in F_net[:, 0]], "T_range_K": [float(dT.min()), float(dT.max())],
+                    "gpu_launches": 2 * K})
+        rt.close()
+    return out
+
+
 def bench_iterative(torch, H, W, steps):
     dev = torch.device("cuda", 0)
     t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
@@ -201,6 +252,8 @@ def main() -> int:
         print(json.dumps(bench_postproc(torch, H, W, args.steps)), flush=True)
     if args.what in ("onedim", "all"):
         for line in bench_onedim(torch, H, W, args.steps):
+            print(json.dumps(line), flush=True)
+        for line in bench_steady_state(torch, H, W):
             print(json.dumps(line), flush=True)
     if args.what in ("iterative", "all"):
         print(json.dumps(bench_iterative(torch, H, W, args.steps)), flush=True)

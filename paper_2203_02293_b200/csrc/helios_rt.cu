@@ -773,9 +773,10 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, 
 //           local memory (kept for comparison builds; SCAP = its capacity in interfaces)
 //   BDIRECT one Gauss point per bin (opacity sampling, L385): every thread has its own bin, so the Planck values are
 //           read coalesced from the workspace instead of being staged (64 KB per block otherwise); PPT = 1
+//   WARPS   warps per block as a compile-time constant, or 0 = taken from the launch
 //   MAXT, MINB  launch bounds (register cap = 65536 / (MAXT MINB)); any block of <= MAXT threads may be launched
 // --------------------------------------------------------------------------------------------
-template <bool NONISO, bool TOA, int PPT, int ROWS, int STK, int SCAP, bool BDIRECT, int MAXT, int MINB>
+template <bool NONISO, bool TOA, int PPT, int ROWS, int STK, int SCAP, bool BDIRECT, int WARPS, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   static_assert(PPT == 1 || PPT == 2 || PPT == 4, "points per thread");
   static_assert(!BDIRECT || PPT == 1, "one Gauss point per bin: one point per thread");
@@ -784,7 +785,8 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   __shared__ double s_T32[32];
   __shared__ int s_is_last, s_col[2];
   const int N = P.N, nlev = P.nlev;
-  const int tid = threadIdx.x, nthr = blockDim.x, nwarps = nthr >> 5;
+  // WARPS > 0: the block size is a compile-time constant (the shapes helios_rt_create picks); 0: any block <= MAXT
+  const int tid = threadIdx.x, nthr = WARPS ? WARPS * 32 : blockDim.x, nwarps = nthr >> 5;
   const int warp = tid >> 5, lane = tid & 31;
   const Lay L = make_lay(N, nlev, nwarps, PPT, P.ng, P.nb, TOA, DEPTH, ROWS, BDIRECT);
   BinOpt *s_bin = (BinOpt *)(smem + L.off_bin);
@@ -1436,16 +1438,16 @@ typedef void (*kernel_fn)(const KParams);
 
 struct Variant {
   bool noniso, toa, bdirect;
-  int ppt, rows, stk, scap;   // scap: capacity (interfaces) of the local-memory stack of the STK = 0 comparison builds
+  int ppt, rows, stk, scap, warps;   // warps: block size compiled in, 0 = any   // scap: capacity (interfaces) of the local-memory stack of the STK = 0 comparison builds
   int maxt, minb;      // launch bounds: register cap = 65536 / (maxt * minb)
   kernel_fn fn;
 };
 
-#define HRT_K(NI, TOA, PPT, ROWS, STK, SCAP, MAXT, MINB) \
-  {NI, TOA, false, PPT, ROWS, STK, SCAP, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, STK, SCAP, false, MAXT, MINB>}
+#define HRT_K(NI, TOA, PPT, ROWS, STK, SCAP, WARPS, MAXT, MINB) \
+  {NI, TOA, false, PPT, ROWS, STK, SCAP, WARPS, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, STK, SCAP, false, WARPS, MAXT, MINB>}
 // one Gauss point per bin (opacity sampling): Planck values read from the workspace; one point per thread
-#define HRT_KB(NI, TOA, ROWS, MAXT, MINB) \
-  {NI, TOA, true, 1, ROWS, 1, 1, MAXT, MINB, rt_step_kernel<NI, TOA, 1, ROWS, 1, 1, true, MAXT, MINB>}
+#define HRT_KB(NI, TOA, ROWS, WARPS, MAXT, MINB) \
+  {NI, TOA, true, 1, ROWS, 1, 1, WARPS, MAXT, MINB, rt_step_kernel<NI, TOA, 1, ROWS, 1, 1, true, WARPS, MAXT, MINB>}
 
 // Compiled instantiations, in order of preference for each (noniso, toa, ppt).  helios_rt_create takes the first
 // match; helios_rt_debug_set_launch (tests, tuning) may select any other.
@@ -1649,7 +1651,7 @@ static int configure_launch(helios_rt *h) {
   const Variant &v = kVariants[h->variant];
   const int N = c.n_layers;
   h->ppt = v.ppt;
-  if (h->warps * 32 > v.maxt) return HELIOS_RT_EINVAL;
+  if (h->warps * 32 > v.maxt || (v.warps != 0 && v.warps != h->warps)) return HELIOS_RT_EINVAL;
   if (!h->toa && v.stk == 0 && N + 1 > v.scap) return HELIOS_RT_EINVAL;
   const int tp = h->warps * 32 * h->ppt;
   h->tiles = (h->npt + tp - 1) / tp;
@@ -1707,10 +1709,13 @@ static int configure_launch(helios_rt *h) {
   return HELIOS_RT_OK;
 }
 
-static int find_variant(bool noniso, bool toa, bool bdirect, int ppt, int rows, int stk, int maxt, int minb) {
+// first instantiation of the class that matches; one compiled for exactly `warps` warps is preferred to a generic one
+static int find_variant(bool noniso, bool toa, bool bdirect, int ppt, int rows, int stk, int maxt, int minb, int warps) {
+  for (int pass = 0; pass < 2; ++pass)
   for (int i = 0; i < kNumVariants; ++i) {
     const Variant &v = kVariants[i];
     if (v.noniso != noniso || v.toa != toa || v.bdirect != bdirect || v.ppt != ppt) continue;
+    if (pass == 0 ? v.warps != warps : v.warps != 0) continue;
     if (rows >= 0 && v.rows != rows) continue;
     if (stk >= 0 && !toa && v.stk != stk) continue;
     if (maxt >= 0 && v.maxt != maxt) continue;
@@ -1741,9 +1746,13 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->iter_warps = default_warps(h->npt, 1, false);
   h->iter_tiles = (h->npt + h->iter_warps * 32 - 1) / (h->iter_warps * 32);
   int ppt = default_ppt(h->npt, ng, h->noniso, h->toa);
-  h->variant = find_variant(h->noniso, h->toa, ng == 1, ppt, -1, -1, -1, -1);
-  if (h->variant < 0) { ppt = 1; h->variant = find_variant(h->noniso, h->toa, ng == 1, 1, -1, -1, -1, -1); }
   h->warps = default_warps(h->npt, ppt, h->noniso);
+  h->variant = find_variant(h->noniso, h->toa, ng == 1, ppt, -1, -1, -1, -1, h->warps);
+  if (h->variant < 0) {
+    ppt = 1;
+    h->warps = default_warps(h->npt, 1, h->noniso);
+    h->variant = find_variant(h->noniso, h->toa, ng == 1, 1, -1, -1, -1, -1, h->warps);
+  }
   int dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -1773,6 +1782,10 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
     bc.sb[0] = sg;            bc.sb[1] = sg + kc;
     bc.ss[0] = sg;            bc.ss[1] = sg + sc;
     bc.gg[0] = 0.0;           bc.gg[1] = (sg + sc > 0.0) ? sc * cfg->cloud_g0[b] / (sg + sc) : 0.0;
+    // omega0 = ss / (kappa_abs + sb) must stay below 1 after rounding (E - omega0 = 0 is the singular conservative limit,
+    // SURVEY.md Q5): a purely scattering constituent is capped one ulp below its extinction
+    for (int cl = 0; cl < 2; ++cl)
+      if (bc.ss[cl] > bc.sb[cl] * (1.0 - 0x1p-52)) bc.ss[cl] = bc.sb[cl] * (1.0 - 0x1p-52);
   }
   build_planck_table(gtab);
   h->inv_dlam = (double *)malloc(sizeof(double) * nb);
@@ -2002,11 +2015,12 @@ extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t p
   const Variant &cur = kVariants[h->variant];
   const int want_ppt = ppt > 0 ? ppt : cur.ppt;
   if (want_ppt > 1 && (h->noniso ? false : (h->cfg.n_gauss % want_ppt) != 0)) return HELIOS_RT_EINVAL;
-  const int v = find_variant(h->noniso, h->toa, cur.bdirect, want_ppt, rows, stk, maxt, minb);
+  const int want_warps = warps > 0 ? warps : h->warps;
+  const int v = find_variant(h->noniso, h->toa, cur.bdirect, want_ppt, rows, stk, maxt, minb, want_warps);
   if (v < 0) return HELIOS_RT_EINVAL;
   const int old_v = h->variant, old_w = h->warps;
   h->variant = v;
-  if (warps > 0) h->warps = warps;
+  h->warps = want_warps;
   int rc = configure_launch(h);
   if (rc) { h->variant = old_v; h->warps = old_w; configure_launch(h); }
   return rc;

@@ -251,3 +251,21 @@ def _make_postproc(columns=None, n_col_level: int = 4, nb: int = 3255, N: int = 
                 lon=lon, lat=lat, area=area, alpha=np.linspace(-np.pi, np.pi, 64, endpoint=False),
                 band=(1.1e-6, 1.7e-6))
     return cfg, inp, meta
+
+
+def make_one_d(zenith_deg=(0.0, 30.0, 60.0, 89.0), cp: float = 2000.0):
+    """Inputs of the "1-D mode" experiment (Sec. 3): one column per stellar zenith angle (the
+    paper's 0, 30, 60, 89 degrees), config 1's column shape, table and spectrum (10 layers, 4 bins x 4 Gauss points),
+    stepped with dt = 300 s (L384) from config 1's initial profile.  The steady state does not depend on the heat
+    capacity, so c_P is lowered from Table 3's 12436 to `cp` J kg^-1 K^-1 as a pseudo-time acceleration (the paper
+    integrates 800 days); the smaller the forcing, the smaller the c_P an explicit step tolerates: 2000 is stable at
+    0-60 degrees, 500 at 89 degrees.  Returns (cfg, inp, meta, extra) with extra = dict(z, p_ref, R_d, dt): the fixed
+    altitude grid (barometric, from the initial mean temperature), the reference pressure of Eq.(20), the gas constant
+    of Table 3 and the time step."""
+    cfg, inp, meta = make(1, columns=slice(0, len(zenith_deg)))
+    mu = np.cos(np.radians(np.asarray(zenith_deg, dtype=np.float64)))
+    R_d = 3553.0
+    z = (R_d * inp["T"].mean() / cfg["gravity"]) * np.log(inp["p"][0, 0] / inp["p"][0])
+    cfg = dict(cfg, cp=float(cp))
+    inp = dict(inp, mu_star=mu)
+    return cfg, inp, meta, dict(z=z, p_ref=float(inp["p"][0, 0]), R_d=R_d, dt=300.0)

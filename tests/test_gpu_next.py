@@ -329,3 +329,56 @@ def test_one_d_mode_loop_matches_the_oracle(torch_cuda, H, graph):
     assert np.allclose(dp.cpu().numpy(), ref_p, rtol=1e-9, atol=0)
     assert np.abs(ref_T - T0).max() > 1e-3       # the loop did move the temperatures
     rt.close()
+
+
+@pytest.mark.parametrize("zenith,cp,n_steps", [((0.0, 30.0, 60.0), 2000.0, 12000), ((89.0,), 500.0, 36000)])
+def test_one_d_mode_steady_state_on_the_device(torch_cuda, H, zenith, cp, n_steps):
+    """PAPER.md Sec. 3 (L401-410): the 1-D mode run to radiative equilibrium, all on the device
+    (one captured time step = RT step + T update + Eq. 20, replayed n_steps times).  At the end: |dT/dt| dt < 1e-7 K,
+    F_net constant with depth and equal to the internal flux (Eq. 10) to 1e-9 of the absorbed stellar flux, and the
+    temperature profile equal to the equilibrium the oracle reaches on its own (same fixed point, different rounding
+    along the way)."""
+    import oracle
+    from oracle import onedim
+    from paper_2203_02293_b200 import workloads as W
+    torch = torch_cuda
+    cfg, inp, meta, ex = W.make_one_d(zenith, cp)
+    n, N = inp["T"].shape
+    g = cfg["gravity"]
+    rt = H.HeliosRT(cfg, n)
+    dT, dz = _t(torch, inp["T"]), _t(torch, ex["z"])
+    dp = torch.empty((n, N), dtype=torch.float64, device="cuda:0")
+    dh = torch.empty((n, N), dtype=torch.float64, device="cuda:0")
+    dmu, dfs = _t(torch, inp["mu_star"]), _t(torch, inp["stellar_flux"])
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        H.advance_1d(0.0, g, ex["R_d"], ex["p_ref"], dz, None, dT, dp, None, stream=s)
+
+        def pair():
+            rt.step(dp, dT, dmu, dfs, inp["f_internal"], {"dTdt": dh}, stream=s)
+            H.advance_1d(ex["dt"], g, ex["R_d"], ex["p_ref"], dz, dh, dT, dp, None, stream=s)
+        pair()
+        s.synchronize()
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr, stream=s):
+            pair()
+        for _ in range(n_steps - 1):
+            gr.replay()
+        out = {k: torch.empty((n, N + 1) if k != "dTdt" else (n, N), dtype=torch.float64, device="cuda:0")
+               for k in ("F_net", "F_down", "dTdt")}
+        rt.step(dp, dT, dmu, dfs, inp["f_internal"], out, stream=s)
+    torch.cuda.synchronize()
+    T = dT.cpu().numpy()
+    F_net, dTdt = out["F_net"].cpu().numpy(), out["dTdt"].cpu().numpy()
+    absorbed = inp["mu_star"] * meta["F_star_tot"]
+    e = cfg["bin_edges"]
+    T_int = (inp["f_internal"] / 5.670374419e-8) ** 0.25
+    F_boa = sum((e[b + 1] - e[b]) * np.pi * oracle.planck_bin_mean(T_int, e[b], e[b + 1]) for b in range(meta["n_bins"]))
+    assert np.all(np.isfinite(T))
+    assert np.abs(dTdt).max() * ex["dt"] < 1e-7
+    assert np.all(np.abs(F_net - F_boa) <= 1e-9 * absorbed[:, None])
+    assert np.all(out["F_down"].cpu().numpy()[:, -1] > 0.5 * absorbed)
+    step = lambda p, T_: oracle.rt_step(cfg, dict(inp, p=p, T=T_), want=("dTdt",), real="f64")["dTdt"]
+    _, T_ref = onedim.run(step, ex["z"], inp["T"], ex["p_ref"], g, ex["R_d"], ex["dt"], n_steps)
+    assert np.allclose(T, T_ref, rtol=1e-7, atol=0)
+    rt.close()

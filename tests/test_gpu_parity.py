@@ -340,6 +340,31 @@ def test_mu_crit_guard_on_device(torch_cuda, H, oracle_mod):
     assert_parity(oracle_mod, cfg, inp, meta, got, ref)
 
 
+def test_conservative_cloud_stays_finite(torch_cuda, H, oracle_mod):
+    """cloud_w0 = 1 (a purely scattering cloud) under the conservative limit E - omega0 -> 0.
+    (a) A cloud 1e12 times more opaque than the most opaque gas point: 1 - omega0 = kappa_abs / kappa_ext is 1e-16 ..
+    1e-12, i.e. at or below the rounding of omega0 itself, so the absorption optical depth (1 - omega0) dtau is not
+    representable and no fp64 result can be held to the long-double oracle; what is required is that nothing divides by
+    zero: the library caps omega0 one ulp below 1, all outputs are finite and the fluxes non-negative.
+    (b) The same cloud at 1e4 times the gas opacity: 1 - omega0 >= 1.4e-8, whose rounding (1e-16 / 1.4e-8) enters
+    zeta+- and alpha through a square root; fluxes agree with the oracle to 1e-6."""
+    cfg, inp, meta = _small()
+    nb = meta["n_bins"]
+    kmax = float(cfg["ktab"].max())
+    for flags in (0, 1, 3):
+        c = dict(cfg, flags=flags, cloud_ext=np.full(nb, 1e12 * kmax), cloud_w0=np.ones(nb),
+                 cloud_g0=np.zeros(nb), cloud_p_top=1e2, cloud_p_bot=3e4)
+        got = run_gpu(torch_cuda, H, c, inp, ("F_up", "F_down", "F_net", "dTdt"))
+        for k in ("F_up", "F_down", "F_net", "dTdt"):
+            assert np.all(np.isfinite(got[k])), (flags, k)
+        assert np.all(got["F_up"] >= 0) and np.all(got["F_down"] >= 0), flags
+        c = dict(c, cloud_ext=np.full(nb, 1e4 * kmax))
+        got = run_gpu(torch_cuda, H, c, inp, ("F_up", "F_down"))
+        ref = oracle_mod.rt_step(c, inp, want=("F_up", "F_down"))
+        for k in ("F_up", "F_down"):
+            assert np.allclose(got[k], ref[k], rtol=1e-6, atol=1e-9 * meta["F_star_tot"]), (flags, k)
+
+
 def test_nan_stays_in_its_column(torch_cuda, H, oracle_mod):
     cfg, inp, meta = _small()
     T = inp["T"].copy(); T[3, 4] = np.nan

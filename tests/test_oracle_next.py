@@ -222,3 +222,41 @@ def test_rt_step_with_iterations_approaches_the_thomas_step():
     ref = oracle.rt_step(cfg, inp, want=("F_net",))["F_net"]
     e = [np.abs(oracle.rt_step(dict(cfg, n_iterations=k), inp, want=("F_net",))["F_net"] - ref).max() for k in (2, 8, 60)]
     assert e[0] > e[1] > e[2] and e[2] < 1e-9 * np.abs(ref).max()
+
+
+# ------------------------------------------------------------------------- 1-D mode run to a steady state (Sec. 3)
+def _equilibrate(oracle_mod, cfg, inp, extra, n_steps):
+    from oracle import onedim
+    g = cfg["gravity"]
+    step = lambda p, T: oracle_mod.rt_step(cfg, dict(inp, p=p, T=T), want=("dTdt",), real="f64")["dTdt"]
+    p, T = onedim.run(step, extra["z"], inp["T"], extra["p_ref"], g, extra["R_d"], extra["dt"], n_steps)
+    return p, T, oracle_mod.rt_step(cfg, dict(inp, p=p, T=T), want=("dTdt", "F_net", "F_up", "F_down"))
+
+
+@pytest.mark.parametrize("zenith,cp,n_steps", [((0.0, 30.0, 60.0), 2000.0, 12000), ((89.0,), 500.0, 36000)])
+def test_one_d_mode_reaches_radiative_equilibrium(oracle_mod, zenith, cp, n_steps):
+    """PAPER.md Sec. 3 (L401-410): RT step + hydrostatic re-balance, stepped until nothing changes.  What makes this
+    physics rather than plumbing: in a steady state every layer's heating rate vanishes, which by the heating-rate
+    reading R14 means the net flux is the same at every interface, and by Eq.(10) (L237-239) that constant is the
+    internal flux sum_b dlam_b pi B_b(T_int) fed in at the bottom -- whatever the zenith angle.  A sign error in the
+    heating rate diverges instead of relaxing; a beam left out of F_down (L235) equilibrates to a net flux that is
+    not F_BOA."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta, extra = W.make_one_d(zenith, cp)
+    p, T, r = _equilibrate(oracle_mod, cfg, inp, extra, n_steps)
+    e = cfg["bin_edges"]
+    SIGMA = 2 * np.pi**5 * 1.380649e-23**4 / (15 * 6.62607015e-34**3 * 299792458.0**2)
+    T_int = (inp["f_internal"] / SIGMA) ** 0.25
+    F_boa = sum((e[b + 1] - e[b]) * np.pi * oracle_mod.planck_bin_mean(T_int, e[b], e[b + 1]) for b in range(meta["n_bins"]))
+    absorbed = inp["mu_star"] * meta["F_star_tot"]
+    assert np.all(np.isfinite(T)) and T.min() > 100.0 and T.max() < 4000.0
+    assert np.abs(T - inp["T"]).max() > 50.0                                   # it went somewhere
+    # F_net constant with depth and equal to the internal flux, to 1e-9 of the stellar flux the column absorbs
+    assert np.all(np.abs(r["F_net"] - F_boa) <= 1e-9 * absorbed[:, None])
+    # ... although the fluxes themselves are of the order of the stellar flux
+    assert np.all(r["F_down"][:, -1] > 0.5 * absorbed)
+    # nothing changes any more: |dT/dt| dt below 1e-7 K per step everywhere
+    assert np.abs(r["dTdt"]).max() * extra["dt"] < 1e-7
+    # hotter under a higher sun
+    if len(zenith) > 1:
+        assert np.all(np.diff(T, axis=0) < 0)
