@@ -91,7 +91,6 @@ struct KParams {
   unsigned row_stride;
   double inv_dlp, inv_dt;   // 1 / mean spacing of the table grids: first guess of the cell search
   double cloud_p_top, cloud_p_bot, inv_g, inv_cp, inv_eps2, e_tau, gcrit_tol, w0_transition, f_toa;
-  int improved;
   // per-step
   const double *p, *T, *mu, *fstar;
   double T_int;
@@ -123,14 +122,14 @@ struct G0Terms {
   double g0;
   double fg;   // Eq.(19): 1.225 - 0.1582 g0 - 0.07465 g0^2
   double fA;   // Eq.(19): -0.1777 + 0.2351 g0   (fit = fg + w0 (fA - 0.05582 w0))
-  double ge;   // g0 / eps2, (B8)
+  double geh;  // g0 / (2 eps2), (B8)
 };
 __device__ __forceinline__ G0Terms g0_terms(double g0, double inv_eps2) {
   G0Terms t;
   t.g0 = g0;
   t.fg = fma(g0, fma(kHC.fc, g0, kHC.fb), kHC.fa);
   t.fA = fma(g0, kHC.fe, kHC.fd);
-  t.ge = g0 * inv_eps2;
+  t.geh = 0.5 * g0 * inv_eps2;
   return t;
 }
 
@@ -141,7 +140,10 @@ __device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__r
   // E, Eq.(19) L374 (readings R5, R6): E = max(1, fit) if w0 > 0.1 else 1
   const double g0 = gt.g0;
   const double fit = fma(w0, fma(kHC.ff, w0, gt.fA), gt.fg);
-  const double E = (P.improved && gt_pos(w0, P.w0_transition) && gt_pos(fit, 1.0)) ? fit : 1.0;
+  // (one predicate, two selects: w0 > transition on the 64-bit pattern; fit >= 1 on the high word alone -- fit = 1
+  // gives E = 1 either way.  Regular two-stream: the transition is +inf, launch_step)
+  const bool use_fit = gt_pos(w0, P.w0_transition) & (__double2hiint(fit) >= 0x3ff00000);
+  const double E = use_fit ? fit : 1.0;
   const double wg = w0 * g0;
   const double num = E - w0;             // E - omega0
   const double den = E * (1.0 - wg);     // E (1 - omega0 g0)
@@ -152,7 +154,7 @@ __device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__r
   const double rs2 = rs * rs;
   const double zp = fma(0.5, s, 0.5), zm = fma(-0.5, s, 0.5);
   double omT;
-  const double Tr = exp_hot<2, true>(min_pos(ha * dtau, 354.0), T32, &omT);   // transmission function (B2), 1 - T
+  const double Tr = exp_hot<2, true>(cap_pos<0x40762000>(ha * dtau), T32, &omT);   // transmission function (B2), 1 - T; argument capped near 354
   const double zmT = zm * Tr;
   const double a = zp - zmT, b = zp + zmT;
   const double inv_ab = rcp_fast(a * b);
@@ -178,14 +180,14 @@ __device__ __forceinline__ void layer_coeffs(const KParams &P, const double *__r
   }
   if (DAY) {
     // (B8) with mu_star = -mu; guard of Eq.(11)/L252 (reading R4)
-    const double ma = mu * (2.0 * ha);
+    const double ma = (mu + mu) * ha;                        // (mu + mu: loop-invariant)
     double D = (ma - 1.0) * (ma + 1.0);                      // 4 E mu^2 (E-w0)(1-w0 g0) - 1
     D = abs_lt(D, P.gcrit_tol) ? -2.0 * mu : D;
     const double invD = rcp_fast(D);
     const double hP = 0.5 * (num * rs2);                     // 1 / (2 E (1 - w0 g0))
-    const double ge = gt.ge;
-    const double lead = (0.5 * w0) * fma(2.0, den, ge) * invD;
-    const double last = (0.5 * w0) * ge * hP;
+    const double geh = gt.geh;                               // g0 / (2 eps2)
+    const double lead = (w0 * (den + geh)) * invD;           // (w0/2) (2 E (1 - w0 g0) + g0/eps2) / D
+    const double last = w0 * (geh * hP);
     const double Gp = fma(lead, hP - mu, last);
     const double Gm = -fma(lead, hP + mu, last);
     // (B7): S_up += t G+ Fa + r G- Fb - G+ Fb ; S_dn += t G- Fb + r G+ Fa - G- Fa
@@ -215,33 +217,6 @@ __device__ __forceinline__ void layer_forward(const KParams &P, const double *__
   U = Un;
 }
 
-// Sum each of the 16 values v[0..15] over the 32 lanes of the warp by recursive halving: 16 shuffle+add
-// steps instead of 16 x 5.  Returns, in lanes L and L^1, the total of v[L >> 1].  Fixed order: deterministic.
-__device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
-  const unsigned full = 0xffffffffu;
-  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const double send = b4 ? v[i] : v[i + 8], keep = b4 ? v[i + 8] : v[i];
-    v[i] = keep + __shfl_xor_sync(full, send, 16);
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const double send = b3 ? v[i] : v[i + 4], keep = b3 ? v[i + 4] : v[i];
-    v[i] = keep + __shfl_xor_sync(full, send, 8);
-  }
-#pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const double send = b2 ? v[i] : v[i + 2], keep = b2 ? v[i + 2] : v[i];
-    v[i] = keep + __shfl_xor_sync(full, send, 4);
-  }
-  {
-    const double send = b1 ? v[0] : v[1], keep = b1 ? v[1] : v[0];
-    v[0] = keep + __shfl_xor_sync(full, send, 2);
-  }
-  return v[0] + __shfl_xor_sync(full, v[0], 1);
-}
-
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -267,8 +242,7 @@ struct Lay {
   unsigned u_stage, u_ring, ring_warp;                   // sweep view: [warp] staging tile; [warp] row ring
 };
 
-// ppt: spectral points per thread; depth: levels per sweep iteration (1 isothermal, 2 non-isothermal); rows: 1 TMA ring,
-// 2 per-lane cp.async buffer;
+// ppt: spectral points per thread; depth: levels per sweep iteration (1 isothermal, 2 non-isothermal); rows: 1 TMA ring;
 // bdirect: one Gauss point per bin -- the Planck block is read from the workspace, not staged
 __host__ __device__ inline Lay make_lay(int N, int nlev, int warps, int ppt, int ng, int nb, bool toa, int depth, int rows,
                                         bool bdirect) {
@@ -296,7 +270,7 @@ __host__ __device__ inline Lay make_lay(int N, int nlev, int warps, int ppt, int
   // sweep scratch
   L.u_stage = utake(toa ? 0 : sizeof(double) * warps * 8 * STAGE_LD);
   u = (u + 127) & ~127u;
-  L.ring_warp = rows == 1 ? (unsigned)(RING * depth * 4 * 32 * ppt * 8) : (rows == 2 ? (unsigned)(depth * 4 * 32 * ppt * 8) : 0);
+  L.ring_warp = rows == 1 ? (unsigned)(RING * depth * 4 * 32 * ppt * 8) : 0;
   L.u_ring = utake((size_t)L.ring_warp * warps);
   L.total = L.off_u + u;
   return L;
@@ -383,11 +357,12 @@ __device__ __forceinline__ void load_rows_s(RowsT<PPT> &r, const double *st, int
 }
 
 // Row feed of the sweep: DEPTH levels per iteration, top-down.  ROWS = 0: the next iteration's rows are held in
-// registers (loads issued one iteration ahead).  ROWS = 1: a per-warp ring of RING stages in shared memory, filled by
-// bulk async copies that lane 0 issues two iterations ahead; each stage has its own mbarrier (expect-tx = the
-// stage's bytes); the warp re-arms a stage itself once all its lanes have consumed it, so warps never wait on each
-// other.  `kc` counts iterations since the barriers were initialised and runs across columns: iteration kc uses
-// stage kc % RING in phase (kc / RING) & 1.
+// registers: an iteration first consumes them (next), then re-loads the same registers for the following iteration
+// (release) -- no copy, the loads are in flight for a whole iteration.  ROWS = 1: a per-warp ring of RING stages in
+// shared memory, filled by bulk async copies that lane 0 issues two iterations ahead; each stage has its own mbarrier
+// (expect-tx = the stage's bytes); the warp re-arms a stage itself once all its lanes have consumed it, so warps never
+// wait on each other.  `kc` counts iterations since the barriers were initialised and runs across columns: iteration
+// kc uses stage kc % RING in phase (kc / RING) & 1.
 template <int PPT, int DEPTH, int ROWS> struct Feed;
 
 template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 0> {
@@ -403,17 +378,15 @@ template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 0> {
   }
   // lv: highest level of the first iteration
   __device__ __forceinline__ void prime(const LevelRec *lv, int /*iterations*/) { load(lv); }
-  // returns the rows of this iteration; lv_next: highest level of the next iteration
-  __device__ __forceinline__ void next(RowsT<PPT> (&cur)[DEPTH], const LevelRec *lv_next) {
-#pragma unroll
-    for (int d = 0; d < DEPTH; ++d) cur[d] = nx[d];
-    load(lv_next);
-  }
-  __device__ __forceinline__ void release(const LevelRec *, bool) {}
+  // the rows of this iteration (valid until release)
+  __device__ __forceinline__ const RowsT<PPT> *next() { return nx; }
+  // call once the iteration's rows have been used; lv_next: highest level of the next iteration
+  __device__ __forceinline__ void release(const LevelRec *lv_next, const LevelRec *, bool) { load(lv_next); }
 };
 
 template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 1> {
   static constexpr uint32_t ROWB = 32 * PPT * 8, STGB = DEPTH * 4 * ROWB;
+  RowsT<PPT> cur[DEPTH];
   const double *ring;    // this warp's ring (generic address)
   uint32_t ring_s, bar_s;
   const double *lnk_w;   // ln(kappa) table + first spectral point of the warp
@@ -440,80 +413,21 @@ template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 1> {
       if (iterations > 1) fill((kc + 1) % RING, lv - DEPTH);
     }
   }
-  __device__ __forceinline__ void next(RowsT<PPT> (&cur)[DEPTH], const LevelRec *) {
+  __device__ __forceinline__ const RowsT<PPT> *next() {
     const uint32_t stage = kc % RING;
     mbar_wait(bar_s + 8 * stage, (kc / RING) & 1u);
     const double *st = ring + (size_t)stage * (STGB / 8);
 #pragma unroll
     for (int d = 0; d < DEPTH; ++d) load_rows_s<PPT>(cur[d], st + d * 4 * 32 * PPT, lane);
+    return cur;
   }
   // call once the iteration's rows are in registers and have been used; lv_refill: highest level of the iteration
   // RING ahead (has = false: none left in this column)
-  __device__ __forceinline__ void release(const LevelRec *lv_refill, bool has) {
+  __device__ __forceinline__ void release(const LevelRec *, const LevelRec *lv_refill, bool has) {
     __syncwarp();
     if (lane == 0 && has) fill(kc % RING, lv_refill);
     ++kc;
   }
-};
-
-// ROWS = 2: per-lane asynchronous copies (cp.async, SASS LDGSTS): every lane copies its own PPT values of each corner
-// row of the NEXT iteration's levels into its own slots of a one-stage per-warp buffer, right after it has consumed
-// this iteration's rows; no other lane touches those slots, so no barrier is involved -- only cp.async.wait_group.
-// Against ROWS = 0 this frees the 8 PPT DEPTH prefetch registers and the moves that rotate them.
-template <int PPT, int DEPTH> struct Feed<PPT, DEPTH, 2> {
-  const double *slot;      // this lane's first slot (generic address); row r of level d at slot + (d * 4 + r) * 32 * PPT
-  uint32_t slot_s;
-  const double *lnk_pt;
-  const LevelRec *lv0, *lv_pending;
-  __device__ __forceinline__ void issue(const LevelRec *lv) {
-#pragma unroll
-    for (int d = 0; d < DEPTH; ++d) {
-      const LevelRec *q = lv - d;
-      q = q < lv0 ? lv0 : q;
-      const uint4 o = *reinterpret_cast<const uint4 *>(&q->o00);
-      const unsigned off[4] = {o.x, o.y, o.z, o.w};
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const double *src = elem_addr(lnk_pt, off[c]);
-        const uint32_t dst = slot_s + (uint32_t)((d * 4 + c) * 32 * PPT * 8);
-        if (PPT == 1) {
-          asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-        } else {
-#pragma unroll
-          for (int h = 0; h < PPT / 2; ++h)
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 16 * h), "l"(src + 2 * h) : "memory");
-        }
-      }
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");
-  }
-  __device__ __forceinline__ void prime(const LevelRec *lv, int) {
-    asm volatile("cp.async.wait_group 0;" ::: "memory");   // the previous column's last (unused) prefetch has landed
-    issue(lv);
-  }
-  __device__ __forceinline__ void next(RowsT<PPT> (&cur)[DEPTH], const LevelRec *lv_next) {
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-#pragma unroll
-    for (int d = 0; d < DEPTH; ++d) {
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const double *a = slot + (d * 4 + c) * 32 * PPT;
-        if (PPT == 1) {
-          cur[d].v[c][0] = *a;
-        } else {
-#pragma unroll
-          for (int h = 0; h < PPT / 2; ++h) {
-            const double2 t = reinterpret_cast<const double2 *>(a)[h];
-            cur[d].v[c][2 * h] = t.x;
-            cur[d].v[c][2 * h + 1] = t.y;
-          }
-        }
-      }
-    }
-    lv_pending = lv_next;
-  }
-  // call once this iteration's rows have been used (their shared-memory loads have completed)
-  __device__ __forceinline__ void release(const LevelRec *, bool) { issue(lv_pending); }
 };
 
 // sum over the warp's lanes of the 8 staged rows (one per interface); row k of the tile belongs to interface
@@ -530,35 +444,54 @@ __device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, 
   __syncwarp();
 }
 
-// back-substitution coefficients of one interface, one warp: 96 PPT doubles.  PPT = 1: [c][W d][R] x 32 lanes;
-// PPT >= 2: 16-byte slots [q: (c, W d)] x 32 lanes, then [h: (R_2h, R_2h+1)] x 32 lanes.  L2 only (.cg).
+// Back-substitution workspace of one warp: rows of 96 PPT doubles, row stride compile-time (immediate offsets).
+// Row i holds (c_i, W d_i) of interface i [F_up[i] = c_i F_up[i-1] + d_i] and R_{i-1} [F_dn = R F_up + U at interface
+// i-1]: the sweep stores R after the layer update, so no copy of the old R is kept.  PPT = 1: [c][W d][R] x 32 lanes;
+// PPT >= 2: 16-byte slots [q: (c, W d)] x 32 lanes, then [h: (R_2h, R_2h+1)] x 32 lanes.  L2 only (.cg).  Rows
+// N+1 .. LP hold the identity (c = 1, W d = 0, R = 0), written once by stack_init_kernel and never discarded: sweep 2
+// runs over whole groups of 8 interfaces with no per-interface test, and R_N = 0 comes from row N+1.
 template <int PPT>
-__device__ __forceinline__ void stk_store(double *w, int lane, const double (&c)[PPT], const double (&wd)[PPT],
+__device__ __forceinline__ void stk_store(double *row, int lane, const double (&c)[PPT], const double (&wd)[PPT],
                                           const double (&R)[PPT]) {
   if (PPT == 1) {
-    __stcg(w + lane, c[0]);
-    __stcg(w + 32 + lane, wd[0]);
-    __stcg(w + 64 + lane, R[0]);
+    __stcg(row + lane, c[0]);
+    __stcg(row + 32 + lane, wd[0]);
+    __stcg(row + 64 + lane, R[0]);
   } else {
-    double2 *v = reinterpret_cast<double2 *>(w) + lane;
+    double2 *v = reinterpret_cast<double2 *>(row) + lane;
 #pragma unroll
     for (int q = 0; q < PPT; ++q) __stcg(v + q * 32, make_double2(c[q], wd[q]));
 #pragma unroll
     for (int h = 0; h < PPT / 2; ++h) __stcg(v + (PPT + h) * 32, make_double2(R[2 * h], R[2 * h + 1]));
   }
 }
+// (c, W d) of row `row`, R of the row after it
 template <int PPT>
-__device__ __forceinline__ void stk_load(const double *w, int lane, double (&c)[PPT], double (&wd)[PPT], double (&R)[PPT]) {
+__device__ __forceinline__ void stk_load(const double *row, int lane, double (&c)[PPT], double (&wd)[PPT], double (&R)[PPT]) {
+  const double *rowR = row + 96 * PPT;
   if (PPT == 1) {
-    c[0] = __ldcg(w + lane);
-    wd[0] = __ldcg(w + 32 + lane);
-    R[0] = __ldcg(w + 64 + lane);
+    c[0] = __ldcg(row + lane);
+    wd[0] = __ldcg(row + 32 + lane);
+    R[0] = __ldcg(rowR + 64 + lane);
   } else {
-    const double2 *v = reinterpret_cast<const double2 *>(w) + lane;
+    const double2 *v = reinterpret_cast<const double2 *>(row) + lane;
+    const double2 *vR = reinterpret_cast<const double2 *>(rowR) + lane;
 #pragma unroll
     for (int q = 0; q < PPT; ++q) { const double2 t = __ldcg(v + q * 32); c[q] = t.x; wd[q] = t.y; }
 #pragma unroll
-    for (int h = 0; h < PPT / 2; ++h) { const double2 t = __ldcg(v + (PPT + h) * 32); R[2 * h] = t.x; R[2 * h + 1] = t.y; }
+    for (int h = 0; h < PPT / 2; ++h) { const double2 t = __ldcg(vR + (PPT + h) * 32); R[2 * h] = t.x; R[2 * h + 1] = t.y; }
+  }
+}
+
+// identity rows of the back-substitution workspace (whole workspace, once per launch shape)
+__global__ void stack_init_kernel(double *stk, size_t n_rows, int ppt) {
+  const size_t rowlen = (size_t)96 * ppt, n = n_rows * rowlen;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t k = i % rowlen;
+    double v;
+    if (ppt == 1) v = k < 32 ? 1.0 : 0.0;
+    else v = (k < (size_t)64 * ppt && (k & 1) == 0) ? 1.0 : 0.0;     // (c, W d) pairs, then R pairs
+    stk[i] = v;
   }
 }
 
@@ -769,14 +702,12 @@ __device__ __forceinline__ void column_epilogue(const KParams &P, const Lay &L, 
 //   PPT     adjacent spectral points of one bin per thread (n_gauss must be a multiple): everything that depends only
 //           on (column, level, bin) is issued once for the group and its PPT dependence chains interleave (ILP)
 //   ROWS    0: k-table rows by register-prefetched loads; 1: by bulk async copies (TMA) into the per-warp ring
-//   STK     back-substitution coefficients: 1 = per-block slab of the global workspace (L2), 0 = thread-private
-//           local memory (kept for comparison builds; SCAP = its capacity in interfaces)
 //   BDIRECT one Gauss point per bin (opacity sampling, L385): every thread has its own bin, so the Planck values are
 //           read coalesced from the workspace instead of being staged (64 KB per block otherwise); PPT = 1
 //   WARPS   warps per block as a compile-time constant, or 0 = taken from the launch
 //   MAXT, MINB  launch bounds (register cap = 65536 / (MAXT MINB)); any block of <= MAXT threads may be launched
 // --------------------------------------------------------------------------------------------
-template <bool NONISO, bool TOA, int PPT, int ROWS, int STK, int SCAP, bool BDIRECT, int WARPS, int MAXT, int MINB>
+template <bool NONISO, bool TOA, int PPT, int ROWS, bool BDIRECT, int WARPS, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   static_assert(PPT == 1 || PPT == 2 || PPT == 4, "points per thread");
   static_assert(!BDIRECT || PPT == 1, "one Gauss point per bin: one point per thread");
@@ -856,11 +787,6 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   Feed<PPT, DEPTH, ROWS> feed;
   if constexpr (ROWS == 0) {
     feed.lnk_pt = P.lnk + pt;
-  } else if constexpr (ROWS == 2) {
-    unsigned char *slot = smem + L.off_u + L.u_ring + (size_t)warp * L.ring_warp + (size_t)lane * PPT * 8;
-    feed.slot = (const double *)slot;
-    feed.slot_s = smem_u32(slot);
-    feed.lnk_pt = P.lnk + pt;
   } else {
     unsigned char *ring = smem + L.off_u + L.u_ring + (size_t)warp * L.ring_warp;
     feed.ring = (const double *)ring;
@@ -871,11 +797,11 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
     feed.lane = lane;
   }
 
-  // this block's slab of the back-substitution workspace: [interface][warp][96 PPT]
-  const size_t istride = (size_t)nwarps * 96 * PPT;
+  // this block's slab of the back-substitution workspace: [warp][LP + 1 rows][96 PPT]
+  constexpr int SROW = 96 * PPT;            // doubles per row
   double *stk_w = nullptr;
-  if (STK == 1 && !TOA)
-    stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * 96 * PPT;
+  if (!TOA)
+    stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * (LP + 1) * SROW;
 
   // ---------------- phase B: columns of this tile's queue ----------------
   // The record block and the tile's Planck block of the NEXT column are fetched by bulk async copies (TMA) into the
@@ -944,9 +870,6 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
 
       // back-substitution state per interface i = 0..N: F_up[i] = c F_up[i-1] + d (weight folded into d) and R with
       // F_dn[i] = R F_up[i] + U.  U itself is not kept: sum_points W (U + beam) is reduced on the way down.
-      double2 l_cd[(STK == 0 && !TOA) ? SCAP : 1][PPT];
-      double l_R[(STK == 0 && !TOA) ? SCAP : 1][PPT];
-
       double R[PPT], U[PPT], Fb[PPT], Ct[PPT], Dt[PPT];
 #pragma unroll
       for (int q = 0; q < PPT; ++q) {
@@ -969,14 +892,10 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
           }
         }
       };
-      auto keep = [&](int i, const double (&c)[PPT], const double (&wd)[PPT], const double (&Ri)[PPT]) {
+      // row i of the workspace: (c_i, W d_i) and R_{i-1}, the R just updated by the layer below interface i
+      auto keep = [&](int i, const double (&c)[PPT], const double (&wd)[PPT], const double (&Rlow)[PPT]) {
         if (TOA) return;
-        if (STK == 1) {
-          stk_store<PPT>(stk_w + (size_t)i * istride, lane, c, wd, Ri);
-        } else {
-#pragma unroll
-          for (int q = 0; q < PPT; ++q) { l_cd[STK == 0 && !TOA ? i : 0][q] = make_double2(c[q], wd[q]); l_R[STK == 0 && !TOA ? i : 0][q] = Ri[q]; }
-        }
+        stk_store<PPT>(stk_w + (size_t)i * SROW, lane, c, wd, Rlow);
       };
 
       // ---------------- sweep 1: TOA -> BOA (one instantiation per day / night: the loop body has no branch) ------
@@ -991,8 +910,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
           feed.prime(lv, N);
           HRT_UNROLL(HRT_UNROLL_ISO)
           for (int j = N - 1; j >= 0; --j, --lv, Bp -= nbtS) {
-            RowsT<PPT> cur[1];
-            feed.next(cur, lv - 1);
+            const RowsT<PPT> *cur = feed.next();
             push_stage(j + 1);
             // S3 + Eqs. 17-18 for the group: shared corner weights and bin constants
             const double2 ca = *reinterpret_cast<const double2 *>(&lv->c00);
@@ -1005,8 +923,8 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
 #pragma unroll
             for (int q = 0; q < PPT; ++q)
               lk[q] = fma(cb.y, cur[0].v[3][q], fma(cb.x, cur[0].v[2][q], fma(ca.y, cur[0].v[1][q], ca.x * cur[0].v[0][q])));
-            feed.release(lv - RING, j - RING >= 0);
-            double cc[PPT], wd[PPT], Ro[PPT];
+            feed.release(lv - 1, lv - RING, j - RING >= 0);
+            double cc[PPT], wd[PPT];
 #pragma unroll
             for (int q = 0; q < PPT; ++q) {
               const double kx = exp_hot<0, false>(lk[q], T32, nullptr) + sbss.x;
@@ -1015,10 +933,9 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
               double Fa = 0.0;
               if (DAY) {
                 tau[q] += dtau;
-                Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);   // (B6)
+                Fa = muF * exp_hot<1, false>(cap_pos<0x40862000>(tau[q] * inv_mu), T32, nullptr);   // (B6)
               }
               double c, d;
-              Ro[q] = R[q];
               layer_forward<DAY, false>(P, T32, w0, gt, dtau, Bj, Bj, mu, Fa, Fb[q], R[q], U[q], c, d);
               Fb[q] = Fa;
               if (TOA) {
@@ -1028,7 +945,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
               cc[q] = c;
               wd[q] = W[q] * d;
             }
-            keep(j + 1, cc, wd, Ro);
+            keep(j + 1, cc, wd, R);
           }
         } else {
           // levels alternate interface (even) / centre (odd); sub-layer s lies between levels s and s+1 and takes
@@ -1059,17 +976,16 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
           feed.prime(lv - 1, N);
 #pragma unroll 1
           for (int j = N - 1; j >= 0; --j, lv -= 2, Bp -= 2 * nbtS) {
-            RowsT<PPT> cur[2];      // [0] centre (lv - 1), [1] lower interface (lv - 2)
-            feed.next(cur, lv - 3);
+            const RowsT<PPT> *cur = feed.next();      // [0] centre (lv - 1), [1] lower interface (lv - 2)
             push_stage(j + 1);
             double kx_c[PPT], w0_c[PPT], g0_c, kx_lo[PPT], w0_lo[PPT], g0_lo;
             optics(cur[0], lv - 1, kx_c, w0_c, g0_c);
             optics(cur[1], lv - 2, kx_lo, w0_lo, g0_lo);
-            feed.release(lv - 1 - 2 * RING, j - RING >= 0);
+            feed.release(lv - 3, lv - 1 - 2 * RING, j - RING >= 0);
             const double B_c = Bp[-nbtS], B_lo = Bp[-2 * nbtS];
             const double dm_u = lv[-1].dm, dm_l = lv[-2].dm;
             const G0Terms gt_u = g0_terms(0.5 * (g0_c + g0_up), P.inv_eps2), gt_l = g0_terms(0.5 * (g0_lo + g0_c), P.inv_eps2);
-            double cc[PPT], wd[PPT], Ro[PPT];
+            double cc[PPT], wd[PPT];
 #pragma unroll
             for (int q = 0; q < PPT; ++q) {
               const double dtau_u = 0.5 * (kx_c[q] + kx_up[q]) * dm_u;
@@ -1078,11 +994,10 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
               if (DAY) {
                 const double tau_c = tau[q] + dtau_u;
                 tau[q] = tau_c + dtau_l;
-                Fc = muF * exp_hot<1, false>(min_pos(tau_c * inv_mu, 708.0), T32, nullptr);   // (B6)
-                Fa = muF * exp_hot<1, false>(min_pos(tau[q] * inv_mu, 708.0), T32, nullptr);
+                Fc = muF * exp_hot<1, false>(cap_pos<0x40862000>(tau_c * inv_mu), T32, nullptr);   // (B6)
+                Fa = muF * exp_hot<1, false>(cap_pos<0x40862000>(tau[q] * inv_mu), T32, nullptr);
               }
               double cu, du, cl, dl;
-              Ro[q] = R[q];
               layer_forward<DAY, true>(P, T32, 0.5 * (w0_c[q] + w0_up[q]), gt_u, dtau_u, B_c, B_up, mu, Fc, Fb[q],
                                        R[q], U[q], cu, du);
               layer_forward<DAY, true>(P, T32, 0.5 * (w0_lo[q] + w0_c[q]), gt_l, dtau_l, B_lo, B_c, mu, Fa, Fc,
@@ -1098,7 +1013,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
               wd[q] = W[q] * d2;
             }
             g0_up = g0_lo; B_up = B_lo;
-            keep(j + 1, cc, wd, Ro);
+            keep(j + 1, cc, wd, R);
           }
         }
       };
@@ -1126,97 +1041,37 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         double wF[PPT];
 #pragma unroll
         for (int q = 0; q < PPT; ++q) wF[q] = 0.0;
-        // The coefficients come back from L2 (several hundred cycles).  Comparison builds (HRT_S2_PF=1) load a group
-        // of 4 interfaces while the previous group is used (two register buffers); it costs registers in sweep 1 and
-        // loses, so 8 interfaces are loaded at a time.
-        constexpr int G = 4;
-#ifndef HRT_S2_PF
-#define HRT_S2_PF 0   /* measured (config 2, same box): 0.739 ms without, 0.784 ms with the two-buffer prefetch */
-#endif
-        constexpr bool PF = (PPT <= 2) && (HRT_S2_PF != 0);
-        double gc[PF ? 2 : 1][PF ? G : 8][PPT], gwd[PF ? 2 : 1][PF ? G : 8][PPT], gR[PF ? 2 : 1][PF ? G : 8][PPT];
-        auto load_one = [&](int bsel, int k, int i) {
-          if (i <= N) {
-            if (STK == 1) {
-              stk_load<PPT>(stk_w + (size_t)i * istride, lane, gc[bsel][k], gwd[bsel][k], gR[bsel][k]);
-            } else {
-#pragma unroll
-              for (int q = 0; q < PPT; ++q) {
-                const double2 a = l_cd[STK == 0 ? i : 0][q];
-                gc[bsel][k][q] = a.x; gwd[bsel][k][q] = a.y; gR[bsel][k][q] = l_R[STK == 0 ? i : 0][q];
-              }
-            }
-          } else {
-            // beyond the top: repeat F_up[N] into rows of the reduction buffer that are never read
-#pragma unroll
-            for (int q = 0; q < PPT; ++q) { gc[bsel][k][q] = 1.0; gwd[bsel][k][q] = 0.0; gR[bsel][k][q] = 0.0; }
-          }
-        };
-#ifdef HRT_S2_BUTTERFLY
-        double v16[16];     // sums over the thread's points of W F_up (rows 0..7) and of W R F_up (rows 8..15)
-#else
-        double sd[8];
-#endif
-        auto use_one = [&](int bsel, int k, int row) {
-          double su = 0.0, s2 = 0.0;
-#pragma unroll
-          for (int q = 0; q < PPT; ++q) {
-            wF[q] = fma(gc[bsel][k][q], wF[q], gwd[bsel][k][q]);
-            su += wF[q];
-            s2 = fma(gR[bsel][k][q], wF[q], s2);
-          }
-#ifdef HRT_S2_BUTTERFLY
-          v16[row] = su;
-          v16[8 + row] = s2;
-#else
-          stage_wr[row * STAGE_LD] = su;
-          sd[row] = s2;
-#endif
-        };
-        if (PF) {
-#pragma unroll
-          for (int k = 0; k < G; ++k) load_one(0, k, k);
-        }
+        // The coefficients come back from L2 (several hundred cycles): the 8 interfaces of a group are loaded at once
+        // (immediate offsets from one row pointer), then used.  Rows above N hold the identity, so the last group needs
+        // no test: it repeats F_up[N] into rows of the reduction buffer that are never read.  (Measured and rejected,
+        // a two-buffer prefetch of the next group, a butterfly instead of the staged transposes.)
+        const double *row = stk_w;
 #pragma unroll 1
-        for (int base = 0; base <= N; base += 8) {
-          if (PF) {
+        for (int base = 0; base <= N; base += 8, row += 8 * SROW) {
+          double gc[8][PPT], gwd[8][PPT], gR[8][PPT], sd[8];
 #pragma unroll
-            for (int k = 0; k < G; ++k) load_one(1, k, base + G + k);
+          for (int k = 0; k < 8; ++k) stk_load<PPT>(row + k * SROW, lane, gc[k], gwd[k], gR[k]);
 #pragma unroll
-            for (int k = 0; k < G; ++k) use_one(0, k, k);
+          for (int k = 0; k < 8; ++k) {
+            double su = 0.0, s2 = 0.0;
 #pragma unroll
-            for (int k = 0; k < G; ++k) load_one(0, k, base + 2 * G + k);
-#pragma unroll
-            for (int k = 0; k < G; ++k) use_one(1, k, G + k);
-          } else {
-#pragma unroll
-            for (int k = 0; k < 8; ++k) load_one(0, k, base + k);
-#pragma unroll
-            for (int k = 0; k < 8; ++k) use_one(0, k, k);
+            for (int q = 0; q < PPT; ++q) {
+              wF[q] = fma(gc[k][q], wF[q], gwd[k][q]);
+              su += wF[q];
+              s2 = fma(gR[k][q], wF[q], s2);
+            }
+            stage_wr[k * STAGE_LD] = su;
+            sd[k] = s2;
           }
-#ifdef HRT_S2_BUTTERFLY
-          {
-            // one recursive-halving butterfly for the 16 values of the 8 interfaces
-            const double tot = warp_reduce16(v16, lane);
-            const int idx = lane >> 1;
-            if (!(lane & 1)) red_w[(idx >> 3) * LP + base + (idx & 7)] = tot;
-          }
-#else
           flush_stage(stage_w, red_w + base, lane);
 #pragma unroll
           for (int k = 0; k < 8; ++k) stage_wr[k * STAGE_LD] = sd[k];
           flush_stage(stage_w, red_w + LP + base, lane);
-#endif
-          if (STK == 1) {
-            // the coefficients of these interfaces are dead: drop their lines from L2 instead of writing them back
-            int n_if = N + 1 - base;
-            n_if = n_if > 8 ? 8 : n_if;
-            const int lines_if = 6 * PPT;               // 96 PPT doubles per interface and warp
-            for (int ln = lane; ln < n_if * lines_if; ln += 32) {
-              const int k = ln / lines_if, r = ln - k * lines_if;
-              l2_discard(stk_w + (size_t)(base + k) * istride + r * 16);
-            }
-          }
+          // rows base .. base+7 are dead (the R part of row base+8 is not: next group's discard): drop the lines of the
+          // real rows from L2 instead of writing them back
+          int n_lines = (N + 1 - base) * (SROW / 16);
+          n_lines = n_lines > 8 * (SROW / 16) ? 8 * (SROW / 16) : n_lines;
+          for (int ln = lane; ln < n_lines; ln += 32) l2_discard(row + ln * 16);
         }
         if (P.F_toa_bin != nullptr) {
 #pragma unroll
@@ -1360,7 +1215,7 @@ __global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int
           double Fa = 0.0;
           if (DAY) {
             tau += dtau;
-            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
+            Fa = muF * exp_hot<1, false>(cap_pos<0x40862000>(tau * inv_mu), T32, nullptr);
           }
           layer_coeffs<DAY, false>(P, T32, w0, g0_terms(g0, P.inv_eps2), dtau, Bj, Bj, mu, Fa, Fb, a_t[j], a_r[j], a_su[j], a_sd[j]);
           bm[j] = Fa;
@@ -1379,7 +1234,7 @@ __global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int
           double Fa = 0.0;
           if (DAY) {
             tau += dtau;
-            Fa = muF * exp_hot<1, false>(min_pos(tau * inv_mu, 708.0), T32, nullptr);
+            Fa = muF * exp_hot<1, false>(cap_pos<0x40862000>(tau * inv_mu), T32, nullptr);
           }
           layer_coeffs<DAY, true>(P, T32, 0.5 * (w0_lo + w0_up), g0_terms(0.5 * (g0_lo + g0_up), P.inv_eps2), dtau, B_lo, B_up,
                                   mu, Fa, Fb, a_t[sl], a_r[sl], a_su[sl], a_sd[sl]);
@@ -1438,16 +1293,16 @@ typedef void (*kernel_fn)(const KParams);
 
 struct Variant {
   bool noniso, toa, bdirect;
-  int ppt, rows, stk, scap, warps;   // warps: block size compiled in, 0 = any   // scap: capacity (interfaces) of the local-memory stack of the STK = 0 comparison builds
+  int ppt, rows, warps;   // warps: block size compiled in, 0 = any
   int maxt, minb;      // launch bounds: register cap = 65536 / (maxt * minb)
   kernel_fn fn;
 };
 
-#define HRT_K(NI, TOA, PPT, ROWS, STK, SCAP, WARPS, MAXT, MINB) \
-  {NI, TOA, false, PPT, ROWS, STK, SCAP, WARPS, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, STK, SCAP, false, WARPS, MAXT, MINB>}
+#define HRT_K(NI, TOA, PPT, ROWS, WARPS, MAXT, MINB) \
+  {NI, TOA, false, PPT, ROWS, WARPS, MAXT, MINB, rt_step_kernel<NI, TOA, PPT, ROWS, false, WARPS, MAXT, MINB>}
 // one Gauss point per bin (opacity sampling): Planck values read from the workspace; one point per thread
 #define HRT_KB(NI, TOA, ROWS, WARPS, MAXT, MINB) \
-  {NI, TOA, true, 1, ROWS, 1, 1, WARPS, MAXT, MINB, rt_step_kernel<NI, TOA, 1, ROWS, 1, 1, true, WARPS, MAXT, MINB>}
+  {NI, TOA, true, 1, ROWS, WARPS, MAXT, MINB, rt_step_kernel<NI, TOA, 1, ROWS, true, WARPS, MAXT, MINB>}
 
 // Compiled instantiations, in order of preference for each (noniso, toa, ppt).  helios_rt_create takes the first
 // match; helios_rt_debug_set_launch (tests, tuning) may select any other.
@@ -1652,7 +1507,6 @@ static int configure_launch(helios_rt *h) {
   const int N = c.n_layers;
   h->ppt = v.ppt;
   if (h->warps * 32 > v.maxt || (v.warps != 0 && v.warps != h->warps)) return HELIOS_RT_EINVAL;
-  if (!h->toa && v.stk == 0 && N + 1 > v.scap) return HELIOS_RT_EINVAL;
   const int tp = h->warps * 32 * h->ppt;
   h->tiles = (h->npt + tp - 1) / tp;
   h->lay = make_lay(N, h->nlev, h->warps, h->ppt, c.n_gauss, c.n_bins, h->toa, h->noniso ? 2 : 1, v.rows, v.bdirect);
@@ -1698,9 +1552,15 @@ static int configure_launch(helios_rt *h) {
       rc = build_slots(h, h->iter_warps * 32, h->iter_lay, h->inv_dlam, &h->d_slot_ptr_iter, &h->d_slots_iter, &h->d_bslot_iter);
     if (rc) return rc;
   }
-  h->stack_block = (size_t)(N + 1) * h->warps * 96 * h->ppt;
-  h->stack_bytes = (!h->toa && v.stk == 1) ? sizeof(double) * h->stack_block * h->tiles * h->workers : 0;
-  if (h->stack_bytes) CK(h, cudaMalloc((void **)&h->d_stack, h->stack_bytes));
+  // back-substitution workspace: per block [warp][LP + 1 rows][96 ppt]; rows above N stay the identity for good
+  h->stack_block = (size_t)(h->lay.LP + 1) * h->warps * 96 * h->ppt;
+  h->stack_bytes = !h->toa ? sizeof(double) * h->stack_block * h->tiles * h->workers : 0;
+  if (h->stack_bytes) {
+    CK(h, cudaMalloc((void **)&h->d_stack, h->stack_bytes));
+    stack_init_kernel<<<h->sm_count * 8, 256>>>(h->d_stack, h->stack_bytes / (sizeof(double) * 96 * h->ppt), h->ppt);
+    CK(h, cudaGetLastError());
+    CK(h, cudaDeviceSynchronize());
+  }
   const int mt = h->tiles > h->iter_tiles ? h->tiles : h->iter_tiles;
   h->partial_bytes = sizeof(double) * (size_t)c.max_columns * mt * 4 * (N + 1);
   CK(h, cudaMalloc((void **)&h->d_partial, h->partial_bytes));
@@ -1717,7 +1577,7 @@ static int find_variant(bool noniso, bool toa, bool bdirect, int ppt, int rows, 
     if (v.noniso != noniso || v.toa != toa || v.bdirect != bdirect || v.ppt != ppt) continue;
     if (pass == 0 ? v.warps != warps : v.warps != 0) continue;
     if (rows >= 0 && v.rows != rows) continue;
-    if (stk >= 0 && !toa && v.stk != stk) continue;
+    if (stk == 0) continue;   // the thread-private stack of round 1 is gone
     if (maxt >= 0 && v.maxt != maxt) continue;
     if (minb >= 0 && v.minb != minb) continue;
     return i;
@@ -1874,8 +1734,8 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.ncol = in->n_columns;
   P.row_stride = h->row_stride; P.inv_dlp = h->inv_dlp; P.inv_dt = h->inv_dt;
   P.cloud_p_top = c.cloud_p_top; P.cloud_p_bot = c.cloud_p_bot; P.inv_g = 1.0 / c.gravity; P.inv_cp = 1.0 / c.cp;
-  P.inv_eps2 = 1.0 / c.eps2; P.e_tau = c.e_tau; P.gcrit_tol = c.gcrit_tol; P.w0_transition = c.w0_transition;
-  P.f_toa = c.f_toa; P.improved = (c.flags & HELIOS_RT_IMPROVED) ? 1 : 0;
+  P.inv_eps2 = 1.0 / c.eps2; P.e_tau = c.e_tau; P.gcrit_tol = c.gcrit_tol; P.w0_transition = (c.flags & HELIOS_RT_IMPROVED) ? c.w0_transition : INFINITY;   // regular two-stream: E = 1
+  P.f_toa = c.f_toa;
   P.p = in->p; P.T = in->T; P.mu = in->mu_star; P.fstar = in->stellar_flux;
   P.T_int = in->f_internal > 0 ? sqrt(sqrt(in->f_internal / kSigmaSB)) : 0.0;
   P.F_up = out->F_up; P.F_down = out->F_down; P.F_net = out->F_net; P.dTdt = out->dTdt; P.F_beam = out->F_beam;
@@ -2029,7 +1889,7 @@ extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t p
 extern "C" int helios_rt_debug_get_launch(const helios_rt *h, int32_t info[16]) {
   if (!h || !info) return HELIOS_RT_EINVAL;
   const Variant &v = kVariants[h->variant];
-  info[0] = h->warps; info[1] = v.ppt; info[2] = v.rows; info[3] = v.stk; info[4] = v.maxt; info[5] = v.minb;
+  info[0] = h->warps; info[1] = v.ppt; info[2] = v.rows; info[3] = 1; info[4] = v.maxt; info[5] = v.minb;
   info[6] = h->tiles; info[7] = h->workers; info[8] = h->occ; info[9] = h->regs; info[10] = h->lmem;
   info[11] = (int32_t)h->lay.total; info[12] = (int32_t)(h->stack_bytes >> 20); info[13] = h->variant;
   info[14] = kNumVariants; info[15] = 0;

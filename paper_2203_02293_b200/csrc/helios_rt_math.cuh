@@ -48,6 +48,13 @@ __device__ __forceinline__ bool abs_lt(double a, double b_pos) {
 }
 // min(x, c) for x >= 0, c > 0 on the integer pipes
 __device__ __forceinline__ double min_pos(double x, double c) { return gt_pos(x, c) ? c : x; }
+// Cap of an exponential's argument, x >= 0, in ONE integer instruction: only the high word is limited to HI (the high
+// word of the cap c, whose low word is 0), so the result is x for x < c and lies in [c, c (1 + 2^-20)) beyond.  Used
+// where anything >= c gives e^-x = 0 to the last bit that matters (c = 354 for e^-2x, 708 for e^-x: >= 2^-1022).
+template <int HI>
+__device__ __forceinline__ double cap_pos(double x) {
+  return __hiloint2double(min(__double2hiint(x), HI), __double2loint(x));
+}
 
 // exp by table: e^x = 2^m T[j] (1 + p(r)), k = 32 m + j = round(32 x / ln 2), r = x - k ln2/32, |r| <= ln2/64,
 // T[j] = 2^(j/32) (32 doubles in shared memory), p = expm1(r) by its degree-6 Taylor polynomial (remainder
@@ -111,7 +118,7 @@ __device__ __forceinline__ double exp_hot(double x, const double *__restrict__ T
     p = fma(r * r, q, r);
   }
   const double Tj = T32[ki & 31];
-  const double Ts = __hiloint2double(__double2hiint(Tj) + ((ki >> 5) << 20), __double2loint(Tj));   // 2^m T[j]
+  const double Ts = __hiloint2double(__double2hiint(Tj) + (ki & ~31) * 32768, __double2loint(Tj));   // 2^m T[j]: (ki >> 5) << 20
   if (OM) *om = fma(-Ts, p, 1.0 - Ts);
   return fma(Ts, p, Ts);
 }
