@@ -118,7 +118,9 @@ __device__ __forceinline__ double exp_hot(double x, const double *__restrict__ T
     p = fma(r * r, q, r);
   }
   const double Tj = T32[ki & 31];
-  const double Ts = __hiloint2double(__double2hiint(Tj) + (ki & ~31) * 32768, __double2loint(Tj));   // 2^m T[j]: (ki >> 5) << 20
+  int hi;                                              // high word of 2^m T[j]: + ((ki >> 5) << 20), one LOP3 + one IMAD
+  asm("mad.lo.s32 %0, %1, 32768, %2;" : "=r"(hi) : "r"(ki & ~31), "r"(__double2hiint(Tj)));
+  const double Ts = __hiloint2double(hi, __double2loint(Tj));
   if (OM) *om = fma(-Ts, p, 1.0 - Ts);
   return fma(Ts, p, Ts);
 }
