@@ -449,12 +449,11 @@ __device__ __forceinline__ void flush_stage(const double *__restrict__ stage_w, 
   __syncwarp();
 }
 
-// Back-substitution workspace of one warp: rows of 96 PPT doubles, row stride compile-time (immediate offsets).
+// Back-substitution workspace of one warp: N + 1 rows of 96 PPT doubles, row stride compile-time (immediate offsets).
 // Row i holds (c_i, W d_i) of interface i [F_up[i] = c_i F_up[i-1] + d_i] and R_{i-1} [F_dn = R F_up + U at interface
-// i-1]: the sweep stores R after the layer update, so no copy of the old R is kept.  PPT = 1: [c][W d][R] x 32 lanes;
-// PPT >= 2: 16-byte slots [q: (c, W d)] x 32 lanes, then [h: (R_2h, R_2h+1)] x 32 lanes.  L2 only (.cg).  Rows
-// N+1 .. LP hold the identity (c = 1, W d = 0, R = 0), written once by stack_init_kernel and never discarded: sweep 2
-// runs over whole groups of 8 interfaces with no per-interface test, and R_N = 0 comes from row N+1.
+// i-1]: the sweep stores R after the layer update, so no copy of the old R is kept (R_N = 0 is not stored).
+// PPT = 1: [c][W d][R] x 32 lanes; PPT >= 2: 16-byte slots [q: (c, W d)] x 32 lanes, then [h: (R_2h, R_2h+1)] x 32
+// lanes.  L2 only (.cg).
 template <int PPT>
 __device__ __forceinline__ void stk_store(double *row, int lane, const double (&c)[PPT], const double (&wd)[PPT],
                                           const double (&R)[PPT]) {
@@ -470,33 +469,26 @@ __device__ __forceinline__ void stk_store(double *row, int lane, const double (&
     for (int h = 0; h < PPT / 2; ++h) __stcg(v + (PPT + h) * 32, make_double2(R[2 * h], R[2 * h + 1]));
   }
 }
-// (c, W d) of row `row`, R of the row after it
+// (c, W d) of a row / the R of a row
 template <int PPT>
-__device__ __forceinline__ void stk_load(const double *row, int lane, double (&c)[PPT], double (&wd)[PPT], double (&R)[PPT]) {
-  const double *rowR = row + 96 * PPT;
+__device__ __forceinline__ void stk_load_cw(const double *row, int lane, double (&c)[PPT], double (&wd)[PPT]) {
   if (PPT == 1) {
     c[0] = __ldcg(row + lane);
     wd[0] = __ldcg(row + 32 + lane);
-    R[0] = __ldcg(rowR + 64 + lane);
   } else {
     const double2 *v = reinterpret_cast<const double2 *>(row) + lane;
-    const double2 *vR = reinterpret_cast<const double2 *>(rowR) + lane;
 #pragma unroll
     for (int q = 0; q < PPT; ++q) { const double2 t = __ldcg(v + q * 32); c[q] = t.x; wd[q] = t.y; }
-#pragma unroll
-    for (int h = 0; h < PPT / 2; ++h) { const double2 t = __ldcg(vR + (PPT + h) * 32); R[2 * h] = t.x; R[2 * h + 1] = t.y; }
   }
 }
-
-// identity rows of the back-substitution workspace (whole workspace, once per launch shape)
-__global__ void stack_init_kernel(double *stk, size_t n_rows, int ppt) {
-  const size_t rowlen = (size_t)96 * ppt, n = n_rows * rowlen;
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const size_t k = i % rowlen;
-    double v;
-    if (ppt == 1) v = k < 32 ? 1.0 : 0.0;
-    else v = (k < (size_t)64 * ppt && (k & 1) == 0) ? 1.0 : 0.0;     // (c, W d) pairs, then R pairs
-    stk[i] = v;
+template <int PPT>
+__device__ __forceinline__ void stk_load_R(const double *row, int lane, double (&R)[PPT]) {
+  if (PPT == 1) {
+    R[0] = __ldcg(row + 64 + lane);
+  } else {
+    const double2 *v = reinterpret_cast<const double2 *>(row) + lane;
+#pragma unroll
+    for (int h = 0; h < PPT / 2; ++h) { const double2 t = __ldcg(v + (PPT + h) * 32); R[2 * h] = t.x; R[2 * h + 1] = t.y; }
   }
 }
 
@@ -802,11 +794,11 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
     feed.lane = lane;
   }
 
-  // this block's slab of the back-substitution workspace: [warp][LP + 1 rows][96 PPT]
+  // this block's slab of the back-substitution workspace: [warp][N + 1 rows][96 PPT]
   constexpr int SROW = 96 * PPT;            // doubles per row
   double *stk_w = nullptr;
   if (!TOA)
-    stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * (LP + 1) * SROW;
+    stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * (N + 1) * SROW;
 
   // ---------------- phase B: columns of this tile's queue ----------------
   // The record block and the tile's Planck block of the NEXT column are fetched by bulk async copies (TMA) into the
@@ -1048,15 +1040,28 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
 #pragma unroll
         for (int q = 0; q < PPT; ++q) wF[q] = 0.0;
         // The coefficients come back from L2 (several hundred cycles): the 8 interfaces of a group are loaded at once
-        // (immediate offsets from one row pointer), then used.  Rows above N hold the identity, so the last group needs
-        // no test: it repeats F_up[N] into rows of the reduction buffer that are never read.  (Measured and rejected,
-        // a two-buffer prefetch of the next group, a butterfly instead of the staged transposes.)
+        // (immediate offsets from one row pointer), then used.  Whole groups need no test; the last group (1..8
+        // interfaces, R_N = 0) tests per interface, uniformly, and repeats F_up[N] into rows of the reduction buffer
+        // that are never read.  (Measured and rejected: a two-buffer prefetch of the next group,
+        // a butterfly instead of the staged transposes.)
         const double *row = stk_w;
-#pragma unroll 1
-        for (int base = 0; base <= N; base += 8, row += 8 * SROW) {
+        auto group = [&](auto full_tag, int base) {
+          constexpr bool FULL = decltype(full_tag)::value;
+          const int nk = N + 1 - base;          // interfaces left (FULL: > 8)
           double gc[8][PPT], gwd[8][PPT], gR[8][PPT], sd[8];
 #pragma unroll
-          for (int k = 0; k < 8; ++k) stk_load<PPT>(row + k * SROW, lane, gc[k], gwd[k], gR[k]);
+          for (int k = 0; k < 8; ++k) {
+            if (FULL || k < nk) stk_load_cw<PPT>(row + k * SROW, lane, gc[k], gwd[k]);
+            else {
+#pragma unroll
+              for (int q = 0; q < PPT; ++q) { gc[k][q] = 1.0; gwd[k][q] = 0.0; }
+            }
+            if (FULL || k < nk - 1) stk_load_R<PPT>(row + (k + 1) * SROW, lane, gR[k]);
+            else {
+#pragma unroll
+              for (int q = 0; q < PPT; ++q) gR[k][q] = 0.0;
+            }
+          }
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
             double su = 0.0, s2 = 0.0;
@@ -1073,12 +1078,15 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
 #pragma unroll
           for (int k = 0; k < 8; ++k) stage_wr[k * STAGE_LD] = sd[k];
           flush_stage(stage_w, red_w + LP + base, lane);
-          // rows base .. base+7 are dead (the R part of row base+8 is not: next group's discard): drop the lines of the
-          // real rows from L2 instead of writing them back
-          int n_lines = (N + 1 - base) * (SROW / 16);
-          n_lines = n_lines > 8 * (SROW / 16) ? 8 * (SROW / 16) : n_lines;
+          // rows base .. base+7 are dead (the R part of row base+8 is not: next group's discard): drop their lines from
+          // L2 instead of writing them back
+          const int n_lines = (FULL ? 8 : nk) * (SROW / 16);
           for (int ln = lane; ln < n_lines; ln += 32) l2_discard(row + ln * 16);
-        }
+        };
+        int base = 0;
+#pragma unroll 1
+        for (; base + 8 <= N; base += 8, row += 8 * SROW) group(std::true_type{}, base);
+        group(std::false_type{}, base);
         if (P.F_toa_bin != nullptr) {
 #pragma unroll
           for (int q = 0; q < PPT; ++q) s_vals[PPT * tid + q] = active ? wF[q] * P.bins[b].inv_dlam : 0.0;
@@ -1558,15 +1566,10 @@ static int configure_launch(helios_rt *h) {
       rc = build_slots(h, h->iter_warps * 32, h->iter_lay, h->inv_dlam, &h->d_slot_ptr_iter, &h->d_slots_iter, &h->d_bslot_iter);
     if (rc) return rc;
   }
-  // back-substitution workspace: per block [warp][LP + 1 rows][96 ppt]; rows above N stay the identity for good
-  h->stack_block = (size_t)(h->lay.LP + 1) * h->warps * 96 * h->ppt;
+  // back-substitution workspace: per block [warp][N + 1 rows][96 ppt]
+  h->stack_block = (size_t)(N + 1) * h->warps * 96 * h->ppt;
   h->stack_bytes = !h->toa ? sizeof(double) * h->stack_block * h->tiles * h->workers : 0;
-  if (h->stack_bytes) {
-    CK(h, cudaMalloc((void **)&h->d_stack, h->stack_bytes));
-    stack_init_kernel<<<h->sm_count * 8, 256>>>(h->d_stack, h->stack_bytes / (sizeof(double) * 96 * h->ppt), h->ppt);
-    CK(h, cudaGetLastError());
-    CK(h, cudaDeviceSynchronize());
-  }
+  if (h->stack_bytes) CK(h, cudaMalloc((void **)&h->d_stack, h->stack_bytes));
   const int mt = h->tiles > h->iter_tiles ? h->tiles : h->iter_tiles;
   h->partial_bytes = sizeof(double) * (size_t)c.max_columns * mt * 4 * (N + 1);
   CK(h, cudaMalloc((void **)&h->d_partial, h->partial_bytes));
