@@ -123,9 +123,11 @@ int helios_rt_create(const helios_rt_config *cfg, helios_rt **out);
 int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
                    void *cuda_stream);
 
-/* Same step with HOST buffers (pinned memory recommended): copies the inputs to device staging
- * owned by the handle, runs the step, copies the requested outputs back and synchronises.  This is
- * the end-to-end path bench.py times ("e2e"). */
+/* Same step with HOST buffers: copies the inputs to device staging owned by the handle, runs the step on the
+ * handle's own stream and synchronises.  Output buffers that are page-locked and mapped (cudaHostAlloc /
+ * cudaHostRegister memory) are written by the kernel directly, column by column while the step runs; pageable ones
+ * (and a per-bin spectrum whose bins straddle thread-block tiles) are staged on the device and copied back.  Inputs
+ * may be pageable or page-locked (page-locked recommended).  This is the end-to-end path bench.py times ("e2e"). */
 int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out);
 
 /* the scheme Thomas's algorithm replaces (L258-270, L397), as a measured comparison:

@@ -1833,6 +1833,14 @@ extern "C" int helios_rt_step_iterative(helios_rt *h, const helios_rt_inputs *in
   return launch_step(h, in, out, (cudaStream_t)cuda_stream, n_iterations);
 }
 
+// device alias of a host pointer that the device can write directly (page-locked, mapped: cudaHostAlloc /
+// cudaHostRegister memory under unified addressing); nullptr for pageable memory
+static double *mapped_alias(double *host) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return a.type == cudaMemoryTypeHost ? (double *)a.devicePointer : nullptr;
+}
+
 extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out) {
   int rc = validate_step(h, in, out);
   if (rc) return rc;
@@ -1846,24 +1854,33 @@ extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, con
   CK(h, cudaMemcpyAsync(d_fs, in->stellar_flux, sizeof(double) * nb, cudaMemcpyHostToDevice, st));
   helios_rt_inputs din = *in;
   din.p = d_p; din.T = d_T; din.mu_star = d_mu; din.stellar_flux = d_fs;
-  helios_rt_outputs dout;
-  double *o = h->d_out;
+  // Outputs.  Page-locked, mapped host buffers are written by the kernel itself (each column's results leave over
+  // PCIe as soon as its last tile has summed them, under the sweeps of the other columns); pageable buffers, and a
+  // per-bin spectrum whose bins straddle tiles (accumulated with atomics), go through device staging and a copy each.
+  const int tp = h->warps * 32 * h->ppt;
+  const bool toa_atomics = h->tiles > 1 && (tp % h->cfg.n_gauss) != 0;
+  double *const host[6] = {out->F_up, out->F_down, out->F_net, out->F_beam, out->dTdt, out->F_up_toa_bin};
   const size_t ni = ncol * (N + 1);
-  dout.F_up = out->F_up ? o : nullptr;                 o += ni;
-  dout.F_down = out->F_down ? o : nullptr;             o += ni;
-  dout.F_net = out->F_net ? o : nullptr;               o += ni;
-  dout.F_beam = out->F_beam ? o : nullptr;             o += ni;
-  dout.dTdt = out->dTdt ? o : nullptr;                 o += ncol * N;
-  dout.F_up_toa_bin = out->F_up_toa_bin ? o : nullptr;
+  const size_t count[6] = {ni, ni, ni, ni, ncol * N, ncol * nb};
+  double *dev[6], *stage = h->d_out;
+  bool staged[6];
+  for (int k = 0; k < 6; ++k) {
+    dev[k] = nullptr;
+    staged[k] = false;
+    if (host[k]) {
+      double *alias = (k == 5 && toa_atomics) ? nullptr : mapped_alias(host[k]);
+      dev[k] = alias ? alias : stage;
+      staged[k] = alias == nullptr;
+    }
+    stage += count[k];
+  }
+  helios_rt_outputs dout;
+  dout.F_up = dev[0]; dout.F_down = dev[1]; dout.F_net = dev[2]; dout.F_beam = dev[3]; dout.dTdt = dev[4];
+  dout.F_up_toa_bin = dev[5];
   rc = launch_step(h, &din, &dout, st);
   if (rc) return rc;
-  if (out->F_up) CK(h, cudaMemcpyAsync(out->F_up, dout.F_up, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
-  if (out->F_down) CK(h, cudaMemcpyAsync(out->F_down, dout.F_down, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
-  if (out->F_net) CK(h, cudaMemcpyAsync(out->F_net, dout.F_net, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
-  if (out->F_beam) CK(h, cudaMemcpyAsync(out->F_beam, dout.F_beam, sizeof(double) * ni, cudaMemcpyDeviceToHost, st));
-  if (out->dTdt) CK(h, cudaMemcpyAsync(out->dTdt, dout.dTdt, sizeof(double) * ncol * N, cudaMemcpyDeviceToHost, st));
-  if (out->F_up_toa_bin)
-    CK(h, cudaMemcpyAsync(out->F_up_toa_bin, dout.F_up_toa_bin, sizeof(double) * ncol * nb, cudaMemcpyDeviceToHost, st));
+  for (int k = 0; k < 6; ++k)
+    if (staged[k]) CK(h, cudaMemcpyAsync(host[k], dev[k], sizeof(double) * count[k], cudaMemcpyDeviceToHost, st));
   CK(h, cudaStreamSynchronize(st));
   return HELIOS_RT_OK;
 }

@@ -29,12 +29,19 @@ def H():
 
 
 def run_gpu(torch, H, cfg, inp, want, host=False, rt=None):
+    """host: False = device buffers (helios_rt_step); True = pageable numpy buffers, "pinned" = page-locked torch
+    buffers (helios_rt_step_host: staged copies / outputs written by the kernel itself)."""
     n = inp["p"].shape[0]
     own = rt is None
     if own:
         rt = H.HeliosRT(cfg, max(n, 1))
     shapes = rt.output_shapes(n)
-    if host:
+    if host == "pinned":
+        pin = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).pin_memory()
+        out = {k: torch.full(shapes[k], float("nan"), dtype=torch.float64).pin_memory() for k in want}
+        rt.step_host(pin(inp["p"]), pin(inp["T"]), pin(inp["mu_star"]), pin(inp["stellar_flux"]), inp["f_internal"], out)
+        res = {k: v.numpy().copy() for k, v in out.items()}
+    elif host:
         out = {k: np.full(shapes[k], np.nan) for k in want}
         rt.step_host(np.ascontiguousarray(inp["p"]), np.ascontiguousarray(inp["T"]),
                      np.ascontiguousarray(inp["mu_star"]), np.ascontiguousarray(inp["stellar_flux"]),
@@ -384,6 +391,20 @@ def test_step_host_equals_device_step(torch_cuda, H, oracle_mod):
         assert np.array_equal(a[k], b[k]), k
     c = run_gpu(torch_cuda, H, cfg, inp, ("dTdt",), host=True)     # a subset of outputs
     assert np.array_equal(c["dTdt"], a["dTdt"])
+    # page-locked output buffers are written by the kernel directly (no staging, no copy back)
+    d = run_gpu(torch_cuda, H, cfg, inp, ALL, host="pinned")
+    for k in ALL:
+        assert np.array_equal(a[k], d[k]), k
+    # TOA spectrum whose bins straddle tiles (atomics): staged even when the buffer is page-locked
+    cfg5, inp5, _ = W_make_toa()
+    e = run_gpu(torch_cuda, H, cfg5, inp5, ("F_up_toa_bin",))
+    f = run_gpu(torch_cuda, H, cfg5, inp5, ("F_up_toa_bin",), host="pinned")
+    assert np.array_equal(e["F_up_toa_bin"], f["F_up_toa_bin"])
+
+
+def W_make_toa():
+    from paper_2203_02293_b200 import workloads as W
+    return W.make(5, columns=slice(1, None, 500))
 
 
 def test_step_argument_errors(torch_cuda, H):
