@@ -111,29 +111,47 @@ def test_fp64_primitives(torch_cuda, H):
 
 
 def test_planck_device_vs_oracle(torch_cuda, H, oracle_mod):
+    """Band Planck on the device against the oracle, 5000 (T, bin) pairs: random bins 0.1 % .. 300 % wide and 2000 bins
+    at the R = 500 sampling of config 6 (0.2 % wide).  The bound is derived, not fitted, in units
+    of eps = 2^-52, relative to the bin mean, with dG the bin's integral in x and G_s the cumulative integral the device
+    differences at the short-wavelength edge (G from infinity, or int_0^x when both edges have x < 1.5):
+        4                  roundings of scale * dG / dlam
+      + 4 G_s / dG         two cumulative integrals, each good to 2 eps (polynomial pieces / series, table exp)
+      + 2 lam / dlam       x = (h c / k lam) (1 / T) is rounded independently at the two edges (1 eps each); moving one
+                           edge by eps x changes the integral by eps x / dx = eps lam / dlam of itself
+      + max(3, x)          the rounding common to both edges (1 / T) scales x: d ln dG / d ln x is 3 in the
+                           Rayleigh-Jeans limit, x - 3 in the Wien tail
+    plus the ORACLE's own error: it differences G(x_hi) - G(x_lo) from infinity in x87 long double (eps 2^-64), which
+    cancels against pi^4/15 = 6.5 for narrow bins at small x: 2^-63 * 6.5 / dG.  (That term, not the device, is what
+    limits the R = 500 bins at lam > 50 um to ~2e-11.)  Measured worst case on B200: 0.56 of the bound."""
     rng = np.random.default_rng(6)
     n = 3000
     T = np.concatenate([rng.uniform(50, 3500, n - 4), [100.0, 400.0, 4798.0, 3000.0]])
     lo = 10 ** rng.uniform(np.log10(0.25e-6), np.log10(150e-6), n)
     hi = lo * (1 + 10 ** rng.uniform(-3, 0.5, n))
+    T = np.concatenate([T, rng.uniform(300, 3500, 2000)])
+    lo_r = 10 ** rng.uniform(np.log10(0.3e-6), np.log10(200e-6), 2000)
+    lo, hi = np.concatenate([lo, lo_r]), np.concatenate([hi, lo_r * (1 + 1 / 500.0)])
     got = H.selftest_planck(T, lo, hi)
-    ref = np.array([oracle_mod.planck_bin_mean(T[i], lo[i], hi[i]) for i in range(n)])
-    # a narrow bin differences two G values: allow the conditioning of G_hi - G_lo
-    # The bin integral differences two cumulative integrals: G (from infinity) or, when both edges have
-    # x < 1.5, int_0^x.  Each carries a few ulp of rounding, so the condition number of the difference is
-    # min(G, int_0^x) / dG at the short-wavelength edge (<= 6.5 / dG).
+    ref = np.array([oracle_mod.planck_bin_mean(T[i], lo[i], hi[i]) for i in range(len(T))])
+    eps = 2.0 ** -52
     C1 = 2 * 1.380649e-23**4 / (6.62607015e-34**3 * 299792458.0**2)
     dG = np.maximum(np.abs(ref) * (hi - lo) / (C1 * T**4), 1e-300)
-    x_lo = 6.62607015e-34 * 299792458.0 / (1.380649e-23 * T * lo)              # larger x of the bin
-    big = np.where(x_lo < 1.5, x_lo**3 / 3.0, 6.5)
-    # ... and x = hc / (lam k T) is itself rounded to fp64 on the device (the oracle carries it in long
-    # double): d ln(dG) / d ln(x) is up to ~x lam/dlam in the Wien tail, 3 lam/dlam below x = 1.5.
-    cond = 1.0 + big / dG + np.maximum(x_lo, 4.0) * lo / (hi - lo)
-    ratio = np.abs(got - ref) / (2.2e-16 * cond * np.abs(ref) + 1e-300)
-    assert ratio.max() <= 40.0, f"worst {ratio.max():.3g} eps*cond at T={T[ratio.argmax()]}, lo={lo[ratio.argmax()]}, hi={hi[ratio.argmax()]}"
-    # bins no narrower than 1 % in wavelength (the paper's tables: 30-300 bins, R=500 sampling is 0.2 %)
-    ok = (ref > 1e-250) & (hi / lo >= 1.01)
-    assert np.max(np.abs(got[ok] - ref[ok]) / ref[ok]) < 2e-11
+    x = 6.62607015e-34 * 299792458.0 / (1.380649e-23 * T * lo)                 # larger x of the bin
+    xs = np.minimum(x, 700.0)
+    G_inf = sum(np.exp(-k * xs) * (xs**3 / k + 3 * xs**2 / k**2 + 6 * xs / k**3 + 6 / k**4) for k in range(1, 60))
+    G_s = np.where(x < 1.5, x**3 / 3.0, G_inf)
+    bound = eps * (4 + 4 * G_s / dG + 2 * lo / (hi - lo) + np.maximum(3.0, x)) + 2.0 ** -63 * 6.5 / dG
+    ok = ref > 1e-280
+    ratio = np.abs(got - ref)[ok] / (bound[ok] * ref[ok])
+    worst = np.flatnonzero(ok)[ratio.argmax()]
+    assert ratio.max() <= 1.0, f"worst {ratio.max():.3g} of the bound at T={T[worst]}, lo={lo[worst]}, hi={hi[worst]}"
+    # in plain numbers: bins no narrower than 1 % in wavelength (the paper's k-tables: 30-300 bins) ...
+    wide = ok & (hi / lo >= 1.01)
+    assert np.max(np.abs(got[wide] - ref[wide]) / ref[wide]) < 2e-12
+    # ... and the R = 500 sampling of the post-processing step (config 6), oracle-limited
+    r500 = ok & (np.arange(len(T)) >= n)
+    assert np.max(np.abs(got[r500] - ref[r500]) / ref[r500]) < 5e-11
 
 
 # ------------------------------------------------------------------------------------ the configs
