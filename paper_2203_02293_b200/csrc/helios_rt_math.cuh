@@ -181,49 +181,70 @@ inline void build_planck_table(double *tab) {
 }
 
 // *low receives int_0^x t^3/(e^t-1) dt when x < 1.5 (else -1).  T32: the 2^(j/32) table in shared memory (exp_hot).
-// Branch-free: all three forms are evaluated on clamped arguments and selected, so that several evaluations unrolled
-// in one thread interleave (S2 is latency-bound: ~65 instructions each, but independent); the polynomial piece uses
-// Estrin's scheme (dependence depth 4 instead of 9).  x <= 0 (T = inf) is not special-cased: callers pass T > 0.
+// Branch-free per lane: the forms are evaluated on clamped arguments and selected (the polynomial piece uses Estrin's
+// scheme: dependence depth 4 instead of 9).  VOTE: a form that no active lane of the warp needs is skipped (warp-uniform
+// branches; phase A's lanes are consecutive levels of a column at one bin edge, so their x lie within a factor ~2.5 and
+// usually share one form).  x <= 0 (T = inf) is not special-cased: callers pass T > 0.
+template <bool VOTE = false>
 __device__ __forceinline__ double planck_G(double x, const double *__restrict__ gtab, const double *__restrict__ T32,
                                            double *low_out) {
-  // x < 1.5: Bernoulli series of int_0^x; coefficients B_k / ((k+3) k!), k = 0,1,2,4,...,30
-  const double xs = fmin(x, kGX0);
-  const double x2 = xs * xs;
-  double s = 8615841276005.0 / (14322.0 * 33.0 * 265252859812191058636308480000000.0);    // k=30
-  s = fma(s, x2, -23749461029.0 / (870.0 * 31.0 * 304888344611713860501504000000.0));      // k=28
-  s = fma(s, x2, 8553103.0 / (6.0 * 29.0 * 403291461126605635584000000.0));                // k=26
-  s = fma(s, x2, -236364091.0 / (2730.0 * 27.0 * 620448401733239439360000.0));             // k=24
-  s = fma(s, x2, 854513.0 / (138.0 * 25.0 * 1124000727777607680000.0));                    // k=22
-  s = fma(s, x2, -174611.0 / (330.0 * 23.0 * 2432902008176640000.0));                      // k=20
-  s = fma(s, x2, 43867.0 / (798.0 * 21.0 * 6402373705728000.0));                           // k=18
-  s = fma(s, x2, -3617.0 / (510.0 * 19.0 * 20922789888000.0));                             // k=16
-  s = fma(s, x2, 7.0 / (6.0 * 17.0 * 87178291200.0));                                      // k=14
-  s = fma(s, x2, -691.0 / (2730.0 * 15.0 * 479001600.0));                                  // k=12
-  s = fma(s, x2, 1.0 / 622702080.0);                                                       // k=10
-  s = fma(s, x2, -1.0 / 13305600.0);                                                       // k=8
-  s = fma(s, x2, 1.0 / 272160.0);                                                          // k=6 : (1/42)/(9*720)
-  s = fma(s, x2, -1.0 / 5040.0);                                                           // k=4 : (-1/30)/(7*24)
-  s = fma(s, x2, 1.0 / 60.0);                                                              // k=2 : (1/6)/(5*2)
-  const double low = x2 * xs * fma(x2, s, fma(-1.0 / 8.0, xs, 1.0 / 3.0));                 // x^3 (1/3 - x/8 + x^2 s)
-  // x >= 1.5: e^-x times a polynomial
-  const double xc = fmin(x, 708.0);                                                        // beyond: G < 1e-298
-  const double u = exp_hot<1, false>(xc, T32, nullptr);
-  int iv = (int)((xc - kGX0) * (1.0 / kGH));
-  iv = iv < 0 ? 0 : (iv > kGIntervals - 1 ? kGIntervals - 1 : iv);
-  const double t = fmin(fmax(xc - (kGX0 + kGH * 0.5 + kGH * (double)iv), -kGH), kGH);
-  const double2 *c = reinterpret_cast<const double2 *>(gtab + iv * kGCoef);
-  const double2 c01 = __ldg(c), c23 = __ldg(c + 1), c45 = __ldg(c + 2), c67 = __ldg(c + 3), c89 = __ldg(c + 4);
-  const double t2 = t * t, t4 = t2 * t2, t8 = t4 * t4;
-  const double p01 = fma(c01.y, t, c01.x), p23 = fma(c23.y, t, c23.x), p45 = fma(c45.y, t, c45.x),
-               p67 = fma(c67.y, t, c67.x), p89 = fma(c89.y, t, c89.x);
-  const double q0 = fma(p23, t2, p01), q1 = fma(p67, t2, p45);
-  const double p_mid = fma(p89, t8, fma(q1, t4, q0));
-  const double p1 = fma(fma(fma(xc, 1.0, 3.0), xc, 6.0), xc, 6.0);               // x^3 + 3x^2 + 6x + 6
-  const double p2 = fma(fma(fma(xc, 0.5, 0.75), xc, 0.75), xc, 0.375);           // x^3/2 + 3x^2/4 + 6x/8 + 6/16
-  const double p_hi = fma(u, p2, p1);
   const bool is_low = x < kGX0;
+  const double xc = fmin(x, 708.0);                                                        // beyond: G < 1e-298
+  const bool is_mid = !is_low && xc < kGX1;
+  bool need_low = true, need_mid = true, need_hi = true;
+  if (VOTE) {
+    const unsigned act = __activemask();
+    need_low = __any_sync(act, is_low);
+    need_mid = __any_sync(act, is_mid);
+    need_hi = __any_sync(act, !is_low && !is_mid);
+  }
+  double low = 0.0;
+  if (need_low) {
+    // x < 1.5: Bernoulli series of int_0^x; coefficients B_k / ((k+3) k!), k = 0,1,2,4,...,30
+    const double xs = fmin(x, kGX0);
+    const double x2 = xs * xs;
+    double s = 8615841276005.0 / (14322.0 * 33.0 * 265252859812191058636308480000000.0);    // k=30
+    s = fma(s, x2, -23749461029.0 / (870.0 * 31.0 * 304888344611713860501504000000.0));      // k=28
+    s = fma(s, x2, 8553103.0 / (6.0 * 29.0 * 403291461126605635584000000.0));                // k=26
+    s = fma(s, x2, -236364091.0 / (2730.0 * 27.0 * 620448401733239439360000.0));             // k=24
+    s = fma(s, x2, 854513.0 / (138.0 * 25.0 * 1124000727777607680000.0));                    // k=22
+    s = fma(s, x2, -174611.0 / (330.0 * 23.0 * 2432902008176640000.0));                      // k=20
+    s = fma(s, x2, 43867.0 / (798.0 * 21.0 * 6402373705728000.0));                           // k=18
+    s = fma(s, x2, -3617.0 / (510.0 * 19.0 * 20922789888000.0));                             // k=16
+    s = fma(s, x2, 7.0 / (6.0 * 17.0 * 87178291200.0));                                      // k=14
+    s = fma(s, x2, -691.0 / (2730.0 * 15.0 * 479001600.0));                                  // k=12
+    s = fma(s, x2, 1.0 / 622702080.0);                                                       // k=10
+    s = fma(s, x2, -1.0 / 13305600.0);                                                       // k=8
+    s = fma(s, x2, 1.0 / 272160.0);                                                          // k=6 : (1/42)/(9*720)
+    s = fma(s, x2, -1.0 / 5040.0);                                                           // k=4 : (-1/30)/(7*24)
+    s = fma(s, x2, 1.0 / 60.0);                                                              // k=2 : (1/6)/(5*2)
+    low = x2 * xs * fma(x2, s, fma(-1.0 / 8.0, xs, 1.0 / 3.0));                              // x^3 (1/3 - x/8 + x^2 s)
+  }
+  // x >= 1.5: e^-x times a polynomial
+  double G_big = 0.0;
+  if (need_mid || need_hi) {
+    const double u = exp_hot<1, false>(xc, T32, nullptr);
+    double p_mid = 0.0, p_hi = 0.0;
+    if (need_mid) {
+      int iv = (int)((xc - kGX0) * (1.0 / kGH));
+      iv = iv < 0 ? 0 : (iv > kGIntervals - 1 ? kGIntervals - 1 : iv);
+      const double t = fmin(fmax(xc - (kGX0 + kGH * 0.5 + kGH * (double)iv), -kGH), kGH);
+      const double2 *c = reinterpret_cast<const double2 *>(gtab + iv * kGCoef);
+      const double2 c01 = __ldg(c), c23 = __ldg(c + 1), c45 = __ldg(c + 2), c67 = __ldg(c + 3), c89 = __ldg(c + 4);
+      const double t2 = t * t, t4 = t2 * t2, t8 = t4 * t4;
+      const double p01 = fma(c01.y, t, c01.x), p23 = fma(c23.y, t, c23.x), p45 = fma(c45.y, t, c45.x),
+                   p67 = fma(c67.y, t, c67.x), p89 = fma(c89.y, t, c89.x);
+      const double q0 = fma(p23, t2, p01), q1 = fma(p67, t2, p45);
+      p_mid = fma(p89, t8, fma(q1, t4, q0));
+    }
+    if (need_hi) {
+      const double p1 = fma(fma(fma(xc, 1.0, 3.0), xc, 6.0), xc, 6.0);               // x^3 + 3x^2 + 6x + 6
+      const double p2 = fma(fma(fma(xc, 0.5, 0.75), xc, 0.75), xc, 0.375);           // x^3/2 + 3x^2/4 + 6x/8 + 6/16
+      p_hi = fma(u, p2, p1);
+    }
+    G_big = u * (is_mid ? p_mid : p_hi);
+  }
   *low_out = is_low ? low : -1.0;
-  const double G_big = u * (xc < kGX1 ? p_mid : p_hi);
   return is_low ? (kPi * kPi * kPi * kPi / 15.0 - low) : (x > 708.0 ? 0.0 : G_big);
 }
 
