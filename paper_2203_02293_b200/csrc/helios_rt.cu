@@ -49,6 +49,9 @@ constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
 #ifndef HRT_UNROLL_ISO
 #define HRT_UNROLL_ISO 1
 #endif
+#ifndef HRT_PA_UNROLL
+#define HRT_PA_UNROLL 2   /* config 2: 0.6787 ms at 2, 0.6845 at 4, 0.6851 at 8 */
+#endif
 #ifndef HRT_VOTE_SEL
 #define HRT_VOTE_SEL (!TOA)
 #endif
@@ -256,7 +259,7 @@ __host__ __device__ inline Lay make_lay(int N, int nlev, int warps, int ppt, int
                                         bool bdirect) {
   Lay L;
   const int tp = warps * 32 * ppt;
-  const int nbt = (tp + ng - 1) / ng + 1;
+  const int nbt = bdirect ? tp : (tp + ng - 1) / ng + 1;   // bins a tile can touch (a tile may start inside a bin; one point per bin: tp)
   L.nbt = nbt < nb ? nbt : nb;
   L.LP = (N + 1 + 7) & ~7;
   L.rec_bytes = (unsigned)((sizeof(LevelRec) * (nlev + 1) + sizeof(double) * (N + 1) + 15) & ~size_t(15));   // LevelRec[nlev+1] | dm[N] | mu
@@ -508,7 +511,7 @@ __device__ __forceinline__ void stk_load_R(const double *row, int lane, double (
 //       B_b goes to the Planck block of each tile that owns points of the bin (slots CSR).  The extra level nlev
 //       carries T_int and yields F_BOA,b = pi B_b(T_int).
 // --------------------------------------------------------------------------------------------
-template <bool NONISO, bool VOTE>
+template <bool NONISO, bool VOTE, bool PACK4>
 __device__ __forceinline__ void prep_item(const KParams &P, const Lay &L, const double *__restrict__ T32, int col, int l) {
   const int N = P.N, nlev = P.nlev;
   const double *pc = P.p + (size_t)col * N;
@@ -588,8 +591,7 @@ __device__ __forceinline__ void prep_item(const KParams &P, const Lay &L, const 
   const double T2 = Tl * Tl;
   const double scale = hot ? ((l == nlev) ? kPlanckC1 * kPi : kPlanckC1) * T2 * T2 : 0.0;   // row nlev: F_BOA = pi B(T_int), L239
   double low_p = 0.0, G_p = planck_G<VOTE>(__ldg(P.c2lam) * invT, P.gtab, T32, &low_p);
-#pragma unroll 4
-  for (int e = 0; e < P.nb; ++e) {
+  auto one_bin = [&](int e) {
     double low_a;
     const double G_a = planck_G<VOTE>(__ldg(P.c2lam + e + 1) * invT, P.gtab, T32, &low_a);
     const int4 raw = __ldg(reinterpret_cast<const int4 *>(P.bslot + e));
@@ -600,18 +602,45 @@ __device__ __forceinline__ void prep_item(const KParams &P, const Lay &L, const 
     else if (raw.y == -2)
       for (int k = __ldg(P.slot_ptr + e) + 1; k < __ldg(P.slot_ptr + e + 1); ++k) Brow[__ldg(P.slots + k)] = B;
     G_p = G_a; low_p = low_a;
+  };
+  if constexpr (PACK4) {
+    int e = 0;
+    if (P.ng == 1 && (L.nbt & 3) == 0) {
+      // one Gauss point per bin (opacity sampling, thousands of bins): every bin has one slot, tiles hold a multiple of
+      // 4 bins and rows are 32-byte aligned, so four consecutive bins leave as ONE 32-byte store (a whole sector) instead
+      // of four 8-byte stores into it (config 6: RT step 10.6 -> 8.0 ms)
+#pragma unroll 1
+      for (; e + 4 <= P.nb; e += 4) {
+        double B4[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          double low_a;
+          const double G_a = planck_G<VOTE>(__ldg(P.c2lam + e + k + 1) * invT, P.gtab, T32, &low_a);
+          B4[k] = scale * planck_dG(G_p, low_p, G_a, low_a) * __ldg(&P.bslot[e + k].inv_dlam);
+          G_p = G_a; low_p = low_a;
+        }
+        double *dst = Brow + __ldg(&P.bslot[e].s0);
+        asm volatile("st.global.L1::no_allocate.v4.b64 [%0], {%1, %2, %3, %4};" ::"l"(dst), "l"(__double_as_longlong(B4[0])),
+                     "l"(__double_as_longlong(B4[1])), "l"(__double_as_longlong(B4[2])), "l"(__double_as_longlong(B4[3]))
+                     : "memory");
+      }
+    }
+    for (; e < P.nb; ++e) one_bin(e);
+  } else {
+HRT_UNROLL(HRT_PA_UNROLL)
+    for (int e = 0; e < P.nb; ++e) one_bin(e);
   }
 }
 
 // phase A over the whole grid: item = (column, level) in column-major order
-template <bool NONISO, bool VOTE>
+template <bool NONISO, bool VOTE, bool PACK4>
 __device__ __forceinline__ void phase_a(const KParams &P, const Lay &L, const double *__restrict__ T32, long gtid, long gthreads,
                                         bool count) {
   const int nlevp = P.nlev + 1;
   const long nitems = (long)P.ncol * nlevp;
   for (long item = gtid; item < nitems; item += gthreads) {
     const int col = (int)(item / nlevp), l = (int)(item - (long)col * nlevp);
-    prep_item<NONISO, VOTE>(P, L, T32, col, l);
+    prep_item<NONISO, VOTE, PACK4>(P, L, T32, col, l);
     if (count) {
       // count the warp's items of each column with one fence + one atomic (the warp barrier + the leader's fence
       // order every lane's stores before the count)
@@ -777,7 +806,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
     __syncthreads();                       // s_T32
     const long nblk = (long)gridDim.x * gridDim.y;
     // (skipping the Planck forms no lane of a warp needs: -1.2 % on config 2, +0.9 % on config 5 -- per-class choice)
-    phase_a<NONISO, HRT_VOTE_SEL>(P, L, s_T32, ((long)blockIdx.y * gridDim.x + blockIdx.x) * nthr + tid, nblk * nthr, true);
+    phase_a<NONISO, HRT_VOTE_SEL, BDIRECT>(P, L, s_T32, ((long)blockIdx.y * gridDim.x + blockIdx.x) * nthr + tid, nblk * nthr, true);
     __syncthreads();
     if (tid == 0) {
       unsigned prev;
@@ -1290,13 +1319,13 @@ __global__ void __launch_bounds__(128) rt_iter_kernel(const KParams P, const int
 // phase A as a launch of its own: for the comparison path (rt_iter_kernel; tp = spectral points per tile of that kernel,
 // count = 0) and for rt_step_kernel when the device cannot host its grid at once (count = 1)
 template <bool NONISO>
-__global__ void __launch_bounds__(128) rt_prep_kernel(const KParams P, const int tp, const int count) {
+__global__ void __launch_bounds__(128) rt_prep_kernel(const KParams P, const int tp, const int count, const int bdirect) {
   __shared__ double s_T32[32];
   // only the block sizes of the layout are used here
-  const Lay L = make_lay(P.N, P.nlev, tp / 32, 1, P.ng, P.nb, true, NONISO ? 2 : 1, 0, true);
+  const Lay L = make_lay(P.N, P.nlev, tp / 32, 1, P.ng, P.nb, true, NONISO ? 2 : 1, 0, bdirect != 0);
   if (threadIdx.x < 32) s_T32[threadIdx.x] = kExp2Tab[threadIdx.x];
   __syncthreads();
-  phase_a<NONISO, true>(P, L, s_T32, (long)blockIdx.x * blockDim.x + threadIdx.x, (long)gridDim.x * blockDim.x, count != 0);
+  phase_a<NONISO, true, true>(P, L, s_T32, (long)blockIdx.x * blockDim.x + threadIdx.x, (long)gridDim.x * blockDim.x, count != 0);
 }
 
 __global__ void zero_kernel(double *p, size_t n) {
@@ -1766,8 +1795,8 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
     const long items = (long)in->n_columns * (h->nlev + 1);
     const int pblocks = (int)((items + 127) / 128 < 16L * h->sm_count ? (items + 127) / 128 : 16L * h->sm_count);
     P.slot_ptr = h->d_slot_ptr_iter; P.slots = h->d_slots_iter; P.bslot = h->d_bslot_iter;
-    if (h->noniso) rt_prep_kernel<true><<<pblocks, 128, 0, st>>>(P, h->iter_warps * 32, 0);
-    else rt_prep_kernel<false><<<pblocks, 128, 0, st>>>(P, h->iter_warps * 32, 0);
+    if (h->noniso) rt_prep_kernel<true><<<pblocks, 128, 0, st>>>(P, h->iter_warps * 32, 0, 0);
+    else rt_prep_kernel<false><<<pblocks, 128, 0, st>>>(P, h->iter_warps * 32, 0, 0);
     CK(h, cudaGetLastError());
     dim3 grid((unsigned)h->iter_tiles, (unsigned)in->n_columns);
     fn<<<grid, h->iter_warps * 32, lay.total, st>>>(P, n_iter);
@@ -1812,8 +1841,9 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
     const long items = (long)in->n_columns * (h->nlev + 1);
     const int pblocks = (int)((items + 127) / 128 < 16L * h->sm_count ? (items + 127) / 128 : 16L * h->sm_count);
     const int tp2 = h->warps * 32 * h->ppt;
-    if (h->noniso) rt_prep_kernel<true><<<pblocks, 128, 0, st>>>(P, tp2, 1);
-    else rt_prep_kernel<false><<<pblocks, 128, 0, st>>>(P, tp2, 1);
+    const int bd = kVariants[h->variant].bdirect ? 1 : 0;
+    if (h->noniso) rt_prep_kernel<true><<<pblocks, 128, 0, st>>>(P, tp2, 1, bd);
+    else rt_prep_kernel<false><<<pblocks, 128, 0, st>>>(P, tp2, 1, bd);
     CK(h, cudaGetLastError());
     lc.numAttrs = 0;
     e = cudaLaunchKernelEx(&lc, kVariants[h->variant].fn, P);
