@@ -787,3 +787,22 @@ def test_heating_rate_beam_only_closed_form(oracle_mod):
         # (kappa is constant with depth, so the non-isothermal sub-layer treatment must give the same profile)
         assert np.allclose(res["dTdt"][0], ref, rtol=1e-11, atol=1e-14 * ref.max())
         assert np.all(np.abs(res["F_up"][0]) <= 1e-40)                        # nothing comes back up (B(50 K) ~ 1e-46)
+
+
+def test_opcount_build_matches_the_oracle_and_counts(oracle_mod):
+    """oracle/opcount.py compiles helios_oracle.c unchanged with an op-counting scalar (BASELINE.md section 3's audit):
+    its results equal the long-double build's, and the counts per layer.point are what BASELINE.md quotes (every
+    dayside layer.point takes 3 exponentials in the method -- kappa is tabulated, so the oracle's 4th is Planck's share --
+    and at least 2 square roots and 16 divisions in the literal form)."""
+    import ctypes as C
+    from oracle import opcount
+    from paper_2203_02293_b200 import workloads as W
+    per = opcount.count(2, True, n_cols=2)
+    assert 3.0 <= per["exp"] <= 4.5 and per["sqrt"] == 2.0 and per["div"] >= 16 and per["log"] == 8.0
+    night = opcount.count(2, False, n_cols=2)
+    assert night["exp"] < per["exp"] and night["div"] < per["div"]          # no direct beam: fewer of both
+    cfg, inp, meta = W.make(1)
+    a = oracle_mod.rt_step(cfg, inp, real="opcount", want=("F_net", "dTdt"))
+    b = oracle_mod.rt_step(cfg, inp, real="ld", want=("F_net", "dTdt"))
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
