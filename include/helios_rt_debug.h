@@ -23,6 +23,11 @@ extern "C" {
 int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t ppt, int32_t rows, int32_t stk, int32_t maxt,
                                int32_t minb);
 
+/* on != 0: every later step of the handle takes the path the library falls back to when the device cannot host the
+ * whole grid of rt_step_kernel at once (cooperative launch refused): phase A as a launch of its own (rt_prep_kernel),
+ * then the sweeps as a plain launch.  Lets the tests run that path through the parity checks. */
+int helios_rt_debug_force_two_launches(helios_rt *h, int32_t on);
+
 /* info[0] = warps per block, [1] = points per thread, [2] = rows, [3] = stk, [4] = maxt, [5] = minb, [6] = tiles per
  * column, [7] = workers per tile (grid = tiles x workers), [8] = resident blocks per SM, [9] = registers per thread,
  * [10] = local-memory bytes per thread, [11] = dynamic shared memory bytes, [12] = back-substitution workspace in MiB,

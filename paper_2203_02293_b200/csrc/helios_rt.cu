@@ -1412,6 +1412,7 @@ struct helios_rt {
   cudaStream_t own_stream, copy_stream;
   cudaEvent_t ev_in[4], ev_done[4];
   int regs, lmem, sm_count;
+  int force_two_launches;   // helios_rt_debug_force_two_launches: always take the fallback path (tests)
   cudaError_t last_err;
 };
 
@@ -1833,7 +1834,7 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
 #ifdef HRT_DIAG_TWO_LAUNCH
   cudaError_t e = cudaErrorNotSupported;
 #else
-  cudaError_t e = cudaLaunchKernelEx(&lc, kVariants[h->variant].fn, P);
+  cudaError_t e = h->force_two_launches ? cudaErrorCooperativeLaunchTooLarge : cudaLaunchKernelEx(&lc, kVariants[h->variant].fn, P);
 #endif
   if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) {
     cudaGetLastError();
@@ -1944,6 +1945,12 @@ extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t p
   int rc = configure_launch(h);
   if (rc) { h->variant = old_v; h->warps = old_w; configure_launch(h); }
   return rc;
+}
+
+extern "C" int helios_rt_debug_force_two_launches(helios_rt *h, int32_t on) {
+  if (!h) return HELIOS_RT_EINVAL;
+  h->force_two_launches = on != 0;
+  return HELIOS_RT_OK;
 }
 
 extern "C" int helios_rt_debug_get_launch(const helios_rt *h, int32_t info[16]) {

@@ -21,7 +21,8 @@ _dp = C.POINTER(C.c_double)
 EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
            "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info", "helios_rt_step_iterative",
            "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_phase_curve_workspace_bytes",
-           "helios_rt_advance_1d", "helios_rt_debug_set_launch", "helios_rt_debug_get_launch")
+           "helios_rt_advance_1d", "helios_rt_debug_set_launch", "helios_rt_debug_get_launch",
+           "helios_rt_debug_force_two_launches")
 # ... and in include/helios_rt_selftest.h (libhelios_rt_selftest.so)
 SELFTEST_EXPORTS = ("helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_selftest_planck_G",
                     "helios_rt_measure_dfma_peak", "helios_rt_measure_latencies")
@@ -86,6 +87,8 @@ def load_library() -> C.CDLL:
         L.helios_rt_phase_curve_workspace_bytes.argtypes = [C.c_int32] * 3
         L.helios_rt_advance_1d.restype = C.c_int
         L.helios_rt_advance_1d.argtypes = [C.c_int32] * 2 + [C.c_double] * 4 + [C.c_void_p] * 6
+        L.helios_rt_debug_force_two_launches.restype = C.c_int
+        L.helios_rt_debug_force_two_launches.argtypes = [C.c_void_p, C.c_int32]
         L.helios_rt_debug_set_launch.restype = C.c_int
         L.helios_rt_debug_set_launch.argtypes = [C.c_void_p] + [C.c_int32] * 6
         L.helios_rt_debug_get_launch.restype = C.c_int
@@ -183,6 +186,10 @@ class HeliosRT:
         """helios_rt_debug_set_launch (include/helios_rt_debug.h; tests and tuning only)."""
         _check(load_library().helios_rt_debug_set_launch(self._h, int(warps), int(ppt), int(rows), int(stk), int(maxt),
                                                          int(minb)), self._h)
+
+    def debug_force_two_launches(self, on: bool = True) -> None:
+        """Tests only (helios_rt_debug.h): take the non-cooperative fallback path (rt_prep_kernel + plain launch)."""
+        _check(load_library().helios_rt_debug_force_two_launches(self._h, int(bool(on))), self._h)
 
     def debug_get_launch(self) -> dict:
         info = (C.c_int32 * 16)()

@@ -307,6 +307,27 @@ def test_every_compiled_variant(torch_cuda, H, oracle_mod, config, stride):
     rt.close()
 
 
+@pytest.mark.parametrize("config,stride", [(2, 173), (3, 259), (5, 701)])
+def test_fallback_two_launches(torch_cuda, H, oracle_mod, config, stride):
+    """The path taken when the device cannot host the whole grid at once (cooperative launch refused): phase A as
+    rt_prep_kernel, then the sweeps as a plain launch.  Same answers as the one-launch path, bit for bit."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config, columns=slice(3, None, stride))
+    want = ("F_up_toa_bin",) if config == 5 else ("F_up", "F_down", "F_net", "dTdt")
+    ref = oracle_mod.rt_step(cfg, inp, want=want)
+    rt = H.HeliosRT(cfg, inp["p"].shape[0])
+    one = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+    rt.debug_force_two_launches(True)
+    two = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+    two_again = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+    rt.debug_force_two_launches(False)
+    back = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+    rt.close()
+    assert_parity(oracle_mod, cfg, inp, meta, two, ref)
+    for k in want:
+        assert np.array_equal(one[k], two[k]) and np.array_equal(two[k], two_again[k]) and np.array_equal(one[k], back[k]), k
+
+
 def test_ragged_shapes(torch_cuda, H, oracle_mod):
     """Odd sizes: 3 bins x 5 Gauss points (15 points, half a warp), 7 layers; 1 layer; the maximum 64 layers; a single
     spectral point; and one Gauss point per bin (the opacity-sampling kernel variant) with all outputs, 150 bins."""
