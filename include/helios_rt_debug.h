@@ -15,8 +15,8 @@ extern "C" {
 /* Re-selects the compiled instantiation of rt_step_kernel and the block size of a handle.  A value <= 0 (warps, ppt)
  * or < 0 (the others) keeps the current / any value.  warps: warps per block (1..maxt/32); ppt: spectral points per
  * thread (1, 2, 4; n_gauss must be a multiple; non-isothermal handles: 1); rows: 0 = k-table rows by register-prefetched
- * loads, 1 = by bulk async copies (TMA) into the per-warp shared-memory ring; stk: 1 = back-substitution coefficients in
- * the global workspace, 0 = thread-private local memory (comparison builds only); maxt, minb: the launch bounds the
+ * loads, 1 = by bulk async copies (TMA) into the per-warp shared-memory ring; stk: kept for
+ * ABI stability (the back-substitution coefficients always live in the global workspace; 0 selects nothing: EINVAL); maxt, minb: the launch bounds the
  * instantiation was compiled with (register cap = 65536 / (maxt * minb)).  HELIOS_RT_EINVAL if no such instantiation was
  * compiled or the shape does not fit an SM; the handle is then unchanged.  Re-allocates the shape-dependent workspace:
  * must not be called while a step of this handle is in flight. */
