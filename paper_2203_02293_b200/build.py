@@ -21,10 +21,14 @@ OBJ = CSRC / "build"
 INC = ROOT / "include"
 LIB = PKG / "libhelios_rt.so"
 LIB_SELFTEST = PKG / "libhelios_rt_selftest.so"
-LIBS = {LIB: ("helios_rt", "helios_post"), LIB_SELFTEST: ("helios_rt_selftest",)}
+LIBS = {LIB: ("helios_rt", "helios_rt_k_iso", "helios_rt_k_toa", "helios_rt_k_noniso", "helios_rt_k_sampling", "helios_post"),
+        LIB_SELFTEST: ("helios_rt_selftest",)}
 
+# -split-compile 4, not 0: nvcc optimises the translation unit in that many parts, and the generated code of the kernels
+# depends on the partition (0 = "as many as there are host threads" made the same source build into binaries 3 % apart
+# from one machine, or one moment, to the next).  4 is fixed so that every build is the same build.
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-split-compile", "0"]
+              "-Xcompiler", "-fPIC", "-split-compile", "4"]
 
 
 def nvcc() -> str:
@@ -60,7 +64,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         _run([nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", "-o", str(tmp), str(src)], verbose)
         os.replace(tmp, obj)
 
-    with ThreadPoolExecutor(max_workers=4) as ex:
+    with ThreadPoolExecutor(max_workers=6) as ex:
         list(ex.map(compile_one, todo))
     for lib, stems in LIBS.items():
         members = [objs[s] for s in stems]
