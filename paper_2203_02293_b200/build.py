@@ -24,11 +24,12 @@ LIB_SELFTEST = PKG / "libhelios_rt_selftest.so"
 LIBS = {LIB: ("helios_rt", "helios_rt_k_iso", "helios_rt_k_toa", "helios_rt_k_noniso", "helios_rt_k_sampling", "helios_post"),
         LIB_SELFTEST: ("helios_rt_selftest",)}
 
-# -split-compile 4, not 0: nvcc optimises the translation unit in that many parts, and the generated code of the kernels
-# depends on the partition (0 = "as many as there are host threads" made the same source build into binaries 3 % apart
-# from one machine, or one moment, to the next).  4 is fixed so that every build is the same build.
+# -split-compile 1 (no parallel split of a translation unit): with any larger value -- and with 0, "as many as there are
+# host threads" -- nvcc's code for the kernels differs from one build of the SAME source to the next (measured: three
+# builds in a row, two different binaries, 3 % apart in step time).  Parallelism comes from compiling
+# the translation units side by side instead.
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-split-compile", "4"]
+              "-Xcompiler", "-fPIC", "-split-compile", "1"]
 
 
 def nvcc() -> str:
