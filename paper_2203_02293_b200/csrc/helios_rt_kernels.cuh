@@ -28,7 +28,7 @@ constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
 #define HRT_PA_UNROLL 2   /* config 2: 0.6787 ms at 2, 0.6845 at 4, 0.6851 at 8 */
 #endif
 #ifndef HRT_VOTE_SEL
-#define HRT_VOTE_SEL (!TOA)
+#define HRT_VOTE_SEL (!TOA || BDIRECT)
 #endif
 #define HRT_PRAGMA(x) _Pragma(#x)
 #define HRT_UNROLL(n) HRT_PRAGMA(unroll n)
@@ -780,7 +780,8 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
 #endif
     __syncthreads();                       // s_T32
     const long nblk = (long)gridDim.x * gridDim.y;
-    // (skipping the Planck forms no lane of a warp needs: -1.2 % on config 2, +0.9 % on config 5 -- per-class choice)
+    // (skipping the Planck forms no lane of a warp needs: -0.5 % on config 2, -1.2 % on configs 3 / 4, -7 % on config 6,
+    // +0.9 % on config 5 -- per-class choice: HRT_VOTE_SEL)
     phase_a<NONISO, HRT_VOTE_SEL, BDIRECT>(P, L, s_T32, ((long)blockIdx.y * gridDim.x + blockIdx.x) * nthr + tid, nblk * nthr, true);
     __syncthreads();
     if (tid == 0) {
