@@ -24,6 +24,13 @@ constexpr int MAXL = HELIOS_RT_MAX_LAYERS;
 #ifndef HRT_UNROLL_ISO
 #define HRT_UNROLL_ISO 1
 #endif
+// An empty asm that "modifies" a loop-invariant value: ptxas then keeps it in a register (or spills it) instead of
+// recomputing it from thread / block indices inside the sweep loops
+#define HRT_PIN_PTR(p) asm volatile("" : "+l"(p))
+#define HRT_PIN_F64(x) asm volatile("" : "+d"(x))
+#ifndef HRT_PIN_LEVEL
+#define HRT_PIN_LEVEL 1
+#endif
 #ifndef HRT_PA_UNROLL
 #define HRT_PA_UNROLL 2   /* config 2: 0.6787 ms at 2, 0.6845 at 4, 0.6851 at 8 */
 #endif
@@ -771,6 +778,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   double *red_w = s_red + (size_t)warp * 4 * LP;
   double *stage_w = (double *)(smem + L.off_u + L.u_stage) + (size_t)warp * 8 * STAGE_LD;
   double *stage_wr = stage_w + lane;
+  if (HRT_PIN_LEVEL >= 2) HRT_PIN_PTR(stage_wr);
 
   // ---------------- phase A: this block's share of the (column, level) items of S1 + S2 ----------------
 #ifdef HRT_DIAG_SKIP_PHASE_A   /* timing-only diagnostic build (_work/): phase A on the handle's first launch only */
@@ -793,6 +801,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   Feed<PPT, DEPTH, ROWS> feed;
   if constexpr (ROWS == 0) {
     feed.lnk_pt = P.lnk + pt;
+    HRT_PIN_PTR(feed.lnk_pt);
   } else {
     unsigned char *ring = smem + L.off_u + L.u_ring + (size_t)warp * L.ring_warp;
     feed.ring = (const double *)ring;
@@ -808,6 +817,10 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   double *stk_w = nullptr;
   if (!TOA)
     stk_w = P.stack + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * P.stack_block + (size_t)warp * (N + 1) * SROW;
+  // the lane's own slots of a row: + lane (PPT = 1) or + lane 16-byte pairs
+  double *stk_wl = stk_w ? stk_w + (PPT == 1 ? lane : 2 * lane) : nullptr;
+  HRT_PIN_PTR(stk_w);
+  if (HRT_PIN_LEVEL >= 2) HRT_PIN_PTR(stk_wl);
 
   // ---------------- phase B: columns of this tile's queue ----------------
   // The record block and the tile's Planck block of the NEXT column are fetched by bulk async copies (TMA) into the
@@ -871,8 +884,9 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
     if (warp_on) {
       const double mu = s_dm[N];
       const bool day = mu > 0.0;
-      const double muF = day ? mu * fstar_b : 0.0;            // mu * F_star[b]
-      const double inv_mu = day ? 1.0 / mu : 0.0;
+      double muF = day ? mu * fstar_b : 0.0;                  // mu * F_star[b]
+      double inv_mu = day ? 1.0 / mu : 0.0;
+      HRT_PIN_F64(muF); HRT_PIN_F64(inv_mu);
 
       // back-substitution state per interface i = 0..N: F_up[i] = c F_up[i-1] + d (weight folded into d) and R with
       // F_dn[i] = R F_up[i] + U.  U itself is not kept: sum_points W (U + beam) is reduced on the way down.
@@ -902,7 +916,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
       int srow_i = N;     // row N: the first one sweep 1 writes
       auto keep = [&](const double (&c)[PPT], const double (&wd)[PPT], const double (&Rlow)[PPT]) {
         if (TOA) return;
-        stk_store<PPT>(stk_w + (size_t)(srow_i--) * SROW, lane, c, wd, Rlow);   // (a running pointer measured 1 % slower)
+        stk_store<PPT>(stk_wl + (size_t)(srow_i--) * SROW, 0, c, wd, Rlow);   // (a running pointer measured 1 % slower)
       };
 
       // ---------------- sweep 1: TOA -> BOA (one instantiation per day / night: the loop body has no branch) ------
@@ -1053,19 +1067,19 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         // interfaces, R_N = 0) tests per interface, uniformly, and repeats F_up[N] into rows of the reduction buffer
         // that are never read.  (Measured and rejected: a two-buffer prefetch of the next group,
         // a butterfly instead of the staged transposes.)
-        const double *row = stk_w;
+        const double *row = stk_w, *row_l = stk_wl;
         auto group = [&](auto full_tag, int base) {
           constexpr bool FULL = decltype(full_tag)::value;
           const int nk = N + 1 - base;          // interfaces left (FULL: > 8)
           double gc[8][PPT], gwd[8][PPT], gR[8][PPT], sd[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
-            if (FULL || k < nk) stk_load_cw<PPT>(row + k * SROW, lane, gc[k], gwd[k]);
+            if (FULL || k < nk) stk_load_cw<PPT>(row_l + k * SROW, 0, gc[k], gwd[k]);
             else {
 #pragma unroll
               for (int q = 0; q < PPT; ++q) { gc[k][q] = 1.0; gwd[k][q] = 0.0; }
             }
-            if (FULL || k < nk - 1) stk_load_R<PPT>(row + (k + 1) * SROW, lane, gR[k]);
+            if (FULL || k < nk - 1) stk_load_R<PPT>(row_l + (k + 1) * SROW, 0, gR[k]);
             else {
 #pragma unroll
               for (int q = 0; q < PPT; ++q) gR[k][q] = 0.0;
@@ -1094,7 +1108,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         };
         int base = 0;
 #pragma unroll 1
-        for (; base + 8 <= N; base += 8, row += 8 * SROW) group(std::true_type{}, base);
+        for (; base + 8 <= N; base += 8, row += 8 * SROW, row_l += 8 * SROW) group(std::true_type{}, base);
         group(std::false_type{}, base);
         if (P.F_toa_bin != nullptr) {
 #pragma unroll
