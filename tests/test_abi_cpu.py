@@ -109,3 +109,23 @@ def test_null_handles(lib):
     assert lib.helios_rt_create(None, C.byref(h)) == -1 and not h
     assert lib.helios_rt_launch_info(None, None) == -1
     assert lib.helios_rt_last_cuda_error(None) == b""
+
+
+def test_kernel_build_is_reproducible(tmp_path):
+    """Two compilations of the headline class with build.py's flags give the same SASS, instruction for instruction
+    (with -split-compile other than 1 they do not, and the step time moves by 3 %)."""
+    import subprocess
+    from paper_2203_02293_b200 import build as B
+    src = B.CSRC / "helios_rt_k_iso.cu"
+    assert "-split-compile" in B.NVCC_FLAGS and B.NVCC_FLAGS[B.NVCC_FLAGS.index("-split-compile") + 1] == "1"
+
+    def sass(tag):
+        obj = tmp_path / f"iso_{tag}.o"
+        subprocess.run([B.nvcc(), *B.NVCC_FLAGS, "-c", "-o", str(obj), str(src)], check=True, capture_output=True)
+        out = subprocess.run(["cuobjdump", "-sass", str(obj)], check=True, capture_output=True, text=True).stdout
+        return [ln.split("*/", 1)[1].split("/*")[0].strip() for ln in out.splitlines() if ln.lstrip().startswith("/*") and "*/" in ln and ";" in ln]
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=2) as ex:      # side by side, as build.py compiles its translation units
+        a, b = ex.map(sass, ("a", "b"))
+    assert len(a) > 10000 and a == b
