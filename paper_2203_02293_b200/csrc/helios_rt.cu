@@ -60,10 +60,10 @@ void collect_variants() {
 
 typedef void (*iter_fn)(const KParams, const int);
 
-// spectral points per thread: isothermal columns whose number of Gauss points is a multiple of it, with enough points
-// to fill the tiles.  2 with the back-substitution pass, 4 in TOA mode.
+// spectral points per thread: columns whose number of Gauss points is a multiple of it, with enough points
+// to fill the tiles.  2 with the back-substitution pass (isothermal and non-isothermal), 4 in isothermal TOA mode.
 int default_ppt(int npt, int ng, bool noniso, bool toa) {
-  const bool can2 = !noniso && ng > 1 && (ng % 2) == 0, can4 = can2 && toa && (ng % 4) == 0;
+  const bool can2 = ng > 1 && (ng % 2) == 0, can4 = can2 && !noniso && toa && (ng % 4) == 0;
   if (npt < 256) return 1;
   return can4 ? 4 : (can2 ? 2 : 1);
 }
@@ -71,7 +71,7 @@ int default_ppt(int npt, int ng, bool noniso, bool toa) {
 // warps per block: tiles of 128 spectral points for long columns; small columns take the
 // block with the fewest padded lanes, ties -> larger block (fewer tiles)
 int default_warps(int npt, int ppt, bool noniso) {
-  if (npt >= 256) return noniso ? 4 : (ppt == 4 ? 1 : (ppt == 2 ? 2 : 4));
+  if (npt >= 256) return ppt == 4 ? 1 : (ppt == 2 ? 2 : 4);
   int best = 1;
   long best_waste = -1;
   for (int w = 1; w <= 4; ++w) {
@@ -638,7 +638,7 @@ extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t p
   if (!h) return HELIOS_RT_EINVAL;
   const Variant &cur = kVariants[h->variant];
   const int want_ppt = ppt > 0 ? ppt : cur.ppt;
-  if (want_ppt > 1 && (h->noniso ? false : (h->cfg.n_gauss % want_ppt) != 0)) return HELIOS_RT_EINVAL;
+  if (want_ppt > 1 && (h->cfg.n_gauss % want_ppt) != 0) return HELIOS_RT_EINVAL;
   const int want_warps = warps > 0 ? warps : h->warps;
   const int v = find_variant(h->noniso, h->toa, cur.bdirect, want_ppt, rows, stk, maxt, minb, want_warps);
   if (v < 0) return HELIOS_RT_EINVAL;
