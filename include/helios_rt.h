@@ -183,6 +183,49 @@ int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t n_phases, c
 /* Size in bytes of the scratch buffer helios_rt_phase_curve needs (>= 8; negative = HELIOS_RT_EINVAL). */
 int64_t helios_rt_phase_curve_workspace_bytes(int32_t n_columns, int32_t n_bins, int32_t n_phases);
 
+/* ---- helios_rt_phase_curve for callers that must not allocate --------------------------------------------------
+ *
+ * Who this is for.  helios_rt_phase_curve needs a scratch buffer (the partial sums per chunk of 128 columns), and
+ * normally the caller gets it from cudaMalloc or from a framework's allocator.  Some callers cannot do either at
+ * the point where they want the phase curve: code running inside a host callback or a plug-in hook of a larger
+ * application that owns all device memory and hands out none; a real-time or fault-handling path that must not
+ * enter the driver's allocator (an allocation can block for milliseconds, fail when the device is full, or
+ * synchronise the whole device and so stall other streams); a worker whose memory budget was fixed at start-up
+ * and is already spent on its handles.  For them this variant brings its own scratch: a fixed array of
+ * HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES that is part of the library image itself (a file-scope
+ * `static __device__` array in helios_post.cu).  The call performs no cudaMalloc / cudaFree and calls no library
+ * routine that allocates; the caller passes inputs and outputs only.
+ *
+ * Same arguments, results and errors as helios_rt_phase_curve, minus `workspace`: the two paths run the same
+ * kernels in the same order, so for the same inputs the outputs are bit-identical.
+ *
+ * What it costs and what to watch:
+ *   - Size limit.  helios_rt_phase_curve_workspace_bytes(n_columns, n_bins, n_phases) must not exceed
+ *     HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES (8 MiB: e.g. 2562 columns x 64 phases x 780 bins, or 10242 columns x
+ *     64 phases x 200 bins).  Anything larger is refused with HELIOS_RT_ETOOBIG before any work is queued; use
+ *     helios_rt_phase_curve with your own buffer for those.
+ *   - Memory.  Every GPU on which this process loads the library's device code carries the 8 MiB from then until
+ *     the process exits, whether or not this function is ever called.
+ *   - First call on a device.  The first call made while a given device is current looks up where the array lives
+ *     on THAT device (cudaGetSymbolAddress; one array exists per device, at different addresses) and remembers the
+ *     answer; later calls on that device only read it.  The look-up may make the CUDA runtime load the library's
+ *     device code, so make this first call during start-up, outside any stream capture.  The device that is current
+ *     at the call must be the device `cuda_stream` and all the pointers belong to.
+ *   - One array, shared.  All calls on a device use the same scratch, and it keeps whatever the last call left in
+ *     it.  Nothing in it needs to start at zero (every element the second kernel reads is first written by the
+ *     first kernel of the same call), so no clearing is done.  But two calls that can overlap on the GPU -- issued on
+ *     different streams, or from different host threads, without an event or synchronisation ordering them -- write
+ *     over each other's partial sums and both results are garbage.  Keep calls on one device stream-ordered.
+ *   - Host threads.  The one-time look-up is guarded by a lock; after it the function is as thread-safe as
+ *     helios_rt_phase_curve, subject to the previous point. */
+#define HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES 8388608
+#define HELIOS_RT_ETOOBIG  -5  /* helios_rt_phase_curve_noalloc: the problem needs more scratch than the built-in
+                                  array holds (HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES)                       */
+int helios_rt_phase_curve_noalloc(int32_t n_columns, int32_t n_bins, int32_t n_phases, const double *F_toa_bin,
+                                  const double *lon, const double *lat, const double *area, const double *alpha,
+                                  const double *bin_edges, double lam1, double lam2, double *F_phase_bin,
+                                  double *F_phase_band, void *cuda_stream);
+
 /* "1-D mode" (Sec. 3): explicit temperature step T <- T + dt * dTdt (dTdt NULL: T unchanged) followed
  * by the hydrostatic re-balance of Eq.(20) on the fixed altitude grid z [n_layers] (m, ascending): p[.][0] =
  * p_ref, p_i = p_{i-1} (1/dz - g/(2 R_d T_{i-1})) / (1/dz + g/(2 R_d T_i)) (sign of the denominator: reading

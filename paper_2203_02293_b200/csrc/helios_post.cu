@@ -3,6 +3,8 @@
 //   helios_rt_extend_top   PAPER.md L385: columns extended isothermally to <= p_min before the post-processing step
 //   helios_rt_phase_curve  Eqs.(25)-(26) L546-552 (+ the wavelength integral of Eq.(23))
 //   helios_rt_advance_1d   Sec. 3 "1-D mode": T <- T + dt dT/dt, hydrostatic re-balance Eq.(20)
+//   helios_rt_phase_curve_noalloc   helios_rt_phase_curve with its scratch in a built-in device array, for callers
+//                          that cannot allocate (described where it is defined, near the end of this file)
 //
 // C ABI: include/helios_rt.h.  All pointers are DEVICE pointers; every call is asynchronous on the given
 // stream, allocates nothing and synchronises nothing, so the calls can be captured in a CUDA graph together
@@ -13,6 +15,8 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+
+#include <mutex>
 
 namespace {
 
@@ -218,6 +222,66 @@ extern "C" int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t 
     if (cudaGetLastError() != cudaSuccess) return HELIOS_RT_ECUDA;
   }
   return HELIOS_RT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// helios_rt_phase_curve_noalloc: the phase curve for callers that may not allocate device memory (a plug-in inside
+// an application that owns the whole device, a real-time path that must stay out of the driver's allocator, a
+// worker whose memory budget is spent; include/helios_rt.h has the full contract).  The partial sums of
+// phase_partial_kernel go to g_phase_scratch, an array that is part of this library's device image, instead of a
+// buffer the caller had to allocate.
+//
+// g_phase_scratch is a DEVICE symbol.  In host code its name is only a host-side stand-in -- it is not a device
+// address, and a kernel handed `g_phase_scratch` from the host would fault (or, on a system where the GPU can reach
+// host memory, quietly use the wrong memory).  Each device holds its own copy at its own address, so the address is
+// asked for once per device, with that device current, and cached by device ordinal.
+// ---------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_phase_scratch[HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES / sizeof(double)];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_scratch_mutex;
+double *g_scratch_addr[kMaxDevices];   // [device ordinal] -> address of g_phase_scratch on that device; nullptr = not asked yet
+
+// Device address of g_phase_scratch on the CURRENT device.  The first call per device asks the runtime (which may
+// load this library's device code: do it before any stream capture); later calls read the cache.  No allocation.
+int phase_scratch_address(double **out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return HELIOS_RT_ENODEV; }
+  if (dev < 0 || dev >= kMaxDevices) return HELIOS_RT_ENODEV;
+  std::lock_guard<std::mutex> lock(g_scratch_mutex);
+  if (!g_scratch_addr[dev]) {
+    void *addr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&addr, g_phase_scratch);
+    if (e != cudaSuccess || !addr) { cudaGetLastError(); return HELIOS_RT_ECUDA; }
+    g_scratch_addr[dev] = static_cast<double *>(addr);
+  }
+  *out = g_scratch_addr[dev];
+  return HELIOS_RT_OK;
+}
+
+}  // namespace
+
+extern "C" int helios_rt_phase_curve_noalloc(int32_t n_columns, int32_t n_bins, int32_t n_phases, const double *F_toa_bin,
+                                             const double *lon, const double *lat, const double *area,
+                                             const double *alpha, const double *bin_edges, double lam1, double lam2,
+                                             double *F_phase_bin, double *F_phase_band, void *cuda_stream) {
+  // Size first: a problem that does not fit the built-in array is refused before anything is queued.
+  const int64_t need = helios_rt_phase_curve_workspace_bytes(n_columns, n_bins, n_phases);
+  if (need < 0) return HELIOS_RT_EINVAL;
+  if (need > (int64_t)HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES) return HELIOS_RT_ETOOBIG;
+  int rc = device_ok();
+  if (rc) return rc;
+  double *scratch = nullptr;
+  rc = phase_scratch_address(&scratch);
+  if (rc) return rc;
+  // Same kernels, same order as the caller-workspace path; only where the partial sums live differs.  The array
+  // keeps the previous call's partial sums; phase_partial_kernel overwrites every element phase_reduce_kernel reads
+  // (chunk < nchunk, phase < n_phases, bin < n_bins), so nothing has to be cleared.  Calls that overlap on the GPU
+  // would share these partial sums and race: callers keep them stream-ordered.
+  return helios_rt_phase_curve(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, bin_edges, lam1, lam2,
+                               F_phase_bin, F_phase_band, scratch, cuda_stream);
 }
 
 extern "C" int helios_rt_advance_1d(int32_t n_columns, int32_t n_layers, double dt, double gravity, double R_d, double p_ref,

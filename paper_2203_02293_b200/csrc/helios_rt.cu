@@ -130,6 +130,8 @@ extern "C" const char *helios_rt_strerror(int code) {
     case HELIOS_RT_ENOMEM: return "out of memory";
     case HELIOS_RT_ECUDA: return "CUDA runtime error (see helios_rt_last_cuda_error)";
     case HELIOS_RT_ENODEV: return "no usable CUDA device (compute capability 10.x required)";
+    case HELIOS_RT_ETOOBIG: return "problem too large for the built-in scratch array of helios_rt_phase_curve_noalloc "
+                                   "(HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES); use helios_rt_phase_curve with your own workspace";
     default: return "unknown error code";
   }
 }

@@ -21,6 +21,7 @@ _dp = C.POINTER(C.c_double)
 EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_rt_destroy",
            "helios_rt_strerror", "helios_rt_last_cuda_error", "helios_rt_launch_info", "helios_rt_step_iterative",
            "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_phase_curve_workspace_bytes",
+           "helios_rt_phase_curve_noalloc",
            "helios_rt_advance_1d", "helios_rt_debug_set_launch", "helios_rt_debug_get_launch",
            "helios_rt_debug_force_two_launches")
 # ... and in include/helios_rt_selftest.h (libhelios_rt_selftest.so)
@@ -83,6 +84,8 @@ def load_library() -> C.CDLL:
         L.helios_rt_extend_top.argtypes = [C.c_int32] * 3 + [C.c_double] + [C.c_void_p] * 5
         L.helios_rt_phase_curve.restype = C.c_int
         L.helios_rt_phase_curve.argtypes = [C.c_int32] * 3 + [C.c_void_p] * 6 + [C.c_double] * 2 + [C.c_void_p] * 4
+        L.helios_rt_phase_curve_noalloc.restype = C.c_int
+        L.helios_rt_phase_curve_noalloc.argtypes = [C.c_int32] * 3 + [C.c_void_p] * 6 + [C.c_double] * 2 + [C.c_void_p] * 3
         L.helios_rt_phase_curve_workspace_bytes.restype = C.c_int64
         L.helios_rt_phase_curve_workspace_bytes.argtypes = [C.c_int32] * 3
         L.helios_rt_advance_1d.restype = C.c_int
@@ -309,6 +312,35 @@ def phase_curve(F_toa_bin, lon, lat, area, alpha, F_phase_bin, bin_edges=None, l
         _dev(F_phase_bin, (na, nb), "F_phase_bin"),
         None if F_phase_band is None else _dev(F_phase_band, (na,), "F_phase_band"), workspace.data_ptr(),
         _stream(stream)))
+
+
+PHASE_CURVE_NOALLOC_MAX_BYTES = 8 << 20   # HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES of include/helios_rt.h
+
+
+def phase_curve_noalloc(F_toa_bin, lon, lat, area, alpha, F_phase_bin, bin_edges=None, lam1=0.0, lam2=0.0,
+                        F_phase_band=None, stream=None) -> None:
+    """helios_rt_phase_curve_noalloc on CUDA tensors: the phase curve (same arguments and bit-identical results as
+    `phase_curve`) for code that is not allowed to allocate device memory where it runs -- a plug-in inside an
+    application that owns the whole GPU, a latency-critical path that must not enter the CUDA allocator, a worker
+    whose memory budget is already spent.  The scratch that `phase_curve` takes as `workspace` is a fixed 8 MiB array
+    inside libhelios_rt.so instead, so:
+
+    * problems needing more than PHASE_CURVE_NOALLOC_MAX_BYTES of scratch (ceil(n/128) * n_phases * n_bins * 8
+      bytes) raise HeliosRTError with code -5; use `phase_curve` with your own workspace for those;
+    * make the first call on each device at start-up, outside any stream capture (it looks up the array's address
+      on that device, once), with the tensors' device as the current device;
+    * every call on a device shares that one array: keep the calls stream-ordered -- two that overlap on the GPU
+      corrupt each other.
+
+    This wrapper creates no tensor either (it passes the pointers of the ones it is given)."""
+    n, nb = F_toa_bin.shape
+    na = alpha.shape[0]
+    _check(load_library().helios_rt_phase_curve_noalloc(
+        n, nb, na, _dev(F_toa_bin, (n, nb), "F_toa_bin"), _dev(lon, (n,), "lon"), _dev(lat, (n,), "lat"),
+        _dev(area, (n,), "area"), _dev(alpha, (na,), "alpha"),
+        None if bin_edges is None else _dev(bin_edges, (nb + 1,), "bin_edges"), float(lam1), float(lam2),
+        _dev(F_phase_bin, (na, nb), "F_phase_bin"),
+        None if F_phase_band is None else _dev(F_phase_band, (na,), "F_phase_band"), _stream(stream)))
 
 
 def advance_1d(dt: float, gravity: float, R_d: float, p_ref: float, z, dTdt, T, p, rho=None, stream=None) -> None:

@@ -59,6 +59,19 @@ def test_strerror(lib):
     assert b"unknown" in lib.helios_rt_strerror(-77)
 
 
+def test_noalloc_phase_curve_size_limit_is_checked_on_the_host(lib):
+    """helios_rt_phase_curve_noalloc refuses a problem whose scratch exceeds the built-in 8 MiB array with ETOOBIG (-5)
+    before it touches the device, so the limit can be checked here without a GPU; malformed sizes stay EINVAL."""
+    from paper_2203_02293_b200 import helios_rt
+    assert helios_rt.PHASE_CURVE_NOALLOC_MAX_BYTES == 8388608
+    assert "8388608" in (ROOT / "include" / "helios_rt.h").read_text()
+    call = lambda n, nb, na: lib.helios_rt_phase_curve_noalloc(n, nb, na, None, None, None, None, None, None, 0.0, 0.0,
+                                                               None, None, None)
+    assert call(2562, 781, 64) == -5 and call(10242, 3256, 64) == -5
+    assert call(-1, 30, 4) == -1 and call(16, 0, 4) == -1
+    assert b"too large" in lib.helios_rt_strerror(-5)
+
+
 def _cfg():
     from paper_2203_02293_b200 import workloads as W
     cfg, inp, meta = W.make(1)
