@@ -119,7 +119,16 @@ int helios_rt_create(const helios_rt_config *cfg, helios_rt **out);
  * enqueued on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream); no host synchronisation, no
  * allocation, no host<->device copy.  Outputs are complete when the stream reaches this point.  NaN inputs
  * propagate to the outputs of their own column only; (p, T) outside the table are clamped to its
- * edge (no extrapolation, not an error). */
+ * edge (no extrapolation, not an error).
+ *
+ * One exception to "one launch" and to bit-reproducibility, for F_up_toa_bin only: when the thread-block tile of the
+ * spectral axis (helios_rt_launch_info: info[0] x points per thread) is not a multiple of n_gauss, some bins have
+ * their Gauss points in two tiles (BASELINE config 5: tiles of 128 points, n_gauss = 20).  Such a step first
+ * launches a zero-fill of F_up_toa_bin (info[6] = 2 for a TOA_SPECTRUM handle; a full-output handle does the same in
+ * the steps that ask for F_up_toa_bin) and the tiles add their parts with atomicAdd.  With at most two
+ * tiles per bin (n_gauss <= tile) the sum of two terms is the same in either order, so the result is still
+ * bit-reproducible; with n_gauss > tile (three or more tiles per bin) the last bits may differ from run to run.
+ * F_up, F_down, F_net, dTdt and F_beam are always summed in a fixed order. */
 int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
                    void *cuda_stream);
 
@@ -151,7 +160,8 @@ const char *helios_rt_last_cuda_error(const helios_rt *h);
 /* Launch geometry of the step kernel, for benchmarks and profiles:
  * info[0] = threads per block, [1] = tiles of the spectral axis per column (the persistent grid is tiles x workers),
  * [2] = dynamic shared memory bytes, [3] = registers per thread, [4] = resident blocks per SM (occupancy API),
- * [5] = local-memory bytes per thread, [6] = kernels launched per step (1), [7] = SM count of the device. */
+ * [5] = local-memory bytes per thread, [6] = kernels launched per step (1; 2 for a TOA_SPECTRUM handle whose bins
+ * straddle tiles, see helios_rt_step), [7] = SM count of the device. */
 int helios_rt_launch_info(const helios_rt *h, int32_t info[8]);
 
 /* ---- the steps either side of the RT step.  DEVICE pointers, fp64,

@@ -18,7 +18,10 @@
 //       2x2 block, so Eqs.(13)-(14) reduce to the scalar recurrences (R, U, c, d) below, carried in registers.
 //       The back-substitution coefficients (c, W d, R) of every interface go to a per-block slab of a global
 //       workspace sized to the resident grid (coalesced 16-byte stores), which the persistent block reuses column
-//       after column, so it lives in L2; its lines are discarded (discard.global.L2) once sweep 2 has read them.
+//       after column.  Where the slabs of the whole grid fit the 126 MB L2 (config 3: 75 MB) they stay there; at the
+//       default config-2 shape they do not (141 MiB: about 40 % of the row stores are written back to HBM and 0.2 GB
+//       read again, 0.83 GB of DRAM traffic per launch; DESIGN.md section 9 has the measurements).  Lines are
+//       discarded (discard.global.L2) once sweep 2 has read them, which saves the write-back of those still in L2.
 //   sweep 2 (BOA -> TOA): back-substitution Eq.(15) fused with S7, the Gauss-/bin-weighted reduction (shared-memory
 //       transposes + warp shuffles, then a fixed-order sum over warps and tiles).
 //
@@ -34,6 +37,8 @@
 
 #include "helios_rt_kernels.cuh"
 
+#include <mutex>
+
 namespace {
 
 using namespace hrt;
@@ -47,15 +52,20 @@ __global__ void zero_kernel(double *p, size_t n) {
     p[i] = 0.0;
 }
 
-// all compiled instantiations of rt_step_kernel, class by class (filled on first use)
+// all compiled instantiations of rt_step_kernel, class by class; filled exactly once (std::call_once), so host threads
+// that create handles at the same time all see the complete table
 Variant kVariants[64];
 int kNumVariants = 0;
+std::once_flag kVariantsOnce;
 void collect_variants() {
-  if (kNumVariants) return;
-  const Variant *tabs[4] = {kVariantsIsoFull, kVariantsIsoToa, kVariantsNoniso, kVariantsSampling};
-  const int n[4] = {kNumIsoFull, kNumIsoToa, kNumNoniso, kNumSampling};
-  for (int t = 0; t < 4; ++t)
-    for (int i = 0; i < n[t] && kNumVariants < 64; ++i) kVariants[kNumVariants++] = tabs[t][i];
+  std::call_once(kVariantsOnce, [] {
+    const Variant *tabs[4] = {kVariantsIsoFull, kVariantsIsoToa, kVariantsNoniso, kVariantsSampling};
+    const int n[4] = {kNumIsoFull, kNumIsoToa, kNumNoniso, kNumSampling};
+    int k = 0;
+    for (int t = 0; t < 4; ++t)
+      for (int i = 0; i < n[t] && k < 64; ++i) kVariants[k++] = tabs[t][i];
+    kNumVariants = k;
+  });
 }
 
 typedef void (*iter_fn)(const KParams, const int);
@@ -105,15 +115,14 @@ struct helios_rt {
   unsigned *d_counter, *d_queue, *d_flags;
   BinSlot *d_bslot, *d_bslot_iter;
   int *d_slot_ptr, *d_slots, *d_slot_ptr_iter, *d_slots_iter;   // bin -> Planck-block slots (step tiling / comparison tiling)
-  unsigned epoch;
   Lay iter_lay;
   double *inv_dlam;          // host copy, [n_bins]
   // device + pinned host staging for step_host
   double *d_in, *d_out, *h_in, *h_out;
-  cudaStream_t own_stream, copy_stream;
-  cudaEvent_t ev_in[4], ev_done[4];
+  cudaStream_t own_stream;   // step_host runs on it
   int regs, lmem, sm_count;
   int force_two_launches;   // helios_rt_debug_force_two_launches: always take the fallback path (tests)
+  int workers_cap;          // helios_rt_debug_set_workers: upper bound of workers per tile (0 = none; tuning runs)
   cudaError_t last_err;
 };
 
@@ -207,11 +216,6 @@ extern "C" int helios_rt_destroy(helios_rt *h) {
   if (h->h_in) cudaFreeHost(h->h_in);
   if (h->h_out) cudaFreeHost(h->h_out);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
-  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
-  for (int i = 0; i < 4; ++i) {
-    if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
-    if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
-  }
   delete h;
   return HELIOS_RT_OK;
 }
@@ -275,6 +279,7 @@ static int configure_launch(helios_rt *h) {
   long workers = (long)h->sm_count * h->occ / h->tiles;
   if (workers < 1) workers = 1;
   if (workers > c.max_columns) workers = c.max_columns;
+  if (h->workers_cap > 0 && workers > h->workers_cap) workers = h->workers_cap;
   h->workers = (int)workers;
   // workspace
   cudaFree(h->d_stack); h->d_stack = nullptr;
@@ -316,14 +321,13 @@ static int configure_launch(helios_rt *h) {
 }
 
 // first instantiation of the class that matches; one compiled for exactly `warps` warps is preferred to a generic one
-static int find_variant(bool noniso, bool toa, bool bdirect, int ppt, int rows, int stk, int maxt, int minb, int warps) {
+static int find_variant(bool noniso, bool toa, bool bdirect, int ppt, int rows, int maxt, int minb, int warps) {
   for (int pass = 0; pass < 2; ++pass)
   for (int i = 0; i < kNumVariants; ++i) {
     const Variant &v = kVariants[i];
     if (v.noniso != noniso || v.toa != toa || v.bdirect != bdirect || v.ppt != ppt) continue;
     if (pass == 0 ? v.warps != warps : v.warps != 0) continue;
     if (rows >= 0 && v.rows != rows) continue;
-    if (stk == 0) continue;   // the thread-private stack of round 1 is gone
     if (maxt >= 0 && v.maxt != maxt) continue;
     if (minb >= 0 && v.minb != minb) continue;
     return i;
@@ -354,11 +358,11 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   h->iter_tiles = (h->npt + h->iter_warps * 32 - 1) / (h->iter_warps * 32);
   int ppt = default_ppt(h->npt, ng, h->noniso, h->toa);
   h->warps = default_warps(h->npt, ppt, h->noniso);
-  h->variant = find_variant(h->noniso, h->toa, ng == 1, ppt, -1, -1, -1, -1, h->warps);
+  h->variant = find_variant(h->noniso, h->toa, ng == 1, ppt, -1, -1, -1, h->warps);
   if (h->variant < 0) {
     ppt = 1;
     h->warps = default_warps(h->npt, 1, h->noniso);
-    h->variant = find_variant(h->noniso, h->toa, ng == 1, 1, -1, -1, -1, -1, h->warps);
+    h->variant = find_variant(h->noniso, h->toa, ng == 1, 1, -1, -1, -1, h->warps);
   }
   int dev = 0;
   cudaGetDevice(&dev);
@@ -427,11 +431,6 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(cudaMalloc((void **)&h->d_in, sizeof(double) * n_in));
   step(cudaMalloc((void **)&h->d_out, sizeof(double) * n_out));
   step(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
-  step(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
-  for (int i = 0; i < 4; ++i) {
-    step(cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming));
-    step(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
-  }
   if (e == cudaSuccess) {
     iter_fn it = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
     if (!h->toa)
@@ -467,8 +466,8 @@ static int validate_step(const helios_rt *h, const helios_rt_inputs *in, const h
   return HELIOS_RT_OK;
 }
 
-// col0: first column of a chunk (step_host pipelines chunks; helios_rt_step passes 0); the chunk's inputs and outputs
-// start at column 0 of the given pointers
+// Enqueues one step on `st`: rt_step_kernel (n_iter == 0) or the comparison scheme rt_prep_kernel + rt_iter_kernel
+// (n_iter > 0).  Pointers in `in` / `out` are device pointers (or device aliases of mapped host memory).
 static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out, cudaStream_t st,
                        int n_iter = 0) {
   const helios_rt_config &c = h->cfg;
@@ -489,7 +488,6 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.F_toa_bin = out->F_up_toa_bin;
   P.ws_rec = h->d_ws_rec; P.ws_B = h->d_ws_B; P.flags = h->d_flags;
   P.slot_ptr = h->d_slot_ptr; P.slots = h->d_slots; P.bslot = h->d_bslot;
-  ++h->epoch;
   P.fused_prep = 0;
   P.stack = h->d_stack; P.stack_block = h->stack_block;
   P.partial = h->d_partial; P.counter = h->d_counter; P.queue = h->d_queue;
@@ -531,16 +529,9 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   attr.val.cooperative = 1;
   lc.attrs = &attr;
   lc.numAttrs = 1;
-  P.fused_prep = h->epoch == 1 ? 1 : 2;   // (2: a later launch of the handle; only diagnostic builds care)
-#ifdef HRT_DIAG_NOCOOP         /* diagnostic builds (_work/): plain launch / phase A as its own launch */
-  lc.numAttrs = 0;
-#endif
-#ifdef HRT_DIAG_TWO_LAUNCH
-  cudaError_t e = cudaErrorNotSupported;
-#else
+  P.fused_prep = 1;
   void *args[1] = {&P};
   cudaError_t e = h->force_two_launches ? cudaErrorCooperativeLaunchTooLarge : cudaLaunchKernelExC(&lc, kVariants[h->variant].fn, args);
-#endif
   if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) {
     cudaGetLastError();
     P.fused_prep = 0;
@@ -629,26 +620,36 @@ extern "C" int helios_rt_launch_info(const helios_rt *h, int32_t info[8]) {
   if (!h || !info) return HELIOS_RT_EINVAL;
   info[0] = h->warps * 32; info[1] = h->tiles; info[2] = (int32_t)h->lay.total; info[3] = h->regs; info[4] = h->occ;
   info[5] = h->lmem;
-  info[6] = 1;   // rt_step_kernel (+1 zero-fill launch when F_up_toa_bin bins straddle tiles)
+  // rt_step_kernel, + 1 zero-fill launch where F_up_toa_bin is accumulated with atomics (bins that straddle tiles)
+  info[6] = (h->toa && h->tiles > 1 && ((h->warps * 32 * h->ppt) % h->cfg.n_gauss) != 0) ? 2 : 1;
   info[7] = h->sm_count;
   return HELIOS_RT_OK;
 }
 
 // ---- include/helios_rt_debug.h: not part of the product API ----
-extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t ppt, int32_t rows, int32_t stk,
-                                          int32_t maxt, int32_t minb) {
+extern "C" int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t ppt, int32_t rows, int32_t maxt,
+                                          int32_t minb) {
   if (!h) return HELIOS_RT_EINVAL;
   const Variant &cur = kVariants[h->variant];
   const int want_ppt = ppt > 0 ? ppt : cur.ppt;
   if (want_ppt > 1 && (h->cfg.n_gauss % want_ppt) != 0) return HELIOS_RT_EINVAL;
   const int want_warps = warps > 0 ? warps : h->warps;
-  const int v = find_variant(h->noniso, h->toa, cur.bdirect, want_ppt, rows, stk, maxt, minb, want_warps);
+  const int v = find_variant(h->noniso, h->toa, cur.bdirect, want_ppt, rows, maxt, minb, want_warps);
   if (v < 0) return HELIOS_RT_EINVAL;
   const int old_v = h->variant, old_w = h->warps;
   h->variant = v;
   h->warps = want_warps;
   int rc = configure_launch(h);
   if (rc) { h->variant = old_v; h->warps = old_w; configure_launch(h); }
+  return rc;
+}
+
+extern "C" int helios_rt_debug_set_workers(helios_rt *h, int32_t workers) {
+  if (!h || workers < 0) return HELIOS_RT_EINVAL;
+  const int old = h->workers_cap;
+  h->workers_cap = workers;
+  int rc = configure_launch(h);
+  if (rc) { h->workers_cap = old; configure_launch(h); }
   return rc;
 }
 
@@ -661,7 +662,7 @@ extern "C" int helios_rt_debug_force_two_launches(helios_rt *h, int32_t on) {
 extern "C" int helios_rt_debug_get_launch(const helios_rt *h, int32_t info[16]) {
   if (!h || !info) return HELIOS_RT_EINVAL;
   const Variant &v = kVariants[h->variant];
-  info[0] = h->warps; info[1] = v.ppt; info[2] = v.rows; info[3] = 1; info[4] = v.maxt; info[5] = v.minb;
+  info[0] = h->warps; info[1] = v.ppt; info[2] = v.rows; info[3] = 0; info[4] = v.maxt; info[5] = v.minb;
   info[6] = h->tiles; info[7] = h->workers; info[8] = h->occ; info[9] = h->regs; info[10] = h->lmem;
   info[11] = (int32_t)h->lay.total; info[12] = (int32_t)(h->stack_bytes >> 20); info[13] = h->variant;
   info[14] = kNumVariants; info[15] = 0;

@@ -781,11 +781,7 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   if (HRT_PIN_LEVEL >= 2) HRT_PIN_PTR(stage_wr);
 
   // ---------------- phase A: this block's share of the (column, level) items of S1 + S2 ----------------
-#ifdef HRT_DIAG_SKIP_PHASE_A   /* timing-only diagnostic build (_work/): phase A on the handle's first launch only */
-  if (P.fused_prep == 1) {
-#else
   if (P.fused_prep) {
-#endif
     __syncthreads();                       // s_T32
     const long nblk = (long)gridDim.x * gridDim.y;
     // (skipping the Planck forms no lane of a warp needs: -0.5 % on config 2, -1.2 % on configs 3 / 4, -7 % on config 6,
@@ -826,9 +822,6 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   // The record block and the tile's Planck block of the NEXT column are fetched by bulk async copies (TMA) into the
   // other shared-memory buffer while this column is swept; thread 0 first waits for the column's publication flag.
   bool all_published = false;               // thread 0: every block has finished phase A -- no more flag polls
-#ifdef HRT_DIAG_SKIP_PHASE_A
-  if (P.fused_prep == 2) all_published = true;
-#endif
   auto fetch_column = [&](int c, int buf) {   // thread 0
     // (the whole grid is resident -- cooperative launch -- and phase A waits for nothing, so this terminates; the
     // poll count is bounded all the same: a wedged GPU is worse than a wrong column)
@@ -1101,8 +1094,9 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
 #pragma unroll
           for (int k = 0; k < 8; ++k) stage_wr[k * STAGE_LD] = sd[k];
           flush_stage(stage_w, red_w + LP + base, lane);
-          // rows base .. base+7 are dead (the R part of row base+8 is not: next group's discard): drop their lines from
-          // L2 instead of writing them back
+          // rows base .. base+7 are dead (the R part of row base+8 is not: next group's discard): drop the lines that
+          // are still in L2 instead of writing them back (at the config-2 shape the oldest rows have already been
+          // evicted to HBM by then: helios_rt.cu header)
           const int n_lines = (FULL ? 8 : nk) * (SROW / 16);
           for (int ln = lane; ln < n_lines; ln += 32) l2_discard(row + ln * 16);
         };

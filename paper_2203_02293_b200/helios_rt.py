@@ -23,7 +23,7 @@ EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_
            "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_phase_curve_workspace_bytes",
            "helios_rt_phase_curve_noalloc",
            "helios_rt_advance_1d", "helios_rt_debug_set_launch", "helios_rt_debug_get_launch",
-           "helios_rt_debug_force_two_launches")
+           "helios_rt_debug_force_two_launches", "helios_rt_debug_set_workers")
 # ... and in include/helios_rt_selftest.h (libhelios_rt_selftest.so)
 SELFTEST_EXPORTS = ("helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_selftest_planck_G",
                     "helios_rt_measure_dfma_peak", "helios_rt_measure_latencies")
@@ -92,8 +92,10 @@ def load_library() -> C.CDLL:
         L.helios_rt_advance_1d.argtypes = [C.c_int32] * 2 + [C.c_double] * 4 + [C.c_void_p] * 6
         L.helios_rt_debug_force_two_launches.restype = C.c_int
         L.helios_rt_debug_force_two_launches.argtypes = [C.c_void_p, C.c_int32]
+        L.helios_rt_debug_set_workers.restype = C.c_int
+        L.helios_rt_debug_set_workers.argtypes = [C.c_void_p, C.c_int32]
         L.helios_rt_debug_set_launch.restype = C.c_int
-        L.helios_rt_debug_set_launch.argtypes = [C.c_void_p] + [C.c_int32] * 6
+        L.helios_rt_debug_set_launch.argtypes = [C.c_void_p] + [C.c_int32] * 5
         L.helios_rt_debug_get_launch.restype = C.c_int
         L.helios_rt_debug_get_launch.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
         _lib = L
@@ -184,11 +186,14 @@ class HeliosRT:
                 "sm_count")
         return dict(zip(keys, list(info)))
 
-    def debug_set_launch(self, warps: int = 0, ppt: int = 0, rows: int = -1, stk: int = -1, maxt: int = -1,
-                         minb: int = -1) -> None:
+    def debug_set_launch(self, warps: int = 0, ppt: int = 0, rows: int = -1, maxt: int = -1, minb: int = -1) -> None:
         """helios_rt_debug_set_launch (include/helios_rt_debug.h; tests and tuning only)."""
-        _check(load_library().helios_rt_debug_set_launch(self._h, int(warps), int(ppt), int(rows), int(stk), int(maxt),
-                                                         int(minb)), self._h)
+        _check(load_library().helios_rt_debug_set_launch(self._h, int(warps), int(ppt), int(rows), int(maxt), int(minb)),
+               self._h)
+
+    def debug_set_workers(self, workers: int) -> None:
+        """helios_rt_debug_set_workers (helios_rt_debug.h; tuning only): cap the persistent workers per tile (0 = no cap)."""
+        _check(load_library().helios_rt_debug_set_workers(self._h, int(workers)), self._h)
 
     def debug_force_two_launches(self, on: bool = True) -> None:
         """Tests only (helios_rt_debug.h): take the non-cooperative fallback path (rt_prep_kernel + plain launch)."""
@@ -197,7 +202,7 @@ class HeliosRT:
     def debug_get_launch(self) -> dict:
         info = (C.c_int32 * 16)()
         _check(load_library().helios_rt_debug_get_launch(self._h, info))
-        keys = ("warps", "ppt", "rows", "stk", "maxt", "minb", "tiles", "workers", "blocks_per_sm", "registers",
+        keys = ("warps", "ppt", "rows", "unused", "maxt", "minb", "tiles", "workers", "blocks_per_sm", "registers",
                 "local_bytes", "smem_bytes", "stack_mib", "variant", "n_variants")
         return dict(zip(keys, list(info)))
 

@@ -271,13 +271,12 @@ def _variants(H, rt):
     out = []
     for ppt in (1, 2, 4):
         for rows in (0, 1):
-            for stk in (0, 1):
-                for maxt in (384, 512, 576, 640, 768, 1024):
-                    try:
-                        rt.debug_set_launch(ppt=ppt, rows=rows, stk=stk, maxt=maxt)
-                    except H.HeliosRTError:
-                        continue
-                    out.append((ppt, rows, stk, maxt))
+            for maxt in (384, 512, 576, 640, 768, 1024):
+                try:
+                    rt.debug_set_launch(ppt=ppt, rows=rows, maxt=maxt)
+                except H.HeliosRTError:
+                    continue
+                out.append((ppt, rows, maxt))
     return out
 
 
@@ -293,8 +292,8 @@ def test_every_compiled_variant(torch_cuda, H, oracle_mod, config, stride):
     variants = _variants(H, rt)
     assert len(variants) >= 1
     seen = set()
-    for ppt, rows, stk, maxt in variants:
-        rt.debug_set_launch(ppt=ppt, rows=rows, stk=stk, maxt=maxt)
+    for ppt, rows, maxt in variants:
+        rt.debug_set_launch(ppt=ppt, rows=rows, maxt=maxt)
         key = rt.debug_get_launch()["variant"]
         if key in seen:
             continue
@@ -303,7 +302,7 @@ def test_every_compiled_variant(torch_cuda, H, oracle_mod, config, stride):
         got2 = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
         assert_parity(oracle_mod, cfg, inp, meta, got, ref)
         for k in want:
-            assert np.array_equal(got[k], got2[k]), (k, ppt, rows, stk, maxt)
+            assert np.array_equal(got[k], got2[k]), (k, ppt, rows, maxt)
     rt.close()
 
 
