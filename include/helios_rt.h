@@ -46,6 +46,12 @@ extern "C" {
 #define HELIOS_RT_ENOMEM   -2  /* host or device allocation failed */
 #define HELIOS_RT_ECUDA    -3  /* a CUDA runtime call failed; helios_rt_last_cuda_error() names it */
 #define HELIOS_RT_ENODEV   -4  /* no CUDA device, or the device is not compute capability 10.x */
+#define HELIOS_RT_ESTUCK   -6  /* a step of this handle gave up waiting for the level data of a column (the flag that
+                                  publishes it never arrived within 2^26 polls: a lost write, a device fault).  The step
+                                  ran to its end, but its outputs are INVALID.  helios_rt_step_host returns it for its
+                                  own step; the asynchronous helios_rt_step cannot know yet, so the NEXT call on the
+                                  handle (step, step_host or step_iterative) returns it instead of launching anything,
+                                  once.  After it the handle is usable again. */
 
 /* flags */
 #define HELIOS_RT_IMPROVED       1u  /* improved two-stream: E from Eq.(19); otherwise E = 1 (regular, L73) */

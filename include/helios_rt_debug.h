@@ -27,6 +27,13 @@ int helios_rt_debug_set_launch(helios_rt *h, int32_t warps, int32_t ppt, int32_t
  * trade, not something the product path sets.  Re-allocates the workspace like set_launch. */
 int helios_rt_debug_set_workers(helios_rt *h, int32_t workers);
 
+/* on != 0: every later step of the handle is launched WITHOUT its phase A, with a poll limit of 64: no column is ever
+ * published, every block gives up waiting and the step must be reported as HELIOS_RT_ESTUCK (by helios_rt_step_host at
+ * once, by the call after an asynchronous helios_rt_step).  Such a step sweeps whatever the workspace holds: call it
+ * only after a normal step of the same handle on the same inputs (an uninitialised workspace holds wild table indices).
+ * Lets a test see the error path that a healthy GPU never takes. */
+int helios_rt_debug_force_stuck(helios_rt *h, int32_t on);
+
 /* on != 0: every later step of the handle takes the path the library falls back to when the device cannot host the
  * whole grid of rt_step_kernel at once (cooperative launch refused): phase A as a launch of its own (rt_prep_kernel),
  * then the sweeps as a plain launch.  Lets the tests run that path through the parity checks. */

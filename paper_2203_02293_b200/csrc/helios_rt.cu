@@ -122,6 +122,8 @@ struct helios_rt {
   cudaStream_t own_stream;   // step_host runs on it
   int regs, lmem, sm_count;
   int force_two_launches;   // helios_rt_debug_force_two_launches: always take the fallback path (tests)
+  int force_stuck;          // helios_rt_debug_force_stuck: the next steps never see their columns published (tests)
+  unsigned *h_err, *d_err;  // error word: page-locked mapped host memory and its device alias (KParams::err)
   int workers_cap;          // helios_rt_debug_set_workers: upper bound of workers per tile (0 = none; tuning runs)
   cudaError_t last_err;
 };
@@ -139,6 +141,8 @@ extern "C" const char *helios_rt_strerror(int code) {
     case HELIOS_RT_ENOMEM: return "out of memory";
     case HELIOS_RT_ECUDA: return "CUDA runtime error (see helios_rt_last_cuda_error)";
     case HELIOS_RT_ENODEV: return "no usable CUDA device (compute capability 10.x required)";
+    case HELIOS_RT_ESTUCK: return "a step of this handle gave up waiting for a column's level data (its publication flag never "
+                                  "arrived); the outputs of that step are invalid";
     case HELIOS_RT_ETOOBIG: return "problem too large for the built-in scratch array of helios_rt_phase_curve_noalloc "
                                    "(HELIOS_RT_PHASE_CURVE_NOALLOC_MAX_BYTES); use helios_rt_phase_curve with your own workspace";
     default: return "unknown error code";
@@ -215,6 +219,7 @@ extern "C" int helios_rt_destroy(helios_rt *h) {
   free(h->inv_dlam);
   if (h->h_in) cudaFreeHost(h->h_in);
   if (h->h_out) cudaFreeHost(h->h_out);
+  if (h->h_err) cudaFreeHost(h->h_err);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   delete h;
   return HELIOS_RT_OK;
@@ -431,6 +436,11 @@ extern "C" int helios_rt_create(const helios_rt_config *cfg, helios_rt **out) {
   step(cudaMalloc((void **)&h->d_in, sizeof(double) * n_in));
   step(cudaMalloc((void **)&h->d_out, sizeof(double) * n_out));
   step(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
+  step(cudaHostAlloc((void **)&h->h_err, 64, cudaHostAllocMapped));
+  if (e == cudaSuccess) {
+    memset(h->h_err, 0, 64);
+    step(cudaHostGetDevicePointer((void **)&h->d_err, h->h_err, 0));
+  }
   if (e == cudaSuccess) {
     iter_fn it = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
     if (!h->toa)
@@ -491,6 +501,7 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   P.fused_prep = 0;
   P.stack = h->d_stack; P.stack_block = h->stack_block;
   P.partial = h->d_partial; P.counter = h->d_counter; P.queue = h->d_queue;
+  P.err = h->d_err; P.poll_limit = h->force_stuck ? 64u : (1u << 26);
   if (n_iter > 0) {
     if (in->n_columns > 65535) return HELIOS_RT_EINVAL;   // the comparison kernel puts columns in gridDim.y
     iter_fn fn = h->noniso ? rt_iter_kernel<true> : rt_iter_kernel<false>;
@@ -531,6 +542,12 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   lc.numAttrs = 1;
   P.fused_prep = 1;
   void *args[1] = {&P};
+  if (h->force_stuck) {   // tests: no phase A at all, so no column is ever published and every block gives up
+    P.fused_prep = 0;
+    lc.numAttrs = 0;
+    CK(h, cudaLaunchKernelExC(&lc, kVariants[h->variant].fn, args));
+    return HELIOS_RT_OK;
+  }
   cudaError_t e = h->force_two_launches ? cudaErrorCooperativeLaunchTooLarge : cudaLaunchKernelExC(&lc, kVariants[h->variant].fn, args);
   if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) {
     cudaGetLastError();
@@ -549,10 +566,20 @@ static int launch_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt
   return HELIOS_RT_OK;
 }
 
+// Reads and clears the handle's error word (written by the kernel through its device alias).  No synchronisation: a
+// step still in flight is seen by a later call.
+static bool take_stuck(helios_rt *h) {
+  volatile unsigned *w = h->h_err;
+  if (!w || *w == 0u) return false;
+  *w = 0u;
+  return true;
+}
+
 extern "C" int helios_rt_step(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out,
                               void *cuda_stream) {
   const int rc = validate_step(h, in, out);
   if (rc) return rc;
+  if (take_stuck(h)) return HELIOS_RT_ESTUCK;   // an EARLIER step of the handle: nothing is launched by this call
   return launch_step(h, in, out, (cudaStream_t)cuda_stream);
 }
 
@@ -561,6 +588,7 @@ extern "C" int helios_rt_step_iterative(helios_rt *h, const helios_rt_inputs *in
   const int rc = validate_step(h, in, out);
   if (rc) return rc;
   if (n_iterations < 1 || h->toa || out->F_up_toa_bin) return HELIOS_RT_EINVAL;
+  if (take_stuck(h)) return HELIOS_RT_ESTUCK;
   return launch_step(h, in, out, (cudaStream_t)cuda_stream, n_iterations);
 }
 
@@ -575,6 +603,7 @@ static double *mapped_alias(double *host) {
 extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, const helios_rt_outputs *out) {
   int rc = validate_step(h, in, out);
   if (rc) return rc;
+  if (take_stuck(h)) return HELIOS_RT_ESTUCK;   // an earlier asynchronous step of the handle
   if (in->n_columns == 0) return HELIOS_RT_OK;
   const size_t ncol = (size_t)in->n_columns, N = (size_t)h->cfg.n_layers, nb = (size_t)h->cfg.n_bins;
   cudaStream_t st = h->own_stream;
@@ -613,7 +642,7 @@ extern "C" int helios_rt_step_host(helios_rt *h, const helios_rt_inputs *in, con
   for (int k = 0; k < 6; ++k)
     if (staged[k]) CK(h, cudaMemcpyAsync(host[k], dev[k], sizeof(double) * count[k], cudaMemcpyDeviceToHost, st));
   CK(h, cudaStreamSynchronize(st));
-  return HELIOS_RT_OK;
+  return take_stuck(h) ? HELIOS_RT_ESTUCK : HELIOS_RT_OK;   // this very step
 }
 
 extern "C" int helios_rt_launch_info(const helios_rt *h, int32_t info[8]) {
@@ -651,6 +680,12 @@ extern "C" int helios_rt_debug_set_workers(helios_rt *h, int32_t workers) {
   int rc = configure_launch(h);
   if (rc) { h->workers_cap = old; configure_launch(h); }
   return rc;
+}
+
+extern "C" int helios_rt_debug_force_stuck(helios_rt *h, int32_t on) {
+  if (!h) return HELIOS_RT_EINVAL;
+  h->force_stuck = on != 0;
+  return HELIOS_RT_OK;
 }
 
 extern "C" int helios_rt_debug_force_two_launches(helios_rt *h, int32_t on) {

@@ -98,6 +98,9 @@ struct KParams {
   unsigned *counter;      // [ncol]   tiles of the column that have published their partial sums
   unsigned *queue;        // [tiles]  next column of each tile's queue;  queue[tiles] = blocks that have finished;
                           // queue[tiles + 1] = blocks that have finished phase A
+  unsigned *err;          // the handle's error word (device alias of page-locked host memory): set to 1 by a block that
+                          // gave up waiting for a column's publication flag (HELIOS_RT_ESTUCK)
+  unsigned poll_limit;    // polls of a publication flag before giving up (2^26; tests force a small value)
 };
 
 // --------------------------------------------------------------------------------------------
@@ -824,7 +827,9 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
   bool all_published = false;               // thread 0: every block has finished phase A -- no more flag polls
   auto fetch_column = [&](int c, int buf) {   // thread 0
     // (the whole grid is resident -- cooperative launch -- and phase A waits for nothing, so this terminates; the
-    // poll count is bounded all the same: a wedged GPU is worse than a wrong column)
+    // poll count is bounded all the same, so that a lost flag cannot wedge the GPU.  A block that gives up says so in
+    // the handle's error word: the step still runs to its end, on whatever the workspace holds, but the host
+    // reports HELIOS_RT_ESTUCK for it -- its outputs are never passed off as results.)
     if (!all_published) {
       unsigned n;
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(n) : "l"(P.queue + P.tiles + 1) : "memory");
@@ -833,7 +838,11 @@ __global__ void __launch_bounds__(MAXT, MINB) rt_step_kernel(const KParams P) {
         unsigned f, polls = 0;
         do {
           asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(P.flags + c) : "memory");
-        } while (f != (unsigned)(nlev + 1) && ++polls < (1u << 26));
+        } while (f != (unsigned)(nlev + 1) && ++polls < P.poll_limit);
+        if (f != (unsigned)(nlev + 1)) {
+          *(volatile unsigned *)P.err = 1u;
+          __threadfence_system();
+        }
       }
       asm volatile("fence.proxy.async.global;" ::: "memory");
     }

@@ -23,7 +23,7 @@ EXPORTS = ("helios_rt_create", "helios_rt_step", "helios_rt_step_host", "helios_
            "helios_rt_extend_top", "helios_rt_phase_curve", "helios_rt_phase_curve_workspace_bytes",
            "helios_rt_phase_curve_noalloc",
            "helios_rt_advance_1d", "helios_rt_debug_set_launch", "helios_rt_debug_get_launch",
-           "helios_rt_debug_force_two_launches", "helios_rt_debug_set_workers")
+           "helios_rt_debug_force_two_launches", "helios_rt_debug_set_workers", "helios_rt_debug_force_stuck")
 # ... and in include/helios_rt_selftest.h (libhelios_rt_selftest.so)
 SELFTEST_EXPORTS = ("helios_rt_selftest_math", "helios_rt_selftest_planck", "helios_rt_selftest_planck_G",
                     "helios_rt_measure_dfma_peak", "helios_rt_measure_latencies")
@@ -92,6 +92,8 @@ def load_library() -> C.CDLL:
         L.helios_rt_advance_1d.argtypes = [C.c_int32] * 2 + [C.c_double] * 4 + [C.c_void_p] * 6
         L.helios_rt_debug_force_two_launches.restype = C.c_int
         L.helios_rt_debug_force_two_launches.argtypes = [C.c_void_p, C.c_int32]
+        L.helios_rt_debug_force_stuck.restype = C.c_int
+        L.helios_rt_debug_force_stuck.argtypes = [C.c_void_p, C.c_int32]
         L.helios_rt_debug_set_workers.restype = C.c_int
         L.helios_rt_debug_set_workers.argtypes = [C.c_void_p, C.c_int32]
         L.helios_rt_debug_set_launch.restype = C.c_int
@@ -190,6 +192,10 @@ class HeliosRT:
         """helios_rt_debug_set_launch (include/helios_rt_debug.h; tests and tuning only)."""
         _check(load_library().helios_rt_debug_set_launch(self._h, int(warps), int(ppt), int(rows), int(maxt), int(minb)),
                self._h)
+
+    def debug_force_stuck(self, on: bool = True) -> None:
+        """Tests only (helios_rt_debug.h): later steps never see their columns published and must report error -6."""
+        _check(load_library().helios_rt_debug_force_stuck(self._h, int(bool(on))), self._h)
 
     def debug_set_workers(self, workers: int) -> None:
         """helios_rt_debug_set_workers (helios_rt_debug.h; tuning only): cap the persistent workers per tile (0 = no cap)."""

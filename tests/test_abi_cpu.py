@@ -54,7 +54,8 @@ def test_product_library_ignores_the_environment():
 
 def test_strerror(lib):
     assert lib.helios_rt_strerror(0) == b"success"
-    for code in (-1, -2, -3, -4):
+    assert b"invalid" in lib.helios_rt_strerror(-6)     # HELIOS_RT_ESTUCK
+    for code in (-1, -2, -3, -4, -5, -6):
         assert len(lib.helios_rt_strerror(code)) > 5
     assert b"unknown" in lib.helios_rt_strerror(-77)
 

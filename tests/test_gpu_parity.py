@@ -327,6 +327,31 @@ def test_fallback_two_launches(torch_cuda, H, oracle_mod, config, stride):
         assert np.array_equal(one[k], two[k]) and np.array_equal(two[k], two_again[k]) and np.array_equal(one[k], back[k]), k
 
 
+@pytest.mark.parametrize("config,stride", [(2, 173), (3, 259), (5, 701)])
+def test_stuck_publication_flag_is_reported_not_guessed(torch_cuda, H, config, stride):
+    """A block that gives up waiting for a column's publication flag must not pass its output off as a result:
+    helios_rt_step_host returns HELIOS_RT_ESTUCK (-6) for its own step; after an asynchronous helios_rt_step the next
+    call on the handle returns it, once, without launching; then the handle works again and reproduces the first
+    answer bit for bit (queues, counters and flags re-armed).  Forced through helios_rt_debug_force_stuck."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config, columns=slice(3, None, stride))
+    want = ("F_up_toa_bin",) if config == 5 else ("F_up", "F_down", "F_net", "dTdt")
+    rt = H.HeliosRT(cfg, inp["p"].shape[0])
+    good = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)
+    rt.debug_force_stuck(True)
+    with pytest.raises(H.HeliosRTError, match=r"error -6"):
+        run_gpu(torch_cuda, H, cfg, inp, want, rt=rt, host="pinned")         # step_host: reported by the step itself
+    run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)                            # asynchronous step: returns OK ...
+    rt.debug_force_stuck(False)
+    with pytest.raises(H.HeliosRTError, match=r"error -6"):
+        run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)                        # ... and the next call reports it
+    again = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt)                    # reported once; the handle is usable
+    host = run_gpu(torch_cuda, H, cfg, inp, want, rt=rt, host="pinned")
+    rt.close()
+    for k in want:
+        assert np.array_equal(good[k], again[k]) and np.array_equal(good[k], host[k]), k
+
+
 def test_ragged_shapes(torch_cuda, H, oracle_mod):
     """Odd sizes: 3 bins x 5 Gauss points (15 points, half a warp), 7 layers; 1 layer; the maximum 64 layers; a single
     spectral point; and one Gauss point per bin (the opacity-sampling kernel variant) with all outputs, 150 bins."""
