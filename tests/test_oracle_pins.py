@@ -806,3 +806,74 @@ def test_opcount_build_matches_the_oracle_and_counts(oracle_mod):
     b = oracle_mod.rt_step(cfg, inp, real="ld", want=("F_net", "dTdt"))
     for k in a:
         assert np.array_equal(a[k], b[k]), k
+
+
+# ---------------------------------------------------------------- round 3: the last two unpinned parts
+# (a) the per-bin TOA spectrum F_up_toa_bin[b] = sum_g w_g F_up[N](b, g) -- the
+#     only output of config 5 and of the post-processing step -- was checked by a numpy re-typing of its own line only;
+# (b) the interfaces of a single-layer column (reading R27) by nothing.
+# Planted mistakes these fail on: "toa_bin += dlam * w_g * Fu", "toa_bin += Fu" (w_g dropped), "Fu[N]" for
+# "Fu[N * stride]" on non-isothermal columns, sqrt(10) -> any other factor in levels().
+
+@pytest.mark.parametrize("config", [1, 5])
+@pytest.mark.parametrize("noniso", [False, True])
+def test_toa_spectrum_integrates_to_the_toa_flux(oracle_mod, config, noniso):
+    """sum_b dlam_b F_up_toa_bin[c, b] = F_up[c, N]: the left side goes through the per-bin accumulation, the right
+    through the interface accumulation that the closed-form pins above cover (pure absorption, opaque limit, energy
+    closure).  Non-isothermal columns have 2N + 1 levels per point: the TOA is level 2N, not N."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(config, columns=slice(0, 6)) if config == 1 else W.make(config, columns=slice(5, None, 640))
+    flags = (cfg["flags"] & ~W.TOA_SPECTRUM & ~W.NONISOTHERMAL) | (W.NONISOTHERMAL if noniso else 0)
+    res = oracle_mod.rt_step(dict(cfg, flags=flags), inp, want=("F_up", "F_up_toa_bin"))
+    dlam = np.diff(np.asarray(cfg["bin_edges"]))
+    assert np.all(dlam > 0) and np.ptp(dlam) > 0.5 * dlam.min()          # unequal bins: a missing / doubled dlam shows
+    integral = res["F_up_toa_bin"] @ dlam
+    assert np.all(integral > 0)
+    assert np.allclose(integral, res["F_up"][:, -1], rtol=1e-13, atol=0)
+    # ... and the spectrum is not the flux at some other level: in these columns F_up changes with height
+    assert np.all(np.abs(res["F_up"][:, meta["n_layers"] // 2] / res["F_up"][:, -1] - 1) > 1e-3)
+
+
+def test_toa_spectrum_pure_absorption_closed_form(oracle_mod):
+    """One isothermal, purely absorbing, night-side column with a (P, T)-independent opacity: per spectral point
+    F_up[N] = pi B (1 - e^{-2 tau}) + e^{-2 tau} (pi B (1 - e^{-2 tau}) + pi B(T_int)), tau = kappa_g (p_0 - p_N) / g
+    (the closed form of test_pure_absorption_closed_form with one source value).  Two bins of different width, three
+    Gauss points with UNEQUAL weights and opacities a decade apart: F_up_toa_bin[b] must be their w_g-weighted sum, per
+    unit wavelength (no dlam), with no cross-talk between bins."""
+    nb, ng = 2, 3
+    kap = np.array([[3e-4, 3e-3, 3e-2], [1e-3, 2e-4, 5e-2]])
+    gw = np.array([0.2, 0.5, 0.3])
+    cfg = _optics_cfg(kap, 0.0, 0.0, 0.0, 0.0, nb=nb, ng=ng)
+    cfg["bin_edges"] = np.array([2e-6, 3e-6, 5e-6])
+    cfg["gauss_w"] = gw
+    N, T0, f_int = 6, 1500.0, 4000.0
+    p = np.logspace(5, 2, N)[None, :]
+    inp = dict(p=p, T=np.full((1, N), T0), mu_star=np.array([-1.0]), stellar_flux=np.array([7.0, 9.0]), f_internal=f_int)
+    for flags in (1, 3):
+        res = oracle_mod.rt_step(dict(cfg, flags=flags), inp, want=("F_up_toa_bin", "F_up"))
+        p_int, _ = oracle_mod.levels(p[0], inp["T"][0])
+        col = (p_int[0] - p_int[-1]) / cfg["gravity"]
+        T_int = (f_int / 5.670374419e-8) ** 0.25
+        expect = np.zeros(nb)
+        for b in range(nb):
+            lo, hi = cfg["bin_edges"][b], cfg["bin_edges"][b + 1]
+            piB, piB_int = np.pi * oracle_mod.planck_bin_mean(T0, lo, hi), np.pi * oracle_mod.planck_bin_mean(T_int, lo, hi)
+            for g in range(ng):
+                tr = np.exp(-2.0 * kap[b, g] * col)
+                expect[b] += gw[g] * (piB * (1 - tr) + tr * (piB * (1 - tr) + piB_int))
+        assert np.allclose(res["F_up_toa_bin"][0], expect, rtol=1e-12, atol=0), flags
+        assert abs(expect[0] / expect[1] - 1) > 0.1                 # the two bins differ: swapping them would show
+
+
+def test_levels_single_layer_reading_R27(oracle_mod):
+    """N = 1 (reading R27): with no neighbour to take a half step from, the one layer spans one decade of pressure
+    centred (in ln p) on its own pressure.  Hand values: p = 2e4 Pa -> interfaces 2e4 * 10^(+-1/2)."""
+    pi, ti = oracle_mod.levels(np.array([2.0e4]), np.array([1234.5]))
+    assert pi.shape == (2,) and ti.shape == (2,)
+    assert pi[0] == pytest.approx(63245.553203367587, rel=1e-15)     # 2e4 * 3.1622776601683793...
+    assert pi[1] == pytest.approx(6324.5553203367587, rel=1e-15)     # 2e4 / 3.1622776601683793...
+    assert pi[0] / pi[1] == pytest.approx(10.0, rel=1e-15) and pi[0] * pi[1] == pytest.approx(4.0e8, rel=1e-15)
+    assert ti[0] == 1234.5 and ti[1] == 1234.5
+    # the same rule is what R9 gives a two-layer column whose layers are one decade apart: the limits agree
+    pi2, _ = oracle_mod.levels(np.array([2.0e4, 2.0e3]), np.array([1000.0, 900.0]))
+    assert pi2[0] == pytest.approx(pi[0], rel=1e-14) and pi2[1] == pytest.approx(pi[1], rel=1e-14)
