@@ -47,7 +47,30 @@ def _timed(torch, fn, steps, flush, stream):
     return float(t.mean()), float(t.min())
 
 
-def bench_postproc(torch, H, W, steps):
+def _postproc_cpu_baseline(cfg, inp, meta, n_cols: int = 12) -> dict:
+    """The oracle (as it stands, double build) on a bounded sample of config 6: the RT step of `n_cols` evenly strided
+    extended columns, then the phase curve of the whole grid from a synthetic spectrum of the right shape -- scaled to one
+    pipeline pass.  A stated baseline, not a target."""
+    import time
+    import oracle
+    from oracle import postproc
+    n, N, ne = meta["n_columns"], meta["n_model_layers"], meta["n_extra"]
+    idx = np.linspace(0, n - 1, n_cols).astype(int)
+    p_ext, T_ext = postproc.extend_top(inp["p"][idx], inp["T"][idx], ne, meta["p_min"])
+    sub = dict(inp, p=p_ext, T=T_ext, mu_star=inp["mu_star"][idx])
+    t0 = time.perf_counter()
+    ref = oracle.rt_step(cfg, sub, real="f64", want=("F_up_toa_bin",))
+    t_step = (time.perf_counter() - t0) * n / n_cols
+    F = np.tile(ref["F_up_toa_bin"], (n // n_cols + 1, 1))[:n]
+    t0 = time.perf_counter()
+    postproc.phase_curve(F, meta["lon"], meta["lat"], meta["area"], meta["alpha"], cfg["bin_edges"], *meta["band"])
+    t_pc = time.perf_counter() - t0
+    return {"value": (t_step + t_pc) * 1e3, "unit": "ms", "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"RT step of {n_cols} evenly strided extended columns scaled to {n}, + the phase curve of the whole grid",
+            "rt_step_s": t_step, "phase_curve_s": t_pc}
+
+
+def bench_postproc(torch, H, W, steps, cpu_baseline: bool = True):
     cfg, inp, meta = W.make(6)
     dev = torch.device("cuda", 0)
     t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
@@ -81,6 +104,18 @@ def bench_postproc(torch, H, W, steps):
     pc_bytes = 8.0 * (n * nb + na * nb + 3 * n + na)       # F read once, phase spectra written once
     pc_flops = 2.0 * n * nb * na                           # one FMA per (column, bin, phase)
     solves = n * nb
+    # fp64-ALU roofline of the opacity-sampling RT step: the locked TOA-mode slots of bench.py (138 day / 90 night per
+    # layer.point) over the extended columns
+    from bench import FP64_LANES_PER_SM, algorithmic_slots
+    info = rt.launch_info()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    slots = algorithmic_slots(meta, cfg["flags"], inp["mu_star"])
+    peak = info["sm_count"] * FP64_LANES_PER_SM * sm_max * 1e6
+    rt_roofline = {"bound": "alu", "achieved": slots / (ms_step * 1e-3) * 1e-12, "peak": peak * 1e-12, "unit": "Tslot/s",
+                   "frac": slots / (ms_step * 1e-3) / peak, "algorithmic_slots_per_step": slots,
+                   "t_alu_ms": slots / peak * 1e3, "kernel_ms": ms_step,
+                   "kernel": "rt_step_kernel<NONISO=0, TOA=1, BDIRECT=1> (one point per bin)",
+                   "slot_lock": "BASELINE.md section 3 (TOA mode: 138 day / 90 night slots per layer.point)"}
     line = {"row": "NEXT-2 post-processing", "metric": "postproc_pipeline_ms", "value": ms_all, "unit": "ms",
             "higher_is_better": False, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config6 {meta['name']}: {n} columns x {N}+{ne} layers x {nb} wavelengths x 1, "
@@ -88,6 +123,8 @@ def bench_postproc(torch, H, W, steps):
                        "launch": rt.launch_info()},
             "stages_ms": {"extend_top": ms_ext, "rt_step": ms_step, "phase_curve": ms_pc, "pipeline_min": ms_all_min},
             "rt_step_solves_per_s": solves / (ms_step * 1e-3),
+            "roofline": rt_roofline,
+            "cpu_baseline": _postproc_cpu_baseline(cfg, inp, meta) if cpu_baseline else None,
             "phase_curve": {"bound": "hbm", "algorithmic_bytes": pc_bytes, "achieved_gbs": pc_bytes / (ms_pc * 1e-3) * 1e-9,
                             "peak_gbs": hbm, "frac": pc_bytes / (ms_pc * 1e-3) * 1e-9 / hbm,
                             "fp64_gflops": pc_flops / (ms_pc * 1e-3) * 1e-9,
