@@ -60,7 +60,7 @@ __global__ void extend_top_kernel(int ncol, int N, int n_extra, double p_min, co
 // phase_curve: out[a][b] = sum_i F[i][b] * w_a[i],  w_a[i] = cos(lat_i) max(cos(lon_i - alpha_a), 0) A_i / (pi R_p^2)
 // (Eqs. 25-26; visibility modulo 2 pi, reading R22).  Two launches, F read once per 32 phases:
 //   phase_partial_kernel  grid = (bin tiles of 128, column chunks of 128, phase tiles of 32).  Each thread first
-//       builds the 32 weights of one column of the chunk in shared memory, then accumulates its bin over the
+//       builds the 32 weights of one column of the chunk in shared memory (angle-addition form), then accumulates its bin over the
 //       chunk's columns in index order: F rows read coalesced, weights broadcast from shared memory two at a time,
 //       32 independent FMA chains in registers.  Writes part[chunk][phase][bin] to the caller's workspace.
 //   phase_reduce_kernel   out[a][b] = sum over chunks in chunk order.
@@ -75,19 +75,30 @@ __global__ void __launch_bounds__(PC_BINS) phase_partial_kernel(int ncol, int nb
                                                                  const double *__restrict__ alpha,
                                                                  double *__restrict__ part) {
   __shared__ __align__(16) double s_w[PC_COLS][PC_PH];
-  __shared__ double s_alpha[PC_PH];
+  __shared__ __align__(16) double2 s_cs[PC_PH];   // (cos alpha, sin alpha) of the tile's phases
   const int tid = threadIdx.x;
   const int bin = blockIdx.x * PC_BINS + tid;
   const int chunk = blockIdx.y, c0 = chunk * PC_COLS;
   const int ph0 = blockIdx.z * PC_PH;
-  if (tid < PC_PH) s_alpha[tid] = (ph0 + tid < nph) ? alpha[ph0 + tid] : 0.0;
+  if (tid < PC_PH) {
+    double sa = 0.0, ca = 0.0;
+    if (ph0 + tid < nph) sincos(alpha[ph0 + tid], &sa, &ca);
+    s_cs[tid] = make_double2(ca, sa);
+  }
   __syncthreads();
   {
+    // cos(lon - alpha) = cos lon cos alpha + sin lon sin alpha: one sincos per column and per phase instead of one cos per
+    // (column, phase) -- the weights were as expensive as the sum they feed (32 fp64 cosines against 128 FMAs per thread
+    // and phase).  The two forms differ by a few 1e-16 (absolute), also in which side of the terminator a column with
+    // |cos| < 1e-16 falls on; its weight is below 1e-16 of the disc either way.
     const int i = c0 + tid;
     if (i < ncol) {
-      const double lo = lon[i], cl = cos(lat[i]) * (area[i] / kPi);
+      double sl, clon;
+      sincos(lon[i], &sl, &clon);
+      const double cl = cos(lat[i]) * (area[i] / kPi);
       for (int k = 0; k < PC_PH; ++k) {
-        const double c = cos(lo - s_alpha[k]);
+        const double2 cs = s_cs[k];
+        const double c = fma(sl, cs.y, clon * cs.x);
         s_w[tid][k] = (c > 0.0) ? cl * c : 0.0;     // Eq.(26)
       }
     } else {
