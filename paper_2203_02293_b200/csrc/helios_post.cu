@@ -35,25 +35,26 @@ int device_ok() {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// extend_top: one thread per column.  n_extra layers above the top layer, equally spaced in ln p with the ratio
-// q = min(p[N-1]/p[N-2], (p_min/p[N-1])^(1/n_extra)) (reading R21); T = T[N-1] (L385).
+// extend_top: one thread per OUTPUT element (column, extended layer), so that consecutive threads write consecutive
+// addresses (one thread per column wrote with a stride of N + n_extra doubles).  n_extra layers above the top layer,
+// equally spaced in ln p with the ratio q = min(p[N-1]/p[N-2], (p_min/p[N-1])^(1/n_extra)) (reading R21);
+// T = T[N-1] (L385).  Every element is the same expression as before: p_top * q^k, bit for bit.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void extend_top_kernel(int ncol, int N, int n_extra, double p_min, const double *__restrict__ p,
-                                  const double *__restrict__ T, double *__restrict__ p_ext, double *__restrict__ T_ext) {
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= ncol) return;
+__global__ void __launch_bounds__(256) extend_top_kernel(int ncol, int N, int n_extra, double p_min,
+                                                         const double *__restrict__ p, const double *__restrict__ T,
+                                                         double *__restrict__ p_ext, double *__restrict__ T_ext) {
+  const int Ne = N + n_extra;
+  const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (e >= (size_t)ncol * Ne) return;
+  const int c = (int)(e / Ne), j = (int)(e - (size_t)c * Ne);
   const double *pc = p + (size_t)c * N, *Tc = T + (size_t)c * N;
-  double *po = p_ext + (size_t)c * (N + n_extra), *To = T_ext + (size_t)c * (N + n_extra);
-  for (int j = 0; j < N; ++j) { po[j] = pc[j]; To[j] = Tc[j]; }
-  if (n_extra == 0) return;
-  const double p_top = pc[N - 1], T_top = Tc[N - 1];
+  if (j < N) { p_ext[e] = pc[j]; T_ext[e] = Tc[j]; return; }
+  const double p_top = pc[N - 1];
   const double q_own = (N > 1) ? p_top / pc[N - 2] : sqrt(0.1);
   const double q_need = pow(p_min / p_top, 1.0 / (double)n_extra);
   const double q = fmin(q_own, q_need);
-  for (int k = 1; k <= n_extra; ++k) {
-    po[N - 1 + k] = p_top * pow(q, (double)k);
-    To[N - 1 + k] = T_top;
-  }
+  p_ext[e] = p_top * pow(q, (double)(j - (N - 1)));
+  T_ext[e] = Tc[N - 1];
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -159,7 +160,8 @@ __global__ void __launch_bounds__(256) phase_band_kernel(int nb, const double *_
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// advance_1d: one thread per column.  T <- T + dt dT/dt (reading R26); p[0] = p_ref and Eq.(20) upward with the
+// advance_1d: one thread per column (columns longer than 62 layers; shorter ones take advance_1d_tile_kernel below, which
+// is this kernel with its loads and stores staged through shared memory).  T <- T + dt dT/dt (reading R26); p[0] = p_ref and Eq.(20) upward with the
 // sign of reading R25; rho = p / (R_d T).
 // ---------------------------------------------------------------------------------------------------------
 __global__ void advance_1d_kernel(int ncol, int N, double dt, double gravity, double R_d, double p_ref,
@@ -187,6 +189,59 @@ __global__ void advance_1d_kernel(int ncol, int N, double dt, double gravity, do
   }
 }
 
+// The same step with coalesced memory traffic: a block of 32 threads owns 32 consecutive columns, whose T, dT/dt and
+// outputs are one contiguous range of 32 N doubles each.  The block copies T and dT/dt into shared memory with
+// consecutive threads on consecutive addresses, each thread then walks ITS column in shared memory (row stride N + 1:
+// odd or not, the 32 rows start in different banks for every N that is not a multiple of 16) with exactly the
+// arithmetic of advance_1d_kernel -- same operations in the same order, so the results are bit-identical -- and the
+// block writes T, p and rho back as linear copies.  Shared memory: 3 x 32 x (N + 1) doubles (N <= 62 fits 48 KB; longer
+// columns take the kernel above).
+constexpr int A1_COLS = 32;
+__global__ void __launch_bounds__(A1_COLS) advance_1d_tile_kernel(int ncol, int N, double dt, double gravity, double R_d,
+                                                                  double p_ref, const double *__restrict__ z,
+                                                                  const double *__restrict__ dTdt, double *__restrict__ T,
+                                                                  double *__restrict__ p, double *__restrict__ rho) {
+  extern __shared__ double a1_smem[];
+  const int ld = N + 1;
+  double *sT = a1_smem, *sH = sT + A1_COLS * ld, *sP = sH + A1_COLS * ld;
+  const int tid = threadIdx.x, c0 = blockIdx.x * A1_COLS;
+  const int nc = (ncol - c0 < A1_COLS) ? ncol - c0 : A1_COLS;
+  const size_t base = (size_t)c0 * N;
+  const int n_el = nc * N;
+  for (int e = tid; e < n_el; e += A1_COLS) {
+    const int c = e / N, i = e - c * N;
+    sT[c * ld + i] = T[base + e];
+    if (dTdt) sH[c * ld + i] = dTdt[base + e];
+  }
+  __syncwarp();
+  if (tid < nc) {
+    double *Tc = sT + tid * ld, *pc = sP + tid * ld;
+    const double *hc = dTdt ? sH + tid * ld : nullptr;
+    const double g2R = gravity / (2.0 * R_d);
+    double T_prev = hc ? __dadd_rn(Tc[0], __dmul_rn(dt, hc[0])) : Tc[0];
+    double p_prev = p_ref;
+    Tc[0] = T_prev;
+    pc[0] = p_prev;
+    for (int i = 1; i < N; ++i) {
+      const double Ti = hc ? __dadd_rn(Tc[i], __dmul_rn(dt, hc[i])) : Tc[i];
+      const double inv_dz = 1.0 / (z[i] - z[i - 1]);
+      const double pi = p_prev * (inv_dz - g2R / T_prev) / (inv_dz + g2R / Ti);
+      Tc[i] = Ti;
+      pc[i] = pi;
+      T_prev = Ti;
+      p_prev = pi;
+    }
+  }
+  __syncwarp();
+  for (int e = tid; e < n_el; e += A1_COLS) {
+    const int c = e / N, i = e - c * N;
+    const double Ti = sT[c * ld + i], pi = sP[c * ld + i];
+    T[base + e] = Ti;
+    p[base + e] = pi;
+    if (rho) rho[base + e] = pi / (R_d * Ti);
+  }
+}
+
 }  // namespace
 
 extern "C" int helios_rt_extend_top(int32_t n_columns, int32_t n_layers, int32_t n_extra, double p_min, const double *p,
@@ -196,8 +251,9 @@ extern "C" int helios_rt_extend_top(int32_t n_columns, int32_t n_layers, int32_t
   const int rc = device_ok();
   if (rc) return rc;
   if (n_columns == 0) return HELIOS_RT_OK;
-  extend_top_kernel<<<(n_columns + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(n_columns, n_layers, n_extra, p_min, p, T,
-                                                                                    p_ext, T_ext);
+  const size_t n_el = (size_t)n_columns * (n_layers + n_extra);
+  extend_top_kernel<<<(unsigned)((n_el + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(n_columns, n_layers, n_extra, p_min, p,
+                                                                                          T, p_ext, T_ext);
   return cudaGetLastError() == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
 }
 
@@ -304,7 +360,12 @@ extern "C" int helios_rt_advance_1d(int32_t n_columns, int32_t n_layers, double 
   const int rc = device_ok();
   if (rc) return rc;
   if (n_columns == 0) return HELIOS_RT_OK;
-  advance_1d_kernel<<<(n_columns + 63) / 64, 64, 0, (cudaStream_t)cuda_stream>>>(n_columns, n_layers, dt, gravity, R_d, p_ref, z,
-                                                                                 dTdt, T, p, rho);
+  const size_t smem = sizeof(double) * 3 * A1_COLS * ((size_t)n_layers + 1);
+  if (smem <= 48 * 1024)
+    advance_1d_tile_kernel<<<(n_columns + A1_COLS - 1) / A1_COLS, A1_COLS, smem, (cudaStream_t)cuda_stream>>>(
+        n_columns, n_layers, dt, gravity, R_d, p_ref, z, dTdt, T, p, rho);
+  else
+    advance_1d_kernel<<<(n_columns + 63) / 64, 64, 0, (cudaStream_t)cuda_stream>>>(n_columns, n_layers, dt, gravity, R_d, p_ref, z,
+                                                                                   dTdt, T, p, rho);
   return cudaGetLastError() == cudaSuccess ? HELIOS_RT_OK : HELIOS_RT_ECUDA;
 }

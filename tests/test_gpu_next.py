@@ -250,11 +250,13 @@ def test_postprocessing_full_size_sampled(torch_cuda, H):
 
 
 # ------------------------------------------------------------------------------------------ NEXT-3
-def test_advance_1d_matches_the_oracle(torch_cuda, H):
+@pytest.mark.parametrize("n,N", [(200, 40), (77, 16), (33, 62), (45, 63), (5, 1), (70, 100)])
+def test_advance_1d_matches_the_oracle(torch_cuda, H, n, N):
+    """Column counts with a ragged last block of 32, layer counts either side of the 62-layer limit of the shared-memory
+    kernel (longer columns take the thread-per-column kernel), a multiple of 16 (bank-aligned rows) and a single layer."""
     from oracle import onedim
     torch = torch_cuda
     rng = np.random.default_rng(10)
-    n, N = 200, 40
     z = np.cumsum(rng.uniform(2e4, 9e4, N))
     T = rng.uniform(600, 2500, (n, N))
     h = rng.normal(0, 1e-3, (n, N))
