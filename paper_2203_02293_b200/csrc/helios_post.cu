@@ -60,28 +60,35 @@ __global__ void __launch_bounds__(256) extend_top_kernel(int ncol, int N, int n_
 // ---------------------------------------------------------------------------------------------------------
 // phase_curve: out[a][b] = sum_i F[i][b] * w_a[i],  w_a[i] = cos(lat_i) max(cos(lon_i - alpha_a), 0) A_i / (pi R_p^2)
 // (Eqs. 25-26; visibility modulo 2 pi, reading R22).  Two launches, F read once per 32 phases:
-//   phase_partial_kernel  grid = (bin tiles of 128, column chunks of 128, phase tiles of 32).  Each thread first
-//       builds the 32 weights of one column of the chunk in shared memory (angle-addition form), then accumulates its bin over the
-//       chunk's columns in index order: F rows read coalesced, weights broadcast from shared memory two at a time,
-//       32 independent FMA chains in registers.  Writes part[chunk][phase][bin] to the caller's workspace.
+//   phase_partial_kernel  grid = (bin tiles of 128 NB, column chunks of 128, phase tiles of NPH).  Each thread first
+//       builds the NPH weights of one column of the chunk in shared memory (angle-addition form), then accumulates its NB
+//       bins over the chunk's columns in index order: F rows read coalesced, weights broadcast from shared memory two at
+//       a time, NB x NPH independent FMA chains in registers.  Writes part[chunk][phase][bin] to the caller's workspace.
 //   phase_reduce_kernel   out[a][b] = sum over chunks in chunk order.
 // Both sums run in a fixed order: deterministic run to run.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int PC_BINS = 128, PC_PH = 32, PC_COLS = 128;
+constexpr int PC_BINS = 128, PC_COLS = 128;
 
+// NB bins per thread (bins tid, tid + 128, ... of a tile of 128 NB bins) x NPH phases per block.  The weights reach the
+// FMAs as broadcast 16-byte shared-memory loads, each of which fills 512 B of registers: at <1, 32> that is 8.25 B per FMA
+// against the ~2 B per FMA an SM can deliver at its DFMA rate, and the kernel ran at a quarter of that rate.  <4, 16>
+// uses every loaded weight for four bins (2.5 B per FMA; 64 accumulators per thread) and is what wide spectra take;
+// <1, 32> stays for spectra of up to 256 bins, where a 512-bin tile would be mostly padding.  Every output is the same
+// chain of FMAs in the same order in both shapes: bit-identical results.
+template <int NB, int NPH>
 __global__ void __launch_bounds__(PC_BINS) phase_partial_kernel(int ncol, int nb, int nph, const double *__restrict__ F,
                                                                  const double *__restrict__ lon,
                                                                  const double *__restrict__ lat,
                                                                  const double *__restrict__ area,
                                                                  const double *__restrict__ alpha,
                                                                  double *__restrict__ part) {
-  __shared__ __align__(16) double s_w[PC_COLS][PC_PH];
-  __shared__ __align__(16) double2 s_cs[PC_PH];   // (cos alpha, sin alpha) of the tile's phases
+  __shared__ __align__(16) double s_w[PC_COLS][NPH];
+  __shared__ __align__(16) double2 s_cs[NPH];   // (cos alpha, sin alpha) of the tile's phases
   const int tid = threadIdx.x;
-  const int bin = blockIdx.x * PC_BINS + tid;
+  const int bin0 = blockIdx.x * (PC_BINS * NB) + tid;
   const int chunk = blockIdx.y, c0 = chunk * PC_COLS;
-  const int ph0 = blockIdx.z * PC_PH;
-  if (tid < PC_PH) {
+  const int ph0 = blockIdx.z * NPH;
+  if (tid < NPH) {
     double sa = 0.0, ca = 0.0;
     if (ph0 + tid < nph) sincos(alpha[ph0 + tid], &sa, &ca);
     s_cs[tid] = make_double2(ca, sa);
@@ -97,36 +104,76 @@ __global__ void __launch_bounds__(PC_BINS) phase_partial_kernel(int ncol, int nb
       double sl, clon;
       sincos(lon[i], &sl, &clon);
       const double cl = cos(lat[i]) * (area[i] / kPi);
-      for (int k = 0; k < PC_PH; ++k) {
+      for (int k = 0; k < NPH; ++k) {
         const double2 cs = s_cs[k];
         const double c = fma(sl, cs.y, clon * cs.x);
         s_w[tid][k] = (c > 0.0) ? cl * c : 0.0;     // Eq.(26)
       }
     } else {
-      for (int k = 0; k < PC_PH; ++k) s_w[tid][k] = 0.0;
+      for (int k = 0; k < NPH; ++k) s_w[tid][k] = 0.0;
     }
   }
   __syncthreads();
-  if (bin >= nb) return;
-  double acc[PC_PH];
+  if (bin0 >= nb) return;
+  double acc[NB][NPH];
 #pragma unroll
-  for (int k = 0; k < PC_PH; ++k) acc[k] = 0.0;
+  for (int q = 0; q < NB; ++q)
+#pragma unroll
+    for (int k = 0; k < NPH; ++k) acc[q][k] = 0.0;
   const int nj = (ncol - c0 < PC_COLS) ? (ncol - c0) : PC_COLS;
-  const double *Fp = F + (size_t)c0 * nb + bin;
-#pragma unroll 2
-  for (int j = 0; j < nj; ++j) {
-    const double f = __ldg(Fp + (size_t)j * nb);
-    const double2 *w2 = reinterpret_cast<const double2 *>(&s_w[j][0]);
+  // bins past the end of the spectrum read the thread's first bin instead (no test in the loop); their sums are dropped
+  const double *Fp[NB];
 #pragma unroll
-    for (int k = 0; k < PC_PH / 2; ++k) {
-      const double2 w = w2[k];
-      acc[2 * k] = fma(w.x, f, acc[2 * k]);         // Eq.(25)
-      acc[2 * k + 1] = fma(w.y, f, acc[2 * k + 1]);
+  for (int q = 0; q < NB; ++q) Fp[q] = F + (size_t)c0 * nb + ((bin0 + q * PC_BINS < nb) ? bin0 + q * PC_BINS : bin0);
+  // F is read once, from HBM: the loads of the next UNR columns (16 per thread) are in flight while this batch is summed
+  // (with one or two columns ahead the kernel sat on its global loads: long_scoreboard 3.8 warps per issue-active cycle,
+  // fp64 pipes 35 % busy at 8 warps per SM).  Rows past the end of a ragged chunk re-read its last row and are not summed.
+  constexpr int UNR = 16 / NB;
+  double fa[UNR][NB];
+#pragma unroll
+  for (int u = 0; u < UNR; ++u) {
+    const size_t row = (size_t)(u < nj ? u : nj - 1) * nb;
+#pragma unroll
+    for (int q = 0; q < NB; ++q) fa[u][q] = __ldg(Fp[q] + row);
+  }
+  for (int j0 = 0; j0 < nj; j0 += UNR) {
+    double fb[UNR][NB];
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      const int jn = j0 + UNR + u;
+      const size_t row = (size_t)(jn < nj ? jn : nj - 1) * nb;
+#pragma unroll
+      for (int q = 0; q < NB; ++q) fb[u][q] = __ldg(Fp[q] + row);
     }
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      if (j0 + u < nj) {
+        const double2 *w2 = reinterpret_cast<const double2 *>(&s_w[j0 + u][0]);
+#pragma unroll
+        for (int k = 0; k < NPH / 2; ++k) {
+          const double2 w = w2[k];
+#pragma unroll
+          for (int q = 0; q < NB; ++q) {
+            acc[q][2 * k] = fma(w.x, fa[u][q], acc[q][2 * k]);         // Eq.(25)
+            acc[q][2 * k + 1] = fma(w.y, fa[u][q], acc[q][2 * k + 1]);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < UNR; ++u)
+#pragma unroll
+      for (int q = 0; q < NB; ++q) fa[u][q] = fb[u][q];
   }
 #pragma unroll
-  for (int k = 0; k < PC_PH; ++k)
-    if (ph0 + k < nph) part[((size_t)chunk * nph + ph0 + k) * nb + bin] = acc[k];
+  for (int q = 0; q < NB; ++q) {
+    const int bin = bin0 + q * PC_BINS;
+    if (bin < nb) {
+#pragma unroll
+      for (int k = 0; k < NPH; ++k)
+        if (ph0 + k < nph) part[((size_t)chunk * nph + ph0 + k) * nb + bin] = acc[q][k];
+    }
+  }
 }
 
 __global__ void __launch_bounds__(256) phase_reduce_kernel(int nchunk, size_t n_out, const double *__restrict__ part,
@@ -278,8 +325,13 @@ extern "C" int helios_rt_phase_curve(int32_t n_columns, int32_t n_bins, int32_t 
   const int nchunk = (n_columns + PC_COLS - 1) / PC_COLS;
   const size_t n_out = (size_t)n_phases * n_bins;
   if (nchunk > 0) {
-    dim3 grid((unsigned)((n_bins + PC_BINS - 1) / PC_BINS), (unsigned)nchunk, (unsigned)((n_phases + PC_PH - 1) / PC_PH));
-    phase_partial_kernel<<<grid, PC_BINS, 0, st>>>(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, workspace);
+    if (n_bins > 2 * PC_BINS) {
+      dim3 grid((unsigned)((n_bins + 4 * PC_BINS - 1) / (4 * PC_BINS)), (unsigned)nchunk, (unsigned)((n_phases + 15) / 16));
+      phase_partial_kernel<4, 16><<<grid, PC_BINS, 0, st>>>(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, workspace);
+    } else {
+      dim3 grid((unsigned)((n_bins + PC_BINS - 1) / PC_BINS), (unsigned)nchunk, (unsigned)((n_phases + 31) / 32));
+      phase_partial_kernel<1, 32><<<grid, PC_BINS, 0, st>>>(n_columns, n_bins, n_phases, F_toa_bin, lon, lat, area, alpha, workspace);
+    }
     if (cudaGetLastError() != cudaSuccess) return HELIOS_RT_ECUDA;
   }
   phase_reduce_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, st>>>(nchunk, n_out, workspace, F_phase_bin);
