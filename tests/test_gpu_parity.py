@@ -356,6 +356,42 @@ def test_stuck_publication_flag_is_reported_not_guessed(torch_cuda, H, config, s
         assert np.array_equal(good[k], again[k]) and np.array_equal(good[k], host[k]), k
 
 
+def test_workers_cap_changes_the_grid_not_the_answer(torch_cuda, H):
+    """helios_rt_debug_set_workers (tuning hook behind bench.py --workers-cap): fewer persistent workers per tile means
+    another grid and a smaller back-substitution workspace, and each column is still summed in the same fixed order --
+    the outputs are bit-identical; 0 restores the default grid."""
+    from paper_2203_02293_b200 import workloads as W
+    cfg, inp, meta = W.make(2, columns=slice(1, None, 9))          # 285 columns: more than the default workers per tile
+    rt = H.HeliosRT(cfg, inp["p"].shape[0])
+    base = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)
+    w0 = rt.debug_get_launch()
+    for cap in (1, 7, 100):
+        rt.debug_set_workers(cap)
+        w = rt.debug_get_launch()
+        assert w["workers"] == min(cap, w0["workers"]) and w["tiles"] == w0["tiles"]
+        got = run_gpu(torch_cuda, H, cfg, inp, ALL, rt=rt)
+        for k in ALL:
+            assert np.array_equal(got[k], base[k]), (k, cap)
+    rt.debug_set_workers(0)
+    assert rt.debug_get_launch()["workers"] == w0["workers"]
+    rt.close()
+
+
+def test_launch_info_counts_the_zero_fill_of_straddling_toa_bins(torch_cuda, H):
+    """helios_rt_launch_info()[6]: one launch per step, except for a TOA-spectrum handle whose tile of the spectral axis is
+    not a multiple of n_gauss (config 5: tiles of 128 points, 20 Gauss points per bin), whose step also launches the
+    zero-fill of the atomically accumulated spectrum (helios_rt.h, helios_rt_step)."""
+    from paper_2203_02293_b200 import workloads as W
+    for config, expect in ((2, 1), (3, 1), (5, 2)):
+        cfg, inp, meta = W.make(config, columns=slice(0, 8))
+        rt = H.HeliosRT(cfg, 8)
+        info, shape = rt.launch_info(), rt.debug_get_launch()
+        tp = info["block"] * shape["ppt"]
+        straddle = bool(cfg["flags"] & W.TOA_SPECTRUM) and shape["tiles"] > 1 and tp % meta["n_gauss"] != 0
+        assert info["launches_per_step"] == expect == (2 if straddle else 1), (config, info, shape)
+        rt.close()
+
+
 def test_ragged_shapes(torch_cuda, H, oracle_mod):
     """Odd sizes: 3 bins x 5 Gauss points (15 points, half a warp), 7 layers; 1 layer; the maximum 64 layers; a single
     spectral point; and one Gauss point per bin (the opacity-sampling kernel variant) with all outputs, 150 bins."""
